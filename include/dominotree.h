@@ -1,0 +1,145 @@
+/*
+ * dominotree.h -- C-ABI boundary of the B200-native DominoTree per-round draft-tree builder.
+ *
+ * The operation is Algorithm 1 of the paper (Sec. 3.2 "DominoTree builder"):
+ * per request and decoding round, (1) take the drafter's L x V marginal logits L_i^base
+ * (PAPER.md:56-62), (2) select the top-M candidate tokens at each block position
+ * (PAPER.md:133, 141), (3) run the best-first max-heap expansion to node budget B
+ * (PAPER.md:93, 109, 145-148), scoring the children of each popped node with Domino's
+ * path-dependent correction  L_i = L_i^base + W2 SiLU(W1 [H_i; S_{i-1}]),  S_{i-1} = GRU(E_{<=i-1})
+ * restricted to the M candidates, and (4) emit the
+ * tree tokens, parents, depths, positions and the ancestor-only tree-attention mask for the
+ * verifier.  Readings of the paper where it is silent are listed in
+ * DESIGN.md ("Readings"): slice log-softmax (A1), PyTorch GRU gate convention (A2),
+ * S_0 = GRUcell(0, E[root]) (A4), T_eff (A7), tie-breaks (A8), dead-leaf padding (A10).
+ *
+ * Everything below runs in hand-written sm_100a CUDA kernels inside libdominotree.so; there is
+ * no CPU fallback.  No torch types cross this boundary: plain pointers and sizes only.
+ *
+ * Pointer convention: every data pointer is a DEVICE pointer owned by the caller and borrowed
+ * for the stream-ordered duration of the call (weights: for the lifetime of the handle).  The
+ * only host pointers are the handle, the dt_weights / dt_outputs structs themselves (read
+ * synchronously during the call) and the `_host` entry point, which says so in its name.
+ *
+ * Error behaviour: every entry point returns DT_OK (0) or a negative dt_status; nothing throws,
+ * aborts or prints.  On error no output buffer content is defined.
+ */
+#ifndef DOMINOTREE_H
+#define DOMINOTREE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dt_handle dt_handle;
+
+/* dtype of marginal_logits, backbone_hidden and all five weight tensors (one dtype for all). */
+typedef enum { DT_BF16 = 0, DT_F32 = 1 } dt_dtype;
+
+typedef enum {
+    DT_OK = 0,
+    DT_ERR_INVALID_ARG = -1, /* null pointer, shape/parameter out of range                       */
+    DT_ERR_UNSUPPORTED = -2, /* shape beyond the compiled limits (see DT_MAX_*)                  */
+    DT_ERR_CUDA = -3,        /* a CUDA runtime call failed (dt_last_cuda_error gives the code)   */
+    DT_ERR_ALLOC = -4        /* device or host allocation failed                                 */
+} dt_status;
+
+/* compiled limits */
+#define DT_MAX_M 256   /* candidate width                                   */
+#define DT_MAX_B 255   /* node budget (N = B+1 <= 256 output slots)         */
+#define DT_MAX_K 32    /* branching factor                                  */
+#define DT_MAX_L 64    /* block depth                                       */
+
+/* Frozen drafter weights.  Row-major, dense, no biases. */
+typedef struct {
+    const void *embed;    /* E    [V, d]     frozen target token embedding    */
+    const void *gru_w_ih; /* W_ih [3g, d]    rows stacked (r, z, n) gates (reading A2) PAPER.md:68   */
+    const void *gru_w_hh; /* W_hh [3g, g]                                                            */
+    const void *corr_w1;  /* W1   [r, d+g]   cols [0,d) act on H_i, [d,d+g) on S_{i-1} PAPER.md:76   */
+    const void *corr_w2;  /* W2   [V, r]     rank-r -> vocabulary projection*/
+    int32_t V, d, g, r;
+    int32_t dtype;        /* dt_dtype */
+} dt_weights;
+
+/* Caller-allocated device outputs; N = B+1 slots per request, slot 0 = the root (reading A10).
+ * All are fully overwritten for `batch` requests, padding slots included. */
+typedef struct {
+    int32_t *tokens;    /* [batch, N]    tokens[b,0] = root_tokens[b]; slots 1.. in pop order */
+    int32_t *parents;   /* [batch, N]    parent slot; -1 for the root; parents[b,i] < i        */
+    int32_t *depths;    /* [batch, N]    0 for the root, 1..L                                                 */
+    int32_t *positions; /* [batch, N]    root_positions[b] + depth (0-based if root_positions is NULL)        */
+    float *scores;      /* [batch, N]    cumulative corrected log-score g(u); 0 for the root   */
+    uint8_t *mask;      /* [batch, N, N] mask[b,i,j] = 1 iff j == i or j is an ancestor of i*/
+    int32_t *n_nodes;   /* [batch]       valid slots incl. root; slots >= n_nodes are dead leaves:            */
+                        /*               token 0, parent 0, depth 1, score -inf, mask row {root, self}        */
+} dt_outputs;
+
+/*
+ * dt_create: validate shapes, allocate the per-handle device workspace for up to `max_batch`
+ * requests of block depth L, candidate width <= max_M, budget <= max_B and branching factor k
+ * (paper: k = 8), and build the weight-only table P = E W_ih^T  [V, 3g] fp32
+ * (the input half of every GRU step, becomes a row gather).  Synchronises the
+ * device; not capture-safe.  Weights are borrowed until dt_destroy.
+ * Errors: INVALID_ARG for null pointers or !(1 <= k <= max_M <= V), !(1 <= max_B), L < 1,
+ * max_batch < 1, V/d/g/r < 1; UNSUPPORTED beyond DT_MAX_*; ALLOC; CUDA.
+ */
+int dt_create(dt_handle **h, const dt_weights *w, int32_t max_batch, int32_t L,
+              int32_t max_M, int32_t max_B, int32_t k);
+
+/*
+ * dt_build_trees: one tree-build round (Algorithm 1) for `batch` independent
+ * requests.
+ *   marginal_logits  [batch, L, V]  device, handle dtype  -- L_i^base
+ *   backbone_hidden  [batch, L, d]  device, handle dtype  -- H_i; row i-1 pairs with
+ *                                                            parent state S_{i-1}
+ *   root_tokens      [batch] int32  device                -- the verified token x_t
+ *   root_positions   [batch] int32  device or NULL
+ *   M in [k, max_M], B in [1, max_B], temperature >= 0 finite (0 means T_eff = 1, reading A7)
+ * Asynchronous and capture-safe: only enqueues work on `stream` (a cudaStream_t), never
+ * allocates, never synchronises, takes no data-dependent host branch -- the caller may capture
+ * the whole round into one CUDA graph.  One handle serves one stream at a time.
+ * Input values are assumed non-NaN (-inf logits are allowed and sort last).
+ */
+int dt_build_trees(dt_handle *h, const void *marginal_logits, const void *backbone_hidden,
+                   const int32_t *root_tokens, const int32_t *root_positions, int32_t batch,
+                   int32_t M, int32_t B, float temperature, const dt_outputs *out, void *stream);
+
+/*
+ * dt_select_topm: step 1 of Algorithm 1 alone: for each of `rows` rows of
+ * `logits` [rows, V] (device, handle dtype) write the token ids and values of the M largest
+ * entries, ordered (value desc, token id asc) with -0 == +0, to cand_id [rows, M] int32 and
+ * cand_val [rows, M] float (device).  rows <= max_batch * L.  Asynchronous, capture-safe.
+ */
+int dt_select_topm(dt_handle *h, const void *logits, int32_t rows, int32_t M,
+                   int32_t *cand_id, float *cand_val, void *stream);
+
+/*
+ * dt_build_trees_host: the same round with HOST buffers (pinned or pageable): copies the inputs
+ * host->device, runs dt_build_trees, copies the outputs device->host and synchronises `stream`.
+ * `out` members are HOST pointers here.  Uses staging buffers owned by the handle.
+ * Not capture-safe (it synchronises).
+ */
+int dt_build_trees_host(dt_handle *h, const void *marginal_logits_host, const void *backbone_hidden_host,
+                        const int32_t *root_tokens_host, const int32_t *root_positions_host,
+                        int32_t batch, int32_t M, int32_t B, float temperature,
+                        const dt_outputs *out_host, void *stream);
+
+/* dt_set_option: tuning knobs for experiments (e.g. "select_chunks"); unknown name -> INVALID_ARG. */
+int dt_set_option(dt_handle *h, const char *name, int64_t value);
+
+/* dt_kernel_launches: number of kernels the last dt_build_trees / dt_select_topm call enqueued. */
+int64_t dt_kernel_launches(const dt_handle *h);
+
+int dt_destroy(dt_handle *h);                 /* frees the workspace; h may be NULL           */
+const char *dt_error_string(int code);        /* static string                                */
+int dt_version(void);                         /* ABI version, currently 1                     */
+size_t dt_workspace_bytes(const dt_handle *h);/* device bytes owned by the handle (incl. P)   */
+int dt_last_cuda_error(const dt_handle *h);   /* cudaError_t of the last DT_ERR_CUDA          */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DOMINOTREE_H */

@@ -1,0 +1,322 @@
+// dt_api.cu -- host side of the C-ABI in include/dominotree.h: handle, validation, workspace,
+// kernel launches.  Every launch goes to the caller's stream; dt_build_trees and dt_select_topm
+// neither allocate nor synchronise, so a round can be captured into one CUDA graph.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <new>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "../../include/dominotree.h"
+#include "dt_expand.cuh"
+#include "dt_precompute.cuh"
+#include "dt_select.cuh"
+
+using namespace dt;
+
+struct dt_handle {
+    dt_weights w;
+    int max_batch, L, max_M, max_B, k;
+    int heap_cap;
+    size_t esize;
+    // device workspace
+    float *P;                       // [V, 3g]
+    char *ws;                       // everything else, carved below
+    size_t ws_bytes, p_bytes;
+    int32_t *cand_id; float *cand_val;
+    unsigned long long *sel_part; unsigned int *sel_counter, *sel_tau;
+    float *C, *states, *heap_g; unsigned long long *heap_tp; int32_t *heap_cnt;
+    // host-call staging (lazy)
+    char *stage; size_t stage_bytes;
+    // options / bookkeeping
+    int64_t opt_select_chunks;
+    int64_t launches;
+    int last_cuda;
+    int num_sms;
+};
+
+#define DT_CUDA(h, call)                                                   \
+    do {                                                                   \
+        cudaError_t e__ = (call);                                          \
+        if (e__ != cudaSuccess) { if (h) (h)->last_cuda = (int)e__; return DT_ERR_CUDA; } \
+    } while (0)
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+extern "C" const char *dt_error_string(int code) {
+    switch (code) {
+        case DT_OK: return "ok";
+        case DT_ERR_INVALID_ARG: return "invalid argument";
+        case DT_ERR_UNSUPPORTED: return "unsupported shape (beyond compiled limits)";
+        case DT_ERR_CUDA: return "CUDA runtime error";
+        case DT_ERR_ALLOC: return "allocation failed";
+        default: return "unknown error";
+    }
+}
+extern "C" int dt_version(void) { return 1; }
+extern "C" size_t dt_workspace_bytes(const dt_handle *h) { return h ? h->ws_bytes + h->p_bytes + h->stage_bytes : 0; }
+extern "C" int dt_last_cuda_error(const dt_handle *h) { return h ? h->last_cuda : 0; }
+extern "C" int64_t dt_kernel_launches(const dt_handle *h) { return h ? h->launches : 0; }
+
+extern "C" int dt_set_option(dt_handle *h, const char *name, int64_t value) {
+    if (!h || !name) return DT_ERR_INVALID_ARG;
+    if (!strcmp(name, "select_chunks")) {
+        if (value < 0 || value > kSelMaxChunks) return DT_ERR_INVALID_ARG;
+        h->opt_select_chunks = value;
+        return DT_OK;
+    }
+    return DT_ERR_INVALID_ARG;
+}
+
+template <typename T>
+static int launch_gemm_nt(dt_handle *h, const void *A, long long lda, const void *Bm, long long ldb,
+                          float *out, long long ldo, int Mr, int Nc, int K, cudaStream_t st) {
+    dim3 grid((Nc + kGemmBN - 1) / kGemmBN, (Mr + kGemmBM - 1) / kGemmBM);
+    gemm_nt_kernel<T><<<grid, 256, 0, st>>>(reinterpret_cast<const T *>(A), lda, reinterpret_cast<const T *>(Bm), ldb,
+                                            out, ldo, Mr, Nc, K);
+    h->launches++;
+    DT_CUDA(h, cudaGetLastError());
+    return DT_OK;
+}
+
+extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch, int32_t L,
+                         int32_t max_M, int32_t max_B, int32_t k) {
+    if (!out || !w) return DT_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!w->embed || !w->gru_w_ih || !w->gru_w_hh || !w->corr_w1 || !w->corr_w2) return DT_ERR_INVALID_ARG;
+    if (w->V < 1 || w->d < 1 || w->g < 1 || w->r < 1) return DT_ERR_INVALID_ARG;
+    if (w->dtype != DT_BF16 && w->dtype != DT_F32) return DT_ERR_INVALID_ARG;
+    if (max_batch < 1 || L < 1 || max_B < 1 || k < 1 || max_M < k || max_M > w->V) return DT_ERR_INVALID_ARG;
+    if (max_M > DT_MAX_M || max_B > DT_MAX_B || k > DT_MAX_K || L > DT_MAX_L) return DT_ERR_UNSUPPORTED;
+
+    dt_handle *h = new (std::nothrow) dt_handle();
+    if (!h) return DT_ERR_ALLOC;
+    memset(h, 0, sizeof(*h));
+    h->w = *w;
+    h->max_batch = max_batch; h->L = L; h->max_M = max_M; h->max_B = max_B; h->k = k;
+    h->heap_cap = max_B * k + k;
+    h->esize = (w->dtype == DT_BF16) ? 2 : 4;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        delete h; return DT_ERR_CUDA;
+    }
+
+    const size_t rows = (size_t)max_batch * L, N = (size_t)max_B + 1;
+    size_t off = 0;
+    auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    const size_t o_cid = carve(rows * max_M * 4), o_cval = carve(rows * max_M * 4);
+    const size_t o_part = carve(rows * kSelMaxChunks * (size_t)max_M * 8);
+    const size_t o_cnt = carve(rows * 4), o_tau = carve(rows * 4);
+    const size_t o_C = carve(rows * w->r * 4);
+    const size_t o_states = carve((size_t)max_batch * N * w->g * 4);
+    const size_t o_hg = carve((size_t)max_batch * h->heap_cap * 4);
+    const size_t o_htp = carve((size_t)max_batch * h->heap_cap * 8);
+    const size_t o_hcnt = carve((size_t)max_batch * 4);
+    h->ws_bytes = off;
+    h->p_bytes = (size_t)w->V * 3 * w->g * 4;
+    if (cudaMalloc(&h->ws, h->ws_bytes) != cudaSuccess) { cudaGetLastError(); delete h; return DT_ERR_ALLOC; }
+    if (cudaMalloc(&h->P, h->p_bytes) != cudaSuccess) { cudaGetLastError(); cudaFree(h->ws); delete h; return DT_ERR_ALLOC; }
+    h->cand_id = (int32_t *)(h->ws + o_cid); h->cand_val = (float *)(h->ws + o_cval);
+    h->sel_part = (unsigned long long *)(h->ws + o_part);
+    h->sel_counter = (unsigned int *)(h->ws + o_cnt); h->sel_tau = (unsigned int *)(h->ws + o_tau);
+    h->C = (float *)(h->ws + o_C); h->states = (float *)(h->ws + o_states);
+    h->heap_g = (float *)(h->ws + o_hg); h->heap_tp = (unsigned long long *)(h->ws + o_htp);
+    h->heap_cnt = (int32_t *)(h->ws + o_hcnt);
+
+    int rc = DT_OK;
+    if (cudaMemset(h->ws, 0, h->ws_bytes) != cudaSuccess) rc = DT_ERR_CUDA;
+    {   // dynamic shared memory of expand_kernel at the handle's maxima
+        const size_t dsm = (size_t)(w->g + w->r + max_M) * 4 + (size_t)max_M * 4;
+        if (dsm > 200 * 1024) rc = DT_ERR_UNSUPPORTED;
+        else if (dsm > 48 * 1024) {
+            cudaError_t e = (w->dtype == DT_BF16)
+                ? cudaFuncSetAttribute(expand_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm)
+                : cudaFuncSetAttribute(expand_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm);
+            if (e != cudaSuccess) rc = DT_ERR_CUDA;
+        }
+    }
+    // P = E W_ih^T  (weight-only table)
+    if (rc == DT_OK) {
+        if (w->dtype == DT_BF16)
+            rc = launch_gemm_nt<__nv_bfloat16>(h, w->embed, w->d, w->gru_w_ih, w->d, h->P, 3LL * w->g, w->V, 3 * w->g, w->d, 0);
+        else
+            rc = launch_gemm_nt<float>(h, w->embed, w->d, w->gru_w_ih, w->d, h->P, 3LL * w->g, w->V, 3 * w->g, w->d, 0);
+    }
+    if (rc == DT_OK && cudaDeviceSynchronize() != cudaSuccess) { h->last_cuda = (int)cudaGetLastError(); rc = DT_ERR_CUDA; }
+    if (rc != DT_OK) { cudaFree(h->ws); cudaFree(h->P); delete h; return rc; }
+    h->launches = 0;
+    *out = h;
+    return DT_OK;
+}
+
+extern "C" int dt_destroy(dt_handle *h) {
+    if (!h) return DT_OK;
+    cudaFree(h->ws); cudaFree(h->P);
+    if (h->stage) cudaFree(h->stage);
+    delete h;
+    return DT_OK;
+}
+
+static int pick_chunks(const dt_handle *h, int rows, int M) {
+    int smax = kSelCap / M;
+    if (smax > kSelMaxChunks) smax = kSelMaxChunks;
+    if (smax < 1) smax = 1;
+    int S;
+    if (h->opt_select_chunks > 0) S = (int)h->opt_select_chunks;
+    else {
+        const int target = 3 * h->num_sms;          // resident CTAs wanted
+        S = (target + rows - 1) / rows;
+    }
+    if (S > smax) S = smax;
+    if (S < 1) S = 1;
+    return S;
+}
+
+static int launch_select(dt_handle *h, const void *logits, int rows, int M, int32_t *cand_id, float *cand_val,
+                         cudaStream_t st) {
+    const int V = h->w.V;
+    const int kvec = (h->w.dtype == DT_BF16) ? 8 : 4;
+    SelectParams p;
+    p.logits = logits; p.rows = rows; p.V = V; p.M = M;
+    p.row_vecs = (V + kvec - 1) / kvec;
+    int S = pick_chunks(h, rows, M);
+    if (S > p.row_vecs) S = p.row_vecs;
+    p.S = S;
+    p.chunk_vecs = (p.row_vecs + S - 1) / S;
+    p.cand_id = cand_id; p.cand_val = cand_val;
+    p.part = h->sel_part; p.row_counter = h->sel_counter; p.row_tau = h->sel_tau;
+    const bool aligned = (V % kvec == 0) && ((reinterpret_cast<uintptr_t>(logits) & 15u) == 0);
+    dim3 grid(S, rows);
+    if (h->w.dtype == DT_BF16) {
+        if (aligned) select_topm_kernel<__nv_bfloat16, true><<<grid, kSelThreads, 0, st>>>(p);
+        else select_topm_kernel<__nv_bfloat16, false><<<grid, kSelThreads, 0, st>>>(p);
+    } else {
+        if (aligned) select_topm_kernel<float, true><<<grid, kSelThreads, 0, st>>>(p);
+        else select_topm_kernel<float, false><<<grid, kSelThreads, 0, st>>>(p);
+    }
+    h->launches++;
+    DT_CUDA(h, cudaGetLastError());
+    return DT_OK;
+}
+
+extern "C" int dt_select_topm(dt_handle *h, const void *logits, int32_t rows, int32_t M,
+                              int32_t *cand_id, float *cand_val, void *stream) {
+    if (!h || !logits || !cand_id || !cand_val) return DT_ERR_INVALID_ARG;
+    if (rows < 0 || rows > h->max_batch * h->L || M < 1 || M > h->max_M) return DT_ERR_INVALID_ARG;
+    h->launches = 0;
+    if (rows == 0) return DT_OK;
+    return launch_select(h, logits, rows, M, cand_id, cand_val, (cudaStream_t)stream);
+}
+
+template <typename T>
+static int launch_expansion(dt_handle *h, ExpandParams &p, cudaStream_t st) {
+    const int g = p.g;
+    init_round_kernel<<<p.batch, 32, 0, st>>>(p);
+    root_state_kernel<<<p.batch, 256, 0, st>>>(h->P, p.root_tokens, g, p.V, p.states, (long long)p.N * g);
+    h->launches += 2;
+    const size_t dsm = (size_t)(g + p.r + p.M) * 4 + (size_t)p.M * 4;   // opt-in above 48 KB done in dt_create
+    const int gru_grid = (g + kGruUnitsPerCta - 1) / kGruUnitsPerCta;
+    for (int t = 0; t < p.B; ++t) {
+        if (t > 0) { gru_step_kernel<T><<<gru_grid, kExpThreads, 0, st>>>(p, t); h->launches++; }
+        expand_kernel<T><<<p.batch, kExpThreads, dsm, st>>>(p, t);
+        h->launches++;
+    }
+    emit_kernel<<<p.batch, kExpThreads, 0, st>>>(p);
+    h->launches++;
+    DT_CUDA(h, cudaGetLastError());
+    return DT_OK;
+}
+
+extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const void *backbone_hidden,
+                              const int32_t *root_tokens, const int32_t *root_positions, int32_t batch,
+                              int32_t M, int32_t B, float temperature, const dt_outputs *out, void *stream) {
+    if (!h || !marginal_logits || !backbone_hidden || !root_tokens || !out) return DT_ERR_INVALID_ARG;
+    if (!out->tokens || !out->parents || !out->depths || !out->positions || !out->scores || !out->mask || !out->n_nodes)
+        return DT_ERR_INVALID_ARG;
+    if (batch < 0 || batch > h->max_batch) return DT_ERR_INVALID_ARG;
+    if (M < h->k || M > h->max_M || B < 1 || B > h->max_B) return DT_ERR_INVALID_ARG;
+    if (!(temperature >= 0.0f) || isinf(temperature)) return DT_ERR_INVALID_ARG;
+    h->launches = 0;
+    if (batch == 0) return DT_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    const dt_weights &w = h->w;
+    const int rows = batch * h->L;
+
+    int rc = launch_select(h, marginal_logits, rows, M, h->cand_id, h->cand_val, st);
+    if (rc) return rc;
+    // C = H W1[:, 0:d]^T   (Fact B PAPER.md:83-89)
+    if (w.dtype == DT_BF16)
+        rc = launch_gemm_nt<__nv_bfloat16>(h, backbone_hidden, w.d, w.corr_w1, (long long)w.d + w.g, h->C, w.r, rows, w.r, w.d, st);
+    else
+        rc = launch_gemm_nt<float>(h, backbone_hidden, w.d, w.corr_w1, (long long)w.d + w.g, h->C, w.r, rows, w.r, w.d, st);
+    if (rc) return rc;
+
+    ExpandParams p;
+    memset(&p, 0, sizeof(p));
+    p.w_hh = w.gru_w_hh; p.w1 = w.corr_w1; p.w2 = w.corr_w2; p.P = h->P;
+    p.V = w.V; p.d = w.d; p.g = w.g; p.r = w.r;
+    p.batch = batch; p.L = h->L; p.M = M; p.B = B; p.k = h->k; p.N = B + 1;
+    p.T_eff = (temperature == 0.0f) ? 1.0f : temperature;          // reading A7
+    p.C = h->C; p.cand_id = h->cand_id; p.cand_val = h->cand_val;
+    p.states = h->states; p.heap_g = h->heap_g; p.heap_tp = h->heap_tp; p.heap_cnt = h->heap_cnt;
+    p.heap_cap = h->heap_cap;
+    p.tokens = out->tokens; p.parents = out->parents; p.depths = out->depths; p.positions = out->positions;
+    p.n_nodes = out->n_nodes; p.scores = out->scores; p.mask = out->mask;
+    p.root_tokens = root_tokens; p.root_positions = root_positions;
+    if (w.dtype == DT_BF16) return launch_expansion<__nv_bfloat16>(h, p, st);
+    return launch_expansion<float>(h, p, st);
+}
+
+extern "C" int dt_build_trees_host(dt_handle *h, const void *logits_h, const void *hidden_h,
+                                   const int32_t *roots_h, const int32_t *rpos_h, int32_t batch,
+                                   int32_t M, int32_t B, float temperature, const dt_outputs *oh, void *stream) {
+    if (!h || !logits_h || !hidden_h || !roots_h || !oh) return DT_ERR_INVALID_ARG;
+    if (!oh->tokens || !oh->parents || !oh->depths || !oh->positions || !oh->scores || !oh->mask || !oh->n_nodes)
+        return DT_ERR_INVALID_ARG;
+    if (batch < 0 || batch > h->max_batch || B < 1 || B > h->max_B) return DT_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t N = (size_t)h->max_B + 1;
+    if (!h->stage) {                            // sized for the handle's maxima, allocated once
+        size_t off = 0;
+        auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+        carve((size_t)h->max_batch * h->L * h->w.V * h->esize);
+        carve((size_t)h->max_batch * h->L * h->w.d * h->esize);
+        carve((size_t)h->max_batch * 4); carve((size_t)h->max_batch * 4);
+        carve((size_t)h->max_batch * N * 4 * 5); carve((size_t)h->max_batch * N * N); carve((size_t)h->max_batch * 4);
+        if (cudaMalloc(&h->stage, off) != cudaSuccess) { cudaGetLastError(); h->stage = nullptr; return DT_ERR_ALLOC; }
+        h->stage_bytes = off;
+    }
+    size_t off = 0;
+    auto carve = [&](size_t bytes) { char *q = h->stage + off; off = align_up(off + bytes, 256); return q; };
+    const size_t lb = (size_t)batch * h->L * h->w.V * h->esize, hb = (size_t)batch * h->L * h->w.d * h->esize;
+    char *d_logits = carve((size_t)h->max_batch * h->L * h->w.V * h->esize);
+    char *d_hidden = carve((size_t)h->max_batch * h->L * h->w.d * h->esize);
+    int32_t *d_roots = (int32_t *)carve((size_t)h->max_batch * 4);
+    int32_t *d_rpos = (int32_t *)carve((size_t)h->max_batch * 4);
+    char *d_i32 = carve((size_t)h->max_batch * N * 4 * 5);
+    uint8_t *d_mask = (uint8_t *)carve((size_t)h->max_batch * N * N);
+    int32_t *d_nn = (int32_t *)carve((size_t)h->max_batch * 4);
+    if (batch == 0) return DT_OK;
+    const size_t Nb = (size_t)B + 1, slab = (size_t)batch * Nb * 4;
+    dt_outputs od;
+    od.tokens = (int32_t *)(d_i32); od.parents = (int32_t *)(d_i32 + slab); od.depths = (int32_t *)(d_i32 + 2 * slab);
+    od.positions = (int32_t *)(d_i32 + 3 * slab); od.scores = (float *)(d_i32 + 4 * slab);
+    od.mask = d_mask; od.n_nodes = d_nn;
+    DT_CUDA(h, cudaMemcpyAsync(d_logits, logits_h, lb, cudaMemcpyHostToDevice, st));
+    DT_CUDA(h, cudaMemcpyAsync(d_hidden, hidden_h, hb, cudaMemcpyHostToDevice, st));
+    DT_CUDA(h, cudaMemcpyAsync(d_roots, roots_h, (size_t)batch * 4, cudaMemcpyHostToDevice, st));
+    if (rpos_h) DT_CUDA(h, cudaMemcpyAsync(d_rpos, rpos_h, (size_t)batch * 4, cudaMemcpyHostToDevice, st));
+    int rc = dt_build_trees(h, d_logits, d_hidden, d_roots, rpos_h ? d_rpos : nullptr, batch, M, B, temperature, &od, st);
+    if (rc) return rc;
+    DT_CUDA(h, cudaMemcpyAsync(oh->tokens, od.tokens, slab, cudaMemcpyDeviceToHost, st));
+    DT_CUDA(h, cudaMemcpyAsync(oh->parents, od.parents, slab, cudaMemcpyDeviceToHost, st));
+    DT_CUDA(h, cudaMemcpyAsync(oh->depths, od.depths, slab, cudaMemcpyDeviceToHost, st));
+    DT_CUDA(h, cudaMemcpyAsync(oh->positions, od.positions, slab, cudaMemcpyDeviceToHost, st));
+    DT_CUDA(h, cudaMemcpyAsync(oh->scores, od.scores, slab, cudaMemcpyDeviceToHost, st));
+    DT_CUDA(h, cudaMemcpyAsync(oh->mask, od.mask, (size_t)batch * Nb * Nb, cudaMemcpyDeviceToHost, st));
+    DT_CUDA(h, cudaMemcpyAsync(oh->n_nodes, od.n_nodes, (size_t)batch * 4, cudaMemcpyDeviceToHost, st));
+    DT_CUDA(h, cudaStreamSynchronize(st));
+    return DT_OK;
+}

@@ -1,0 +1,74 @@
+// dt_common.cuh -- shared device helpers for the DominoTree builder kernels (sm_100a).
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace dt {
+
+constexpr int kWarp = 32;
+
+// ---- element type helpers: T is __nv_bfloat16 or float -------------------------------------
+template <typename T> struct ElemTraits;
+template <> struct ElemTraits<__nv_bfloat16> {
+    static constexpr int kVec = 8;              // elements per 16-byte vector
+    static __device__ __forceinline__ float to_f32(__nv_bfloat16 v) { return __bfloat162float(v); }
+};
+template <> struct ElemTraits<float> {
+    static constexpr int kVec = 4;
+    static __device__ __forceinline__ float to_f32(float v) { return v; }
+};
+
+__device__ __forceinline__ float bf16_bits_to_f32(uint32_t hi16) { return __uint_as_float(hi16 << 16); }
+
+// Unpack the 8 bf16 of a uint4 into floats (element 0 = lowest address).
+__device__ __forceinline__ void unpack8(const uint4 &v, float (&f)[8]) {
+    f[0] = __uint_as_float(v.x << 16); f[1] = __uint_as_float(v.x & 0xFFFF0000u);
+    f[2] = __uint_as_float(v.y << 16); f[3] = __uint_as_float(v.y & 0xFFFF0000u);
+    f[4] = __uint_as_float(v.z << 16); f[5] = __uint_as_float(v.z & 0xFFFF0000u);
+    f[6] = __uint_as_float(v.w << 16); f[7] = __uint_as_float(v.w & 0xFFFF0000u);
+}
+
+// Order-preserving map float -> uint32 (larger float <=> larger key), with -0 folded onto +0 so
+// that equal values give equal keys.  NaN is outside the contract (dominotree.h).
+__device__ __forceinline__ uint32_t ord_key(float v) {
+    uint32_t b = __float_as_uint(v);
+    if (b == 0x80000000u) b = 0u;
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__device__ __forceinline__ float ord_key_inv(uint32_t k) {
+    uint32_t b = (k & 0x80000000u) ? (k & 0x7FFFFFFFu) : ~k;
+    return __uint_as_float(b);
+}
+
+// 128-bit streaming global load (read-once data: do not allocate in L1).
+__device__ __forceinline__ uint4 ld_stream_v4(const void *p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+// 128-bit read-only load that may stay in L1/L2 (weights, reused rows).
+__device__ __forceinline__ uint4 ld_ro_v4(const void *p) {
+    return __ldg(reinterpret_cast<const uint4 *>(p));
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+__device__ __forceinline__ float sigmoidf_acc(float x) { return 1.0f / (1.0f + expf(-x)); }
+
+// generic element load -> float
+template <typename T> __device__ __forceinline__ float ldf(const T *p, size_t i) {
+    return ElemTraits<T>::to_f32(p[i]);
+}
+
+}  // namespace dt
