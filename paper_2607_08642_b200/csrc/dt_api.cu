@@ -203,10 +203,11 @@ static int launch_select(dt_handle *h, const void *logits, int rows, int M, int3
 
 extern "C" int dt_select_topm(dt_handle *h, const void *logits, int32_t rows, int32_t M,
                               int32_t *cand_id, float *cand_val, void *stream) {
-    if (!h || !logits || !cand_id || !cand_val) return DT_ERR_INVALID_ARG;
+    if (!h) return DT_ERR_INVALID_ARG;
     if (rows < 0 || rows > h->max_batch * h->L || M < 1 || M > h->max_M) return DT_ERR_INVALID_ARG;
     h->launches = 0;
     if (rows == 0) return DT_OK;
+    if (!logits || !cand_id || !cand_val) return DT_ERR_INVALID_ARG;
     return launch_select(h, logits, rows, M, cand_id, cand_val, (cudaStream_t)stream);
 }
 
@@ -232,14 +233,15 @@ static int launch_expansion(dt_handle *h, ExpandParams &p, cudaStream_t st) {
 extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const void *backbone_hidden,
                               const int32_t *root_tokens, const int32_t *root_positions, int32_t batch,
                               int32_t M, int32_t B, float temperature, const dt_outputs *out, void *stream) {
-    if (!h || !marginal_logits || !backbone_hidden || !root_tokens || !out) return DT_ERR_INVALID_ARG;
-    if (!out->tokens || !out->parents || !out->depths || !out->positions || !out->scores || !out->mask || !out->n_nodes)
-        return DT_ERR_INVALID_ARG;
+    if (!h || !out) return DT_ERR_INVALID_ARG;
     if (batch < 0 || batch > h->max_batch) return DT_ERR_INVALID_ARG;
     if (M < h->k || M > h->max_M || B < 1 || B > h->max_B) return DT_ERR_INVALID_ARG;
     if (!(temperature >= 0.0f) || isinf(temperature)) return DT_ERR_INVALID_ARG;
     h->launches = 0;
-    if (batch == 0) return DT_OK;
+    if (batch == 0) return DT_OK;               // empty batch: nothing to read or write
+    if (!marginal_logits || !backbone_hidden || !root_tokens) return DT_ERR_INVALID_ARG;
+    if (!out->tokens || !out->parents || !out->depths || !out->positions || !out->scores || !out->mask || !out->n_nodes)
+        return DT_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const dt_weights &w = h->w;
     const int rows = batch * h->L;
@@ -272,10 +274,12 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
 extern "C" int dt_build_trees_host(dt_handle *h, const void *logits_h, const void *hidden_h,
                                    const int32_t *roots_h, const int32_t *rpos_h, int32_t batch,
                                    int32_t M, int32_t B, float temperature, const dt_outputs *oh, void *stream) {
-    if (!h || !logits_h || !hidden_h || !roots_h || !oh) return DT_ERR_INVALID_ARG;
+    if (!h || !oh) return DT_ERR_INVALID_ARG;
+    if (batch < 0 || batch > h->max_batch || B < 1 || B > h->max_B) return DT_ERR_INVALID_ARG;
+    if (batch == 0) return DT_OK;
+    if (!logits_h || !hidden_h || !roots_h) return DT_ERR_INVALID_ARG;
     if (!oh->tokens || !oh->parents || !oh->depths || !oh->positions || !oh->scores || !oh->mask || !oh->n_nodes)
         return DT_ERR_INVALID_ARG;
-    if (batch < 0 || batch > h->max_batch || B < 1 || B > h->max_B) return DT_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t N = (size_t)h->max_B + 1;
     if (!h->stage) {                            // sized for the handle's maxima, allocated once
@@ -298,7 +302,6 @@ extern "C" int dt_build_trees_host(dt_handle *h, const void *logits_h, const voi
     char *d_i32 = carve((size_t)h->max_batch * N * 4 * 5);
     uint8_t *d_mask = (uint8_t *)carve((size_t)h->max_batch * N * N);
     int32_t *d_nn = (int32_t *)carve((size_t)h->max_batch * 4);
-    if (batch == 0) return DT_OK;
     const size_t Nb = (size_t)B + 1, slab = (size_t)batch * Nb * 4;
     dt_outputs od;
     od.tokens = (int32_t *)(d_i32); od.parents = (int32_t *)(d_i32 + slab); od.depths = (int32_t *)(d_i32 + 2 * slab);
