@@ -130,6 +130,24 @@ int dt_build_trees_host(dt_handle *h, const void *marginal_logits_host, const vo
 /* dt_set_option: tuning knobs for experiments (e.g. "select_chunks"); unknown name -> INVALID_ARG. */
 int dt_set_option(dt_handle *h, const char *name, int64_t value);
 
+/*
+ * Phase timing (measurement aid, off by default).  dt_phase_timing(h, n_slots) creates n_slots
+ * sets of CUDA events (n_slots = 0 frees them; not capture-safe).  While enabled, every
+ * dt_build_trees call records the boundaries of its phases on `stream` into the slot chosen by
+ * dt_phase_slot -- inside a stream capture as external event-record nodes, so each replay of the
+ * captured graph re-records them.  dt_phase_elapsed_ms returns the device time of one phase of
+ * the last completed round that used `slot` (the caller synchronises first); phases:
+ *   DT_PHASE_SELECT (a1), DT_PHASE_PRECOMPUTE (a3, a4), DT_PHASE_EXPAND (a5-a8), DT_PHASE_EMIT (a9).
+ */
+#define DT_PHASE_SELECT 0
+#define DT_PHASE_PRECOMPUTE 1
+#define DT_PHASE_EXPAND 2
+#define DT_PHASE_EMIT 3
+#define DT_NUM_PHASES 4
+int dt_phase_timing(dt_handle *h, int32_t n_slots);
+int dt_phase_slot(dt_handle *h, int32_t slot);
+int dt_phase_elapsed_ms(dt_handle *h, int32_t slot, int32_t phase, float *ms);
+
 /* dt_kernel_launches: number of kernels the last dt_build_trees / dt_select_topm call enqueued. */
 int64_t dt_kernel_launches(const dt_handle *h);
 

@@ -19,7 +19,8 @@ LIB_PATH = os.path.join(_PKG, "libdominotree.so")
 DT_BF16, DT_F32 = 0, 1
 EXPORTS = ("dt_create", "dt_build_trees", "dt_select_topm", "dt_build_trees_host", "dt_set_option",
            "dt_kernel_launches", "dt_destroy", "dt_error_string", "dt_version", "dt_workspace_bytes",
-           "dt_last_cuda_error")
+           "dt_last_cuda_error", "dt_phase_timing", "dt_phase_slot", "dt_phase_elapsed_ms")
+PHASES = ("select", "precompute", "expand", "emit")
 
 
 class DominoTreeError(RuntimeError):
@@ -75,6 +76,12 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.dt_workspace_bytes.restype = ctypes.c_size_t
     lib.dt_last_cuda_error.argtypes = [vp]
     lib.dt_last_cuda_error.restype = ctypes.c_int
+    lib.dt_phase_timing.argtypes = [vp, i32]
+    lib.dt_phase_timing.restype = ctypes.c_int
+    lib.dt_phase_slot.argtypes = [vp, i32]
+    lib.dt_phase_slot.restype = ctypes.c_int
+    lib.dt_phase_elapsed_ms.argtypes = [vp, i32, i32, ctypes.POINTER(f32)]
+    lib.dt_phase_elapsed_ms.restype = ctypes.c_int
     if path is None:
         _lib = lib
     return lib
@@ -215,6 +222,23 @@ class DominoTreeBuilder:
     # -- misc -------------------------------------------------------------------------------------
     def set_option(self, name: str, value: int):
         _check(self.lib, self.lib.dt_set_option(self._h, name.encode(), int(value)), f"dt_set_option({name})")
+
+    def phase_timing(self, n_slots: int):
+        """dt_phase_timing: create (or with 0 free) n_slots sets of phase-boundary CUDA events."""
+        _check(self.lib, self.lib.dt_phase_timing(self._h, int(n_slots)), "dt_phase_timing", self._h)
+
+    def phase_slot(self, slot: int):
+        _check(self.lib, self.lib.dt_phase_slot(self._h, int(slot)), "dt_phase_slot", self._h)
+
+    def phase_ms(self, slot: int) -> Dict[str, float]:
+        """Device milliseconds of each phase of the last completed round recorded into `slot`."""
+        out = {}
+        for i, name in enumerate(PHASES):
+            ms = ctypes.c_float()
+            _check(self.lib, self.lib.dt_phase_elapsed_ms(self._h, int(slot), i, ctypes.byref(ms)),
+                   "dt_phase_elapsed_ms", self._h)
+            out[name] = float(ms.value)
+        return out
 
     @property
     def kernel_launches(self) -> int:

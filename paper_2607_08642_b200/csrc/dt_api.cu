@@ -31,6 +31,8 @@ struct dt_handle {
     char *stage; size_t stage_bytes;
     // options / bookkeeping
     int64_t opt_select_chunks;
+    // phase timing (optional): n_slots x kPhaseEvents events, recorded on the caller's stream
+    cudaEvent_t *ph_ev; int ph_slots, ph_slot;
     int64_t launches;
     int last_cuda;
     int num_sms;
@@ -43,6 +45,48 @@ struct dt_handle {
     } while (0)
 
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// Phase boundaries of one round: [0] start, [1] after select (a1), [2] after precompute (a3, a4),
+// [3] after the expansion loop (a5-a8), [4] after the emitter (a9).
+constexpr int kPhaseEvents = DT_NUM_PHASES + 1;
+
+// Record boundary `i` of the selected slot.  Inside a stream capture the record becomes an external
+// event-record node, so every replay of the graph re-records it.
+static int phase_mark(dt_handle *h, int i, cudaStream_t st) {
+    if (!h->ph_ev) return DT_OK;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    DT_CUDA(h, cudaStreamIsCapturing(st, &cs));
+    cudaEvent_t ev = h->ph_ev[(size_t)h->ph_slot * kPhaseEvents + i];
+    DT_CUDA(h, cudaEventRecordWithFlags(ev, st, cs == cudaStreamCaptureStatusActive ? cudaEventRecordExternal
+                                                                                   : cudaEventRecordDefault));
+    return DT_OK;
+}
+
+extern "C" int dt_phase_timing(dt_handle *h, int32_t n_slots) {
+    if (!h || n_slots < 0 || n_slots > 4096) return DT_ERR_INVALID_ARG;
+    if (h->ph_ev) {
+        for (int i = 0; i < h->ph_slots * kPhaseEvents; ++i) cudaEventDestroy(h->ph_ev[i]);
+        free(h->ph_ev); h->ph_ev = nullptr; h->ph_slots = 0; h->ph_slot = 0;
+    }
+    if (n_slots == 0) return DT_OK;
+    h->ph_ev = (cudaEvent_t *)calloc((size_t)n_slots * kPhaseEvents, sizeof(cudaEvent_t));
+    if (!h->ph_ev) return DT_ERR_ALLOC;
+    for (int i = 0; i < n_slots * kPhaseEvents; ++i) DT_CUDA(h, cudaEventCreate(&h->ph_ev[i]));
+    h->ph_slots = n_slots;
+    return DT_OK;
+}
+extern "C" int dt_phase_slot(dt_handle *h, int32_t slot) {
+    if (!h || !h->ph_ev || slot < 0 || slot >= h->ph_slots) return DT_ERR_INVALID_ARG;
+    h->ph_slot = slot;
+    return DT_OK;
+}
+extern "C" int dt_phase_elapsed_ms(dt_handle *h, int32_t slot, int32_t phase, float *ms) {
+    if (!h || !h->ph_ev || !ms || slot < 0 || slot >= h->ph_slots || phase < 0 || phase >= DT_NUM_PHASES)
+        return DT_ERR_INVALID_ARG;
+    const cudaEvent_t *e = h->ph_ev + (size_t)slot * kPhaseEvents;
+    DT_CUDA(h, cudaEventElapsedTime(ms, e[phase], e[phase + 1]));
+    return DT_OK;
+}
 
 extern "C" const char *dt_error_string(int code) {
     switch (code) {
@@ -153,6 +197,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
 
 extern "C" int dt_destroy(dt_handle *h) {
     if (!h) return DT_OK;
+    dt_phase_timing(h, 0);
     cudaFree(h->ws); cudaFree(h->P);
     if (h->stage) cudaFree(h->stage);
     delete h;
@@ -217,6 +262,8 @@ static int launch_expansion(dt_handle *h, ExpandParams &p, cudaStream_t st) {
     init_round_kernel<<<p.batch, 32, 0, st>>>(p);
     root_state_kernel<<<p.batch, 256, 0, st>>>(h->P, p.root_tokens, g, p.V, p.states, (long long)p.N * g);
     h->launches += 2;
+    int rc = phase_mark(h, 2, st);
+    if (rc) return rc;
     const size_t dsm = (size_t)(g + p.r + p.M) * 4 + (size_t)p.M * 4;   // opt-in above 48 KB done in dt_create
     const int gru_grid = (g + kGruUnitsPerCta - 1) / kGruUnitsPerCta;
     for (int t = 0; t < p.B; ++t) {
@@ -224,10 +271,11 @@ static int launch_expansion(dt_handle *h, ExpandParams &p, cudaStream_t st) {
         expand_kernel<T><<<p.batch, kExpThreads, dsm, st>>>(p, t);
         h->launches++;
     }
+    if ((rc = phase_mark(h, 3, st))) return rc;
     emit_kernel<<<p.batch, kExpThreads, 0, st>>>(p);
     h->launches++;
     DT_CUDA(h, cudaGetLastError());
-    return DT_OK;
+    return phase_mark(h, 4, st);
 }
 
 extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const void *backbone_hidden,
@@ -246,8 +294,11 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
     const dt_weights &w = h->w;
     const int rows = batch * h->L;
 
-    int rc = launch_select(h, marginal_logits, rows, M, h->cand_id, h->cand_val, st);
+    int rc = phase_mark(h, 0, st);
     if (rc) return rc;
+    rc = launch_select(h, marginal_logits, rows, M, h->cand_id, h->cand_val, st);
+    if (rc) return rc;
+    if ((rc = phase_mark(h, 1, st))) return rc;
     // C = H W1[:, 0:d]^T   (Fact B PAPER.md:83-89)
     if (w.dtype == DT_BF16)
         rc = launch_gemm_nt<__nv_bfloat16>(h, backbone_hidden, w.d, w.corr_w1, (long long)w.d + w.g, h->C, w.r, rows, w.r, w.d, st);
