@@ -10,6 +10,7 @@
 
 #include "../../include/dominotree.h"
 #include "dt_expand.cuh"
+#include "dt_fused.cuh"
 #include "dt_precompute.cuh"
 #include "dt_select.cuh"
 
@@ -27,6 +28,10 @@ struct dt_handle {
     int32_t *cand_id; float *cand_val;
     unsigned long long *sel_part; unsigned int *sel_counter, *sel_tau;
     float *C, *states, *heap_g; unsigned long long *heap_tp; int32_t *heap_cnt;
+    // fused persistent expansion (bf16): state copies, split-K partials, hand-over words
+    __nv_bfloat16 *s_hi, *s_lo; float *partial; int2 *desc; unsigned int *sync;
+    int fused_ok, max_smem_optin;
+    int64_t opt_expand_path;        // 0 auto, 1 per-step kernels, 2 fused upc=8, 3 fused upc=16
     // host-call staging (lazy)
     char *stage; size_t stage_bytes;
     // options / bookkeeping
@@ -105,6 +110,11 @@ extern "C" int64_t dt_kernel_launches(const dt_handle *h) { return h ? h->launch
 
 extern "C" int dt_set_option(dt_handle *h, const char *name, int64_t value) {
     if (!h || !name) return DT_ERR_INVALID_ARG;
+    if (!strcmp(name, "expand_path")) {
+        if (value < 0 || value > 3) return DT_ERR_INVALID_ARG;
+        h->opt_expand_path = value;
+        return DT_OK;
+    }
     if (!strcmp(name, "select_chunks")) {
         if (value < 0 || value > kSelMaxChunks) return DT_ERR_INVALID_ARG;
         h->opt_select_chunks = value;
@@ -147,14 +157,26 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         delete h; return DT_ERR_CUDA;
     }
 
-    const size_t rows = (size_t)max_batch * L, N = (size_t)max_B + 1;
+    const size_t rows = (size_t)max_batch * L;
     size_t off = 0;
     auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
     const size_t o_cid = carve(rows * max_M * 4), o_cval = carve(rows * max_M * 4);
     const size_t o_part = carve(rows * kSelMaxChunks * (size_t)max_M * 8);
     const size_t o_cnt = carve(rows * 4), o_tau = carve(rows * 4);
     const size_t o_C = carve(rows * w->r * 4);
-    const size_t o_states = carve((size_t)max_batch * N * w->g * 4);
+    const size_t slots = (size_t)max_B + 2;                  // fused layout: slot 0 = zeros, node t at t+1
+    const size_t o_states = carve((size_t)max_batch * slots * w->g * 4);
+    // fused path eligibility (shape part; the grid / smem fit is checked per call)
+    h->fused_ok = (w->dtype == DT_BF16) && (w->g % 32 == 0) && (w->r % 8 == 0) && max_M <= 256 &&
+                  ((reinterpret_cast<uintptr_t>(w->gru_w_hh) & 15u) == 0) && ((reinterpret_cast<uintptr_t>(w->corr_w2) & 15u) == 0);
+    size_t o_shi = 0, o_slo = 0, o_partial = 0, o_desc = 0, o_sync = 0;
+    if (h->fused_ok) {
+        o_shi = carve((size_t)max_batch * slots * w->g * 2);
+        o_slo = carve((size_t)max_batch * slots * w->g * 2);
+        o_partial = carve((size_t)(w->g / 8) * max_batch * w->r * 4);
+        o_desc = carve((size_t)2 * max_batch * sizeof(int2));
+        o_sync = carve(64 * 4);
+    }
     const size_t o_hg = carve((size_t)max_batch * h->heap_cap * 4);
     const size_t o_htp = carve((size_t)max_batch * h->heap_cap * 8);
     const size_t o_hcnt = carve((size_t)max_batch * 4);
@@ -168,6 +190,18 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     h->C = (float *)(h->ws + o_C); h->states = (float *)(h->ws + o_states);
     h->heap_g = (float *)(h->ws + o_hg); h->heap_tp = (unsigned long long *)(h->ws + o_htp);
     h->heap_cnt = (int32_t *)(h->ws + o_hcnt);
+    if (h->fused_ok) {
+        h->s_hi = (__nv_bfloat16 *)(h->ws + o_shi); h->s_lo = (__nv_bfloat16 *)(h->ws + o_slo);
+        h->partial = (float *)(h->ws + o_partial); h->desc = (int2 *)(h->ws + o_desc);
+        h->sync = (unsigned int *)(h->ws + o_sync);
+        bool ok = cudaDeviceGetAttribute(&h->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess;
+        h->max_smem_optin -= 1024;                  // room for the kernels' static shared memory
+        if (!ok ||
+            cudaFuncSetAttribute(fused_expand_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->max_smem_optin) != cudaSuccess ||
+            cudaFuncSetAttribute(fused_expand_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->max_smem_optin) != cudaSuccess) {
+            cudaGetLastError(); h->fused_ok = 0;
+        }
+    }
 
     int rc = DT_OK;
     if (cudaMemset(h->ws, 0, h->ws_bytes) != cudaSuccess) rc = DT_ERR_CUDA;
@@ -256,6 +290,48 @@ extern "C" int dt_select_topm(dt_handle *h, const void *logits, int32_t rows, in
     return launch_select(h, logits, rows, M, cand_id, cand_val, (cudaStream_t)stream);
 }
 
+// Fused persistent expansion (dt_fused.cuh).  Returns 1 if the shape does not fit (caller falls back
+// to the per-step kernels), DT_OK after enqueueing, or a negative error.
+static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st) {
+    if (!h->fused_ok || h->opt_expand_path == 1) return 1;
+    int upc = 0;
+    for (int cand : {16, 8}) {      // batch-independent preference => batch-invariant results
+        if (h->opt_expand_path == 2 && cand != 8) continue;
+        if (h->opt_expand_path == 3 && cand != 16) continue;
+        if (p.g % cand) continue;
+        if (p.g / cand + p.batch > h->num_sms) continue;
+        const int mt = (3 * cand + 15) / 16;
+        if (fused_gru_smem(p.g, p.r, cand, mt) > (size_t)h->max_smem_optin) continue;
+        upc = cand; break;
+    }
+    if (!upc) return 1;
+    FusedParams f;
+    memset(&f, 0, sizeof(f));
+    f.e = p;
+    f.upc = upc; f.n_gru = p.g / upc; f.m_tiles = (3 * upc + 15) / 16;
+    f.slot_stride = h->max_B + 2;
+    f.s_hi = h->s_hi; f.s_lo = h->s_lo; f.s32 = h->states; f.partial = h->partial; f.desc = h->desc; f.sync = h->sync;
+    f.w2_smem = 1;
+    size_t rs = fused_req_smem(p.r, p.M, p.N, p.heap_cap, 1);
+    if (rs > (size_t)h->max_smem_optin) { f.w2_smem = 0; rs = fused_req_smem(p.r, p.M, p.N, p.heap_cap, 0); }
+    if (rs > (size_t)h->max_smem_optin) return 1;
+    const size_t gs = fused_gru_smem(p.g, p.r, upc, f.m_tiles);
+    const size_t dsm = gs > rs ? gs : rs;
+    fused_init_kernel<<<(p.batch + 127) / 128, 128, 0, st>>>(f);
+    h->launches++;
+    int rc = phase_mark(h, 2, st);
+    if (rc) return rc;
+    void *args[] = {&f};
+    const dim3 grid(f.n_gru + p.batch), block(kFusThreads);
+    cudaError_t e = (upc == 8)
+        ? cudaLaunchCooperativeKernel((const void *)fused_expand_kernel<8>, grid, block, args, dsm, st)
+        : cudaLaunchCooperativeKernel((const void *)fused_expand_kernel<16>, grid, block, args, dsm, st);
+    h->launches++;
+    DT_CUDA(h, e);
+    if ((rc = phase_mark(h, 3, st))) return rc;
+    return phase_mark(h, 4, st);
+}
+
 template <typename T>
 static int launch_expansion(dt_handle *h, ExpandParams &p, cudaStream_t st) {
     const int g = p.g;
@@ -318,7 +394,11 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
     p.tokens = out->tokens; p.parents = out->parents; p.depths = out->depths; p.positions = out->positions;
     p.n_nodes = out->n_nodes; p.scores = out->scores; p.mask = out->mask;
     p.root_tokens = root_tokens; p.root_positions = root_positions;
-    if (w.dtype == DT_BF16) return launch_expansion<__nv_bfloat16>(h, p, st);
+    if (w.dtype == DT_BF16) {
+        rc = launch_fused(h, p, st);
+        if (rc <= 0) return rc;
+        return launch_expansion<__nv_bfloat16>(h, p, st);
+    }
     return launch_expansion<float>(h, p, st);
 }
 

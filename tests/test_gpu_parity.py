@@ -151,6 +151,47 @@ def test_tree_stress_path_dependence():
     assert ne + nt == 8
 
 
+def _small_bf16_case(gu, g, r, k, max_M, max_B):
+    """Small bf16 shapes that take the fused persistent expansion kernel (dt_fused.cuh)."""
+    cfg = wl.CONFIGS["tiny"].replace(dtype="bf16", g=g, r=r, d=96, V=2000, L=5, embed_std=1.0)
+    key = f"smallbf16-{g}-{r}-{k}-{max_M}-{max_B}"
+    return gu.get_case(key, cfg, max_batch=40, max_M=max_M, max_B=max_B, k=k)
+
+
+@pytest.mark.parametrize("path", [0, 1, 2, 3])
+@pytest.mark.parametrize("batch,M,B,k", [(1, 8, 8, 8), (5, 20, 17, 3), (33, 24, 40, 8), (40, 9, 6, 1)])
+def test_tree_small_bf16_all_expand_paths(path, batch, M, B, k):
+    """Ragged small shapes (batch > one 32-request MMA pass, M and r not powers of two, short trees
+    with k = 1) through every expansion path: auto, per-step kernels, fused upc=8, fused upc=16."""
+    gu = _gu()
+    case = _small_bf16_case(gu, 64, 40, k, 32, 48)
+    inp = wl.make_inputs(case.cfg, batch=batch, seed=900 + batch, regime="flat" if batch % 2 else "peaked")
+    case.builder.set_option("expand_path", path)
+    try:
+        ne, nt = gu.check_batch(case, inp, M, B, 0.6, BF16_TOL)
+        launches = case.builder.kernel_launches
+    finally:
+        case.builder.set_option("expand_path", 0)
+    assert ne + nt == batch
+    if path != 1:
+        assert launches <= 5, launches            # select, GEMM, init, fused kernel: no per-pop launches
+
+
+def test_tree_fused_short_tree_and_leaf_pops():
+    """k = 1 chain longer than L (tree exhausted: n_nodes < B+1, dead-leaf padding) and B large
+    enough that depth-L leaves are popped (nodes that are never expanded) on the fused path."""
+    gu = _gu()
+    case = _small_bf16_case(gu, 32, 16, 1, 32, 48)
+    inp = wl.make_inputs(case.cfg, batch=3, seed=31)
+    ne, nt = gu.check_batch(case, inp, 4, 12, 0.0, BF16_TOL)
+    assert ne + nt == 3
+    out = case.run_gpu(inp, 4, 12, 0.0)
+    assert out.n_nodes.tolist() == [6, 6, 6]          # root + L = 5 chain nodes
+    case2 = _small_bf16_case(gu, 32, 16, 2, 32, 48)
+    ne, nt = gu.check_batch(case2, inp, 6, 48, 1.0, BF16_TOL)
+    assert ne + nt == 3
+
+
 @pytest.mark.parametrize("regime", ["flat", "peaked"])
 def test_tree_qwen4b(regime):
     """BASELINE configs[1]."""
