@@ -28,6 +28,10 @@ struct dt_handle {
     int32_t *cand_id; float *cand_val;
     unsigned long long *sel_part; unsigned int *sel_counter, *sel_tau;
     float *C, *states, *heap_g; unsigned long long *heap_tp; int32_t *heap_cnt;
+    // tensor-core precompute GEMM (bf16): split-K partials + tile tickets; side stream + fork/join events so the
+    // GEMM overlaps the HBM-bound select inside the same round (and the same captured graph)
+    float *mma_partial; unsigned int *mma_tickets; int mma_ok;
+    cudaStream_t side; cudaEvent_t ev_fork, ev_join;
     // fused persistent expansion (bf16): state copies, split-K partials, hand-over words
     __nv_bfloat16 *s_hi, *s_lo; float *partial; int2 *desc; unsigned int *sync;
     int fused_ok, max_smem_optin;
@@ -134,6 +138,29 @@ static int launch_gemm_nt(dt_handle *h, const void *A, long long lda, const void
     return DT_OK;
 }
 
+// C = H W1[:, 0:d]^T on the tensor cores (dt_gemm_mma.cuh), split-K kMmaSplits ways.
+constexpr int kMmaSplits = 8;
+static int launch_gemm_mma(dt_handle *h, const void *A, long long lda, const void *Bm, long long ldb,
+                           float *out, long long ldo, int Mr, int Nc, int K, cudaStream_t st) {
+    GemmMmaParams g;
+    g.A = reinterpret_cast<const __nv_bfloat16 *>(A); g.lda = lda;
+    g.Bm = reinterpret_cast<const __nv_bfloat16 *>(Bm); g.ldb = ldb;
+    g.out = out; g.ldo = ldo; g.M = Mr; g.N = Nc; g.K = K;
+    const int tm = (Mr + kMmaBM - 1) / kMmaBM, tn = (Nc + kMmaBN - 1) / kMmaBN;
+    // The K split depends on K only, never on the batch: every output element is then summed in the same order
+    // whatever the batch size (batch invariance).
+    const int kt = (K + kMmaBK - 1) / kMmaBK;
+    int splits = kt < kMmaSplits ? kt : kMmaSplits;
+    g.k_per_split = ((kt + splits - 1) / splits) * kMmaBK;
+    splits = (K + g.k_per_split - 1) / g.k_per_split;
+    g.splits = splits; g.partial = h->mma_partial; g.tile_counter = h->mma_tickets;
+    dim3 grid(tn, tm, splits);
+    gemm_nt_bf16_mma_kernel<<<grid, kMmaThreads, 0, st>>>(g);
+    h->launches++;
+    DT_CUDA(h, cudaGetLastError());
+    return DT_OK;
+}
+
 extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch, int32_t L,
                          int32_t max_M, int32_t max_B, int32_t k) {
     if (!out || !w) return DT_ERR_INVALID_ARG;
@@ -177,6 +204,15 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         o_desc = carve((size_t)2 * max_batch * sizeof(int2));
         o_sync = carve(64 * 4);
     }
+    // MMA GEMM eligibility: bf16, 16-byte aligned rows of H and W1
+    h->mma_ok = (w->dtype == DT_BF16) && (w->d % 8 == 0) && ((w->d + w->g) % 8 == 0) &&
+                ((reinterpret_cast<uintptr_t>(w->corr_w1) & 15u) == 0);
+    const size_t mma_tiles = ((rows + kMmaBM - 1) / kMmaBM) * (size_t)((w->r + kMmaBN - 1) / kMmaBN);
+    size_t o_mpart = 0, o_mtick = 0;
+    if (h->mma_ok) {
+        o_mpart = carve(mma_tiles * kMmaSplits * (size_t)kMmaBM * kMmaBN * 4);
+        o_mtick = carve(mma_tiles * 4);
+    }
     const size_t o_hg = carve((size_t)max_batch * h->heap_cap * 4);
     const size_t o_htp = carve((size_t)max_batch * h->heap_cap * 8);
     const size_t o_hcnt = carve((size_t)max_batch * 4);
@@ -190,6 +226,12 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     h->C = (float *)(h->ws + o_C); h->states = (float *)(h->ws + o_states);
     h->heap_g = (float *)(h->ws + o_hg); h->heap_tp = (unsigned long long *)(h->ws + o_htp);
     h->heap_cnt = (int32_t *)(h->ws + o_hcnt);
+    if (h->mma_ok) { h->mma_partial = (float *)(h->ws + o_mpart); h->mma_tickets = (unsigned int *)(h->ws + o_mtick); }
+    if (cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError(); cudaFree(h->ws); cudaFree(h->P); delete h; return DT_ERR_CUDA;
+    }
     if (h->fused_ok) {
         h->s_hi = (__nv_bfloat16 *)(h->ws + o_shi); h->s_lo = (__nv_bfloat16 *)(h->ws + o_slo);
         h->partial = (float *)(h->ws + o_partial); h->desc = (int2 *)(h->ws + o_desc);
@@ -232,6 +274,9 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
 extern "C" int dt_destroy(dt_handle *h) {
     if (!h) return DT_OK;
     dt_phase_timing(h, 0);
+    if (h->side) cudaStreamDestroy(h->side);
+    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    if (h->ev_join) cudaEventDestroy(h->ev_join);
     cudaFree(h->ws); cudaFree(h->P);
     if (h->stage) cudaFree(h->stage);
     delete h;
@@ -372,11 +417,22 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
 
     int rc = phase_mark(h, 0, st);
     if (rc) return rc;
+    // C = H W1[:, 0:d]^T   (Fact B PAPER.md:83-89).  bf16: tensor cores, forked onto the handle's side
+    // stream so it overlaps the HBM-bound select (fork/join by events: capture-safe, becomes a parallel graph branch).
+    const bool mma = h->mma_ok && ((reinterpret_cast<uintptr_t>(backbone_hidden) & 15u) == 0) &&
+                     rows <= h->max_batch * h->L;
+    if (mma) {
+        DT_CUDA(h, cudaEventRecord(h->ev_fork, st));
+        DT_CUDA(h, cudaStreamWaitEvent(h->side, h->ev_fork, 0));
+        rc = launch_gemm_mma(h, backbone_hidden, w.d, w.corr_w1, (long long)w.d + w.g, h->C, w.r, rows, w.r, w.d, h->side);
+        if (rc) return rc;
+        DT_CUDA(h, cudaEventRecord(h->ev_join, h->side));
+    }
     rc = launch_select(h, marginal_logits, rows, M, h->cand_id, h->cand_val, st);
     if (rc) return rc;
     if ((rc = phase_mark(h, 1, st))) return rc;
-    // C = H W1[:, 0:d]^T   (Fact B PAPER.md:83-89)
-    if (w.dtype == DT_BF16)
+    if (mma) DT_CUDA(h, cudaStreamWaitEvent(st, h->ev_join, 0));
+    else if (w.dtype == DT_BF16)
         rc = launch_gemm_nt<__nv_bfloat16>(h, backbone_hidden, w.d, w.corr_w1, (long long)w.d + w.g, h->C, w.r, rows, w.r, w.d, st);
     else
         rc = launch_gemm_nt<float>(h, backbone_hidden, w.d, w.corr_w1, (long long)w.d + w.g, h->C, w.r, rows, w.r, w.d, st);
