@@ -33,7 +33,7 @@ struct dt_handle {
     float *mma_partial; unsigned int *mma_tickets; int mma_ok;
     cudaStream_t side; cudaEvent_t ev_fork, ev_join;
     // fused persistent expansion (bf16): state copies, split-K partials, hand-over words
-    __nv_bfloat16 *s_hi, *s_lo; float *partial; int2 *desc; unsigned int *sync;
+    __nv_bfloat16 *s_hi, *s_lo; float *partial; unsigned long long *desc; unsigned int *flags;
     int fused_ok, max_smem_optin;
     int64_t opt_expand_path;        // 0 auto, 1 per-step kernels, 2 fused upc=8, 3 fused upc=16
     // host-call staging (lazy)
@@ -201,8 +201,8 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         o_shi = carve((size_t)max_batch * slots * w->g * 2);
         o_slo = carve((size_t)max_batch * slots * w->g * 2);
         o_partial = carve((size_t)(w->g / 8) * max_batch * w->r * 4);
-        o_desc = carve((size_t)2 * max_batch * sizeof(int2));
-        o_sync = carve(64 * 4);
+        o_desc = carve((size_t)max_batch * 8);
+        o_sync = carve(256 * 4);
     }
     // MMA GEMM eligibility: bf16, 16-byte aligned rows of H and W1
     h->mma_ok = (w->dtype == DT_BF16) && (w->d % 8 == 0) && ((w->d + w->g) % 8 == 0) &&
@@ -234,8 +234,8 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     }
     if (h->fused_ok) {
         h->s_hi = (__nv_bfloat16 *)(h->ws + o_shi); h->s_lo = (__nv_bfloat16 *)(h->ws + o_slo);
-        h->partial = (float *)(h->ws + o_partial); h->desc = (int2 *)(h->ws + o_desc);
-        h->sync = (unsigned int *)(h->ws + o_sync);
+        h->partial = (float *)(h->ws + o_partial); h->desc = (unsigned long long *)(h->ws + o_desc);
+        h->flags = (unsigned int *)(h->ws + o_sync);
         bool ok = cudaDeviceGetAttribute(&h->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess;
         h->max_smem_optin -= 1024;                  // room for the kernels' static shared memory
         if (!ok ||
@@ -344,7 +344,7 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st) {
         if (h->opt_expand_path == 2 && cand != 8) continue;
         if (h->opt_expand_path == 3 && cand != 16) continue;
         if (p.g % cand) continue;
-        if (p.g / cand + p.batch > h->num_sms) continue;
+        if (p.g / cand + p.batch > h->num_sms || p.g / cand > 256) continue;
         const int mt = (3 * cand + 15) / 16;
         if (fused_gru_smem(p.g, p.r, cand, mt) > (size_t)h->max_smem_optin) continue;
         upc = cand; break;
@@ -355,14 +355,14 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st) {
     f.e = p;
     f.upc = upc; f.n_gru = p.g / upc; f.m_tiles = (3 * upc + 15) / 16;
     f.slot_stride = h->max_B + 2;
-    f.s_hi = h->s_hi; f.s_lo = h->s_lo; f.s32 = h->states; f.partial = h->partial; f.desc = h->desc; f.sync = h->sync;
+    f.s_hi = h->s_hi; f.s_lo = h->s_lo; f.s32 = h->states; f.partial = h->partial; f.desc = h->desc; f.flags = h->flags;
     f.w2_smem = 1;
-    size_t rs = fused_req_smem(p.r, p.M, p.N, p.heap_cap, 1);
-    if (rs > (size_t)h->max_smem_optin) { f.w2_smem = 0; rs = fused_req_smem(p.r, p.M, p.N, p.heap_cap, 0); }
+    size_t rs = fused_req_smem(p.r, p.M, p.N, p.k, 1);
+    if (rs > (size_t)h->max_smem_optin) { f.w2_smem = 0; rs = fused_req_smem(p.r, p.M, p.N, p.k, 0); }
     if (rs > (size_t)h->max_smem_optin) return 1;
     const size_t gs = fused_gru_smem(p.g, p.r, upc, f.m_tiles);
     const size_t dsm = gs > rs ? gs : rs;
-    fused_init_kernel<<<(p.batch + 127) / 128, 128, 0, st>>>(f);
+    fused_init_kernel<<<((p.batch > f.n_gru ? p.batch : f.n_gru) + 127) / 128, 128, 0, st>>>(f);
     h->launches++;
     int rc = phase_mark(h, 2, st);
     if (rc) return rc;
@@ -510,3 +510,10 @@ extern "C" int dt_build_trees_host(dt_handle *h, const void *logits_h, const voi
     DT_CUDA(h, cudaStreamSynchronize(st));
     return DT_OK;
 }
+
+#ifdef DT_TRACE
+// measurement builds only (-DDT_TRACE): copy the in-kernel timeline of the last fused round to `host` (2*256*8 u64)
+extern "C" int dt_trace_read(unsigned long long *host) {
+    return cudaMemcpyFromSymbol(host, dt::g_dt_trace, sizeof(unsigned long long) * 2 * 256 * 8) == cudaSuccess ? 0 : -3;
+}
+#endif

@@ -66,6 +66,14 @@ __device__ __forceinline__ float warp_max(float v) {
 
 __device__ __forceinline__ float sigmoidf_acc(float x) { return 1.0f / (1.0f + expf(-x)); }
 
+// Fast gate functions for the fused expansion kernel: ex2.approx-based, relative error ~1e-6 -- two orders
+// below the 1e-4 ordering margin.
+__device__ __forceinline__ float sigmoidf_fast(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
+__device__ __forceinline__ float tanhf_fast(float x) {
+    const float xc = fminf(fmaxf(x, -15.f), 15.f);
+    return 1.0f - __fdividef(2.0f, 1.0f + __expf(2.0f * xc));
+}
+
 // generic element load -> float
 template <typename T> __device__ __forceinline__ float ldf(const T *p, size_t i) {
     return ElemTraits<T>::to_f32(p[i]);

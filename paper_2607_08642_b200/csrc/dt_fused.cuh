@@ -8,18 +8,24 @@
 //    produce GRU units [j*upc, (j+1)*upc) and the matching columns of W1[:, d:] in shared memory for
 //    the whole round.  Step t: for the node every request popped t-th, hidden half W_hh S_parent on
 //    the tensor cores (mma.sync m16n8k16, states split bf16 hi + lo so the bf16 x bf16 products are
-//    exact and the state is carried to ~2^-17 relative), gates with the input half gathered from the
+//    exact and the state is carried to ~2^-17 relative; split-K over the warps, each warp streaming
+//    its k-blocks of the parents' states from L2 through a private cp.async ring), gates with the input half gathered from the
 //    table P = E W_ih^T, new state S_t, and this CTA's split-K share of
 //    W1[:, d:] S_t written as a partial [batch, r].
 //  * Request CTAs (one per request) own that request's heap in shared memory.  Step t: sum the
 //    partials in CTA order (fixed order => deterministic, batch-invariant), a = SiLU(C + .),
 //    z_m = (base_m + W2[cand_m, :] a) / T_eff over the M candidate rows of the node's depth
 //    (rows staged into shared memory by cp.async while the GRU CTAs work),
-//    slice log-softmax (reading A1), top-k, push, pop the maximum (reading A8) into slot t+1.
+//    slice log-softmax (reading A1), top-k, merge into the sorted frontier, pop entry 0 (reading A8)
+//    into slot t+1.
 //    After the last pop the same CTA emits positions, padding and the ancestor mask (a9).
 //
-// The two roles hand over through two monotone counters in global memory (release: fence + atomic
-// add; acquire: ld.acquire spin by one thread + bar.sync) and a double-buffered node descriptor.
+// The two roles hand over through self-describing words in global memory, one per producer, so no
+// shared counter is contended: request b publishes {epoch, parent state slot, token} in desc[b] and
+// GRU CTA c publishes its completed step count in flags[c]; consumers poll with L1-bypassing loads
+// (one lane per producer), fence, and release the CTA through one barrier.
+// The request CTA keeps its frontier as a SORTED array (one entry per thread, truncated to the pops
+// that remain), so a pop is "take entry 0" and a push is a rank-and-scatter merge of the k children.
 #pragma once
 #include "dt_expand.cuh"
 #include "dt_gemm_mma.cuh"
@@ -31,6 +37,10 @@ constexpr int kFusWarps = 8;
 constexpr int kFusWPad = 32;      // bf16 elements of padding per W_hh row in smem (64 B: conflict-free LDS.128)
 constexpr int kFusRedLd = 40;     // floats per row of the split-K reduction buffer
 constexpr int kFusChunk = 32;     // requests per MMA pass (4 n8 tiles)
+constexpr int kFusKB = 32;        // k per MMA block (two k16 steps)
+constexpr int kFusRing = 3;       // state blocks in flight per warp (cp.async ring)
+constexpr int kFusW2Pad = 32;     // bf16 elements of padding per staged W2 row (row stride = 16 banks mod 32)
+constexpr int kFusMaxFront = 256; // frontier entries kept (>= DT_MAX_B)
 
 struct FusedParams {
     ExpandParams e;
@@ -40,51 +50,79 @@ struct FusedParams {
     __nv_bfloat16 *s_hi, *s_lo;    // [batch, slot_stride, g]
     float *s32;                    // [batch, slot_stride, g]
     float *partial;                // [n_gru, batch, r]
-    int2 *desc;                    // [2, batch]  {state slot of the parent or -1 = skip, token}
-    unsigned int *sync;            // [0] ready (request -> GRU), [32] done (GRU -> request)
+    unsigned long long *desc;      // [batch]  hand-over word request -> GRU: epoch(16) | state slot + 1 (16) | token (32)
+    unsigned int *flags;           // [n_gru]  hand-over word GRU -> request: steps completed by that GRU CTA
 };
 
-__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int *p) {
+// Optional in-kernel timeline (compile with -DDT_TRACE; measurement builds only, never the product build):
+// thread 0 of GRU CTA 0 (role 0) and of request CTA 0 (role 1) stamp %globaltimer at fixed points of every step.
+#ifdef DT_TRACE
+__device__ unsigned long long g_dt_trace[2][256][8];
+__device__ __forceinline__ unsigned long long dt_globaltimer() {
+    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
+}
+#define DT_TR(role, first_cta, t, i) do { if (threadIdx.x == 0 && (int)blockIdx.x == (first_cta)) g_dt_trace[role][t][i] = dt_globaltimer(); } while (0)
+#else
+#define DT_TR(role, first_cta, t, i) do { } while (0)
+#endif
+
+// ---- hand-over words -------------------------------------------------------------------------------
+// Both directions use one self-describing word per producer (no shared counter, so no serialised
+// atomics): the consumer's lanes poll the producers' words with relaxed loads that bypass L1, then
+// fence.  The producer fences after a CTA barrier and stores its word.
+__device__ __forceinline__ unsigned int ld_relaxed_u32(const unsigned int *p) {
     unsigned int v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-// All threads of the CTA call: waits until *ctr >= target.
-__device__ __forceinline__ void cta_wait_counter(const unsigned int *ctr, unsigned int target) {
-    if (threadIdx.x == 0) {
-        while (ld_acquire_u32(ctr) < target) { }
-    }
-    __syncthreads();
+__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long *p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
 }
-// All threads call after their global writes: publishes them and bumps *ctr by one.
-__device__ __forceinline__ void cta_signal_counter(unsigned int *ctr) {
-    __syncthreads();
-    if (threadIdx.x == 0) { __threadfence(); atomicAdd(ctr, 1u); }
+__device__ __forceinline__ void st_relaxed_u32(unsigned int *p, unsigned int v) {
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void st_relaxed_u64(unsigned long long *p, unsigned long long v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long fused_desc_pack(int epoch, int sidx, int tok) {
+    return ((unsigned long long)(unsigned int)epoch << 48) | ((unsigned long long)(unsigned int)(sidx + 1) << 32) |
+           (unsigned long long)(unsigned int)tok;
 }
 
-// Zero the hand-over words and write the step-0 descriptor (the root: parent state = zeros, reading A4).
+// Zero the GRU flags and write the step-0 descriptor (the root: parent state = zeros, reading A4).
 __global__ void fused_init_kernel(FusedParams p) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i == 0) { p.sync[0] = 0u; p.sync[32] = 0u; }
+    if (i < p.n_gru) p.flags[i] = 0u;
     if (i < p.e.batch) {
         int tok = p.e.root_tokens[i];
         tok = min(max(tok, 0), p.e.V - 1);
-        p.desc[i] = make_int2(0, tok);
+        p.desc[i] = fused_desc_pack(1, 0, tok);
     }
 }
 
 // shared-memory footprints (bytes) of the two roles
 __host__ __device__ inline size_t fused_gru_smem(int g, int r, int upc, int m_tiles) {
     size_t w = (size_t)3 * upc * (g + kFusWPad) * 2;
-    size_t red = (size_t)kFusWarps * m_tiles * 16 * kFusRedLd * 4;
-    size_t w1 = (size_t)r * upc * 4;
-    size_t snew = (size_t)upc * (kFusChunk + 1) * 4;
-    return w + red + w1 + snew + 3 * kFusChunk * 4;
+    size_t ring = (size_t)kFusWarps * kFusRing * (2 * kFusChunk * kFusKB * 2);          // hi + lo blocks
+    size_t red = (size_t)kFusWarps * m_tiles * 16 * kFusRedLd * 4;                      // aliases the ring
+    size_t w1 = (size_t)r * 16 * 2;
+    size_t snew = (size_t)2 * kFusChunk * 16 * 2;
+    (void)upc;
+    return w + (ring > red ? ring : red) + w1 + snew + 3 * kFusChunk * 4 + 64;
 }
-__host__ __device__ inline size_t fused_req_smem(int r, int M, int N, int heap_cap, int w2_smem) {
-    size_t s = (size_t)r * 4 + (size_t)M * 12 + (size_t)N * 16 + (size_t)heap_cap * 12 + 64;
-    if (w2_smem) s += (size_t)M * (r + 8) * 2;
-    return (s + 15) / 16 * 16 + 16;
+__host__ __device__ inline size_t fused_req_smem(int r, int M, int N, int k, int w2_smem) {
+    auto al = [](size_t x) { return (x + 15) / 16 * 16; };
+    size_t s = al((size_t)2 * kFusMaxFront * 8) + al((size_t)k * 8) + al((size_t)M * 8) + al((size_t)2 * kFusMaxFront * 4) +
+               al((size_t)k * 4) + al((size_t)r * 4) + 3 * al((size_t)M * 4) + 4 * al((size_t)N * 4);
+    if (w2_smem) s += al((size_t)M * (r + kFusW2Pad) * 2);
+    return s + 16;
+}
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
+    unsigned int s = (unsigned int)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
 }
 
 // ------------------------------------------------------------------------------------------ GRU role
@@ -93,7 +131,7 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
     constexpr int MT = (3 * UPC + 15) / 16;
     constexpr int ROWS = 3 * UPC;
     constexpr int PP = UPC * kFusChunk / kFusThreads;          // epilogue (unit, request) pairs per thread
-    constexpr int kNewLd = kFusChunk + 1;
+    constexpr int kBlkBytes = 2 * kFusChunk * kFusKB * 2;      // one k-block of states: [hi|lo][32 cols][32 k] bf16
     const ExpandParams &e = p.e;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, gq = lane >> 2, c4 = lane & 3;
     const int g = e.g, r = e.r, batch = e.batch;
@@ -102,11 +140,16 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
     const size_t stride = (size_t)p.slot_stride;
 
     __nv_bfloat16 *sW = reinterpret_cast<__nv_bfloat16 *>(smem_raw);
-    float *sRed = reinterpret_cast<float *>(sW + (size_t)ROWS * ldw);
-    float *sW1 = sRed + (size_t)kFusWarps * MT * 16 * kFusRedLd;
-    float *sNew = sW1 + (size_t)r * UPC;
-    int *sIdx = reinterpret_cast<int *>(sNew + UPC * kNewLd);
+    unsigned char *sRingAll = reinterpret_cast<unsigned char *>(sW + (size_t)ROWS * ldw);
+    const size_t ring_bytes = (size_t)kFusWarps * kFusRing * kBlkBytes;
+    const size_t red_bytes = (size_t)kFusWarps * MT * 16 * kFusRedLd * 4;
+    float *sRed = reinterpret_cast<float *>(sRingAll);                                  // aliases the ring
+    unsigned int *sW1b = reinterpret_cast<unsigned int *>(sRingAll + (ring_bytes > red_bytes ? ring_bytes : red_bytes));  // [r][16] bf16
+    __nv_bfloat16 *sNewH = reinterpret_cast<__nv_bfloat16 *>(sW1b + (size_t)r * 8);     // [32 requests][16 units]
+    __nv_bfloat16 *sNewL = sNewH + kFusChunk * 16;
+    int *sIdx = reinterpret_cast<int *>(sNewL + kFusChunk * 16);
     int *sTok = sIdx + kFusChunk;
+    unsigned char *myRing = sRingAll + (size_t)warp * kFusRing * kBlkBytes;
 
     // resident weights: rows (gate, u0 + ul) of W_hh, columns d + u0 + ul of W1
     {
@@ -119,27 +162,56 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
             *reinterpret_cast<uint4 *>(sW + (size_t)lr * ldw + v * 8) = q;
         }
         const __nv_bfloat16 *w1 = reinterpret_cast<const __nv_bfloat16 *>(e.w1);
-        for (int i = tid; i < r * UPC; i += kFusThreads) {
-            const int j = i / UPC, ul = i - j * UPC;
-            sW1[i] = __bfloat162float(w1[(size_t)j * (e.d + g) + e.d + u0 + ul]);
+        __nv_bfloat16 *sW1h = reinterpret_cast<__nv_bfloat16 *>(sW1b);
+        for (int i = tid; i < r * 16; i += kFusThreads) {       // K padded to 16 with zeros when UPC == 8
+            const int j = i >> 4, ul = i & 15;
+            sW1h[i] = (ul < UPC) ? w1[(size_t)j * (e.d + g) + e.d + u0 + ul] : __float2bfloat16_rn(0.f);
         }
+        for (int i = tid; i < 2 * kFusChunk * 16; i += kFusThreads) sNewH[i] = __float2bfloat16_rn(0.f);   // H and L are adjacent
     }
     __syncthreads();
 
-    const int nblk = g / 32;
+    // split-K over the warps: warp w owns k-blocks [blk0, blk1) of 32 k each
+    const int nblk = g / kFusKB;
     const int blk0 = warp * nblk / kFusWarps, blk1 = (warp + 1) * nblk / kFusWarps;
 
     for (int t = 0; t < e.B; ++t) {
-        if (t > 0) cta_wait_counter(&p.sync[0], (unsigned int)batch * (unsigned int)t);
-        const int2 *desc = p.desc + (size_t)(t & 1) * batch;
         for (int c0 = 0; c0 < batch; c0 += kFusChunk) {
             const int nb = min(kFusChunk, batch - c0);
             const int ntiles = (nb + 7) >> 3;
-            if (tid < kFusChunk) {
-                int2 dsc = (tid < nb) ? __ldcg(desc + c0 + tid) : make_int2(-1, 0);
-                sIdx[tid] = dsc.x; sTok[tid] = dsc.y;
+            // wait for the descriptors of step t (lane = request), then broadcast through shared memory
+            if (warp == 0) {
+                int sidx = -1, tok = 0;
+                if (lane < nb) {
+                    unsigned long long dsc;
+                    do { dsc = ld_relaxed_u64(p.desc + c0 + lane); } while ((int)(dsc >> 48) != t + 1);
+                    sidx = (int)((dsc >> 32) & 0xFFFFu) - 1;
+                    tok = (int)(dsc & 0xFFFFFFFFull);
+                }
+                __threadfence();
+                sIdx[lane] = sidx; sTok[lane] = tok;
             }
             __syncthreads();
+            if (c0 == 0) DT_TR(0, 0, t, 0);
+
+            // stream this warp's k-blocks of the parents' states (bf16 hi | lo) into its ring
+            auto issue_block = [&](int blk) {
+                unsigned char *dst = myRing + (size_t)((blk - blk0) % kFusRing) * kBlkBytes;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const int idx = i * 32 + lane;                   // 256 16-byte pieces: [hl][col][piece]
+                    const int hl = idx >> 7, col = (idx >> 2) & 31, pc = idx & 3;
+                    const int sidx = sIdx[col];
+                    const size_t off = (sidx > 0) ? ((size_t)(c0 + col) * stride + sidx) * g : 0;   // 0 = zero slot
+                    const __nv_bfloat16 *src = (hl ? p.s_lo : p.s_hi) + off + (size_t)blk * kFusKB + pc * 8;
+                    cp_async16(dst + (size_t)idx * 16, src);
+                }
+                cp_async_commit();
+            };
+#pragma unroll
+            for (int i = 0; i < kFusRing; ++i) {
+                if (blk0 + i < blk1) issue_block(blk0 + i); else cp_async_commit();
+            }
 
             // epilogue operands (input half from P, previous state): issued now, consumed after the MMAs
             float pr[PP], pz[PP], pn[PP], hp[PP];
@@ -155,7 +227,8 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
                 }
             }
 
-            // hidden half W_hh S_parent: split-K over the warps, 32 k per block (two k16 MMA steps)
+            // hidden half W_hh S_parent on the tensor cores; A (weights) and B (states) use the same
+            // k permutation inside a block, so 16-byte loads feed both operands directly
             float acc[MT][4][4];
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt)
@@ -163,42 +236,54 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
                 for (int nt = 0; nt < 4; ++nt)
 #pragma unroll
                     for (int q = 0; q < 4; ++q) acc[mt][nt][q] = 0.f;
-            size_t boff[4];
-#pragma unroll
-            for (int nt = 0; nt < 4; ++nt) {
-                const int n = nt * 8 + gq;
-                const int sidx = sIdx[n];
-                boff[nt] = (sidx > 0) ? ((size_t)(c0 + n) * stride + sidx) * g : 0;     // 0 = zero slot of request 0
-            }
             for (int blk = blk0; blk < blk1; ++blk) {
-                const int k0 = blk * 32 + 8 * c4;
+                cp_async_wait<kFusRing - 1>();
+                __syncwarp();
+                const unsigned char *src = myRing + (size_t)((blk - blk0) % kFusRing) * kBlkBytes;
                 uint4 bh[4], bl4[4];
 #pragma unroll
                 for (int nt = 0; nt < 4; ++nt) {
-                    if (nt < ntiles) {
-                        bh[nt] = __ldcg(reinterpret_cast<const uint4 *>(p.s_hi + boff[nt] + k0));
-                        bl4[nt] = __ldcg(reinterpret_cast<const uint4 *>(p.s_lo + boff[nt] + k0));
-                    } else { bh[nt] = make_uint4(0, 0, 0, 0); bl4[nt] = make_uint4(0, 0, 0, 0); }
+                    bh[nt] = *reinterpret_cast<const uint4 *>(src + (size_t)((nt * 8 + gq) * 4 + c4) * 16);
+                    bl4[nt] = *reinterpret_cast<const uint4 *>(src + (size_t)(128 + (nt * 8 + gq) * 4 + c4) * 16);
                 }
+                __syncwarp();
+                if (blk + kFusRing < blk1) issue_block(blk + kFusRing); else cp_async_commit();
+                const int k0 = blk * kFusKB + 8 * c4;
+                unsigned int aA[MT][4], aB[MT][4];
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) {
                     const int r0 = mt * 16 + gq, r1 = r0 + 8;
                     uint4 A0 = make_uint4(0, 0, 0, 0), A1 = make_uint4(0, 0, 0, 0);
                     if (r0 < ROWS) A0 = *reinterpret_cast<const uint4 *>(sW + (size_t)r0 * ldw + k0);
                     if (r1 < ROWS) A1 = *reinterpret_cast<const uint4 *>(sW + (size_t)r1 * ldw + k0);
-                    const unsigned int aA[4] = {A0.x, A1.x, A0.y, A1.y};
-                    const unsigned int aB[4] = {A0.z, A1.z, A0.w, A1.w};
-#pragma unroll
-                    for (int nt = 0; nt < 4; ++nt) {
-                        if (nt < ntiles) {
-                            mma_bf16_16816(acc[mt][nt], aA, bh[nt].x, bh[nt].y);
-                            mma_bf16_16816(acc[mt][nt], aB, bh[nt].z, bh[nt].w);
-                            mma_bf16_16816(acc[mt][nt], aA, bl4[nt].x, bl4[nt].y);
-                            mma_bf16_16816(acc[mt][nt], aB, bl4[nt].z, bl4[nt].w);
-                        }
-                    }
+                    aA[mt][0] = A0.x; aA[mt][1] = A1.x; aA[mt][2] = A0.y; aA[mt][3] = A1.y;
+                    aB[mt][0] = A0.z; aB[mt][1] = A1.z; aB[mt][2] = A0.w; aB[mt][3] = A1.w;
                 }
+                // four passes over the MT x 4 independent accumulators: consecutive MMAs never chain
+#pragma unroll
+                for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt)
+                        if (nt < ntiles) mma_bf16_16816(acc[mt][nt], aA[mt], bh[nt].x, bh[nt].y);
+#pragma unroll
+                for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt)
+                        if (nt < ntiles) mma_bf16_16816(acc[mt][nt], aB[mt], bh[nt].z, bh[nt].w);
+#pragma unroll
+                for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt)
+                        if (nt < ntiles) mma_bf16_16816(acc[mt][nt], aA[mt], bl4[nt].x, bl4[nt].y);
+#pragma unroll
+                for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt)
+                        if (nt < ntiles) mma_bf16_16816(acc[mt][nt], aB[mt], bl4[nt].z, bl4[nt].w);
             }
+            cp_async_wait<0>();
+            __syncthreads();                                    // every warp is done with its ring: reuse it as sRed
+            if (c0 == 0) DT_TR(0, 0, t, 1);
             {
                 float *red = sRed + (size_t)warp * MT * 16 * kFusRedLd;
 #pragma unroll
@@ -211,6 +296,7 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
                     }
             }
             __syncthreads();
+            if (c0 == 0) DT_TR(0, 0, t, 2);
             // gates (reading A2): r, z, n rows of unit ul are local rows ul, UPC + ul, 2 UPC + ul
 #pragma unroll
             for (int i = 0; i < PP; ++i) {
@@ -225,71 +311,67 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
                 }
                 float hnew = 0.f;
                 if (sIdx[bl] >= 0) {
-                    const float rg = sigmoidf_acc(pr[i] + hr);
-                    const float zg = sigmoidf_acc(pz[i] + hz);
-                    const float ng = tanhf(pn[i] + rg * hn);
+                    const float rg = sigmoidf_fast(pr[i] + hr);
+                    const float zg = sigmoidf_fast(pz[i] + hz);
+                    const float ng = tanhf_fast(pn[i] + rg * hn);
                     hnew = (1.0f - zg) * ng + zg * hp[i];
                 }
-                sNew[ul * kNewLd + bl] = hnew;
+                const __nv_bfloat16 hi = __float2bfloat16_rn(hnew);
+                const __nv_bfloat16 lo = __float2bfloat16_rn(hnew - __bfloat162float(hi));
+                if (sIdx[bl] >= 0) {                             // publish S_t (slot t+1): fp32 and the bf16 hi/lo split
+                    const size_t o = ((size_t)(c0 + bl) * stride + (t + 1)) * g + u0 + ul;
+                    __stcg(p.s32 + o, hnew);
+                    p.s_hi[o] = hi;
+                    p.s_lo[o] = lo;
+                }
+                sNewH[bl * 16 + ul] = hi;
+                sNewL[bl * 16 + ul] = lo;
             }
             __syncthreads();
-            // publish S_t (slot t+1): fp32 and the bf16 hi/lo split, UPC consecutive units per request row
-            for (int idx = tid; idx < UPC * nb; idx += kFusThreads) {
-                const int bl = idx / UPC, ul = idx - bl * UPC;
-                if (sIdx[bl] >= 0) {
-                    const float h = sNew[ul * kNewLd + bl];
-                    const size_t o = ((size_t)(c0 + bl) * stride + (t + 1)) * g + u0 + ul;
-                    const __nv_bfloat16 hi = __float2bfloat16_rn(h);
-                    __stcg(p.s32 + o, h);
-                    p.s_hi[o] = hi;
-                    p.s_lo[o] = __float2bfloat16_rn(h - __bfloat162float(hi));
+            if (c0 == 0) DT_TR(0, 0, t, 3);
+            // this CTA's split-K share of W1[:, d:] S_t on the tensor cores:
+            // [r x 16] (bf16 weights, exact) x [16 x 32] (new states, bf16 hi + lo)
+            for (int mt = warp; mt < (r + 15) / 16; mt += kFusWarps) {
+                const int j0 = mt * 16 + gq, j1 = j0 + 8;
+                unsigned int a[4] = {0u, 0u, 0u, 0u};
+                if (j0 < r) { a[0] = sW1b[j0 * 8 + c4]; a[2] = sW1b[j0 * 8 + 4 + c4]; }
+                if (j1 < r) { a[1] = sW1b[j1 * 8 + c4]; a[3] = sW1b[j1 * 8 + 4 + c4]; }
+                float c[4][4];
+#pragma unroll
+                for (int nt = 0; nt < 4; ++nt) {
+                    c[nt][0] = c[nt][1] = c[nt][2] = c[nt][3] = 0.f;
+                    const unsigned int *bh32 = reinterpret_cast<const unsigned int *>(sNewH) + (nt * 8 + gq) * 8;
+                    const unsigned int *bl32 = reinterpret_cast<const unsigned int *>(sNewL) + (nt * 8 + gq) * 8;
+                    mma_bf16_16816(c[nt], a, bh32[c4], bh32[4 + c4]);
+                    mma_bf16_16816(c[nt], a, bl32[c4], bl32[4 + c4]);
                 }
-            }
-            // this CTA's split-K share of W1[:, d:] S_t
-            for (int j = tid; j < r; j += kFusThreads) {
-                float w1r[UPC];
 #pragma unroll
-                for (int ul = 0; ul < UPC; ++ul) w1r[ul] = sW1[j * UPC + ul];
-                for (int bl = 0; bl < nb; ++bl) {
-                    float s = 0.f;
-#pragma unroll
-                    for (int ul = 0; ul < UPC; ++ul) s = fmaf(w1r[ul], sNew[ul * kNewLd + bl], s);
-                    __stcg(p.partial + ((size_t)cta * batch + c0 + bl) * r + j, s);
+                for (int nt = 0; nt < 4; ++nt) {
+                    const int col = nt * 8 + 2 * c4;
+                    float *o0 = p.partial + ((size_t)cta * batch + c0 + col) * r;
+                    if (col < nb) { if (j0 < r) __stcg(o0 + j0, c[nt][0]); if (j1 < r) __stcg(o0 + j1, c[nt][2]); }
+                    if (col + 1 < nb) { if (j0 < r) __stcg(o0 + r + j0, c[nt][1]); if (j1 < r) __stcg(o0 + r + j1, c[nt][3]); }
                 }
             }
             __syncthreads();
         }
-        cta_signal_counter(&p.sync[32]);
+        DT_TR(0, 0, t, 4);
+        if (tid == 0) { __threadfence(); st_relaxed_u32(p.flags + cta, (unsigned int)(t + 1)); }
+        DT_TR(0, 0, t, 5);
     }
 }
 
 // -------------------------------------------------------------------------------------- request role
-__device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
-    unsigned int s = (unsigned int)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
-}
-
-// dot(w[0..n) bf16 in SHARED memory (16 B aligned, n % 8 == 0), s[0..n) fp32 in shared memory).
-__device__ __forceinline__ float warp_dot_smem_bf16(const __nv_bfloat16 *w, const float *s, int n, int lane) {
-    float acc = 0.f;
-    for (int v = lane; v < n / 8; v += 32) {
-        const uint4 q = *reinterpret_cast<const uint4 *>(w + (size_t)v * 8);
-        const float *sp = s + (size_t)v * 8;
-        float f[8];
-        unpack8(q, f);
-#pragma unroll
-        for (int i = 0; i < 8; ++i) acc = fmaf(f[i], sp[i], acc);
-    }
-    return warp_sum(acc);
+// Frontier entries are ordered by the pop comparator of reading A8, (g desc, token asc, parent asc),
+// packed so that a larger (hi, lo) pair pops first: hi = ord_key(g), lo = ~token << 32 | ~parent.
+__device__ __forceinline__ bool front_gt(unsigned int ah, unsigned long long al, unsigned int bh, unsigned long long bl) {
+    return ah > bh || (ah == bh && al > bl);
 }
 
 struct FusedReqSmem {
-    float red[8];
-    float redk[8];
-    unsigned long long redtp[8];
-    int redi[8];
-    float zmax, lse;
-    int n_valid, cnt;
+    int n_valid;        // tree slots filled so far (root included)
+    int n_front;        // live frontier entries
+    int cur;            // which of the two frontier buffers is live
 };
 
 __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned char *smem_raw) {
@@ -297,24 +379,27 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     const ExpandParams &e = p.e;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int b = blockIdx.x - p.n_gru;
-    const int g = e.g, r = e.r, M = e.M, k = e.k, N = e.N, L = e.L, batch = e.batch;
-    (void)g;
-    const int ldw2 = r + 8;
+    const int r = e.r, M = e.M, k = e.k, N = e.N, L = e.L, batch = e.batch, B = e.B;
+    const int ldw2 = r + kFusW2Pad;
 
-    // carve: [W2 rows (bf16, 16 B aligned)] [heap tp u64] [fp32 / int arrays]
-    __nv_bfloat16 *sW2 = reinterpret_cast<__nv_bfloat16 *>(smem_raw);
-    size_t off = p.w2_smem ? ((size_t)M * ldw2 * 2 + 15) / 16 * 16 : 0;
-    unsigned long long *htp = reinterpret_cast<unsigned long long *>(smem_raw + off);
-    off += (size_t)e.heap_cap * 8;
-    float *hg = reinterpret_cast<float *>(smem_raw + off);
-    float *sA = hg + e.heap_cap;
-    float *sZ = sA + r;
-    float *sBase = sZ + M;
-    int *sTok = reinterpret_cast<int *>(sBase + M);
-    int *nTok = sTok + M;
-    int *nPar = nTok + N;
-    int *nDep = nPar + N;
-    float *nSco = reinterpret_cast<float *>(nDep + N);
+    // carve, every array 16-byte aligned: [W2 rows bf16] [frontier lo u64 x2] [new lo] [rank keys] [frontier hi u32 x2]
+    // [new hi] [a] [z] [base] [cand tok] [tree tok / par / dep / score]
+    size_t off = 0;
+    auto carve = [&](size_t bytes) { unsigned char *q = smem_raw + off; off += (bytes + 15) / 16 * 16; return q; };
+    __nv_bfloat16 *sW2 = reinterpret_cast<__nv_bfloat16 *>(carve(p.w2_smem ? (size_t)M * ldw2 * 2 : 0));
+    unsigned long long *fLo = reinterpret_cast<unsigned long long *>(carve((size_t)2 * kFusMaxFront * 8));
+    unsigned long long *nLo = reinterpret_cast<unsigned long long *>(carve((size_t)k * 8));
+    unsigned long long *sKey = reinterpret_cast<unsigned long long *>(carve((size_t)M * 8));
+    unsigned int *fHi = reinterpret_cast<unsigned int *>(carve((size_t)2 * kFusMaxFront * 4));
+    unsigned int *nHi = reinterpret_cast<unsigned int *>(carve((size_t)k * 4));
+    float *sA = reinterpret_cast<float *>(carve((size_t)r * 4));
+    float *sZ = reinterpret_cast<float *>(carve((size_t)M * 4));
+    float *sBase = reinterpret_cast<float *>(carve((size_t)M * 4));
+    int *sTok = reinterpret_cast<int *>(carve((size_t)M * 4));
+    int *nTok = reinterpret_cast<int *>(carve((size_t)N * 4));
+    int *nPar = reinterpret_cast<int *>(carve((size_t)N * 4));
+    int *nDep = reinterpret_cast<int *>(carve((size_t)N * 4));
+    float *nSco = reinterpret_cast<float *>(carve((size_t)N * 4));
 
     const __nv_bfloat16 *w2 = reinterpret_cast<const __nv_bfloat16 *>(e.w2);
 
@@ -338,27 +423,48 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
 
     if (tid == 0) {
         nTok[0] = e.root_tokens[b]; nPar[0] = -1; nDep[0] = 0; nSco[0] = 0.f;
-        sm.n_valid = 1; sm.cnt = 0;
+        sm.n_valid = 1; sm.n_front = 0; sm.cur = 0;
     }
     __syncthreads();
     stage_depth(0);
 
-    for (int t = 0; t < e.B; ++t) {
+    for (int t = 0; t < B; ++t) {
         const int n_valid = sm.n_valid;
-        int cnt = sm.cnt;
+        const int n_front = sm.n_front, cur = sm.cur;
         const bool node_ok = (t < n_valid);
         const int depth = node_ok ? nDep[t] : L;
+        const bool expand = node_ok && depth < L;               // block-uniform
         // Every request CTA waits for the GRU CTAs' step t, expanded or not: nobody runs ahead, so the
-        // double-buffered descriptor and the partial buffer are never overwritten while still in use.
-        cta_wait_counter(&p.sync[32], (unsigned int)p.n_gru * (unsigned int)(t + 1));
-        if (node_ok && depth < L) {                 // block-uniform
+        // descriptor word and the partial buffer are never overwritten while still in use.
+        if (warp == 0) {
+            for (int q = lane; q < p.n_gru; q += 32)
+                while (ld_relaxed_u32(p.flags + q) < (unsigned int)(t + 1)) { }
+            __threadfence();
+        }
+        __syncthreads();
+        DT_TR(1, p.n_gru, t, 0);
+        // the live frontier is entries 1 .. n_front of buffer `cur` (entry 0 was popped by the previous step)
+        const unsigned int *oHi = fHi + cur * kFusMaxFront + 1;
+        const unsigned long long *oLo = fLo + cur * kFusMaxFront + 1;
+        unsigned int *wHi = fHi + (cur ^ 1) * kFusMaxFront;
+        unsigned long long *wLo = fLo + (cur ^ 1) * kFusMaxFront;
+        int n_new = 0;
+        if (expand) {
             const size_t row = (size_t)b * L + depth;           // H_{depth+1} <-> row index depth (A12)
             // a = SiLU(C + W1[:, d:] S_t): split-K partials summed in CTA order
             for (int j = tid; j < r; j += kFusThreads) {
                 const float *pp = p.partial + (size_t)b * r + j;
                 const size_t ps = (size_t)batch * r;
+                const float cval = e.C[row * r + j];
                 float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
                 int q = 0;
+                for (; q + 32 <= p.n_gru; q += 32) {
+                    float v[32];
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) v[i] = __ldcg(pp + (size_t)(q + i) * ps);
+#pragma unroll
+                    for (int i = 0; i < 32; i += 4) { s0 += v[i]; s1 += v[i + 1]; s2 += v[i + 2]; s3 += v[i + 3]; }
+                }
                 for (; q + 4 <= p.n_gru; q += 4) {
                     s0 += __ldcg(pp + (size_t)q * ps);
                     s1 += __ldcg(pp + (size_t)(q + 1) * ps);
@@ -366,97 +472,145 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                     s3 += __ldcg(pp + (size_t)(q + 3) * ps);
                 }
                 for (; q < p.n_gru; ++q) s0 += __ldcg(pp + (size_t)q * ps);
-                const float x = e.C[row * r + j] + ((s0 + s1) + (s2 + s3));
+                const float x = cval + ((s0 + s1) + (s2 + s3));
                 sA[j] = x * sigmoidf_acc(x);
             }
             cp_async_wait<0>();
             __syncthreads();
+            DT_TR(1, p.n_gru, t, 1);
             // z_m = ((base_m - base_0) + W2[cand_m, :] a) / T_eff     PAPER.md:143-144 (shift-invariant)
+            // four lanes per candidate row, interleaved 16-byte pieces
             const float base0 = sBase[0];
-            for (int m = warp; m < M; m += kFusWarps) {
-                float acc = p.w2_smem ? warp_dot_smem_bf16(sW2 + (size_t)m * ldw2, sA, r, lane)
-                                      : warp_dot(w2 + (size_t)sTok[m] * r, sA, r, lane);
-                if (lane == 0) sZ[m] = __fdiv_rn((sBase[m] - base0) + acc, e.T_eff);
-            }
-            __syncthreads();
-            // slice log-softmax (reading A1): one candidate per thread (M <= 256)
-            const float z = (tid < M) ? sZ[tid] : -INFINITY;
-            const float wm = warp_max(z);
-            if (lane == 0) sm.red[warp] = wm;
-            __syncthreads();
-            if (tid == 0) { float m = sm.red[0]; for (int i = 1; i < 8; ++i) m = fmaxf(m, sm.red[i]); sm.zmax = m; }
-            __syncthreads();
-            const float zmax = sm.zmax;
-            const float ex = (tid < M) ? expf(z - zmax) : 0.f;
-            const float ws = warp_sum(ex);
-            if (lane == 0) sm.redk[warp] = ws;
-            __syncthreads();
-            if (tid == 0) { float s = 0.f; for (int i = 0; i < 8; ++i) s += sm.redk[i]; sm.lse = logf(s); }
-            __syncthreads();
-            const float lp = (z - zmax) - sm.lse;
-            if (tid < M) sZ[tid] = lp;
-            __syncthreads();
-            // top-k by (logp desc, token asc): rank by counting; push
-            if (tid < M) {
-                const int mytok = sTok[tid];
-                int rank = 0;
-                for (int m = 0; m < M; ++m) {
-                    const float o = sZ[m];
-                    rank += (o > lp) || (o == lp && sTok[m] < mytok);
-                }
-                if (rank < k) {
-                    hg[cnt + rank] = nSco[t] + lp;
-                    htp[cnt + rank] = ((unsigned long long)(unsigned int)mytok << 32) | (unsigned int)t;
-                }
-            }
-            cnt += k;
-            __syncthreads();
-        }
-
-        // pop the maximum under (g desc, token asc, parent asc) into slot t+1
-        int next_dep = L;                           // depth of the node popped now (L = none / leaf)
-        if (cnt > 0) {
-            float bg = -INFINITY; unsigned long long btp = ~0ull; int bi = -1;
-            for (int i = tid; i < cnt; i += kFusThreads) {
-                const float gi = hg[i]; const unsigned long long tp = htp[i];
-                if (bi < 0 || gi > bg || (gi == bg && tp < btp)) { bg = gi; btp = tp; bi = i; }
-            }
+            {
+                const int q4 = tid & 3, nvec = r / 8;
+                for (int mb = 0; mb < M; mb += kFusThreads / 4) {     // warp-uniform trip count (shuffles below)
+                    const int m = mb + (tid >> 2);
+                    float acc = 0.f;
+                    if (m >= M) {
+                    } else if (p.w2_smem) {
+                        const __nv_bfloat16 *wr = sW2 + (size_t)m * ldw2;
+                        for (int v = q4; v < nvec; v += 4) {
+                            const uint4 q = *reinterpret_cast<const uint4 *>(wr + (size_t)v * 8);
+                            const float4 a0 = *reinterpret_cast<const float4 *>(sA + (size_t)v * 8);
+                            const float4 a1 = *reinterpret_cast<const float4 *>(sA + (size_t)v * 8 + 4);
+                            float f[8];
+                            unpack8(q, f);
+                            acc = fmaf(f[0], a0.x, acc); acc = fmaf(f[1], a0.y, acc); acc = fmaf(f[2], a0.z, acc); acc = fmaf(f[3], a0.w, acc);
+                            acc = fmaf(f[4], a1.x, acc); acc = fmaf(f[5], a1.y, acc); acc = fmaf(f[6], a1.z, acc); acc = fmaf(f[7], a1.w, acc);
+                        }
+                    } else {
+                        const __nv_bfloat16 *wr = w2 + (size_t)sTok[m] * r;
+                        for (int v = q4; v < nvec; v += 4) {
+                            const uint4 q = ld_ro_v4(wr + (size_t)v * 8);
+                            const float *sp = sA + (size_t)v * 8;
+                            float f[8];
+                            unpack8(q, f);
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                const float og = __shfl_xor_sync(0xffffffffu, bg, o);
-                const unsigned long long otp = __shfl_xor_sync(0xffffffffu, btp, o);
-                const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-                if (oi >= 0 && (bi < 0 || og > bg || (og == bg && otp < btp))) { bg = og; btp = otp; bi = oi; }
-            }
-            if (lane == 0) { sm.redk[warp] = bg; sm.redtp[warp] = btp; sm.redi[warp] = bi; }
-            __syncthreads();
-            if (tid == 0) {
-                for (int w = 0; w < kFusWarps; ++w) {
-                    const float og = sm.redk[w]; const unsigned long long otp = sm.redtp[w]; const int oi = sm.redi[w];
-                    if (oi >= 0 && (bi < 0 || og > bg || (og == bg && otp < btp))) { bg = og; btp = otp; bi = oi; }
+                            for (int i = 0; i < 8; ++i) acc = fmaf(f[i], sp[i], acc);
+                        }
+                    }
+                    acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+                    acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+                    if (q4 == 0 && m < M) sZ[m] = __fdiv_rn((sBase[m] - base0) + acc, e.T_eff);
                 }
-                const int par = (int)(btp & 0xFFFFFFFFull), tok = (int)(btp >> 32);
-                const int dep = nDep[par] + 1;
-                nTok[t + 1] = tok; nPar[t + 1] = par; nDep[t + 1] = dep; nSco[t + 1] = bg;
-                hg[bi] = hg[cnt - 1];
-                htp[bi] = htp[cnt - 1];
-                sm.n_valid = t + 2; sm.cnt = cnt - 1;
-                if (t + 1 < e.B)
-                    p.desc[(size_t)((t + 1) & 1) * batch + b] = make_int2(dep < L ? par + 1 : -1, tok);
             }
             __syncthreads();
-            next_dep = nDep[t + 1];
-        } else {
-            if (tid == 0) {
-                sm.cnt = 0;
-                if (t + 1 < e.B) p.desc[(size_t)((t + 1) & 1) * batch + b] = make_int2(-1, 0);
+            DT_TR(1, p.n_gru, t, 2);
+            // slice log-softmax (reading A1): every warp reduces the whole slice itself (no CTA barrier)
+            float zmax = -INFINITY;
+            for (int m = lane; m < M; m += 32) zmax = fmaxf(zmax, sZ[m]);
+            zmax = warp_max(zmax);
+            float ssum = 0.f;
+            for (int m = lane; m < M; m += 32) ssum += expf(sZ[m] - zmax);
+            const float lse = logf(warp_sum(ssum));
+            const float gpar = nSco[t];
+            if (tid < M) {
+                const float lp = (sZ[tid] - zmax) - lse;
+                sKey[tid] = ((unsigned long long)ord_key(lp) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned int)sTok[tid]);
             }
+            __syncthreads();
+            // top-k by (logp desc, token asc): rank by counting, `tpc` lanes per candidate (a power of two <= 8,
+            // lanes of one candidate are neighbours in a warp); the k winners become the new entries
+            {
+                int tpc = 1;
+                while (tpc < 8 && M * tpc * 2 <= kFusThreads) tpc <<= 1;
+                const int m = tid / tpc, part = tid - m * tpc;
+                const bool act = (m < M);
+                const unsigned long long mk = act ? sKey[m] : 0ull;
+                int rank = 0;
+                if (act) {
+                    const int per = (((M + tpc - 1) / tpc) + 1) & ~1;                // even, so 16-byte loads stay aligned
+                    const int m0 = part * per, m1 = min(M, m0 + per);
+                    int q = m0;
+                    for (; q + 2 <= m1; q += 2) {
+                        const ulonglong2 o = *reinterpret_cast<const ulonglong2 *>(sKey + q);
+                        rank += (o.x > mk) + (o.y > mk);
+                    }
+                    if (q < m1) rank += (sKey[q] > mk);
+                }
+                for (int o = 1; o < tpc; o <<= 1) rank += __shfl_xor_sync(0xffffffffu, rank, o);
+                if (act && part == 0 && rank < k) {
+                    const float lpm = (sZ[m] - zmax) - lse;
+                    nHi[rank] = ord_key(gpar + lpm);
+                    nLo[rank] = ((unsigned long long)(0xFFFFFFFFu - (unsigned int)sTok[m]) << 32) |
+                                (unsigned long long)(0xFFFFFFFFu - (unsigned int)t);
+                }
+            }
+            n_new = k;
+            __syncthreads();
+            DT_TR(1, p.n_gru, t, 3);
         }
-        if (t + 1 < e.B) {
-            cta_signal_counter(&p.sync[0]);
-            if (next_dep < L) stage_depth(next_dep);   // overlaps the GRU CTAs' step t+1
-            else __syncthreads();
+        // merge the new entries into the sorted frontier (other buffer), truncated to the pops that remain
+        const int cap = B - t;                                  // pops still to do, this one included
+        int tot = n_front + n_new;
+        if (tot > 0) {
+            if (tid < n_front) {
+                const unsigned int h = oHi[tid]; const unsigned long long l = oLo[tid];
+                int c = 0;
+                for (int j = 0; j < n_new; ++j) c += front_gt(nHi[j], nLo[j], h, l);
+                const int pos = tid + c;
+                if (pos < cap) { wHi[pos] = h; wLo[pos] = l; }
+            }
+            if (tid >= kFusThreads - n_new) {                   // the last n_new threads place the new entries
+                const int j = tid - (kFusThreads - n_new);
+                const unsigned int h = nHi[j]; const unsigned long long l = nLo[j];
+                int c = 0;
+                for (int j2 = 0; j2 < n_new; ++j2) c += front_gt(nHi[j2], nLo[j2], h, l);
+                int lo = 0, hi = n_front;                        // first old entry that does not beat (h, l)
+                while (lo < hi) {
+                    const int mid = (lo + hi) >> 1;
+                    if (front_gt(oHi[mid], oLo[mid], h, l)) lo = mid + 1; else hi = mid;
+                }
+                const int pos = lo + c;
+                if (pos < cap) { wHi[pos] = h; wLo[pos] = l; }
+            }
+            if (tot > cap) tot = cap;
         }
+        __syncthreads();
+        // pop entry 0 into slot t+1; the live frontier becomes entries 1..tot-1 of the other buffer
+        int next_dep = L;                                       // depth of the node popped now (L = none / leaf)
+        if (tot > 0) {
+            const unsigned int h = wHi[0]; const unsigned long long l = wLo[0];
+            const int tok = (int)(0xFFFFFFFFu - (unsigned int)(l >> 32));
+            const int par = (int)(0xFFFFFFFFu - (unsigned int)(l & 0xFFFFFFFFull));
+            const int dep = nDep[par] + 1;
+            next_dep = dep;
+            if (tid == 0) {
+                if (t + 1 < B) {
+                    __threadfence();
+                    st_relaxed_u64(p.desc + b, fused_desc_pack(t + 2, dep < L ? par + 1 : -1, tok));
+                }
+                nTok[t + 1] = tok; nPar[t + 1] = par; nDep[t + 1] = dep; nSco[t + 1] = ord_key_inv(h);
+                sm.n_valid = t + 2; sm.n_front = tot - 1; sm.cur = cur ^ 1;
+            }
+        } else if (tid == 0) {
+            sm.n_front = 0;
+            if (t + 1 < B) { __threadfence(); st_relaxed_u64(p.desc + b, fused_desc_pack(t + 2, -1, 0)); }
+        }
+        DT_TR(1, p.n_gru, t, 4);
+        __syncthreads();
+        if (t + 1 < B && next_dep < L) stage_depth(next_dep);   // overlaps the GRU CTAs' step t+1
+        DT_TR(1, p.n_gru, t, 5);
     }
     __syncthreads();
 
