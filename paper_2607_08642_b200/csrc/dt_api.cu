@@ -35,7 +35,7 @@ struct dt_handle {
     // fused persistent expansion (bf16): state copies, split-K partials, hand-over words
     __nv_bfloat16 *s_hi, *s_lo; float *partial; unsigned long long *desc; unsigned int *flags;
     int fused_ok, max_smem_optin;
-    int64_t opt_expand_path;        // 0 auto, 1 per-step kernels, 2 fused upc=8, 3 fused upc=16
+    int64_t opt_expand_path;        // 0 auto, 1 per-step kernels, 2 fused mma.sync upc=8, 3 fused mma.sync upc=16, 4 fused tcgen05
     // host-call staging (lazy)
     char *stage; size_t stage_bytes;
     // options / bookkeeping
@@ -115,7 +115,7 @@ extern "C" int64_t dt_kernel_launches(const dt_handle *h) { return h ? h->launch
 extern "C" int dt_set_option(dt_handle *h, const char *name, int64_t value) {
     if (!h || !name) return DT_ERR_INVALID_ARG;
     if (!strcmp(name, "expand_path")) {
-        if (value < 0 || value > 3) return DT_ERR_INVALID_ARG;
+        if (value < 0 || value > 4) return DT_ERR_INVALID_ARG;
         h->opt_expand_path = value;
         return DT_OK;
     }
@@ -240,7 +240,8 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         h->max_smem_optin -= 1024;                  // room for the kernels' static shared memory
         if (!ok ||
             cudaFuncSetAttribute(fused_expand_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->max_smem_optin) != cudaSuccess ||
-            cudaFuncSetAttribute(fused_expand_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->max_smem_optin) != cudaSuccess) {
+            cudaFuncSetAttribute(fused_expand_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->max_smem_optin) != cudaSuccess ||
+            cudaFuncSetAttribute(fused_expand_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->max_smem_optin) != cudaSuccess) {
             cudaGetLastError(); h->fused_ok = 0;
         }
     }
@@ -340,7 +341,17 @@ extern "C" int dt_select_topm(dt_handle *h, const void *logits, int32_t rows, in
 static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st) {
     if (!h->fused_ok || h->opt_expand_path == 1) return 1;
     int upc = 0;
-    for (int cand : {16, 8}) {      // batch-independent preference => batch-invariant results
+    bool tcgen = false;
+    // tcgen05 + TMEM GRU CTAs (16 units each) whenever the shape allows; the choice never depends on the batch
+    // beyond fitting on the chip, so results stay batch-invariant
+    if ((h->opt_expand_path == 0 || h->opt_expand_path == 4) && p.g % kTcKC == 0 && p.r % 8 == 0 && p.r <= 256 &&
+        p.g / kTcUPC + p.batch <= h->num_sms && p.g / kTcUPC <= 256 && (size_t)16 * p.g * 2 <= (size_t)kTcSlots * kTcSlotBytes &&
+        fused_tc_smem(p.g, p.r) <= (size_t)h->max_smem_optin) {
+        tcgen = true; upc = kTcUPC;
+    }
+    if (h->opt_expand_path == 4 && !tcgen) return 1;
+    for (int cand : {16, 8}) {      // mma.sync fallback; batch-independent preference => batch-invariant results
+        if (tcgen) break;
         if (h->opt_expand_path == 2 && cand != 8) continue;
         if (h->opt_expand_path == 3 && cand != 16) continue;
         if (p.g % cand) continue;
@@ -360,7 +371,7 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st) {
     size_t rs = fused_req_smem(p.r, p.M, p.N, p.k, 1);
     if (rs > (size_t)h->max_smem_optin) { f.w2_smem = 0; rs = fused_req_smem(p.r, p.M, p.N, p.k, 0); }
     if (rs > (size_t)h->max_smem_optin) return 1;
-    const size_t gs = fused_gru_smem(p.g, p.r, upc, f.m_tiles);
+    const size_t gs = tcgen ? fused_tc_smem(p.g, p.r) : fused_gru_smem(p.g, p.r, upc, f.m_tiles);
     const size_t dsm = gs > rs ? gs : rs;
     fused_init_kernel<<<((p.batch > f.n_gru ? p.batch : f.n_gru) + 127) / 128, 128, 0, st>>>(f);
     h->launches++;
@@ -368,9 +379,9 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st) {
     if (rc) return rc;
     void *args[] = {&f};
     const dim3 grid(f.n_gru + p.batch), block(kFusThreads);
-    cudaError_t e = (upc == 8)
-        ? cudaLaunchCooperativeKernel((const void *)fused_expand_kernel<8>, grid, block, args, dsm, st)
-        : cudaLaunchCooperativeKernel((const void *)fused_expand_kernel<16>, grid, block, args, dsm, st);
+    cudaError_t e = tcgen ? cudaLaunchCooperativeKernel((const void *)fused_expand_kernel<0>, grid, block, args, dsm, st)
+                  : (upc == 8) ? cudaLaunchCooperativeKernel((const void *)fused_expand_kernel<8>, grid, block, args, dsm, st)
+                               : cudaLaunchCooperativeKernel((const void *)fused_expand_kernel<16>, grid, block, args, dsm, st);
     h->launches++;
     DT_CUDA(h, e);
     if ((rc = phase_mark(h, 3, st))) return rc;

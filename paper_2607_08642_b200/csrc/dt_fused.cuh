@@ -29,6 +29,7 @@
 #pragma once
 #include "dt_expand.cuh"
 #include "dt_gemm_mma.cuh"
+#include "dt_tcgen05.cuh"
 
 namespace dt {
 
@@ -62,7 +63,10 @@ __device__ __forceinline__ unsigned long long dt_globaltimer() {
     unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
 }
 #define DT_TR(role, first_cta, t, i) do { if (threadIdx.x == 0 && (int)blockIdx.x == (first_cta)) g_dt_trace[role][t][i] = dt_globaltimer(); } while (0)
+// fine-grained stamps of GRU CTA 0 at step 5: rows 200.. of role 0
+#define DT_TRF(t, i) do { if (threadIdx.x == 0 && blockIdx.x == 0 && (t) == 5) g_dt_trace[0][200 + (i) / 8][(i) % 8] = dt_globaltimer(); } while (0)
 #else
+#define DT_TRF(t, i) do { } while (0)
 #define DT_TR(role, first_cta, t, i) do { } while (0)
 #endif
 
@@ -361,6 +365,253 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
     }
 }
 
+// ------------------------------------------------------------------------- GRU role, tcgen05 + TMEM
+// Same work as fused_gru_role<16>, on the 5th-generation tensor cores: legacy mma.sync runs at about
+// 256 MAC/clk/SM on B200 (measured, profiles/), which made the 3072 x 1024 x 64 hidden half 6 us per
+// step; tcgen05.mma does it in ~1 us.  One CTA owns 16 GRU units = 48 rows of W_hh (M = 64 tile, rows
+// 48..63 are phantom and ignored), N = 64 columns per pass (32 requests x {bf16 hi, bf16 lo} of the
+// parent state), K = g streamed in 128-wide chunks through a 6-slot cp.async ring.  The accumulator
+// lives in TMEM; a second, tiny tcgen05 GEMM [r x 16] x [16 x 64] gives this CTA's split-K share of
+// W1[:, d:] S_t.  Operand layout: K-major core matrices, no swizzle (dt_tcgen05.cuh).
+constexpr int kTcUPC = 16;
+constexpr int kTcKC = 128;            // k per ring slot
+constexpr int kTcSlots = 6;
+constexpr int kTcSlotBytes = 64 * kTcKC * 2;          // 64 columns x 128 k bf16 = 16 KB
+constexpr int kTcCols = 256;          // TMEM columns: D1 [0,64), D2 tiles at 64 and 128
+
+__host__ __device__ inline size_t fused_tc_smem(int g, int r) {
+    const size_t a = (size_t)48 * g * 2;                              // W_hh slice as core matrices
+    const size_t ring = (size_t)kTcSlots * kTcSlotBytes;              // must cover the phantom rows: >= 16 * g * 2
+    const size_t a2 = (size_t)((r + 127) / 128) * 128 * 32;           // W1[:, d + u0 ..] slice [r_pad x 16] bf16
+    const size_t b2 = 64 * 32;                                        // new states [64 cols x 16] bf16
+    const size_t sh = 48 * 33 * 4;                                    // hidden-half pre-activations
+    return a + ring + a2 + b2 + sh + 3 * kFusChunk * 4 + 8 * 8 + 64 + 1024;
+}
+
+__device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned char *smem_raw) {
+    constexpr int UPC = kTcUPC;
+    constexpr int PP = UPC * kFusChunk / kFusThreads;          // (unit, request) pairs per thread = 2
+    const ExpandParams &e = p.e;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int g = e.g, r = e.r, batch = e.batch;
+    const int cta = blockIdx.x, u0 = cta * UPC;
+    const size_t stride = (size_t)p.slot_stride;
+    const int n_kc = g / kTcKC;                                // ring chunks per pass
+    const int m2_tiles = (r + 127) / 128;
+
+    // carve (smem_raw is 1024-byte aligned by the kernel)
+    unsigned char *sA = smem_raw;                                             // 6 row groups x (g/8 chunks x 128 B)
+    const uint32_t sboA = (uint32_t)g * 16;                                   // bytes between 8-row groups
+    unsigned char *sRing = sA + (size_t)48 * g * 2;
+    unsigned char *sA2 = sRing + (size_t)kTcSlots * kTcSlotBytes;             // [r_pad/8 groups][2 chunks][8 rows][16 B]
+    unsigned char *sB2 = sA2 + (size_t)m2_tiles * 128 * 32;                   // [8 groups][2 chunks][8 cols][16 B]
+    float *sH = reinterpret_cast<float *>(sB2 + 64 * 32);                     // [48][33]
+    int *sIdx = reinterpret_cast<int *>(sH + 48 * 33);
+    int *sTok = sIdx + kFusChunk;
+    unsigned long long *mbar = reinterpret_cast<unsigned long long *>(sTok + 2 * kFusChunk);   // [0],[1] slot free, [2] D1, [3] D2
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(mbar + 8);
+
+    // resident weights in core-matrix layout
+    {
+        const __nv_bfloat16 *whh = reinterpret_cast<const __nv_bfloat16 *>(e.w_hh);
+        const int vpr = g / 8;
+        for (int i = tid; i < 48 * vpr; i += kFusThreads) {
+            const int m = i / vpr, c = i - m * vpr;                // local row m = gate * 16 + ul, k-chunk c
+            const int gate = m >> 4, ul = m & 15;
+            const uint4 q = ld_ro_v4(whh + ((size_t)gate * g + u0 + ul) * g + (size_t)c * 8);
+            *reinterpret_cast<uint4 *>(sA + (size_t)(m >> 3) * sboA + (size_t)c * 128 + (m & 7) * 16) = q;
+        }
+        const __nv_bfloat16 *w1 = reinterpret_cast<const __nv_bfloat16 *>(e.w1);
+        for (int i = tid; i < m2_tiles * 128 * 16; i += kFusThreads) {
+            const int j = i >> 4, ul = i & 15;
+            const __nv_bfloat16 v = (j < r) ? w1[(size_t)j * (e.d + g) + e.d + u0 + ul] : __float2bfloat16_rn(0.f);
+            *reinterpret_cast<__nv_bfloat16 *>(sA2 + (size_t)(j >> 3) * 256 + (ul >> 3) * 128 + (j & 7) * 16 + (ul & 7) * 2) = v;
+        }
+        if (tid == 0) {
+            for (int i = 0; i < 4; ++i) tc::mbar_init(tc::smem_u32(mbar + i), 1);
+            tc::mbar_init_fence();
+        }
+        if (warp == 0) tc::tmem_alloc<kTcCols>(tmem_slot);
+    }
+    tc::fence_proxy_async();
+    tc::fence_before_sync();
+    __syncthreads();
+    tc::fence_after_sync();
+    const uint32_t tmem = *tmem_slot;
+    const uint32_t idesc1 = tc::make_idesc_bf16(64, 64), idesc2 = tc::make_idesc_bf16(128, 64);
+    const uint32_t aA = tc::smem_u32(sA), aRing = tc::smem_u32(sRing), aA2 = tc::smem_u32(sA2), aB2 = tc::smem_u32(sB2);
+    const uint32_t mb0 = tc::smem_u32(mbar);
+    const uint64_t descA0 = tc::make_desc(aA, 128, sboA), descB0 = tc::make_desc(aRing, 128, kTcKC * 16);
+    uint32_t ph_free = 0, ph_d1 = 0, ph_d2 = 0;                 // mbarrier phases (uniform across the CTA)
+
+    // this thread's share of one ring slot: 4 pieces of 16 B = columns n = 8 * (2 i + tid / 128) + tid % 8, k-chunk (tid / 8) % 16
+    const int my_n0 = tid & 7, my_cl = (tid >> 3) & 15, my_nh = tid >> 7;
+
+    for (int t = 0; t < e.B; ++t) {
+        for (int c0 = 0; c0 < batch; c0 += kFusChunk) {
+            const int nb = min(kFusChunk, batch - c0);
+            if (warp == 0) {
+                int sidx = -1, tok = 0;
+                if (lane < nb) {
+                    unsigned long long dsc;
+                    do { dsc = ld_relaxed_u64(p.desc + c0 + lane); } while ((int)(dsc >> 48) != t + 1);
+                    sidx = (int)((dsc >> 32) & 0xFFFFu) - 1;
+                    tok = (int)(dsc & 0xFFFFFFFFull);
+                }
+                __threadfence();
+                sIdx[lane] = sidx; sTok[lane] = tok;
+            }
+            __syncthreads();
+            if (c0 == 0) DT_TR(0, 0, t, 0);
+
+            // source rows of this thread's four ring pieces (column n < 32: hi of request n, else lo of request n - 32)
+            const __nv_bfloat16 *src[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int n = 8 * (2 * i + my_nh) + my_n0;
+                const int sidx = sIdx[n & 31];
+                const size_t off = (sidx > 0) ? ((size_t)(c0 + (n & 31)) * stride + sidx) * g : 0;   // 0 = zero slot
+                src[i] = ((n >> 5) ? p.s_lo : p.s_hi) + off + (size_t)my_cl * 8;
+            }
+            DT_TRF(t, 40);
+            auto issue_chunk = [&](int kc) {
+                unsigned char *dst = sRing + (size_t)(kc % kTcSlots) * kTcSlotBytes + (size_t)my_cl * 128 + my_n0 * 16;
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    cp_async16(dst + (size_t)(2 * i + my_nh) * (kTcKC * 16), src[i] + (size_t)kc * kTcKC);
+            };
+#pragma unroll 1
+            for (int kc = 0; kc < kTcSlots; ++kc) { if (kc < n_kc) issue_chunk(kc); cp_async_commit(); }
+            DT_TRF(t, 41);
+
+            // epilogue operands (input half from P, previous state): issued now, consumed after the MMAs
+            float pr[PP], pz[PP], pn[PP], hp[PP];
+#pragma unroll
+            for (int i = 0; i < PP; ++i) {
+                const int idx = tid + i * kFusThreads, ul = idx >> 5, bl = idx & 31;
+                const int sidx = sIdx[bl];
+                pr[i] = pz[i] = pn[i] = hp[i] = 0.f;
+#ifndef DT_EXP_NOP
+                if (sidx >= 0) {
+                    const float *prow = e.P + (size_t)sTok[bl] * 3 * g + u0 + ul;
+                    pr[i] = __ldg(prow); pz[i] = __ldg(prow + g); pn[i] = __ldg(prow + 2 * g);
+                    if (sidx > 0) hp[i] = __ldcg(p.s32 + ((size_t)(c0 + bl) * stride + sidx) * g + u0 + ul);
+                }
+#endif
+            }
+
+            DT_TRF(t, 42);
+            // hidden half: D1[64 x 64] = W_hh slice [64 x g] . [S_hi | S_lo]^T, K streamed through the ring
+#pragma unroll 1
+            for (int kc = 0; kc < n_kc; ++kc) {
+                DT_TRF(t, kc * 5 + 0);
+                cp_async_wait<kTcSlots - 1>();
+                DT_TRF(t, kc * 5 + 1);
+                tc::fence_proxy_async();
+                DT_TRF(t, kc * 5 + 2);
+                __syncthreads();
+                DT_TRF(t, kc * 5 + 3);
+                if (tid == 0) {
+                    tc::fence_after_sync();
+                    // descriptors advance by 256 B (two core matrices) per K = 16 step: +16 in the address field
+                    const uint64_t da = descA0 + (uint64_t)(kc * (kTcKC / 16) * 16);
+                    const uint64_t db = descB0 + (uint64_t)((kc % kTcSlots) * (kTcSlotBytes / 16));
+#pragma unroll
+                    for (int s8 = 0; s8 < kTcKC / 16; ++s8)
+                        tc::mma_bf16(tmem, da + (uint64_t)(s8 * 16), db + (uint64_t)(s8 * 16), idesc1, (kc | s8) ? 1u : 0u);
+                    if (kc + kTcSlots < n_kc) tc::commit(mb0 + 8 * (kc & 1));       // this slot is refilled below
+                    if (kc == n_kc - 1) tc::commit(mb0 + 16);
+                }
+                DT_TRF(t, kc * 5 + 4);
+                if (kc + kTcSlots < n_kc) {                  // refill the slot once its MMAs have read it
+                    tc::mbar_wait(mb0 + 8 * (kc & 1), (ph_free >> (kc & 1)) & 1u);
+                    ph_free ^= 1u << (kc & 1);
+                    issue_chunk(kc + kTcSlots);
+                }
+                cp_async_commit();
+            }
+            cp_async_wait<0>();
+            DT_TRF(t, 43);
+            tc::mbar_wait(mb0 + 16, ph_d1); ph_d1 ^= 1u;
+            DT_TRF(t, 44);
+            tc::fence_after_sync();
+            if (c0 == 0) DT_TR(0, 0, t, 1);
+            // TMEM -> shared: row m = 16 w + i sits in lane 32 w + i (i < 16) for an M = 64 accumulator
+            __syncwarp();
+            if (warp < 3) {
+                float vh[32], vl[32];
+                tc::tmem_ld32(tmem + ((uint32_t)(32 * warp) << 16), vh);
+                tc::tmem_ld32(tmem + ((uint32_t)(32 * warp) << 16) + 32, vl);
+                if (lane < 16) {
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) sH[(16 * warp + lane) * 33 + c] = vh[c] + vl[c];
+                }
+            }
+            tc::fence_before_sync();
+            __syncthreads();
+            if (c0 == 0) DT_TR(0, 0, t, 2);
+            // gates (reading A2): rows ul, 16 + ul, 32 + ul are the r, z, n pre-activations of unit ul
+#pragma unroll
+            for (int i = 0; i < PP; ++i) {
+                const int idx = tid + i * kFusThreads, ul = idx >> 5, bl = idx & 31;
+                float hnew = 0.f;
+                if (sIdx[bl] >= 0) {
+                    const float rg = sigmoidf_fast(pr[i] + sH[ul * 33 + bl]);
+                    const float zg = sigmoidf_fast(pz[i] + sH[(16 + ul) * 33 + bl]);
+                    const float ng = tanhf_fast(pn[i] + rg * sH[(32 + ul) * 33 + bl]);
+                    hnew = (1.0f - zg) * ng + zg * hp[i];
+                }
+                const __nv_bfloat16 hi = __float2bfloat16_rn(hnew);
+                const __nv_bfloat16 lo = __float2bfloat16_rn(hnew - __bfloat162float(hi));
+                if (sIdx[bl] >= 0) {                             // publish S_t (slot t+1): fp32 and the bf16 hi/lo split
+                    const size_t o = ((size_t)(c0 + bl) * stride + (t + 1)) * g + u0 + ul;
+                    __stcg(p.s32 + o, hnew);
+                    p.s_hi[o] = hi;
+                    p.s_lo[o] = lo;
+                }
+                // operand B of the W1 GEMM: column bl (hi) and 32 + bl (lo), k = ul
+                unsigned char *q = sB2 + (size_t)(bl >> 3) * 256 + (ul >> 3) * 128 + (bl & 7) * 16 + (ul & 7) * 2;
+                *reinterpret_cast<__nv_bfloat16 *>(q) = hi;
+                *reinterpret_cast<__nv_bfloat16 *>(q + 4 * 256) = lo;
+            }
+            tc::fence_proxy_async();
+            __syncthreads();
+            if (c0 == 0) DT_TR(0, 0, t, 3);
+            // this CTA's split-K share of W1[:, d:] S_t: D2[r x 64] = W1 slice [r x 16] . [S_hi | S_lo]^T
+            if (tid == 0) {
+                tc::fence_after_sync();
+                const uint64_t db = tc::make_desc(aB2, 128, 256);
+                for (int mt = 0; mt < m2_tiles; ++mt)
+                    tc::mma_bf16(tmem + 64 + 64 * mt, tc::make_desc(aA2 + (uint32_t)mt * 4096, 128, 256), db, idesc2, 0u);
+                tc::commit(mb0 + 24);
+            }
+            tc::mbar_wait(mb0 + 24, ph_d2); ph_d2 ^= 1u;
+            tc::fence_after_sync();
+            __syncwarp();
+            for (int mt = warp >> 2; mt < m2_tiles; mt += 2) {
+                float vh[32], vl[32];
+                const uint32_t ta = tmem + ((uint32_t)(32 * (warp & 3)) << 16) + 64 + 64 * mt;
+                tc::tmem_ld32(ta, vh);
+                tc::tmem_ld32(ta + 32, vl);
+                const int j = mt * 128 + 32 * (warp & 3) + lane;
+                if (j < r) {
+                    float *o = p.partial + ((size_t)cta * batch + c0) * r + j;
+#pragma unroll
+                    for (int c = 0; c < 32; ++c)
+                        if (c < nb) __stcg(o + (size_t)c * r, vh[c] + vl[c]);
+                }
+            }
+            tc::fence_before_sync();
+            __syncthreads();
+        }
+        DT_TR(0, 0, t, 4);
+        if (tid == 0) { __threadfence(); st_relaxed_u32(p.flags + cta, (unsigned int)(t + 1)); }
+        DT_TR(0, 0, t, 5);
+    }
+    __syncthreads();
+    if (warp == 0) tc::tmem_free<kTcCols>(tmem);
+}
+
 // -------------------------------------------------------------------------------------- request role
 // Frontier entries are ordered by the pop comparator of reading A8, (g desc, token asc, parent asc),
 // packed so that a larger (hi, lo) pair pops first: hi = ord_key(g), lo = ~token << 32 | ~parent.
@@ -640,9 +891,11 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
 
 template <int UPC>
 __global__ void __launch_bounds__(kFusThreads, 1) fused_expand_kernel(FusedParams p) {
-    extern __shared__ __align__(16) unsigned char fused_smem[];
-    if ((int)blockIdx.x < p.n_gru) fused_gru_role<UPC>(p, fused_smem);
-    else fused_req_role(p, fused_smem);
+    extern __shared__ __align__(1024) unsigned char fused_smem[];
+    if ((int)blockIdx.x < p.n_gru) {
+        if constexpr (UPC == 0) fused_gru_role_tc(p, fused_smem);
+        else fused_gru_role<UPC>(p, fused_smem);
+    } else fused_req_role(p, fused_smem);
 }
 
 }  // namespace dt
