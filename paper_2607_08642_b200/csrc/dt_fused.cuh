@@ -372,19 +372,21 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
 // 48..63 are phantom and ignored), N = 64 columns per pass (32 requests x {bf16 hi, bf16 lo} of the
 // parent state), K = g streamed in 128-wide chunks through a 6-slot cp.async ring.  The accumulator
 // lives in TMEM; a second, tiny tcgen05 GEMM [r x 16] x [16 x 64] gives this CTA's split-K share of
-// W1[:, d:] S_t.  Operand layout: K-major core matrices, no swizzle (dt_tcgen05.cuh).
+// W1[:, d:] S_t.  Operand layout of the big GEMM: K-major, 128-byte swizzle (a warp-wide cp.async moves four whole
+// 128-byte state rows and lands conflict-free); the tiny one uses unswizzled core matrices (dt_tcgen05.cuh).
 constexpr int kTcUPC = 16;
-constexpr int kTcKC = 128;            // k per ring slot
-constexpr int kTcSlots = 6;
-constexpr int kTcSlotBytes = 64 * kTcKC * 2;          // 64 columns x 128 k bf16 = 16 KB
-constexpr int kTcCols = 256;          // TMEM columns: D1 [0,64), D2 tiles at 64 and 128
+constexpr int kTcKC = 256;            // k per ring slot = four 64-wide swizzle blocks, one per issuing warp
+constexpr int kTcSlots = 3;
+constexpr int kTcSlotBytes = 64 * kTcKC * 2;          // 64 columns x 256 k bf16 = 32 KB
+constexpr int kTcIssuers = 4;         // warps 0..3 each issue the MMAs of one k-block into their own accumulator
+constexpr int kTcCols = 512;          // TMEM columns: D1[w] at 64 w (w < 4), D2 tiles at 256 and 320
 
 __host__ __device__ inline size_t fused_tc_smem(int g, int r) {
     const size_t a = (size_t)48 * g * 2;                              // W_hh slice as core matrices
     const size_t ring = (size_t)kTcSlots * kTcSlotBytes;              // must cover the phantom rows: >= 16 * g * 2
     const size_t a2 = (size_t)((r + 127) / 128) * 128 * 32;           // W1[:, d + u0 ..] slice [r_pad x 16] bf16
     const size_t b2 = 64 * 32;                                        // new states [64 cols x 16] bf16
-    const size_t sh = 48 * 33 * 4;                                    // hidden-half pre-activations
+    const size_t sh = 48 * 34 * 4;                                    // hidden-half pre-activations
     return a + ring + a2 + b2 + sh + 3 * kFusChunk * 4 + 8 * 8 + 64 + 1024;
 }
 
@@ -400,13 +402,13 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
     const int m2_tiles = (r + 127) / 128;
 
     // carve (smem_raw is 1024-byte aligned by the kernel)
-    unsigned char *sA = smem_raw;                                             // 6 row groups x (g/8 chunks x 128 B)
+    unsigned char *sA = smem_raw;                                             // 6 row groups x (g/64 swizzle atoms of 1 KB)
     const uint32_t sboA = (uint32_t)g * 16;                                   // bytes between 8-row groups
     unsigned char *sRing = sA + (size_t)48 * g * 2;
     unsigned char *sA2 = sRing + (size_t)kTcSlots * kTcSlotBytes;             // [r_pad/8 groups][2 chunks][8 rows][16 B]
     unsigned char *sB2 = sA2 + (size_t)m2_tiles * 128 * 32;                   // [8 groups][2 chunks][8 cols][16 B]
-    float *sH = reinterpret_cast<float *>(sB2 + 64 * 32);                     // [48][33]
-    int *sIdx = reinterpret_cast<int *>(sH + 48 * 33);
+    float *sH = reinterpret_cast<float *>(sB2 + 64 * 32);                     // [48][34]
+    int *sIdx = reinterpret_cast<int *>(sH + 48 * 34);
     int *sTok = sIdx + kFusChunk;
     unsigned long long *mbar = reinterpret_cast<unsigned long long *>(sTok + 2 * kFusChunk);   // [0],[1] slot free, [2] D1, [3] D2
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(mbar + 8);
@@ -419,7 +421,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             const int m = i / vpr, c = i - m * vpr;                // local row m = gate * 16 + ul, k-chunk c
             const int gate = m >> 4, ul = m & 15;
             const uint4 q = ld_ro_v4(whh + ((size_t)gate * g + u0 + ul) * g + (size_t)c * 8);
-            *reinterpret_cast<uint4 *>(sA + (size_t)(m >> 3) * sboA + (size_t)c * 128 + (m & 7) * 16) = q;
+            *reinterpret_cast<uint4 *>(sA + (size_t)(m >> 3) * sboA + (size_t)(c >> 3) * 1024 + (m & 7) * 128 + (((c & 7) ^ (m & 7)) << 4)) = q;
         }
         const __nv_bfloat16 *w1 = reinterpret_cast<const __nv_bfloat16 *>(e.w1);
         for (int i = tid; i < m2_tiles * 128 * 16; i += kFusThreads) {
@@ -428,7 +430,10 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             *reinterpret_cast<__nv_bfloat16 *>(sA2 + (size_t)(j >> 3) * 256 + (ul >> 3) * 128 + (j & 7) * 16 + (ul & 7) * 2) = v;
         }
         if (tid == 0) {
-            for (int i = 0; i < 4; ++i) tc::mbar_init(tc::smem_u32(mbar + i), 1);
+            tc::mbar_init(tc::smem_u32(mbar + 0), kTcIssuers);      // slot free
+            tc::mbar_init(tc::smem_u32(mbar + 1), kTcIssuers);
+            tc::mbar_init(tc::smem_u32(mbar + 2), kTcIssuers);      // D1 complete (one commit per issuing warp)
+            tc::mbar_init(tc::smem_u32(mbar + 3), 1);               // D2 complete
             tc::mbar_init_fence();
         }
         if (warp == 0) tc::tmem_alloc<kTcCols>(tmem_slot);
@@ -441,11 +446,13 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
     const uint32_t idesc1 = tc::make_idesc_bf16(64, 64), idesc2 = tc::make_idesc_bf16(128, 64);
     const uint32_t aA = tc::smem_u32(sA), aRing = tc::smem_u32(sRing), aA2 = tc::smem_u32(sA2), aB2 = tc::smem_u32(sB2);
     const uint32_t mb0 = tc::smem_u32(mbar);
-    const uint64_t descA0 = tc::make_desc(aA, 128, sboA), descB0 = tc::make_desc(aRing, 128, kTcKC * 16);
+    const uint64_t descA0 = tc::make_desc_sw128(aA, sboA), descB0 = tc::make_desc_sw128(aRing, 1024);
     uint32_t ph_free = 0, ph_d1 = 0, ph_d2 = 0;                 // mbarrier phases (uniform across the CTA)
 
-    // this thread's share of one ring slot: 4 pieces of 16 B = columns n = 8 * (2 i + tid / 128) + tid % 8, k-chunk (tid / 8) % 16
-    const int my_n0 = tid & 7, my_cl = (tid >> 3) & 15, my_nh = tid >> 7;
+    // this thread's share of one ring slot: the 16-byte piece `my_c` of the 128-byte rows of request `my_rq`
+    // (hi and lo, both 64-wide k-blocks of the slot); a warp instruction moves 4 whole 128-byte rows
+    const int my_c = tid & 7, my_rq = tid >> 3;
+    const uint32_t my_dst = (uint32_t)((my_rq >> 3) * 1024 + (my_rq & 7) * 128 + ((my_c ^ (my_rq & 7)) << 4));
 
     for (int t = 0; t < e.B; ++t) {
         for (int c0 = 0; c0 < batch; c0 += kFusChunk) {
@@ -464,21 +471,19 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             __syncthreads();
             if (c0 == 0) DT_TR(0, 0, t, 0);
 
-            // source rows of this thread's four ring pieces (column n < 32: hi of request n, else lo of request n - 32)
-            const __nv_bfloat16 *src[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const int n = 8 * (2 * i + my_nh) + my_n0;
-                const int sidx = sIdx[n & 31];
-                const size_t off = (sidx > 0) ? ((size_t)(c0 + (n & 31)) * stride + sidx) * g : 0;   // 0 = zero slot
-                src[i] = ((n >> 5) ? p.s_lo : p.s_hi) + off + (size_t)my_cl * 8;
-            }
+            // source rows of this thread's ring pieces (column n < 32: hi of request n, else lo of request n - 32)
+            const int my_sidx = sIdx[my_rq];
+            const size_t my_off = (my_sidx > 0) ? ((size_t)(c0 + my_rq) * stride + my_sidx) * g : 0;   // 0 = zero slot
+            const __nv_bfloat16 *src_hi = p.s_hi + my_off + (size_t)my_c * 8, *src_lo = p.s_lo + my_off + (size_t)my_c * 8;
             DT_TRF(t, 40);
             auto issue_chunk = [&](int kc) {
-                unsigned char *dst = sRing + (size_t)(kc % kTcSlots) * kTcSlotBytes + (size_t)my_cl * 128 + my_n0 * 16;
+                unsigned char *dst = sRing + (size_t)(kc % kTcSlots) * kTcSlotBytes + my_dst;
+                const size_t k0 = (size_t)kc * kTcKC;
 #pragma unroll
-                for (int i = 0; i < 4; ++i)
-                    cp_async16(dst + (size_t)(2 * i + my_nh) * (kTcKC * 16), src[i] + (size_t)kc * kTcKC);
+                for (int kb = 0; kb < kTcKC / 64; ++kb) {           // per k-block: columns 0..31 = hi, 32..63 = lo (+4 atoms)
+                    cp_async16(dst + kb * 8192, src_hi + k0 + kb * 64);
+                    cp_async16(dst + kb * 8192 + 4096, src_lo + k0 + kb * 64);
+                }
             };
 #pragma unroll 1
             for (int kc = 0; kc < kTcSlots; ++kc) { if (kc < n_kc) issue_chunk(kc); cp_async_commit(); }
@@ -488,7 +493,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             float pr[PP], pz[PP], pn[PP], hp[PP];
 #pragma unroll
             for (int i = 0; i < PP; ++i) {
-                const int idx = tid + i * kFusThreads, ul = idx >> 5, bl = idx & 31;
+                const int idx = tid + i * kFusThreads, ul = idx & 15, bl = idx >> 4;   // lanes along the units: 64 B per row
                 const int sidx = sIdx[bl];
                 pr[i] = pz[i] = pn[i] = hp[i] = 0.f;
 #ifndef DT_EXP_NOP
@@ -511,14 +516,15 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                 DT_TRF(t, kc * 5 + 2);
                 __syncthreads();
                 DT_TRF(t, kc * 5 + 3);
-                if (tid == 0) {
+                if (warp < kTcIssuers && lane == 0) {
+                    // warp w issues k-block w of the slot (A: +1 KB per block, B: +8 KB) as four K = 16 steps (+32 B)
+                    // into its own accumulator D1[w]; the epilogue adds the four
                     tc::fence_after_sync();
-                    // descriptors advance by 256 B (two core matrices) per K = 16 step: +16 in the address field
-                    const uint64_t da = descA0 + (uint64_t)(kc * (kTcKC / 16) * 16);
-                    const uint64_t db = descB0 + (uint64_t)((kc % kTcSlots) * (kTcSlotBytes / 16));
+                    const uint64_t da = descA0 + (uint64_t)((kc * (kTcKC / 64) + warp) * 64);
+                    const uint64_t db = descB0 + (uint64_t)((kc % kTcSlots) * (kTcSlotBytes / 16) + warp * 512);
 #pragma unroll
-                    for (int s8 = 0; s8 < kTcKC / 16; ++s8)
-                        tc::mma_bf16(tmem, da + (uint64_t)(s8 * 16), db + (uint64_t)(s8 * 16), idesc1, (kc | s8) ? 1u : 0u);
+                    for (int s4 = 0; s4 < 4; ++s4)
+                        tc::mma_bf16(tmem + 64 * warp, da + (uint64_t)(s4 * 2), db + (uint64_t)(s4 * 2), idesc1, (kc | s4) ? 1u : 0u);
                     if (kc + kTcSlots < n_kc) tc::commit(mb0 + 8 * (kc & 1));       // this slot is refilled below
                     if (kc == n_kc - 1) tc::commit(mb0 + 16);
                 }
@@ -539,12 +545,18 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             // TMEM -> shared: row m = 16 w + i sits in lane 32 w + i (i < 16) for an M = 64 accumulator
             __syncwarp();
             if (warp < 3) {
-                float vh[32], vl[32];
-                tc::tmem_ld32(tmem + ((uint32_t)(32 * warp) << 16), vh);
-                tc::tmem_ld32(tmem + ((uint32_t)(32 * warp) << 16) + 32, vl);
+                float acc[32], v[32];
+#pragma unroll
+                for (int c = 0; c < 32; ++c) acc[c] = 0.f;
+#pragma unroll
+                for (int q = 0; q < 2 * kTcIssuers; ++q) {       // four accumulators x {hi, lo} column halves
+                    tc::tmem_ld32(tmem + ((uint32_t)(32 * warp) << 16) + 32 * q, v);
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) acc[c] += v[c];
+                }
                 if (lane < 16) {
 #pragma unroll
-                    for (int c = 0; c < 32; ++c) sH[(16 * warp + lane) * 33 + c] = vh[c] + vl[c];
+                    for (int c = 0; c < 32; ++c) sH[(16 * warp + lane) * 34 + c] = acc[c];
                 }
             }
             tc::fence_before_sync();
@@ -553,12 +565,12 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             // gates (reading A2): rows ul, 16 + ul, 32 + ul are the r, z, n pre-activations of unit ul
 #pragma unroll
             for (int i = 0; i < PP; ++i) {
-                const int idx = tid + i * kFusThreads, ul = idx >> 5, bl = idx & 31;
+                const int idx = tid + i * kFusThreads, ul = idx & 15, bl = idx >> 4;
                 float hnew = 0.f;
                 if (sIdx[bl] >= 0) {
-                    const float rg = sigmoidf_fast(pr[i] + sH[ul * 33 + bl]);
-                    const float zg = sigmoidf_fast(pz[i] + sH[(16 + ul) * 33 + bl]);
-                    const float ng = tanhf_fast(pn[i] + rg * sH[(32 + ul) * 33 + bl]);
+                    const float rg = sigmoidf_fast(pr[i] + sH[ul * 34 + bl]);
+                    const float zg = sigmoidf_fast(pz[i] + sH[(16 + ul) * 34 + bl]);
+                    const float ng = tanhf_fast(pn[i] + rg * sH[(32 + ul) * 34 + bl]);
                     hnew = (1.0f - zg) * ng + zg * hp[i];
                 }
                 const __nv_bfloat16 hi = __float2bfloat16_rn(hnew);
@@ -582,7 +594,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                 tc::fence_after_sync();
                 const uint64_t db = tc::make_desc(aB2, 128, 256);
                 for (int mt = 0; mt < m2_tiles; ++mt)
-                    tc::mma_bf16(tmem + 64 + 64 * mt, tc::make_desc(aA2 + (uint32_t)mt * 4096, 128, 256), db, idesc2, 0u);
+                    tc::mma_bf16(tmem + 256 + 64 * mt, tc::make_desc(aA2 + (uint32_t)mt * 4096, 128, 256), db, idesc2, 0u);
                 tc::commit(mb0 + 24);
             }
             tc::mbar_wait(mb0 + 24, ph_d2); ph_d2 ^= 1u;
@@ -590,7 +602,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             __syncwarp();
             for (int mt = warp >> 2; mt < m2_tiles; mt += 2) {
                 float vh[32], vl[32];
-                const uint32_t ta = tmem + ((uint32_t)(32 * (warp & 3)) << 16) + 64 + 64 * mt;
+                const uint32_t ta = tmem + ((uint32_t)(32 * (warp & 3)) << 16) + 256 + 64 * mt;
                 tc::tmem_ld32(ta, vh);
                 tc::tmem_ld32(ta + 32, vl);
                 const int j = mt * 128 + 32 * (warp & 3) + lane;

@@ -2,7 +2,7 @@
 // (tcgen05.mma with shared-memory operand descriptors and TMEM accumulators), mbarriers and the
 // proxy fences they need.  Used by the GRU role of the fused expansion kernel (dt_fused.cuh).
 //
-// Operand layout used throughout: K-major, no swizzle.  A "core matrix" is 8 rows x 16 bytes
+// Operand layouts: K-major.  Without swizzle a "core matrix" is 8 rows x 16 bytes
 // (8 bf16 along K), stored as 128 contiguous bytes; the descriptor gives the byte distance between
 // the two core matrices that one K=16 MMA step spans along K (LBO) and between consecutive 8-row
 // groups (SBO).  Element (row m, k) of an operand therefore lives at
@@ -21,6 +21,13 @@ __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)_
 __device__ __forceinline__ uint64_t make_desc(uint32_t smem_addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
     return (uint64_t)((smem_addr >> 4) & 0x3FFFu) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16) |
            ((uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32) | (1ull << 46);
+}
+// Same for the 128-byte-swizzled K-major layout: rows of 128 B (64 bf16 along K) in 1024-byte atoms of 8 rows, the
+// 16-byte piece index XORed with (row % 8); SBO = distance between 8-row atoms, LBO unused (1).  Atoms must be
+// 1024-byte aligned; a K = 16 step inside the 64-wide block advances the start address by 32 B.
+__device__ __forceinline__ uint64_t make_desc_sw128(uint32_t smem_addr, uint32_t sbo_bytes) {
+    return (uint64_t)((smem_addr >> 4) & 0x3FFFu) | (1ull << 16) | ((uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32) |
+           (1ull << 46) | (2ull << 61);
 }
 // 32-bit instruction descriptor for kind::f16: bf16 x bf16 -> fp32, both operands K-major.
 __host__ __device__ constexpr uint32_t make_idesc_bf16(int M, int N) {

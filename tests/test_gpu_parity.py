@@ -179,10 +179,10 @@ def test_tree_small_bf16_all_expand_paths(path, batch, M, B, k):
 
 @pytest.mark.parametrize("batch,M,B,k", [(1, 8, 8, 8), (5, 20, 17, 3), (33, 24, 40, 8), (40, 9, 6, 1)])
 def test_tree_small_bf16_tcgen05_path(batch, M, B, k):
-    """The tcgen05 + TMEM GRU role (expand_path 4) on a small shape it accepts (g a multiple of 128, r <= 256 and
+    """The tcgen05 + TMEM GRU role (expand_path 4) on a small shape it accepts (g a multiple of 256, r <= 256 and
     not a multiple of 16), ragged batch / M / B, against the oracle."""
     gu = _gu()
-    case = _small_bf16_case(gu, 128, 40, k, 32, 48)
+    case = _small_bf16_case(gu, 256, 40, k, 32, 48)
     inp = wl.make_inputs(case.cfg, batch=batch, seed=700 + batch, regime="flat" if batch % 2 else "peaked")
     case.builder.set_option("expand_path", 4)
     try:
