@@ -104,3 +104,294 @@ template <> struct SelOps<float> {
     }
 };
 
+
+struct SelectSmem {
+    unsigned long long cand[kSelCap];       // 8 warp-private segments of kSelSeg keys; reused for sorting / merging
+    unsigned long long fin[kSelFin];        // survivors of the final prune
+    unsigned int wcnt[kSelWarps];           // keys in each warp's segment
+    unsigned int claim[kSelWarps];          // c_w: >= q lanes of warp w have seen an element with ordered key >= c_w
+    unsigned int claimM[kSelWarps];         // >= M elements of warp w have ordered key >= claimM[w] (after a compaction)
+    unsigned int cnt2;
+    unsigned int is_last;
+};
+
+// In-place descending bitonic sort of n (power of two) u64 keys in smem; all kSelThreads threads call.
+__device__ __forceinline__ void block_bitonic_desc(unsigned long long *s, int n) {
+    const int tid = threadIdx.x;
+    for (int k = 2; k <= n; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int i = tid; i < n; i += kSelThreads) {
+                int ixj = i ^ j;
+                if (ixj > i) {
+                    unsigned long long a = s[i], b = s[ixj];
+                    bool desc = ((i & k) == 0);
+                    if (desc ? (a < b) : (a > b)) { s[i] = b; s[ixj] = a; }
+                }
+            }
+            __syncthreads();
+        }
+    }
+}
+// Same for one warp on its own segment (n a power of two <= kSelSeg); the 32 lanes of the warp call.
+__device__ __forceinline__ void warp_bitonic_desc(unsigned long long *s, int n, int lane) {
+    for (int k = 2; k <= n; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int i = lane; i < n; i += 32) {
+                int ixj = i ^ j;
+                if (ixj > i) {
+                    unsigned long long a = s[i], b = s[ixj];
+                    bool desc = ((i & k) == 0);
+                    if (desc ? (a < b) : (a > b)) { s[i] = b; s[ixj] = a; }
+                }
+            }
+            __syncwarp();
+        }
+    }
+}
+
+__device__ __forceinline__ int next_pow2(int x) { int p = 1; while (p < x) p <<= 1; return p; }
+
+// q-th largest (1-based, q <= 32) of the 32 lanes' keys: the largest T with #{key >= T} >= q, built bit by bit
+// from the top with one ballot per bit.  NBITS = 16 resolves only the top 16 bits (bf16 keys; the caller completes
+// the low half, which is 0xFFFF for negative values and 0 otherwise).
+template <int NBITS>
+__device__ __forceinline__ unsigned int warp_qth_largest(unsigned int key, int q) {
+    unsigned int T = 0;
+#pragma unroll
+    for (int b = 31; b > 31 - NBITS; --b) {
+        const unsigned int cand = T | (1u << b);
+        if (__popc(__ballot_sync(0xffffffffu, key >= cand)) >= q) T = cand;
+    }
+    return T;
+}
+
+// Rank `n` distinct keys (n <= kSelThreads * per-thread loop) by counting and hand the top M to `emit(rank, key)`.
+template <typename F>
+__device__ __forceinline__ void block_rank_emit(const unsigned long long *keys, int n, int M, F emit) {
+    for (int i = threadIdx.x; i < n; i += kSelThreads) {
+        const unsigned long long mk = keys[i];
+        int rank = 0;
+        int j = 0;
+        for (; j + 2 <= n; j += 2) {
+            const ulonglong2 o = *reinterpret_cast<const ulonglong2 *>(keys + j);
+            rank += (o.x > mk) + (o.y > mk);
+        }
+        if (j < n) rank += (keys[j] > mk);
+        if (rank < M) emit(rank, mk);
+    }
+}
+
+template <typename T, bool ALIGNED>
+__global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParams p) {
+    using Ops = SelOps<T>;
+    using Run = typename Ops::Run;
+    constexpr int kVec = ElemTraits<T>::kVec;
+    constexpr int kNBits = (sizeof(T) == 2) ? 16 : 32;
+    constexpr unsigned int kFull = 0xffffffffu;
+    __shared__ __align__(16) SelectSmem sm;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int row = blockIdx.y, s = blockIdx.x;
+    const int M = p.M, V = p.V;
+    const int q = (M + kSelWarps - 1) / kSelWarps;             // lanes per warp that must back a claim (<= 32)
+    const T *rowp = reinterpret_cast<const T *>(p.logits) + (size_t)row * V;
+    const int v0 = s * p.chunk_vecs;
+    const int v1 = min(p.row_vecs, v0 + p.chunk_vecs);
+    const int tile_vecs = kSelThreads * kSelU;
+    const int n_tiles = (max(v1 - v0, 0) + tile_vecs - 1) / tile_vecs;
+    unsigned long long *seg = sm.cand + warp * kSelSeg;
+    volatile unsigned int *vclaim = sm.claim, *vclaimM = sm.claimM, *vwcnt = sm.wcnt;
+
+    if (tid < kSelWarps) { sm.wcnt[tid] = 0; sm.claim[tid] = 0; sm.claimM[tid] = 0; }
+    if (tid == 0) { sm.cnt2 = 0; sm.is_last = 0; }
+    __syncthreads();
+
+    auto load_tile = [&](int t, uint4 (&buf)[kSelU]) {
+#pragma unroll
+        for (int u = 0; u < kSelU; ++u) {
+            int gv = v0 + t * tile_vecs + u * kSelThreads + tid;
+            if (gv < v1) {
+                if (ALIGNED) buf[u] = ld_stream_v4(rowp + (size_t)gv * kVec);
+                else buf[u] = Ops::load_scalar(rowp, (long long)gv * kVec, V);
+            } else buf[u] = Ops::lowest_vec();
+        }
+    };
+
+    unsigned int tau_ord = 0;                // ordered-key lower bound on the row's M-th largest value
+    unsigned long long wtau_key = 0ull;      // exact key bound for this warp's own pushes (after a compaction)
+    Run run = Ops::lowest();                 // this lane's running maximum (two packed halves)
+
+    // Publish this warp's claim: the q-th largest of its 32 lane maxima.
+    auto publish_claim = [&]() {
+        unsigned int k0, k1;
+        Ops::sub_keys(run, k0, k1);
+        unsigned int c = warp_qth_largest<kNBits>(max(k0, k1), q);
+        // bf16: only the top 16 bits were resolved; keys of negative values end in 0xFFFF, of non-negative ones in 0
+        if (kNBits == 16 && !(c & 0x80000000u)) c |= 0xFFFFu;
+        if (lane == 0) vclaim[warp] = c;
+    };
+    // tau = max(min_w claim[w], max_w claimM[w], the row-shared word); claims only grow, stale reads stay valid.
+    auto read_tau = [&]() {
+        unsigned int cw = (lane < kSelWarps) ? vclaim[lane] : 0xFFFFFFFFu;
+        unsigned int cm = (lane < kSelWarps) ? vclaimM[lane] : 0u;
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) {
+            cw = min(cw, __shfl_xor_sync(kFull, cw, o));
+            cm = max(cm, __shfl_xor_sync(kFull, cm, o));
+        }
+        unsigned int t = max(__shfl_sync(kFull, cw, 0), __shfl_sync(kFull, cm, 0));
+        if (p.S > 1) {
+            unsigned int g = 0;
+            if (lane == 0) g = (warp == 0) ? atomicMax(&p.row_tau[row], t) : *reinterpret_cast<volatile unsigned int *>(&p.row_tau[row]);
+            t = max(t, __shfl_sync(kFull, g, 0));
+        }
+        tau_ord = max(tau_ord, t);
+    };
+    // Keep the top M of this warp's segment (sort), remember the exact bound, publish the strong claim.
+    auto compact = [&]() {
+        __syncwarp();
+        int n = (int)vwcnt[warp];
+        const int np2 = next_pow2(max(n, 2));
+        for (int i = n + lane; i < np2; i += 32) seg[i] = 0ull;
+        __syncwarp();
+        warp_bitonic_desc(seg, np2, lane);
+        if (n >= M) {
+            wtau_key = seg[M - 1];
+            n = M;
+            const unsigned int o = (unsigned int)(wtau_key >> 32);
+            if (lane == 0) vclaimM[warp] = o;
+            tau_ord = max(tau_ord, o);
+        }
+        __syncwarp();
+        if (lane == 0) vwcnt[warp] = (unsigned int)n;
+        __syncwarp();
+    };
+    // Slow path for one vector: append every element that can still be in the top M.
+    auto push_vec = [&](const uint4 &v, int gv, float tau_f) {
+        float f[kVec];
+        Ops::elems(v, f);
+#pragma unroll
+        for (int i = 0; i < kVec; ++i) {
+            if (f[i] >= tau_f) {
+                const unsigned int idx = (unsigned int)gv * kVec + i;
+                const unsigned long long key = ((unsigned long long)ord_key(f[i]) << 32) | (unsigned long long)(0xFFFFFFFFu - idx);
+                if (key > wtau_key && idx < (unsigned int)V) {
+                    const unsigned int pos = atomicAdd(&sm.wcnt[warp], 1u);
+                    seg[pos] = key;
+                }
+            }
+        }
+    };
+
+    uint4 A[kSelU], Bn[kSelU];
+    if (n_tiles > 0) {
+        load_tile(0, A);
+#pragma unroll
+        for (int u = 0; u < kSelU; ++u) run = Ops::rmax(run, Ops::vmax(A[u]));
+    }
+    publish_claim();
+    __syncthreads();                          // the only CTA barrier before the epilogue: every warp has a claim
+    read_tau();
+
+    for (int t = 0; t < n_tiles; ++t) {
+        if (t + 1 < n_tiles) load_tile(t + 1, Bn);
+        const Run tau = Ops::make_tau(tau_ord);
+        Run m[kSelU];
+#pragma unroll
+        for (int u = 0; u < kSelU; ++u) m[u] = Ops::vmax(A[u]);
+        const Run mt = Ops::rmax(Ops::rmax(m[0], m[1]), Ops::rmax(m[2], m[3]));
+        run = Ops::rmax(run, mt);
+        if (__any_sync(kFull, Ops::pass(mt, tau))) {            // some lane of the warp holds an element >= tau
+            const float tau_f = ord_key_inv(tau_ord);
+#pragma unroll
+            for (int u = 0; u < kSelU; ++u) {
+                const bool hu = Ops::pass(m[u], tau);
+                if (__any_sync(kFull, hu)) {
+                    if ((int)vwcnt[warp] > kSelSeg - 32 * kVec) compact();     // this slot adds at most 32 * kVec keys
+                    if (hu) push_vec(A[u], v0 + t * tile_vecs + u * kSelThreads + tid, tau_f);
+                    __syncwarp();
+                }
+            }
+        }
+        if (t > 0 && (((t + 1) & t) == 0) && (t + 1 < n_tiles)) { publish_claim(); __syncwarp(); read_tau(); }
+#pragma unroll
+        for (int u = 0; u < kSelU; ++u) A[u] = Bn[u];
+    }
+
+    // Epilogue: final tau, prune every segment, rank the survivors, emit.
+    publish_claim();
+    __syncthreads();
+    read_tau();
+    {
+        const int n = (int)sm.wcnt[warp];
+        for (int i = lane; i < n; i += 32) {
+            const unsigned long long key = seg[i];
+            if ((unsigned int)(key >> 32) >= tau_ord) {
+                const unsigned int pos = atomicAdd(&sm.cnt2, 1u);
+                if (pos < (unsigned int)kSelFin) sm.fin[pos] = key;
+            }
+        }
+    }
+    __syncthreads();
+    const int c2 = (int)sm.cnt2;
+
+    unsigned long long *part = p.part + ((size_t)row * p.S + s) * M;
+    auto out_single = [&](int rank, unsigned long long key) {
+        p.cand_id[(size_t)row * M + rank] = (int32_t)(0xFFFFFFFFu - (unsigned int)(key & 0xFFFFFFFFull));
+        p.cand_val[(size_t)row * M + rank] = ord_key_inv((unsigned int)(key >> 32));
+    };
+    auto out_part = [&](int rank, unsigned long long key) { part[rank] = key; };
+
+    if (c2 <= kSelFin) {
+        if (p.S == 1) { block_rank_emit(sm.fin, c2, M, out_single); return; }
+        block_rank_emit(sm.fin, c2, M, out_part);
+        for (int i = c2 + tid; i < M; i += kSelThreads) part[i] = 0ull;      // chunk with fewer than M elements
+    } else {
+        // adversarial rows (more than kSelFin survivors): sort everything that was kept
+        const int n = (int)sm.wcnt[warp];
+        for (int i = n + lane; i < kSelSeg; i += 32) seg[i] = 0ull;
+        __syncthreads();
+        block_bitonic_desc(sm.cand, kSelCap);
+        for (int i = tid; i < M; i += kSelThreads) { if (p.S == 1) out_single(i, sm.cand[i]); else out_part(i, sm.cand[i]); }
+        if (p.S == 1) return;
+    }
+
+    // Chunked row: the last chunk to arrive merges the S sorted partial lists.
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        unsigned int ticket = atomicAdd(&p.row_counter[row], 1u);
+        sm.is_last = (ticket == (unsigned int)(p.S - 1));
+    }
+    __syncthreads();
+    if (!sm.is_last) return;
+    __threadfence();
+    // every chunk's final tau went into row_tau: prune the S * M keys with it, then rank
+    const unsigned int gtau = *reinterpret_cast<volatile unsigned int *>(&p.row_tau[row]);
+    if (tid == 0) sm.cnt2 = 0;
+    __syncthreads();
+    const int tot = p.S * M;
+    const unsigned long long *allp = p.part + (size_t)row * p.S * M;
+    for (int i = tid; i < tot; i += kSelThreads) {
+        const unsigned long long key = __ldcg(allp + i);
+        sm.cand[i] = key;
+        if ((unsigned int)(key >> 32) >= gtau && key != 0ull) {
+            const unsigned int pos = atomicAdd(&sm.cnt2, 1u);
+            if (pos < (unsigned int)kSelFin) sm.fin[pos] = key;
+        }
+    }
+    __syncthreads();
+    const int c3 = (int)sm.cnt2;
+    if (c3 <= kSelFin) {
+        block_rank_emit(sm.fin, c3, M, out_single);
+    } else {
+        const int n2 = next_pow2(max(tot, 2));
+        for (int i = tot + tid; i < n2; i += kSelThreads) sm.cand[i] = 0ull;
+        __syncthreads();
+        block_bitonic_desc(sm.cand, n2);
+        for (int i = tid; i < M; i += kSelThreads) out_single(i, sm.cand[i]);
+    }
+    if (tid == 0) { p.row_counter[row] = 0u; p.row_tau[row] = 0u; }
+}
+
+}  // namespace dt
