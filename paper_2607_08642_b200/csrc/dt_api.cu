@@ -428,10 +428,12 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
 
     int rc = phase_mark(h, 0, st);
     if (rc) return rc;
-    // C = H W1[:, 0:d]^T   (Fact B PAPER.md:83-89).  bf16: tensor cores, forked onto the handle's side
-    // stream so it overlaps the HBM-bound select (fork/join by events: capture-safe, becomes a parallel graph branch).
+    // C = H W1[:, 0:d]^T   (Fact B PAPER.md:83-89).  bf16: tensor cores.
     const bool mma = h->mma_ok && ((reinterpret_cast<uintptr_t>(backbone_hidden) & 15u) == 0) &&
                      rows <= h->max_batch * h->L;
+    // bf16: tensor cores, forked onto the handle's side stream so it overlaps the HBM-bound select (fork/join by
+    // events: capture-safe, becomes a parallel graph branch).  Measured at C5: overlapped select + GEMM 64 us,
+    // back to back 51 + 35 us.
     if (mma) {
         DT_CUDA(h, cudaEventRecord(h->ev_fork, st));
         DT_CUDA(h, cudaStreamWaitEvent(h->side, h->ev_fork, 0));

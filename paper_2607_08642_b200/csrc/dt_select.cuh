@@ -31,7 +31,8 @@ constexpr int kSelU = 4;            // 16-byte vectors per thread per tile
 constexpr int kSelCap = 4096;       // candidate buffer capacity (u64 keys), power of two
 constexpr int kSelWarps = kSelThreads / 32;
 constexpr int kSelSeg = kSelCap / kSelWarps;       // candidate segment per warp (512 keys)
-constexpr int kSelFin = 1024;       // survivors ranked by counting; more than that falls back to a bitonic sort
+constexpr int kSelFin = 512;        // survivors ranked by counting; more than that falls back to a bitonic sort
+constexpr int kSelQ = 64;           // per-warp queue of vectors waiting for the element filter
 constexpr int kSelMaxChunks = 32;   // chunks per row; S * M <= kSelCap must hold
 
 struct SelectParams {
@@ -108,6 +109,8 @@ template <> struct SelOps<float> {
 struct SelectSmem {
     unsigned long long cand[kSelCap];       // 8 warp-private segments of kSelSeg keys; reused for sorting / merging
     unsigned long long fin[kSelFin];        // survivors of the final prune
+    uint4 qv[kSelWarps][kSelQ];             // per-warp queue: vectors that hold an element >= tau ...
+    int qi[kSelWarps][kSelQ];               // ... and their vector index in the row
     unsigned int wcnt[kSelWarps];           // keys in each warp's segment
     unsigned int claim[kSelWarps];          // c_w: >= q lanes of warp w have seen an element with ordered key >= c_w
     unsigned int claimM[kSelWarps];         // >= M elements of warp w have ordered key >= claimM[w] (after a compaction)
@@ -181,6 +184,72 @@ __device__ __forceinline__ void block_rank_emit(const unsigned long long *keys, 
     }
 }
 
+// Per-warp slow-path state kept in registers by the kernel and handed to the out-of-line helpers.
+struct SelWarpCtx {
+    unsigned int tau_ord;                // ordered-key lower bound on the row's M-th largest value
+    unsigned long long wtau_key;         // exact key bound for this warp's own pushes (after a compaction)
+    int qcnt;                            // vectors waiting in this warp's queue (warp-uniform)
+};
+
+// Keep the top M of this warp's segment (sort), remember the exact bound, publish the strong claim.
+__device__ __noinline__ SelWarpCtx sel_compact(SelectSmem &sm, SelWarpCtx c, int M) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    unsigned long long *seg = sm.cand + warp * kSelSeg;
+    volatile unsigned int *vwcnt = sm.wcnt, *vclaimM = sm.claimM;
+    __syncwarp();
+    int n = (int)vwcnt[warp];
+    const int np2 = next_pow2(max(n, 2));
+    for (int i = n + lane; i < np2; i += 32) seg[i] = 0ull;
+    __syncwarp();
+    warp_bitonic_desc(seg, np2, lane);
+    if (n >= M) {
+        c.wtau_key = seg[M - 1];
+        n = M;
+        const unsigned int o = (unsigned int)(c.wtau_key >> 32);
+        if (lane == 0) vclaimM[warp] = o;
+        c.tau_ord = max(c.tau_ord, o);
+    }
+    __syncwarp();
+    if (lane == 0) vwcnt[warp] = (unsigned int)n;
+    __syncwarp();
+    return c;
+}
+
+// Filter the queued vectors, one vector per lane: append every element that can still be in the top M.
+template <typename T>
+__device__ __noinline__ SelWarpCtx sel_drain(SelectSmem &sm, SelWarpCtx c, int M, int V) {
+    using Ops = SelOps<T>;
+    constexpr int kVec = ElemTraits<T>::kVec;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    unsigned long long *seg = sm.cand + warp * kSelSeg;
+    volatile unsigned int *vwcnt = sm.wcnt;
+    __syncwarp();
+    for (int base = 0; base < c.qcnt; base += 32) {
+        if ((int)vwcnt[warp] > kSelSeg - 32 * kVec) c = sel_compact(sm, c, M);      // this batch adds at most 32 * kVec keys
+        if (base + lane < c.qcnt) {
+            const float tau_f = ord_key_inv(c.tau_ord);
+            const uint4 v = sm.qv[warp][base + lane];
+            const int gv = sm.qi[warp][base + lane];
+            float f[kVec];
+            Ops::elems(v, f);
+#pragma unroll
+            for (int i = 0; i < kVec; ++i) {
+                if (f[i] >= tau_f) {
+                    const unsigned int idx = (unsigned int)gv * kVec + i;
+                    const unsigned long long key = ((unsigned long long)ord_key(f[i]) << 32) | (unsigned long long)(0xFFFFFFFFu - idx);
+                    if (key > c.wtau_key && idx < (unsigned int)V) {
+                        const unsigned int pos = atomicAdd(&sm.wcnt[warp], 1u);
+                        seg[pos] = key;
+                    }
+                }
+            }
+        }
+        __syncwarp();
+    }
+    c.qcnt = 0;
+    return c;
+}
+
 template <typename T, bool ALIGNED>
 __global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParams p) {
     using Ops = SelOps<T>;
@@ -206,7 +275,14 @@ __global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParam
     if (tid == 0) { sm.cnt2 = 0; sm.is_last = 0; }
     __syncthreads();
 
+    const int n_full = max(v1 - v0, 0) / tile_vecs;            // tiles that need no bounds checks
     auto load_tile = [&](int t, uint4 (&buf)[kSelU]) {
+        if (ALIGNED && t < n_full) {
+            const T *q = rowp + (size_t)(v0 + t * tile_vecs + tid) * kVec;
+#pragma unroll
+            for (int u = 0; u < kSelU; ++u) buf[u] = ld_stream_v4(q + (size_t)u * kSelThreads * kVec);
+            return;
+        }
 #pragma unroll
         for (int u = 0; u < kSelU; ++u) {
             int gv = v0 + t * tile_vecs + u * kSelThreads + tid;
@@ -217,18 +293,18 @@ __global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParam
         }
     };
 
-    unsigned int tau_ord = 0;                // ordered-key lower bound on the row's M-th largest value
-    unsigned long long wtau_key = 0ull;      // exact key bound for this warp's own pushes (after a compaction)
+    SelWarpCtx c;
+    c.tau_ord = 0; c.wtau_key = 0ull; c.qcnt = 0;
     Run run = Ops::lowest();                 // this lane's running maximum (two packed halves)
 
     // Publish this warp's claim: the q-th largest of its 32 lane maxima.
     auto publish_claim = [&]() {
         unsigned int k0, k1;
         Ops::sub_keys(run, k0, k1);
-        unsigned int c = warp_qth_largest<kNBits>(max(k0, k1), q);
+        unsigned int cl = warp_qth_largest<kNBits>(max(k0, k1), q);
         // bf16: only the top 16 bits were resolved; keys of negative values end in 0xFFFF, of non-negative ones in 0
-        if (kNBits == 16 && !(c & 0x80000000u)) c |= 0xFFFFu;
-        if (lane == 0) vclaim[warp] = c;
+        if (kNBits == 16 && !(cl & 0x80000000u)) cl |= 0xFFFFu;
+        if (lane == 0) vclaim[warp] = cl;
     };
     // tau = max(min_w claim[w], max_w claimM[w], the row-shared word); claims only grow, stale reads stay valid.
     auto read_tau = [&]() {
@@ -245,42 +321,7 @@ __global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParam
             if (lane == 0) g = (warp == 0) ? atomicMax(&p.row_tau[row], t) : *reinterpret_cast<volatile unsigned int *>(&p.row_tau[row]);
             t = max(t, __shfl_sync(kFull, g, 0));
         }
-        tau_ord = max(tau_ord, t);
-    };
-    // Keep the top M of this warp's segment (sort), remember the exact bound, publish the strong claim.
-    auto compact = [&]() {
-        __syncwarp();
-        int n = (int)vwcnt[warp];
-        const int np2 = next_pow2(max(n, 2));
-        for (int i = n + lane; i < np2; i += 32) seg[i] = 0ull;
-        __syncwarp();
-        warp_bitonic_desc(seg, np2, lane);
-        if (n >= M) {
-            wtau_key = seg[M - 1];
-            n = M;
-            const unsigned int o = (unsigned int)(wtau_key >> 32);
-            if (lane == 0) vclaimM[warp] = o;
-            tau_ord = max(tau_ord, o);
-        }
-        __syncwarp();
-        if (lane == 0) vwcnt[warp] = (unsigned int)n;
-        __syncwarp();
-    };
-    // Slow path for one vector: append every element that can still be in the top M.
-    auto push_vec = [&](const uint4 &v, int gv, float tau_f) {
-        float f[kVec];
-        Ops::elems(v, f);
-#pragma unroll
-        for (int i = 0; i < kVec; ++i) {
-            if (f[i] >= tau_f) {
-                const unsigned int idx = (unsigned int)gv * kVec + i;
-                const unsigned long long key = ((unsigned long long)ord_key(f[i]) << 32) | (unsigned long long)(0xFFFFFFFFu - idx);
-                if (key > wtau_key && idx < (unsigned int)V) {
-                    const unsigned int pos = atomicAdd(&sm.wcnt[warp], 1u);
-                    seg[pos] = key;
-                }
-            }
-        }
+        c.tau_ord = max(c.tau_ord, t);
     };
 
     uint4 A[kSelU], Bn[kSelU];
@@ -293,30 +334,40 @@ __global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParam
     __syncthreads();                          // the only CTA barrier before the epilogue: every warp has a claim
     read_tau();
 
-    for (int t = 0; t < n_tiles; ++t) {
-        if (t + 1 < n_tiles) load_tile(t + 1, Bn);
-        const Run tau = Ops::make_tau(tau_ord);
-        Run m[kSelU];
+    // Vectors that hold an element >= tau are queued (a few instructions, whichever lanes hit); when more than 32
+    // wait, the warp filters them one vector per lane (sel_drain), so the element filter always runs with full lanes.
+    uint4 *qv = sm.qv[warp];
+    int *qi = sm.qi[warp];
+    auto process = [&](const uint4 (&X)[kSelU], int t) {
+        const Run tau = Ops::make_tau(c.tau_ord);
+        const int gv0 = v0 + t * tile_vecs + tid;
 #pragma unroll
-        for (int u = 0; u < kSelU; ++u) m[u] = Ops::vmax(A[u]);
-        const Run mt = Ops::rmax(Ops::rmax(m[0], m[1]), Ops::rmax(m[2], m[3]));
-        run = Ops::rmax(run, mt);
-        if (__any_sync(kFull, Ops::pass(mt, tau))) {            // some lane of the warp holds an element >= tau
-            const float tau_f = ord_key_inv(tau_ord);
-#pragma unroll
-            for (int u = 0; u < kSelU; ++u) {
-                const bool hu = Ops::pass(m[u], tau);
-                if (__any_sync(kFull, hu)) {
-                    if ((int)vwcnt[warp] > kSelSeg - 32 * kVec) compact();     // this slot adds at most 32 * kVec keys
-                    if (hu) push_vec(A[u], v0 + t * tile_vecs + u * kSelThreads + tid, tau_f);
-                    __syncwarp();
+        for (int u = 0; u < kSelU; ++u) {
+            const Run m = Ops::vmax(X[u]);
+            run = Ops::rmax(run, m);
+            const bool hu = Ops::pass(m, tau);
+            const unsigned int bal = __ballot_sync(kFull, hu);
+            if (bal) {                                   // some lane of the warp holds an element >= tau in this vector slot
+                if (hu) {
+                    const int pos = c.qcnt + __popc(bal & ((1u << lane) - 1u));
+                    qv[pos] = X[u];
+                    qi[pos] = gv0 + u * kSelThreads;
                 }
+                c.qcnt += __popc(bal);
+                if (c.qcnt > 32) c = sel_drain<T>(sm, c, M, V);
             }
         }
         if (t > 0 && (((t + 1) & t) == 0) && (t + 1 < n_tiles)) { publish_claim(); __syncwarp(); read_tau(); }
-#pragma unroll
-        for (int u = 0; u < kSelU; ++u) A[u] = Bn[u];
+    };
+    for (int t = 0; t < n_tiles; t += 2) {      // ping-pong between the two register tiles
+        if (t + 1 < n_tiles) load_tile(t + 1, Bn);
+        process(A, t);
+        if (t + 1 < n_tiles) {
+            if (t + 2 < n_tiles) load_tile(t + 2, A);
+            process(Bn, t + 1);
+        }
     }
+    c = sel_drain<T>(sm, c, M, V);
 
     // Epilogue: final tau, prune every segment, rank the survivors, emit.
     publish_claim();
@@ -326,7 +377,7 @@ __global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParam
         const int n = (int)sm.wcnt[warp];
         for (int i = lane; i < n; i += 32) {
             const unsigned long long key = seg[i];
-            if ((unsigned int)(key >> 32) >= tau_ord) {
+            if ((unsigned int)(key >> 32) >= c.tau_ord) {
                 const unsigned int pos = atomicAdd(&sm.cnt2, 1u);
                 if (pos < (unsigned int)kSelFin) sm.fin[pos] = key;
             }
