@@ -72,8 +72,11 @@ __device__ __forceinline__ unsigned long long dt_globaltimer() {
 
 // ---- hand-over words -------------------------------------------------------------------------------
 // Both directions use one self-describing word per producer (no shared counter, so no serialised
-// atomics): the consumer's lanes poll the producers' words with relaxed loads that bypass L1, then
-// fence.  The producer fences after a CTA barrier and stores its word.
+// atomics).  GRU -> request: the GRU CTA's threads store states / partials, a CTA barrier, then thread 0
+// fences at gpu scope (the data is in L2 before the flag can be seen) and stores the flag.  Consumers
+// poll with relaxed gpu-scope loads and read ALL hand-over data with L1-bypassing loads (ld.global.cg,
+// cp.async.cg), i.e. from L2, the single point of coherence, after the control dependency on the polled
+// word; they need no fence of their own.  Request -> GRU: the descriptor word is the whole payload.
 __device__ __forceinline__ unsigned int ld_relaxed_u32(const unsigned int *p) {
     unsigned int v;
     asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -119,7 +122,7 @@ __host__ __device__ inline size_t fused_gru_smem(int g, int r, int upc, int m_ti
 __host__ __device__ inline size_t fused_req_smem(int r, int M, int N, int k, int w2_smem) {
     auto al = [](size_t x) { return (x + 15) / 16 * 16; };
     size_t s = al((size_t)2 * kFusMaxFront * 8) + al((size_t)k * 8) + al((size_t)M * 8) + al((size_t)2 * kFusMaxFront * 4) +
-               al((size_t)k * 4) + al((size_t)r * 4) + 3 * al((size_t)M * 4) + 4 * al((size_t)N * 4);
+               al((size_t)k * 4) + 9 * al((size_t)r * 4) + 3 * al((size_t)M * 4) + 4 * al((size_t)N * 4);
     if (w2_smem) s += al((size_t)M * (r + kFusW2Pad) * 2);
     return s + 16;
 }
@@ -192,7 +195,6 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
                     sidx = (int)((dsc >> 32) & 0xFFFFu) - 1;
                     tok = (int)(dsc & 0xFFFFFFFFull);
                 }
-                __threadfence();
                 sIdx[lane] = sidx; sTok[lane] = tok;
             }
             __syncthreads();
@@ -465,7 +467,6 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                     sidx = (int)((dsc >> 32) & 0xFFFFu) - 1;
                     tok = (int)(dsc & 0xFFFFFFFFull);
                 }
-                __threadfence();
                 sIdx[lane] = sidx; sTok[lane] = tok;
             }
             __syncthreads();
@@ -656,6 +657,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     unsigned int *fHi = reinterpret_cast<unsigned int *>(carve((size_t)2 * kFusMaxFront * 4));
     unsigned int *nHi = reinterpret_cast<unsigned int *>(carve((size_t)k * 4));
     float *sA = reinterpret_cast<float *>(carve((size_t)r * 4));
+    float *sP = reinterpret_cast<float *>(carve((size_t)8 * r * 4));        // group sums of the split-K partials
     float *sZ = reinterpret_cast<float *>(carve((size_t)M * 4));
     float *sBase = reinterpret_cast<float *>(carve((size_t)M * 4));
     int *sTok = reinterpret_cast<int *>(carve((size_t)M * 4));
@@ -702,7 +704,6 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         if (warp == 0) {
             for (int q = lane; q < p.n_gru; q += 32)
                 while (ld_relaxed_u32(p.flags + q) < (unsigned int)(t + 1)) { }
-            __threadfence();
         }
         __syncthreads();
         DT_TR(1, p.n_gru, t, 0);
@@ -714,29 +715,42 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         int n_new = 0;
         if (expand) {
             const size_t row = (size_t)b * L + depth;           // H_{depth+1} <-> row index depth (A12)
-            // a = SiLU(C + W1[:, d:] S_t): split-K partials summed in CTA order
-            for (int j = tid; j < r; j += kFusThreads) {
-                const float *pp = p.partial + (size_t)b * r + j;
-                const size_t ps = (size_t)batch * r;
-                const float cval = e.C[row * r + j];
-                float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-                int q = 0;
-                for (; q + 32 <= p.n_gru; q += 32) {
-                    float v[32];
+            // a = SiLU(C + W1[:, d:] S_t): the n_gru split-K partials are summed in a fixed order (batch-invariant):
+            // G thread groups each sum a contiguous range of GRU CTAs with 16-byte loads, then the groups are added
+            {
+                const int r4 = r >> 2;
+                const int G = min(8, kFusThreads / r4);
+                const int per = (p.n_gru + G - 1) / G;
+                const int jq = tid % r4, qg = tid / r4;
+                if (qg < G) {
+                    const size_t ps4 = ((size_t)batch * r) >> 2;
+                    const float4 *pp = reinterpret_cast<const float4 *>(p.partial + (size_t)b * r) + jq;
+                    const int q0 = qg * per, q1 = min(p.n_gru, q0 + per);
+                    float4 s0 = make_float4(0.f, 0.f, 0.f, 0.f), s1 = s0;
+                    int q = q0;
+                    for (; q + 16 <= q1; q += 16) {
+                        float4 v[16];
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) v[i] = __ldcg(pp + (size_t)(q + i) * ps);
+                        for (int i = 0; i < 16; ++i) v[i] = __ldcg(pp + (size_t)(q + i) * ps4);
 #pragma unroll
-                    for (int i = 0; i < 32; i += 4) { s0 += v[i]; s1 += v[i + 1]; s2 += v[i + 2]; s3 += v[i + 3]; }
+                        for (int i = 0; i < 16; i += 2) {
+                            s0.x += v[i].x; s0.y += v[i].y; s0.z += v[i].z; s0.w += v[i].w;
+                            s1.x += v[i + 1].x; s1.y += v[i + 1].y; s1.z += v[i + 1].z; s1.w += v[i + 1].w;
+                        }
+                    }
+                    for (; q < q1; ++q) {
+                        const float4 v = __ldcg(pp + (size_t)q * ps4);
+                        s0.x += v.x; s0.y += v.y; s0.z += v.z; s0.w += v.w;
+                    }
+                    *reinterpret_cast<float4 *>(sP + (size_t)qg * r + 4 * jq) = make_float4(s0.x + s1.x, s0.y + s1.y, s0.z + s1.z, s0.w + s1.w);
                 }
-                for (; q + 4 <= p.n_gru; q += 4) {
-                    s0 += __ldcg(pp + (size_t)q * ps);
-                    s1 += __ldcg(pp + (size_t)(q + 1) * ps);
-                    s2 += __ldcg(pp + (size_t)(q + 2) * ps);
-                    s3 += __ldcg(pp + (size_t)(q + 3) * ps);
+                __syncthreads();
+                for (int j = tid; j < r; j += kFusThreads) {
+                    float acc = sP[j];
+                    for (int gq = 1; gq < G; ++gq) acc += sP[(size_t)gq * r + j];
+                    const float x = e.C[row * r + j] + acc;
+                    sA[j] = x * sigmoidf_acc(x);
                 }
-                for (; q < p.n_gru; ++q) s0 += __ldcg(pp + (size_t)q * ps);
-                const float x = cval + ((s0 + s1) + (s2 + s3));
-                sA[j] = x * sigmoidf_acc(x);
             }
             cp_async_wait<0>();
             __syncthreads();
@@ -787,35 +801,30 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             for (int m = lane; m < M; m += 32) ssum += expf(sZ[m] - zmax);
             const float lse = logf(warp_sum(ssum));
             const float gpar = nSco[t];
-            if (tid < M) {
-                const float lp = (sZ[tid] - zmax) - lse;
-                sKey[tid] = ((unsigned long long)ord_key(lp) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned int)sTok[tid]);
-            }
-            __syncthreads();
-            // top-k by (logp desc, token asc): rank by counting, `tpc` lanes per candidate (a power of two <= 8,
-            // lanes of one candidate are neighbours in a warp); the k winners become the new entries
+            // top-k by (logp desc, token asc): rank by counting on z (logp is a monotone map of z), `tpc` lanes per
+            // candidate (a power of two <= 8, lanes of one candidate are neighbours in a warp); the k winners become
+            // the new entries
             {
                 int tpc = 1;
                 while (tpc < 8 && M * tpc * 2 <= kFusThreads) tpc <<= 1;
                 const int m = tid / tpc, part = tid - m * tpc;
                 const bool act = (m < M);
-                const unsigned long long mk = act ? sKey[m] : 0ull;
+                const float mz = act ? sZ[m] : 0.f;
+                const int mtok = act ? sTok[m] : 0;
                 int rank = 0;
                 if (act) {
-                    const int per = (((M + tpc - 1) / tpc) + 1) & ~1;                // even, so 16-byte loads stay aligned
+                    const int per = (M + tpc - 1) / tpc;
                     const int m0 = part * per, m1 = min(M, m0 + per);
-                    int q = m0;
-                    for (; q + 2 <= m1; q += 2) {
-                        const ulonglong2 o = *reinterpret_cast<const ulonglong2 *>(sKey + q);
-                        rank += (o.x > mk) + (o.y > mk);
+                    for (int q = m0; q < m1; ++q) {
+                        const float oz = sZ[q];
+                        rank += (oz > mz) || (oz == mz && sTok[q] < mtok);
                     }
-                    if (q < m1) rank += (sKey[q] > mk);
                 }
                 for (int o = 1; o < tpc; o <<= 1) rank += __shfl_xor_sync(0xffffffffu, rank, o);
                 if (act && part == 0 && rank < k) {
-                    const float lpm = (sZ[m] - zmax) - lse;
+                    const float lpm = (mz - zmax) - lse;
                     nHi[rank] = ord_key(gpar + lpm);
-                    nLo[rank] = ((unsigned long long)(0xFFFFFFFFu - (unsigned int)sTok[m]) << 32) |
+                    nLo[rank] = ((unsigned long long)(0xFFFFFFFFu - (unsigned int)mtok) << 32) |
                                 (unsigned long long)(0xFFFFFFFFu - (unsigned int)t);
                 }
             }
@@ -823,9 +832,29 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             __syncthreads();
             DT_TR(1, p.n_gru, t, 3);
         }
-        // merge the new entries into the sorted frontier (other buffer), truncated to the pops that remain
+        // The node popped now is the better of the old frontier head and the best new entry: thread 0 publishes its
+        // descriptor BEFORE the merge, so the GRU CTAs start step t+1 while this CTA is still merging.
         const int cap = B - t;                                  // pops still to do, this one included
         int tot = n_front + n_new;
+        if (tid == 0) {
+            if (tot > 0) {
+                unsigned int h = 0; unsigned long long l = 0ull; bool have = false;
+                if (n_front > 0) { h = oHi[0]; l = oLo[0]; have = true; }
+                for (int j = 0; j < n_new; ++j)
+                    if (!have || front_gt(nHi[j], nLo[j], h, l)) { h = nHi[j]; l = nLo[j]; have = true; }
+                const int tok = (int)(0xFFFFFFFFu - (unsigned int)(l >> 32));
+                const int par = (int)(0xFFFFFFFFu - (unsigned int)(l & 0xFFFFFFFFull));
+                const int dep = nDep[par] + 1;
+                if (t + 1 < B) st_relaxed_u64(p.desc + b, fused_desc_pack(t + 2, dep < L ? par + 1 : -1, tok));
+                nTok[t + 1] = tok; nPar[t + 1] = par; nDep[t + 1] = dep; nSco[t + 1] = ord_key_inv(h);
+                sm.n_valid = t + 2; sm.n_front = min(tot, cap) - 1; sm.cur = cur ^ 1;
+            } else {
+                sm.n_front = 0;
+                if (t + 1 < B) st_relaxed_u64(p.desc + b, fused_desc_pack(t + 2, -1, 0));
+            }
+        }
+        DT_TR(1, p.n_gru, t, 4);
+        // merge the new entries into the sorted frontier (other buffer), truncated to the pops that remain
         if (tot > 0) {
             if (tid < n_front) {
                 const unsigned int h = oHi[tid]; const unsigned long long l = oLo[tid];
@@ -850,28 +879,9 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             if (tot > cap) tot = cap;
         }
         __syncthreads();
-        // pop entry 0 into slot t+1; the live frontier becomes entries 1..tot-1 of the other buffer
+        // the popped node is entry 0 of the other buffer; the live frontier becomes its entries 1..tot-1
         int next_dep = L;                                       // depth of the node popped now (L = none / leaf)
-        if (tot > 0) {
-            const unsigned int h = wHi[0]; const unsigned long long l = wLo[0];
-            const int tok = (int)(0xFFFFFFFFu - (unsigned int)(l >> 32));
-            const int par = (int)(0xFFFFFFFFu - (unsigned int)(l & 0xFFFFFFFFull));
-            const int dep = nDep[par] + 1;
-            next_dep = dep;
-            if (tid == 0) {
-                if (t + 1 < B) {
-                    __threadfence();
-                    st_relaxed_u64(p.desc + b, fused_desc_pack(t + 2, dep < L ? par + 1 : -1, tok));
-                }
-                nTok[t + 1] = tok; nPar[t + 1] = par; nDep[t + 1] = dep; nSco[t + 1] = ord_key_inv(h);
-                sm.n_valid = t + 2; sm.n_front = tot - 1; sm.cur = cur ^ 1;
-            }
-        } else if (tid == 0) {
-            sm.n_front = 0;
-            if (t + 1 < B) { __threadfence(); st_relaxed_u64(p.desc + b, fused_desc_pack(t + 2, -1, 0)); }
-        }
-        DT_TR(1, p.n_gru, t, 4);
-        __syncthreads();
+        if (tot > 0) next_dep = nDep[t + 1];
         if (t + 1 < B && next_dep < L) stage_depth(next_dep);   // overlaps the GRU CTAs' step t+1
         DT_TR(1, p.n_gru, t, 5);
     }
