@@ -124,7 +124,7 @@ __host__ __device__ inline size_t fused_req_smem(int r, int M, int N, int k, int
     size_t s = al((size_t)2 * kFusMaxFront * 8) + al((size_t)k * 8) + al((size_t)M * 8) + al((size_t)2 * kFusMaxFront * 4) +
                al((size_t)k * 4) + 9 * al((size_t)r * 4) + 3 * al((size_t)M * 4) + 4 * al((size_t)N * 4);
     if (w2_smem) s += al((size_t)M * (r + kFusW2Pad) * 2);
-    return s + 16;
+    return s + 16 + 64;
 }
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
@@ -658,6 +658,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     unsigned int *nHi = reinterpret_cast<unsigned int *>(carve((size_t)k * 4));
     float *sA = reinterpret_cast<float *>(carve((size_t)r * 4));
     float *sP = reinterpret_cast<float *>(carve((size_t)8 * r * 4));        // group sums of the split-K partials
+    float *sWst = reinterpret_cast<float *>(carve((size_t)2 * kFusWarps * 4)); // per-warp softmax (max, sum)
     float *sZ = reinterpret_cast<float *>(carve((size_t)M * 4));
     float *sBase = reinterpret_cast<float *>(carve((size_t)M * 4));
     int *sTok = reinterpret_cast<int *>(carve((size_t)M * 4));
@@ -701,6 +702,9 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         const bool expand = node_ok && depth < L;               // block-uniform
         // Every request CTA waits for the GRU CTAs' step t, expanded or not: nobody runs ahead, so the
         // descriptor word and the partial buffer are never overwritten while still in use.
+        // C = H W1h^T of the node's depth does not depend on the GRU CTAs: fetch it while waiting for them
+        float cpre = 0.f;
+        if (expand && tid < r) cpre = e.C[((size_t)b * L + depth) * r + tid];
         if (warp == 0) {
             for (int q = lane; q < p.n_gru; q += 32)
                 while (ld_relaxed_u32(p.flags + q) < (unsigned int)(t + 1)) { }
@@ -748,7 +752,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                 for (int j = tid; j < r; j += kFusThreads) {
                     float acc = sP[j];
                     for (int gq = 1; gq < G; ++gq) acc += sP[(size_t)gq * r + j];
-                    const float x = e.C[row * r + j] + acc;
+                    const float x = ((j == tid) ? cpre : e.C[row * r + j]) + acc;
                     sA[j] = x * sigmoidf_acc(x);
                 }
             }
@@ -760,6 +764,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             const float base0 = sBase[0];
             {
                 const int q4 = tid & 3, nvec = r / 8;
+                float wmx = -INFINITY, wsm = 0.f;                     // this warp's running (max, sum exp(z - max))
                 for (int mb = 0; mb < M; mb += kFusThreads / 4) {     // warp-uniform trip count (shuffles below)
                     const int m = mb + (tid >> 2);
                     float acc = 0.f;
@@ -788,18 +793,31 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                     }
                     acc += __shfl_xor_sync(0xffffffffu, acc, 1);
                     acc += __shfl_xor_sync(0xffffffffu, acc, 2);
-                    if (q4 == 0 && m < M) sZ[m] = __fdiv_rn((sBase[m] - base0) + acc, e.T_eff);
+                    float z = -INFINITY;
+                    if (m < M) { z = __fdiv_rn((sBase[m] - base0) + acc, e.T_eff); if (q4 == 0) sZ[m] = z; }
+                    // slice log-softmax statistics (reading A1), online: the 8 candidates of this warp pass ...
+                    float zm = fmaxf(z, __shfl_xor_sync(0xffffffffu, z, 4));
+                    zm = fmaxf(zm, __shfl_xor_sync(0xffffffffu, zm, 8));
+                    zm = fmaxf(zm, __shfl_xor_sync(0xffffffffu, zm, 16));
+                    const float nmx = fmaxf(wmx, zm);
+                    float ex = (q4 == 0 && m < M) ? expf(z - nmx) : 0.f;
+                    ex += __shfl_xor_sync(0xffffffffu, ex, 4);
+                    ex += __shfl_xor_sync(0xffffffffu, ex, 8);
+                    ex += __shfl_xor_sync(0xffffffffu, ex, 16);
+                    if (nmx > -INFINITY) { wsm = wsm * expf(wmx - nmx) + ex; wmx = nmx; }
                 }
+                if (lane == 0) { sWst[2 * warp] = wmx; sWst[2 * warp + 1] = wsm; }
             }
             __syncthreads();
             DT_TR(1, p.n_gru, t, 2);
-            // slice log-softmax (reading A1): every warp reduces the whole slice itself (no CTA barrier)
+            // ... then every thread merges the 8 warps' (max, sum) pairs in warp order
             float zmax = -INFINITY;
-            for (int m = lane; m < M; m += 32) zmax = fmaxf(zmax, sZ[m]);
-            zmax = warp_max(zmax);
+#pragma unroll
+            for (int w = 0; w < kFusWarps; ++w) zmax = fmaxf(zmax, sWst[2 * w]);
             float ssum = 0.f;
-            for (int m = lane; m < M; m += 32) ssum += expf(sZ[m] - zmax);
-            const float lse = logf(warp_sum(ssum));
+#pragma unroll
+            for (int w = 0; w < kFusWarps; ++w) { const float mw = sWst[2 * w]; if (mw > -INFINITY) ssum += sWst[2 * w + 1] * expf(mw - zmax); }
+            const float lse = logf(ssum);
             const float gpar = nSco[t];
             // top-k by (logp desc, token asc): rank by counting on z (logp is a monotone map of z), `tpc` lanes per
             // candidate (a power of two <= 8, lanes of one candidate are neighbours in a warp); the k winners become
@@ -815,7 +833,18 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                 if (act) {
                     const int per = (M + tpc - 1) / tpc;
                     const int m0 = part * per, m1 = min(M, m0 + per);
-                    for (int q = m0; q < m1; ++q) {
+                    int q = m0;
+                    if (!(per & 3)) {
+                        for (; q + 4 <= m1; q += 4) {
+                            const float4 oz = *reinterpret_cast<const float4 *>(sZ + q);
+                            const int4 ot = *reinterpret_cast<const int4 *>(sTok + q);
+                            rank += (oz.x > mz) || (oz.x == mz && ot.x < mtok);
+                            rank += (oz.y > mz) || (oz.y == mz && ot.y < mtok);
+                            rank += (oz.z > mz) || (oz.z == mz && ot.z < mtok);
+                            rank += (oz.w > mz) || (oz.w == mz && ot.w < mtok);
+                        }
+                    }
+                    for (; q < m1; ++q) {
                         const float oz = sZ[q];
                         rank += (oz > mz) || (oz == mz && sTok[q] < mtok);
                     }
