@@ -40,6 +40,8 @@ struct dt_handle {
     char *stage; size_t stage_bytes;
     // options / bookkeeping
     int64_t opt_select_chunks;
+    int64_t opt_select_kernel;      // 0 auto, 1 register-tile kernel only
+    int sel_bulk_ok;
     // phase timing (optional): n_slots x kPhaseEvents events, recorded on the caller's stream
     cudaEvent_t *ph_ev; int ph_slots, ph_slot;
     int64_t launches;
@@ -117,6 +119,11 @@ extern "C" int dt_set_option(dt_handle *h, const char *name, int64_t value) {
     if (!strcmp(name, "expand_path")) {
         if (value < 0 || value > 4) return DT_ERR_INVALID_ARG;
         h->opt_expand_path = value;
+        return DT_OK;
+    }
+    if (!strcmp(name, "select_kernel")) {
+        if (value < 0 || value > 1) return DT_ERR_INVALID_ARG;
+        h->opt_select_kernel = value;
         return DT_OK;
     }
     if (!strcmp(name, "select_chunks")) {
@@ -246,6 +253,10 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         }
     }
 
+    h->sel_bulk_ok =
+        cudaFuncSetAttribute(select_topm_bulk_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSelBulkDynSmem) == cudaSuccess &&
+        cudaFuncSetAttribute(select_topm_bulk_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSelBulkDynSmem) == cudaSuccess;
+    if (!h->sel_bulk_ok) cudaGetLastError();
     int rc = DT_OK;
     if (cudaMemset(h->ws, 0, h->ws_bytes) != cudaSuccess) rc = DT_ERR_CUDA;
     {   // dynamic shared memory of expand_kernel at the handle's maxima
@@ -284,8 +295,8 @@ extern "C" int dt_destroy(dt_handle *h) {
     return DT_OK;
 }
 
-static int pick_chunks(const dt_handle *h, int rows, int M) {
-    int smax = kSelCap / M;
+static int pick_chunks(const dt_handle *h, int rows, int M, int cap) {
+    int smax = cap / M;                             // the merging CTA holds S * M keys in its candidate buffer
     if (smax > kSelMaxChunks) smax = kSelMaxChunks;
     if (smax < 1) smax = 1;
     int S;
@@ -303,18 +314,24 @@ static int launch_select(dt_handle *h, const void *logits, int rows, int M, int3
                          cudaStream_t st) {
     const int V = h->w.V;
     const int kvec = (h->w.dtype == DT_BF16) ? 8 : 4;
+    const bool aligned = (V % kvec == 0) && ((reinterpret_cast<uintptr_t>(logits) & 15u) == 0);
+    // bulk-copy kernel (cp.async.bulk ring per warp) for 16-byte aligned rows, else the register-tile kernel
+    const bool bulk = aligned && h->opt_select_kernel != 1 && h->sel_bulk_ok;
     SelectParams p;
     p.logits = logits; p.rows = rows; p.V = V; p.M = M;
     p.row_vecs = (V + kvec - 1) / kvec;
-    int S = pick_chunks(h, rows, M);
+    int S = pick_chunks(h, rows, M, SelectSmemBig::kCap);
     if (S > p.row_vecs) S = p.row_vecs;
     p.S = S;
     p.chunk_vecs = (p.row_vecs + S - 1) / S;
+    if (bulk) p.chunk_vecs = (p.chunk_vecs + kSelTileVecs - 1) / kSelTileVecs * kSelTileVecs;   // chunks start on tile boundaries
     p.cand_id = cand_id; p.cand_val = cand_val;
     p.part = h->sel_part; p.row_counter = h->sel_counter; p.row_tau = h->sel_tau;
-    const bool aligned = (V % kvec == 0) && ((reinterpret_cast<uintptr_t>(logits) & 15u) == 0);
     dim3 grid(S, rows);
-    if (h->w.dtype == DT_BF16) {
+    if (bulk) {
+        if (h->w.dtype == DT_BF16) select_topm_bulk_kernel<__nv_bfloat16><<<grid, kSelThreads, kSelBulkDynSmem, st>>>(p);
+        else select_topm_bulk_kernel<float><<<grid, kSelThreads, kSelBulkDynSmem, st>>>(p);
+    } else if (h->w.dtype == DT_BF16) {
         if (aligned) select_topm_kernel<__nv_bfloat16, true><<<grid, kSelThreads, 0, st>>>(p);
         else select_topm_kernel<__nv_bfloat16, false><<<grid, kSelThreads, 0, st>>>(p);
     } else {

@@ -28,11 +28,10 @@ namespace dt {
 
 constexpr int kSelThreads = 256;
 constexpr int kSelU = 4;            // 16-byte vectors per thread per tile
-constexpr int kSelCap = 4096;       // candidate buffer capacity (u64 keys), power of two
+constexpr int kSelCap = 4096;       // largest candidate buffer (u64 keys): bounds S * M for chunked rows
 constexpr int kSelWarps = kSelThreads / 32;
-constexpr int kSelSeg = kSelCap / kSelWarps;       // candidate segment per warp (512 keys)
-constexpr int kSelFin = 512;        // survivors ranked by counting; more than that falls back to a bitonic sort
-constexpr int kSelQ = 64;           // per-warp queue of vectors waiting for the element filter
+constexpr int kSelTileBytes = 4096; // bulk-copy tile of one warp: 256 vectors of 16 bytes
+constexpr int kSelStages = 2;       // bulk-copy tiles in flight per warp (ring slots)
 constexpr int kSelMaxChunks = 32;   // chunks per row; S * M <= kSelCap must hold
 
 struct SelectParams {
@@ -70,6 +69,17 @@ template <> struct SelOps<__nv_bfloat16> {
         k1 = ord_key(__uint_as_float(b & 0xFFFF0000u));
     }
     static __device__ __forceinline__ void elems(const uint4 &v, float (&f)[8]) { unpack8(v, f); }
+    // bit i set <=> element i >= tau (packed compares, two elements per instruction)
+    static __device__ __forceinline__ unsigned int ge_mask(const uint4 &v, Run tau) {
+        const unsigned int m0 = __hge2_mask(from_bits(v.x), tau), m1 = __hge2_mask(from_bits(v.y), tau);
+        const unsigned int m2 = __hge2_mask(from_bits(v.z), tau), m3 = __hge2_mask(from_bits(v.w), tau);
+        return ((m0 & 1u) | ((m0 >> 15) & 2u)) | (((m1 & 1u) | ((m1 >> 15) & 2u)) << 2) |
+               (((m2 & 1u) | ((m2 >> 15) & 2u)) << 4) | (((m3 & 1u) | ((m3 >> 15) & 2u)) << 6);
+    }
+    static __device__ __forceinline__ float elem(const uint4 &v, int i) {
+        const unsigned int w = (i < 4) ? ((i < 2) ? v.x : v.y) : ((i < 6) ? v.z : v.w);
+        return __uint_as_float((i & 1) ? (w & 0xFFFF0000u) : (w << 16));
+    }
     static __device__ __forceinline__ uint4 load_scalar(const __nv_bfloat16 *row, long long e0, int V) {
         uint32_t w[4];
 #pragma unroll
@@ -97,6 +107,13 @@ template <> struct SelOps<float> {
     static __device__ __forceinline__ void elems(const uint4 &v, float (&f)[4]) {
         f[0] = __uint_as_float(v.x); f[1] = __uint_as_float(v.y); f[2] = __uint_as_float(v.z); f[3] = __uint_as_float(v.w);
     }
+    static __device__ __forceinline__ unsigned int ge_mask(const uint4 &v, Run tau) {
+        return (__uint_as_float(v.x) >= tau.a ? 1u : 0u) | (__uint_as_float(v.y) >= tau.a ? 2u : 0u) |
+               (__uint_as_float(v.z) >= tau.a ? 4u : 0u) | (__uint_as_float(v.w) >= tau.a ? 8u : 0u);
+    }
+    static __device__ __forceinline__ float elem(const uint4 &v, int i) {
+        return __uint_as_float((i < 2) ? ((i == 0) ? v.x : v.y) : ((i == 2) ? v.z : v.w));
+    }
     static __device__ __forceinline__ uint4 load_scalar(const float *row, long long e0, int V) {
         uint32_t w[4];
 #pragma unroll
@@ -106,17 +123,22 @@ template <> struct SelOps<float> {
 };
 
 
-struct SelectSmem {
-    unsigned long long cand[kSelCap];       // 8 warp-private segments of kSelSeg keys; reused for sorting / merging
-    unsigned long long fin[kSelFin];        // survivors of the final prune
-    uint4 qv[kSelWarps][kSelQ];             // per-warp queue: vectors that hold an element >= tau ...
-    int qi[kSelWarps][kSelQ];               // ... and their vector index in the row
-    unsigned int wcnt[kSelWarps];           // keys in each warp's segment
-    unsigned int claim[kSelWarps];          // c_w: >= q lanes of warp w have seen an element with ordered key >= c_w
-    unsigned int claimM[kSelWarps];         // >= M elements of warp w have ordered key >= claimM[w] (after a compaction)
+// Shared-memory state of one CTA.  SEG = keys per warp-private candidate segment (M <= SEG / 2),
+// FIN = survivors the epilogue ranks by counting, QCAP = per-warp queue of vectors awaiting the element filter.
+template <int SEG, int FIN, int QCAP>
+struct SelectSmemT {
+    static constexpr int kSeg = SEG, kCap = SEG * kSelWarps, kFin = FIN, kQ = QCAP;
+    unsigned long long cand[SEG * kSelWarps];   // 8 warp-private segments; reused for sorting / merging
+    unsigned long long fin[FIN];                // survivors of the final prune
+    uint4 qv[kSelWarps][QCAP];                  // per-warp queue: vectors that hold an element >= tau ...
+    int qi[kSelWarps][QCAP];                    // ... and their vector index in the row
+    unsigned int wcnt[kSelWarps];               // keys in each warp's segment
+    unsigned int claim[kSelWarps];              // c_w: >= q lanes of warp w have seen an element with ordered key >= c_w
+    unsigned int claimM[kSelWarps];             // >= M elements of warp w have ordered key >= claimM[w] (after a compaction)
     unsigned int cnt2;
     unsigned int is_last;
 };
+using SelectSmemBig = SelectSmemT<512, 512, 64>;      // any M <= 256 (47 KB static)
 
 // In-place descending bitonic sort of n (power of two) u64 keys in smem; all kSelThreads threads call.
 __device__ __forceinline__ void block_bitonic_desc(unsigned long long *s, int n) {
@@ -135,7 +157,7 @@ __device__ __forceinline__ void block_bitonic_desc(unsigned long long *s, int n)
         }
     }
 }
-// Same for one warp on its own segment (n a power of two <= kSelSeg); the 32 lanes of the warp call.
+// Same for one warp on its own segment (n a power of two); the 32 lanes of the warp call.
 __device__ __forceinline__ void warp_bitonic_desc(unsigned long long *s, int n, int lane) {
     for (int k = 2; k <= n; k <<= 1) {
         for (int j = k >> 1; j > 0; j >>= 1) {
@@ -168,7 +190,7 @@ __device__ __forceinline__ unsigned int warp_qth_largest(unsigned int key, int q
     return T;
 }
 
-// Rank `n` distinct keys (n <= kSelThreads * per-thread loop) by counting and hand the top M to `emit(rank, key)`.
+// Rank `n` distinct keys by counting and hand the top M to `emit(rank, key)`; all threads call.
 template <typename F>
 __device__ __forceinline__ void block_rank_emit(const unsigned long long *keys, int n, int M, F emit) {
     for (int i = threadIdx.x; i < n; i += kSelThreads) {
@@ -184,7 +206,7 @@ __device__ __forceinline__ void block_rank_emit(const unsigned long long *keys, 
     }
 }
 
-// Per-warp slow-path state kept in registers by the kernel and handed to the out-of-line helpers.
+// Per-warp slow-path state kept in registers by the kernels and handed to the out-of-line helpers by value.
 struct SelWarpCtx {
     unsigned int tau_ord;                // ordered-key lower bound on the row's M-th largest value
     unsigned long long wtau_key;         // exact key bound for this warp's own pushes (after a compaction)
@@ -192,9 +214,10 @@ struct SelWarpCtx {
 };
 
 // Keep the top M of this warp's segment (sort), remember the exact bound, publish the strong claim.
-__device__ __noinline__ SelWarpCtx sel_compact(SelectSmem &sm, SelWarpCtx c, int M) {
+template <typename SM>
+__device__ __noinline__ SelWarpCtx sel_compact(SM &sm, SelWarpCtx c, int M) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    unsigned long long *seg = sm.cand + warp * kSelSeg;
+    unsigned long long *seg = sm.cand + warp * SM::kSeg;
     volatile unsigned int *vwcnt = sm.wcnt, *vclaimM = sm.claimM;
     __syncwarp();
     int n = (int)vwcnt[warp];
@@ -216,31 +239,31 @@ __device__ __noinline__ SelWarpCtx sel_compact(SelectSmem &sm, SelWarpCtx c, int
 }
 
 // Filter the queued vectors, one vector per lane: append every element that can still be in the top M.
-template <typename T>
-__device__ __noinline__ SelWarpCtx sel_drain(SelectSmem &sm, SelWarpCtx c, int M, int V) {
+// A batch adds at most SEG / 2 keys; the segment is compacted first when it could overflow.
+template <typename T, typename SM>
+__device__ __noinline__ SelWarpCtx sel_drain(SM &sm, SelWarpCtx c, int M, int V) {
     using Ops = SelOps<T>;
     constexpr int kVec = ElemTraits<T>::kVec;
+    constexpr int kBatchKeys = SM::kSeg / 2;
+    constexpr int kLanes = (kBatchKeys / kVec) < 32 ? (kBatchKeys / kVec) : 32;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    unsigned long long *seg = sm.cand + warp * kSelSeg;
+    unsigned long long *seg = sm.cand + warp * SM::kSeg;
     volatile unsigned int *vwcnt = sm.wcnt;
     __syncwarp();
-    for (int base = 0; base < c.qcnt; base += 32) {
-        if ((int)vwcnt[warp] > kSelSeg - 32 * kVec) c = sel_compact(sm, c, M);      // this batch adds at most 32 * kVec keys
-        if (base + lane < c.qcnt) {
-            const float tau_f = ord_key_inv(c.tau_ord);
+    for (int base = 0; base < c.qcnt; base += kLanes) {
+        if ((int)vwcnt[warp] > SM::kSeg - kBatchKeys) c = sel_compact(sm, c, M);
+        if (lane < kLanes && base + lane < c.qcnt) {
             const uint4 v = sm.qv[warp][base + lane];
             const int gv = sm.qi[warp][base + lane];
-            float f[kVec];
-            Ops::elems(v, f);
-#pragma unroll
-            for (int i = 0; i < kVec; ++i) {
-                if (f[i] >= tau_f) {
-                    const unsigned int idx = (unsigned int)gv * kVec + i;
-                    const unsigned long long key = ((unsigned long long)ord_key(f[i]) << 32) | (unsigned long long)(0xFFFFFFFFu - idx);
-                    if (key > c.wtau_key && idx < (unsigned int)V) {
-                        const unsigned int pos = atomicAdd(&sm.wcnt[warp], 1u);
-                        seg[pos] = key;
-                    }
+            unsigned int mask = Ops::ge_mask(v, Ops::make_tau(c.tau_ord));      // usually one bit
+            while (mask) {
+                const int i = __ffs(mask) - 1;
+                mask &= mask - 1;
+                const unsigned int idx = (unsigned int)gv * kVec + i;
+                const unsigned long long key = ((unsigned long long)ord_key(Ops::elem(v, i)) << 32) | (unsigned long long)(0xFFFFFFFFu - idx);
+                if (key > c.wtau_key && idx < (unsigned int)V) {
+                    const unsigned int pos = atomicAdd(&sm.wcnt[warp], 1u);
+                    seg[pos] = key;
                 }
             }
         }
@@ -250,136 +273,77 @@ __device__ __noinline__ SelWarpCtx sel_drain(SelectSmem &sm, SelWarpCtx c, int M
     return c;
 }
 
-template <typename T, bool ALIGNED>
-__global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParams p) {
-    using Ops = SelOps<T>;
-    using Run = typename Ops::Run;
-    constexpr int kVec = ElemTraits<T>::kVec;
+// Publish this warp's claim: the q-th largest of its 32 lane maxima.
+template <typename T, typename SM>
+__device__ __forceinline__ void sel_publish_claim(SM &sm, typename SelOps<T>::Run run, int q) {
     constexpr int kNBits = (sizeof(T) == 2) ? 16 : 32;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    unsigned int k0, k1;
+    SelOps<T>::sub_keys(run, k0, k1);
+    unsigned int cl = warp_qth_largest<kNBits>(max(k0, k1), q);
+    // bf16: only the top 16 bits were resolved; keys of negative values end in 0xFFFF, of non-negative ones in 0
+    if (kNBits == 16 && !(cl & 0x80000000u)) cl |= 0xFFFFu;
+    if (lane == 0) *reinterpret_cast<volatile unsigned int *>(&sm.claim[warp]) = cl;
+}
+// tau = max(min_w claim[w], max_w claimM[w], the row-shared word); claims only grow, stale reads stay valid.
+template <typename SM>
+__device__ __forceinline__ unsigned int sel_read_tau(SM &sm, const SelectParams &p, int row) {
     constexpr unsigned int kFull = 0xffffffffu;
-    __shared__ __align__(16) SelectSmem sm;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    volatile unsigned int *vclaim = sm.claim, *vclaimM = sm.claimM;
+    unsigned int cw = (lane < kSelWarps) ? vclaim[lane] : 0xFFFFFFFFu;
+    unsigned int cm = (lane < kSelWarps) ? vclaimM[lane] : 0u;
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) {
+        cw = min(cw, __shfl_xor_sync(kFull, cw, o));
+        cm = max(cm, __shfl_xor_sync(kFull, cm, o));
+    }
+    unsigned int t = max(__shfl_sync(kFull, cw, 0), __shfl_sync(kFull, cm, 0));
+    if (p.S > 1) {
+        unsigned int g = 0;
+        if (lane == 0) g = (warp == 0) ? atomicMax(&p.row_tau[row], t) : *reinterpret_cast<volatile unsigned int *>(&p.row_tau[row]);
+        t = max(t, __shfl_sync(kFull, g, 0));
+    }
+    return t;
+}
+// One vector slot of a warp: lanes whose vector holds an element >= tau queue it; a full queue is drained.
+template <typename T, typename SM>
+__device__ __forceinline__ SelWarpCtx sel_slot(SM &sm, SelWarpCtx c, const uint4 &x, bool hit, int gv, int M, int V) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#ifdef DT_EXP_SELDRY
+    hit = false;
+#endif
+    const unsigned int bal = __ballot_sync(0xffffffffu, hit);
+    if (bal) {
+        if (hit) {
+            const int pos = c.qcnt + __popc(bal & ((1u << lane) - 1u));
+            sm.qv[warp][pos] = x;
+            sm.qi[warp][pos] = gv;
+        }
+        c.qcnt += __popc(bal);
+#ifdef DT_EXP_NODRAIN
+        if (c.qcnt > SM::kQ - 32) c.qcnt = 0;
+#else
+        if (c.qcnt > SM::kQ - 32) c = sel_drain<T>(sm, c, M, V);
+#endif
+    }
+    return c;
+}
 
+// Epilogue shared by both kernels: prune every segment with the final tau, rank the survivors, emit; chunked rows
+// publish their top M and the last chunk to arrive merges.  All threads call, after a CTA barrier.
+template <typename SM>
+__device__ __forceinline__ void sel_epilogue(SM &sm, const SelectParams &p, int row, int s, unsigned int tau_ord) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int row = blockIdx.y, s = blockIdx.x;
-    const int M = p.M, V = p.V;
-    const int q = (M + kSelWarps - 1) / kSelWarps;             // lanes per warp that must back a claim (<= 32)
-    const T *rowp = reinterpret_cast<const T *>(p.logits) + (size_t)row * V;
-    const int v0 = s * p.chunk_vecs;
-    const int v1 = min(p.row_vecs, v0 + p.chunk_vecs);
-    const int tile_vecs = kSelThreads * kSelU;
-    const int n_tiles = (max(v1 - v0, 0) + tile_vecs - 1) / tile_vecs;
-    unsigned long long *seg = sm.cand + warp * kSelSeg;
-    volatile unsigned int *vclaim = sm.claim, *vclaimM = sm.claimM, *vwcnt = sm.wcnt;
-
-    if (tid < kSelWarps) { sm.wcnt[tid] = 0; sm.claim[tid] = 0; sm.claimM[tid] = 0; }
-    if (tid == 0) { sm.cnt2 = 0; sm.is_last = 0; }
-    __syncthreads();
-
-    const int n_full = max(v1 - v0, 0) / tile_vecs;            // tiles that need no bounds checks
-    auto load_tile = [&](int t, uint4 (&buf)[kSelU]) {
-        if (ALIGNED && t < n_full) {
-            const T *q = rowp + (size_t)(v0 + t * tile_vecs + tid) * kVec;
-#pragma unroll
-            for (int u = 0; u < kSelU; ++u) buf[u] = ld_stream_v4(q + (size_t)u * kSelThreads * kVec);
-            return;
-        }
-#pragma unroll
-        for (int u = 0; u < kSelU; ++u) {
-            int gv = v0 + t * tile_vecs + u * kSelThreads + tid;
-            if (gv < v1) {
-                if (ALIGNED) buf[u] = ld_stream_v4(rowp + (size_t)gv * kVec);
-                else buf[u] = Ops::load_scalar(rowp, (long long)gv * kVec, V);
-            } else buf[u] = Ops::lowest_vec();
-        }
-    };
-
-    SelWarpCtx c;
-    c.tau_ord = 0; c.wtau_key = 0ull; c.qcnt = 0;
-    Run run = Ops::lowest();                 // this lane's running maximum (two packed halves)
-
-    // Publish this warp's claim: the q-th largest of its 32 lane maxima.
-    auto publish_claim = [&]() {
-        unsigned int k0, k1;
-        Ops::sub_keys(run, k0, k1);
-        unsigned int cl = warp_qth_largest<kNBits>(max(k0, k1), q);
-        // bf16: only the top 16 bits were resolved; keys of negative values end in 0xFFFF, of non-negative ones in 0
-        if (kNBits == 16 && !(cl & 0x80000000u)) cl |= 0xFFFFu;
-        if (lane == 0) vclaim[warp] = cl;
-    };
-    // tau = max(min_w claim[w], max_w claimM[w], the row-shared word); claims only grow, stale reads stay valid.
-    auto read_tau = [&]() {
-        unsigned int cw = (lane < kSelWarps) ? vclaim[lane] : 0xFFFFFFFFu;
-        unsigned int cm = (lane < kSelWarps) ? vclaimM[lane] : 0u;
-#pragma unroll
-        for (int o = 4; o > 0; o >>= 1) {
-            cw = min(cw, __shfl_xor_sync(kFull, cw, o));
-            cm = max(cm, __shfl_xor_sync(kFull, cm, o));
-        }
-        unsigned int t = max(__shfl_sync(kFull, cw, 0), __shfl_sync(kFull, cm, 0));
-        if (p.S > 1) {
-            unsigned int g = 0;
-            if (lane == 0) g = (warp == 0) ? atomicMax(&p.row_tau[row], t) : *reinterpret_cast<volatile unsigned int *>(&p.row_tau[row]);
-            t = max(t, __shfl_sync(kFull, g, 0));
-        }
-        c.tau_ord = max(c.tau_ord, t);
-    };
-
-    uint4 A[kSelU], Bn[kSelU];
-    if (n_tiles > 0) {
-        load_tile(0, A);
-#pragma unroll
-        for (int u = 0; u < kSelU; ++u) run = Ops::rmax(run, Ops::vmax(A[u]));
-    }
-    publish_claim();
-    __syncthreads();                          // the only CTA barrier before the epilogue: every warp has a claim
-    read_tau();
-
-    // Vectors that hold an element >= tau are queued (a few instructions, whichever lanes hit); when more than 32
-    // wait, the warp filters them one vector per lane (sel_drain), so the element filter always runs with full lanes.
-    uint4 *qv = sm.qv[warp];
-    int *qi = sm.qi[warp];
-    auto process = [&](const uint4 (&X)[kSelU], int t) {
-        const Run tau = Ops::make_tau(c.tau_ord);
-        const int gv0 = v0 + t * tile_vecs + tid;
-#pragma unroll
-        for (int u = 0; u < kSelU; ++u) {
-            const Run m = Ops::vmax(X[u]);
-            run = Ops::rmax(run, m);
-            const bool hu = Ops::pass(m, tau);
-            const unsigned int bal = __ballot_sync(kFull, hu);
-            if (bal) {                                   // some lane of the warp holds an element >= tau in this vector slot
-                if (hu) {
-                    const int pos = c.qcnt + __popc(bal & ((1u << lane) - 1u));
-                    qv[pos] = X[u];
-                    qi[pos] = gv0 + u * kSelThreads;
-                }
-                c.qcnt += __popc(bal);
-                if (c.qcnt > 32) c = sel_drain<T>(sm, c, M, V);
-            }
-        }
-        if (t > 0 && (((t + 1) & t) == 0) && (t + 1 < n_tiles)) { publish_claim(); __syncwarp(); read_tau(); }
-    };
-    for (int t = 0; t < n_tiles; t += 2) {      // ping-pong between the two register tiles
-        if (t + 1 < n_tiles) load_tile(t + 1, Bn);
-        process(A, t);
-        if (t + 1 < n_tiles) {
-            if (t + 2 < n_tiles) load_tile(t + 2, A);
-            process(Bn, t + 1);
-        }
-    }
-    c = sel_drain<T>(sm, c, M, V);
-
-    // Epilogue: final tau, prune every segment, rank the survivors, emit.
-    publish_claim();
-    __syncthreads();
-    read_tau();
+    const int M = p.M;
+    unsigned long long *seg = sm.cand + warp * SM::kSeg;
     {
         const int n = (int)sm.wcnt[warp];
         for (int i = lane; i < n; i += 32) {
             const unsigned long long key = seg[i];
-            if ((unsigned int)(key >> 32) >= c.tau_ord) {
+            if ((unsigned int)(key >> 32) >= tau_ord) {
                 const unsigned int pos = atomicAdd(&sm.cnt2, 1u);
-                if (pos < (unsigned int)kSelFin) sm.fin[pos] = key;
+                if (pos < (unsigned int)SM::kFin) sm.fin[pos] = key;
             }
         }
     }
@@ -393,16 +357,16 @@ __global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParam
     };
     auto out_part = [&](int rank, unsigned long long key) { part[rank] = key; };
 
-    if (c2 <= kSelFin) {
+    if (c2 <= SM::kFin) {
         if (p.S == 1) { block_rank_emit(sm.fin, c2, M, out_single); return; }
         block_rank_emit(sm.fin, c2, M, out_part);
         for (int i = c2 + tid; i < M; i += kSelThreads) part[i] = 0ull;      // chunk with fewer than M elements
     } else {
-        // adversarial rows (more than kSelFin survivors): sort everything that was kept
+        // adversarial rows (more than kFin survivors): sort everything that was kept
         const int n = (int)sm.wcnt[warp];
-        for (int i = n + lane; i < kSelSeg; i += 32) seg[i] = 0ull;
+        for (int i = n + lane; i < SM::kSeg; i += 32) seg[i] = 0ull;
         __syncthreads();
-        block_bitonic_desc(sm.cand, kSelCap);
+        block_bitonic_desc(sm.cand, SM::kCap);
         for (int i = tid; i < M; i += kSelThreads) { if (p.S == 1) out_single(i, sm.cand[i]); else out_part(i, sm.cand[i]); }
         if (p.S == 1) return;
     }
@@ -421,19 +385,19 @@ __global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParam
     const unsigned int gtau = *reinterpret_cast<volatile unsigned int *>(&p.row_tau[row]);
     if (tid == 0) sm.cnt2 = 0;
     __syncthreads();
-    const int tot = p.S * M;
+    const int tot = p.S * M;                                   // <= SM::kCap (launcher)
     const unsigned long long *allp = p.part + (size_t)row * p.S * M;
     for (int i = tid; i < tot; i += kSelThreads) {
         const unsigned long long key = __ldcg(allp + i);
         sm.cand[i] = key;
         if ((unsigned int)(key >> 32) >= gtau && key != 0ull) {
             const unsigned int pos = atomicAdd(&sm.cnt2, 1u);
-            if (pos < (unsigned int)kSelFin) sm.fin[pos] = key;
+            if (pos < (unsigned int)SM::kFin) sm.fin[pos] = key;
         }
     }
     __syncthreads();
     const int c3 = (int)sm.cnt2;
-    if (c3 <= kSelFin) {
+    if (c3 <= SM::kFin) {
         block_rank_emit(sm.fin, c3, M, out_single);
     } else {
         const int n2 = next_pow2(max(tot, 2));
@@ -443,6 +407,215 @@ __global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParam
         for (int i = tid; i < M; i += kSelThreads) out_single(i, sm.cand[i]);
     }
     if (tid == 0) { p.row_counter[row] = 0u; p.row_tau[row] = 0u; }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Register-tile kernel: any alignment, any M <= 256.  Each thread keeps two tiles of four 16-byte vectors in
+// registers (ping-pong) and loads them with 128-bit streaming loads (scalar loads when the row is unaligned).
+template <typename T, bool ALIGNED>
+__global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParams p) {
+    using Ops = SelOps<T>;
+    using Run = typename Ops::Run;
+    using SM = SelectSmemBig;
+    constexpr int kVec = ElemTraits<T>::kVec;
+    __shared__ __align__(16) SM sm;
+
+    const int tid = threadIdx.x;
+    const int row = blockIdx.y, s = blockIdx.x;
+    const int M = p.M, V = p.V;
+    const int q = (M + kSelWarps - 1) / kSelWarps;             // lanes per warp that must back a claim (<= 32)
+    const T *rowp = reinterpret_cast<const T *>(p.logits) + (size_t)row * V;
+    const int v0 = s * p.chunk_vecs;
+    const int v1 = min(p.row_vecs, v0 + p.chunk_vecs);
+    const int tile_vecs = kSelThreads * kSelU;
+    const int n_tiles = (max(v1 - v0, 0) + tile_vecs - 1) / tile_vecs;
+
+    if (tid < kSelWarps) { sm.wcnt[tid] = 0; sm.claim[tid] = 0; sm.claimM[tid] = 0; }
+    if (tid == 0) { sm.cnt2 = 0; sm.is_last = 0; }
+    __syncthreads();
+
+    const int n_full = max(v1 - v0, 0) / tile_vecs;            // tiles that need no bounds checks
+    auto load_tile = [&](int t, uint4 (&buf)[kSelU]) {
+        if (ALIGNED && t < n_full) {
+            const T *qp = rowp + (size_t)(v0 + t * tile_vecs + tid) * kVec;
+#pragma unroll
+            for (int u = 0; u < kSelU; ++u) buf[u] = ld_stream_v4(qp + (size_t)u * kSelThreads * kVec);
+            return;
+        }
+#pragma unroll
+        for (int u = 0; u < kSelU; ++u) {
+            int gv = v0 + t * tile_vecs + u * kSelThreads + tid;
+            if (gv < v1) {
+                if (ALIGNED) buf[u] = ld_stream_v4(rowp + (size_t)gv * kVec);
+                else buf[u] = Ops::load_scalar(rowp, (long long)gv * kVec, V);
+            } else buf[u] = Ops::lowest_vec();
+        }
+    };
+
+    SelWarpCtx c;
+    c.tau_ord = 0; c.wtau_key = 0ull; c.qcnt = 0;
+    Run run = Ops::lowest();                 // this lane's running maximum (two packed halves)
+
+    uint4 A[kSelU], Bn[kSelU];
+    if (n_tiles > 0) {
+        load_tile(0, A);
+#pragma unroll
+        for (int u = 0; u < kSelU; ++u) run = Ops::rmax(run, Ops::vmax(A[u]));
+    }
+    sel_publish_claim<T>(sm, run, q);
+    __syncthreads();                          // the only CTA barrier before the epilogue: every warp has a claim
+    c.tau_ord = max(c.tau_ord, sel_read_tau(sm, p, row));
+
+    auto process = [&](const uint4 (&X)[kSelU], int t) {
+        const Run tau = Ops::make_tau(c.tau_ord);
+        const int gv0 = v0 + t * tile_vecs + tid;
+#pragma unroll
+        for (int u = 0; u < kSelU; ++u) {
+            const Run m = Ops::vmax(X[u]);
+            run = Ops::rmax(run, m);
+            c = sel_slot<T>(sm, c, X[u], Ops::pass(m, tau), gv0 + u * kSelThreads, M, V);
+        }
+#ifndef DT_EXP_NOCLAIM
+        if (t > 0 && (((t + 1) & t) == 0) && (t + 1 < n_tiles)) {
+            sel_publish_claim<T>(sm, run, q);
+            __syncwarp();
+            c.tau_ord = max(c.tau_ord, sel_read_tau(sm, p, row));
+        }
+#endif
+    };
+    for (int t = 0; t < n_tiles; t += 2) {      // ping-pong between the two register tiles
+        if (t + 1 < n_tiles) load_tile(t + 1, Bn);
+        process(A, t);
+        if (t + 1 < n_tiles) {
+            if (t + 2 < n_tiles) load_tile(t + 2, A);
+            process(Bn, t + 1);
+        }
+    }
+    c = sel_drain<T>(sm, c, M, V);
+
+    sel_publish_claim<T>(sm, run, q);
+    __syncthreads();
+    c.tau_ord = max(c.tau_ord, sel_read_tau(sm, p, row));
+    sel_epilogue(sm, p, row, s, c.tau_ord);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Bulk-copy kernel (16-byte aligned rows, M <= 128): every warp streams its own 2 KB tiles from HBM into a private
+// ring in shared memory with cp.async.bulk (one elected lane issues; completion on an mbarrier), kSelStages tiles
+// in flight per warp, and reads them back with conflict-free 128-bit shared loads.  No load instruction or
+// register is spent per vector on the global side, so more bytes are in flight per SM (3 CTAs x 8 warps x 2 tiles).
+__device__ __forceinline__ void sel_mbar_init(unsigned int bar, unsigned int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void sel_mbar_wait(unsigned int bar, unsigned int parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n"
+        "DT_SEL_WAIT:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DT_SEL_DONE;\n\t"
+        "bra DT_SEL_WAIT;\n"
+        "DT_SEL_DONE:\n\t}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void sel_bulk_load(unsigned int dst, const void *src, unsigned int bytes, unsigned int bar) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+constexpr int kSelTileVecs = kSelTileBytes / 16;
+constexpr int kBulkU = kSelTileVecs / 32;        // vectors per lane per tile
+constexpr size_t kSelBulkDynSmem = (size_t)kSelWarps * kSelStages * kSelTileBytes + (size_t)kSelWarps * kSelStages * 8;
+
+template <typename T>
+__global__ void __launch_bounds__(kSelThreads, 2) select_topm_bulk_kernel(SelectParams p) {
+    using Ops = SelOps<T>;
+    using Run = typename Ops::Run;
+    using SM = SelectSmemBig;
+    constexpr int kVec = ElemTraits<T>::kVec;
+    __shared__ __align__(16) SM sm;
+    extern __shared__ __align__(128) unsigned char sel_dyn[];
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int row = blockIdx.y, s = blockIdx.x;
+    const int M = p.M, V = p.V;
+    const int q = (M + kSelWarps - 1) / kSelWarps;
+    const T *rowp = reinterpret_cast<const T *>(p.logits) + (size_t)row * V;
+    const int v0 = s * p.chunk_vecs;
+    const int v1 = min(p.row_vecs, v0 + p.chunk_vecs);
+    const int n_ctiles = (max(v1 - v0, 0) + kSelTileVecs - 1) / kSelTileVecs;       // 2 KB tiles of the chunk
+    const int n_w = (n_ctiles > warp) ? (n_ctiles - warp + kSelWarps - 1) / kSelWarps : 0;   // tiles of this warp
+
+    unsigned char *ring = sel_dyn + (size_t)warp * kSelStages * kSelTileBytes;
+    const unsigned int ring_a = (unsigned int)__cvta_generic_to_shared(ring);
+    const unsigned int bar_a = (unsigned int)__cvta_generic_to_shared(sel_dyn + (size_t)kSelWarps * kSelStages * kSelTileBytes) +
+                               (unsigned int)warp * kSelStages * 8;
+
+    if (tid < kSelWarps) { sm.wcnt[tid] = 0; sm.claim[tid] = 0; sm.claimM[tid] = 0; }
+    if (tid == 0) { sm.cnt2 = 0; sm.is_last = 0; }
+    if (lane == 0) {
+        for (int i = 0; i < kSelStages; ++i) sel_mbar_init(bar_a + 8 * i, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // tile i of this warp = chunk tile warp + 8 i: vectors [tv0, tv0 + nv)
+    auto issue = [&](int i) {
+        const int tv0 = v0 + (warp + kSelWarps * i) * kSelTileVecs;
+        const int nv = min(kSelTileVecs, v1 - tv0);
+        const int slot = i % kSelStages;
+        sel_bulk_load(ring_a + slot * kSelTileBytes, rowp + (size_t)tv0 * kVec, (unsigned int)nv * 16u, bar_a + 8 * slot);
+    };
+    if (lane == 0) for (int i = 0; i < kSelStages && i < n_w; ++i) issue(i);
+
+    SelWarpCtx c;
+    c.tau_ord = 0; c.wtau_key = 0ull; c.qcnt = 0;
+    Run run = Ops::lowest();
+    auto load_slot = [&](int i, uint4 (&X)[kBulkU]) {            // lane's vectors u * 32 + lane of tile i
+        const int nv = min(kSelTileVecs, v1 - (v0 + (warp + kSelWarps * i) * kSelTileVecs));
+        const uint4 *src = reinterpret_cast<const uint4 *>(ring + (size_t)(i % kSelStages) * kSelTileBytes);
+#pragma unroll
+        for (int u = 0; u < kBulkU; ++u) X[u] = (u * 32 + lane < nv) ? src[u * 32 + lane] : Ops::lowest_vec();
+    };
+
+    // first tile: fold into the running maxima so that every warp can back a claim before any push
+    uint4 X[kBulkU];
+    if (n_w > 0) {
+        sel_mbar_wait(bar_a, 0);
+        load_slot(0, X);
+#pragma unroll
+        for (int u = 0; u < kBulkU; ++u) run = Ops::rmax(run, Ops::vmax(X[u]));
+    }
+    sel_publish_claim<T>(sm, run, q);
+    __syncthreads();
+    c.tau_ord = max(c.tau_ord, sel_read_tau(sm, p, row));
+
+    for (int i = 0; i < n_w; ++i) {
+        if (i > 0) { sel_mbar_wait(bar_a + 8 * (i % kSelStages), (unsigned int)((i / kSelStages) & 1)); load_slot(i, X); }
+        __syncwarp();                                           // every lane has read the slot: refill it
+        if (lane == 0 && i + kSelStages < n_w) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic reads above, async write below
+            issue(i + kSelStages);
+        }
+        const Run tau = Ops::make_tau(c.tau_ord);
+        const int gv0 = v0 + (warp + kSelWarps * i) * kSelTileVecs + lane;
+#pragma unroll
+        for (int u = 0; u < kBulkU; ++u) {
+            const Run m = Ops::vmax(X[u]);
+            run = Ops::rmax(run, m);
+            c = sel_slot<T>(sm, c, X[u], Ops::pass(m, tau), gv0 + u * 32, M, V);
+        }
+        if (i > 0 && (((i + 1) & i) == 0) && (i + 1 < n_w)) {
+            sel_publish_claim<T>(sm, run, q);
+            __syncwarp();
+            c.tau_ord = max(c.tau_ord, sel_read_tau(sm, p, row));
+        }
+    }
+    c = sel_drain<T>(sm, c, M, V);
+
+    sel_publish_claim<T>(sm, run, q);
+    __syncthreads();
+    c.tau_ord = max(c.tau_ord, sel_read_tau(sm, p, row));
+    sel_epilogue(sm, p, row, s, c.tau_ord);
 }
 
 }  // namespace dt
