@@ -53,6 +53,27 @@ def test_select_qwen_rows_exact_all_chunkings(M, chunks):
         case.builder.set_option("select_chunks", 0)
 
 
+@pytest.mark.parametrize("chunks", [1, 4])
+def test_select_register_tile_kernel_on_aligned_rows(chunks):
+    """The register-tile kernel (select_kernel = 1; the default for aligned rows is the bulk-copy kernel) on
+    Qwen-sized rows and on the adversarial rows, M = 64 and M = 256 (largest supported)."""
+    gu = _gu()
+    case = gu.get_case("qwen8b-m256", wl.CONFIGS["qwen8b"], max_batch=1, max_M=256, max_B=16, k=8)
+    inp = wl.make_inputs(case.cfg, batch=1, regime="peaked")
+    rows = wl.adversarial_select_rows(case.cfg.V, case.cfg.torch_dtype)
+    adv = torch.stack(list(rows.values()))
+    case.builder.set_option("select_chunks", chunks)
+    try:
+        for kern in (1, 0):
+            case.builder.set_option("select_kernel", kern)
+            _check_select(case.builder, inp["logits"], 256)
+            _check_select(case.builder, inp["logits"], 64)
+            _check_select(case.builder, adv, 256)
+    finally:
+        case.builder.set_option("select_kernel", 0)
+        case.builder.set_option("select_chunks", 0)
+
+
 @pytest.mark.parametrize("dtype", ["bf16", "f32"])
 @pytest.mark.parametrize("chunks", [1, 3])
 def test_select_adversarial_rows(dtype, chunks):
