@@ -295,7 +295,7 @@ extern "C" int dt_destroy(dt_handle *h) {
     return DT_OK;
 }
 
-static int pick_chunks(const dt_handle *h, int rows, int M, int cap) {
+static int pick_chunks(const dt_handle *h, int rows, int M, int cap, int row_vecs) {
     int smax = cap / M;                             // the merging CTA holds S * M keys in its candidate buffer
     if (smax > kSelMaxChunks) smax = kSelMaxChunks;
     if (smax < 1) smax = 1;
@@ -304,6 +304,11 @@ static int pick_chunks(const dt_handle *h, int rows, int M, int cap) {
     else {
         const int target = 3 * h->num_sms;          // resident CTAs wanted
         S = (target + rows - 1) / rows;
+        // A chunk must keep all 8 warps of its CTA busy for a few tiles, or their threshold claims are worthless
+        // and everything is pushed (measured at batch 1, V = 151 936: S = 4 -> 16 us, S = 28 -> 390 us).
+        int by_len = row_vecs / 4096;
+        if (by_len < 1) by_len = 1;
+        if (S > by_len) S = by_len;
     }
     if (S > smax) S = smax;
     if (S < 1) S = 1;
@@ -320,7 +325,7 @@ static int launch_select(dt_handle *h, const void *logits, int rows, int M, int3
     SelectParams p;
     p.logits = logits; p.rows = rows; p.V = V; p.M = M;
     p.row_vecs = (V + kvec - 1) / kvec;
-    int S = pick_chunks(h, rows, M, SelectSmemBig::kCap);
+    int S = pick_chunks(h, rows, M, SelectSmemBig::kCap, p.row_vecs);
     if (S > p.row_vecs) S = p.row_vecs;
     p.S = S;
     p.chunk_vecs = (p.row_vecs + S - 1) / S;
