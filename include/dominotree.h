@@ -127,6 +127,25 @@ int dt_build_trees_host(dt_handle *h, const void *marginal_logits_host, const vo
                         int32_t batch, int32_t M, int32_t B, float temperature,
                         const dt_outputs *out_host, void *stream);
 
+/*
+ * dt_commit_paths: longest-accepted-path commit over the trees of one round (Sec. 3.5: "we
+ * commit the highest-scoring root-to-leaf path along which every edge is accepted").  `tree` holds the DEVICE
+ * outputs of dt_build_trees for the same batch and B (tokens, parents, depths, scores, n_nodes are read; N = B+1).
+ * Exactly one of the two acceptance inputs is non-NULL:
+ *   target_next [batch, N] int32 device -- greedy verification: the token the target model predicts after each
+ *                tree node; the edge parent u -> node i is accepted iff tokens[i] == target_next[u];
+ *   edge_ok     [batch, N] uint8 device -- any other rule: edge into node i accepted iff edge_ok[i] != 0.
+ * A node is reachable iff every edge of its root path is accepted; the path ends at the reachable node of greatest
+ * depth, then highest draft score, then lowest slot (dead-leaf padding slots never qualify).  Outputs (device):
+ *   accept_len  [batch]        number of accepted draft tokens (depth of the end node, 0 = only the root)
+ *   path_slots  [batch, L+1]   tree slots of the path, root first, padded with -1
+ *   bonus_token [batch] or NULL  target_next at the end node (-1 in edge_ok mode)
+ * Asynchronous, capture-safe.  Errors: INVALID_ARG for null pointers, both or neither acceptance input, batch or B
+ * out of range.
+ */
+int dt_commit_paths(dt_handle *h, const dt_outputs *tree, int32_t batch, int32_t B, const int32_t *target_next,
+                    const uint8_t *edge_ok, int32_t *accept_len, int32_t *path_slots, int32_t *bonus_token, void *stream);
+
 /* dt_set_option: tuning knobs for experiments (e.g. "select_chunks"); unknown name -> INVALID_ARG. */
 int dt_set_option(dt_handle *h, const char *name, int64_t value);
 

@@ -17,7 +17,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libdominotree.so")
 
 DT_BF16, DT_F32 = 0, 1
-EXPORTS = ("dt_create", "dt_build_trees", "dt_select_topm", "dt_build_trees_host", "dt_set_option",
+EXPORTS = ("dt_create", "dt_build_trees", "dt_select_topm", "dt_build_trees_host", "dt_commit_paths", "dt_set_option",
            "dt_kernel_launches", "dt_destroy", "dt_error_string", "dt_version", "dt_workspace_bytes",
            "dt_last_cuda_error", "dt_phase_timing", "dt_phase_slot", "dt_phase_elapsed_ms")
 PHASES = ("select", "precompute", "expand", "emit")
@@ -60,6 +60,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.dt_build_trees.restype = ctypes.c_int
     lib.dt_build_trees_host.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, f32, ctypes.POINTER(_Outputs), vp]
     lib.dt_build_trees_host.restype = ctypes.c_int
+    lib.dt_commit_paths.argtypes = [vp, ctypes.POINTER(_Outputs), i32, i32, vp, vp, vp, vp, vp, vp]
+    lib.dt_commit_paths.restype = ctypes.c_int
     lib.dt_select_topm.argtypes = [vp, vp, i32, i32, vp, vp, vp]
     lib.dt_select_topm.restype = ctypes.c_int
     lib.dt_set_option.argtypes = [vp, ctypes.c_char_p, i64]
@@ -197,6 +199,29 @@ class DominoTreeBuilder:
         st = stream if stream is not None else torch.cuda.current_stream()
         rc = self.lib.dt_select_topm(self._h, lg.data_ptr(), lg.shape[0], M, ids.data_ptr(), vals.data_ptr(), st.cuda_stream)
         _check(self.lib, rc, "dt_select_topm", self._h)
+
+    def commit_paths(self, tree: TreeBatch, B: int, target_next=None, edge_ok=None, stream=None):
+        """dt_commit_paths: longest accepted path of every tree -> (accept_len [batch], path_slots [batch, L+1],
+        bonus_token [batch]) on the device.  Pass target_next (int32 [batch, B+1], greedy verification) or
+        edge_ok (uint8 [batch, B+1])."""
+        import torch
+        batch = tree.tokens.shape[0]
+        if target_next is not None:
+            self._check_in(target_next, (batch, B + 1), torch.int32, True)
+        if edge_ok is not None:
+            self._check_in(edge_ok, (batch, B + 1), torch.uint8, True)
+        dev = tree.tokens.device
+        acc = torch.empty((batch,), dtype=torch.int32, device=dev)
+        path = torch.empty((batch, self.L + 1), dtype=torch.int32, device=dev)
+        bonus = torch.empty((batch,), dtype=torch.int32, device=dev)
+        st = stream if stream is not None else torch.cuda.current_stream()
+        os_ = tree._struct()
+        rc = self.lib.dt_commit_paths(self._h, ctypes.byref(os_), batch, B,
+                                      target_next.data_ptr() if target_next is not None else None,
+                                      edge_ok.data_ptr() if edge_ok is not None else None,
+                                      acc.data_ptr(), path.data_ptr(), bonus.data_ptr(), st.cuda_stream)
+        _check(self.lib, rc, "dt_commit_paths", self._h)
+        return acc, path, bonus
 
     def build_trees_host(self, marginal_logits, backbone_hidden, root_tokens, root_positions, M: int, B: int,
                          temperature: float, out: Optional[TreeBatch] = None, stream=None) -> TreeBatch:

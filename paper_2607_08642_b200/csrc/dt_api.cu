@@ -9,6 +9,7 @@
 #include <string.h>
 
 #include "../../include/dominotree.h"
+#include "dt_commit.cuh"
 #include "dt_expand.cuh"
 #include "dt_fused.cuh"
 #include "dt_precompute.cuh"
@@ -491,6 +492,27 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
         return launch_expansion<__nv_bfloat16>(h, p, st);
     }
     return launch_expansion<float>(h, p, st);
+}
+
+extern "C" int dt_commit_paths(dt_handle *h, const dt_outputs *tree, int32_t batch, int32_t B, const int32_t *target_next,
+                               const uint8_t *edge_ok, int32_t *accept_len, int32_t *path_slots, int32_t *bonus_token,
+                               void *stream) {
+    if (!h || !tree) return DT_ERR_INVALID_ARG;
+    if (batch < 0 || batch > h->max_batch || B < 1 || B > h->max_B) return DT_ERR_INVALID_ARG;
+    if ((target_next != nullptr) == (edge_ok != nullptr)) return DT_ERR_INVALID_ARG;
+    h->launches = 0;
+    if (batch == 0) return DT_OK;
+    if (!tree->tokens || !tree->parents || !tree->depths || !tree->scores || !tree->n_nodes || !accept_len || !path_slots)
+        return DT_ERR_INVALID_ARG;
+    CommitParams c;
+    c.tokens = tree->tokens; c.parents = tree->parents; c.depths = tree->depths; c.n_nodes = tree->n_nodes;
+    c.scores = tree->scores; c.target_next = target_next; c.edge_ok = edge_ok;
+    c.accept_len = accept_len; c.path_slots = path_slots; c.bonus_token = bonus_token;
+    c.N = B + 1; c.L = h->L;
+    commit_paths_kernel<<<batch, 256, 0, (cudaStream_t)stream>>>(c);
+    h->launches++;
+    DT_CUDA(h, cudaGetLastError());
+    return DT_OK;
 }
 
 extern "C" int dt_build_trees_host(dt_handle *h, const void *logits_h, const void *hidden_h,
