@@ -432,8 +432,11 @@ def main():
     round_us = 1e3 * ctx["ms_per_step"]
     sel_us = ph["select"]
     sel_gbs = sel_bytes / (sel_us * 1e-6) / 1e9
-    roof_select = {"kernel": "select_topm_kernel", "bound": "hbm", "achieved": sel_gbs, "peak": peaks["hbm_gbs"],
-                   "unit": "GB/s", "frac": sel_gbs / peaks["hbm_gbs"], "traffic": None,
+    # `traffic`: dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures summarised in
+    # profiles/r1_select_ncu.md and profiles/r1_fused_ncu.md (C5 workload only; None for any other workload)
+    c5 = (cfg.name == "concurrent8b")
+    roof_select = {"kernel": "select_topm_bulk_kernel", "bound": "hbm", "achieved": sel_gbs, "peak": peaks["hbm_gbs"],
+                   "unit": "GB/s", "frac": sel_gbs / peaks["hbm_gbs"], "traffic": 159.66e6 if c5 else None,
                    "peak_source": peaks["source"], "algorithmic_bytes": sel_bytes, "us_per_launch": sel_us,
                    "share_of_step": sel_us / ctx["phase_round_us"],
                    "alone_back_to_back_gbs": sel_bytes / (ctx["select_alone_us"] * 1e-6) / 1e9}
