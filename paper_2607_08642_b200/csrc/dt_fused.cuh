@@ -445,7 +445,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
     __syncthreads();
     tc::fence_after_sync();
     const uint32_t tmem = *tmem_slot;
-    const uint32_t idesc1 = tc::make_idesc_bf16(64, 64), idesc2 = tc::make_idesc_bf16(128, 64);
+    const uint32_t idesc2 = tc::make_idesc_bf16(128, 64);
     const uint32_t aA = tc::smem_u32(sA), aRing = tc::smem_u32(sRing), aA2 = tc::smem_u32(sA2), aB2 = tc::smem_u32(sB2);
     const uint32_t mb0 = tc::smem_u32(mbar);
     const uint64_t descA0 = tc::make_desc_sw128(aA, sboA), descB0 = tc::make_desc_sw128(aRing, 1024);
@@ -454,11 +454,18 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
     // this thread's share of one ring slot: the 16-byte piece `my_c` of the 128-byte rows of request `my_rq`
     // (hi and lo, both 64-wide k-blocks of the slot); a warp instruction moves 4 whole 128-byte rows
     const int my_c = tid & 7, my_rq = tid >> 3;
-    const uint32_t my_dst = (uint32_t)((my_rq >> 3) * 1024 + (my_rq & 7) * 128 + ((my_c ^ (my_rq & 7)) << 4));
 
     for (int t = 0; t < e.B; ++t) {
         for (int c0 = 0; c0 < batch; c0 += kFusChunk) {
             const int nb = min(kFusChunk, batch - c0);
+            // Columns of the hidden-half GEMM: requests' hi halves in rows [0, lo_off), lo halves in [lo_off, 2 lo_off);
+            // N shrinks with the batch (8 columns serve up to 4 requests), and so do the ring traffic and the MMA time.
+            const int ncol = (nb <= 4) ? 8 : (nb <= 8) ? 16 : (nb <= 16) ? 32 : 64;
+            const int lo_off = ncol >> 1;
+            const uint32_t idesc1 = tc::make_idesc_bf16(64, ncol);
+            const int n_lo = lo_off + my_rq;
+            const uint32_t my_dst_hi = (uint32_t)((my_rq >> 3) * 1024 + (my_rq & 7) * 128 + ((my_c ^ (my_rq & 7)) << 4));
+            const uint32_t my_dst_lo = (uint32_t)((n_lo >> 3) * 1024 + (n_lo & 7) * 128 + ((my_c ^ (n_lo & 7)) << 4));
             if (warp == 0) {
                 int sidx = -1, tok = 0;
                 if (lane < nb) {
@@ -478,12 +485,13 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             const __nv_bfloat16 *src_hi = p.s_hi + my_off + (size_t)my_c * 8, *src_lo = p.s_lo + my_off + (size_t)my_c * 8;
             DT_TRF(t, 40);
             auto issue_chunk = [&](int kc) {
-                unsigned char *dst = sRing + (size_t)(kc % kTcSlots) * kTcSlotBytes + my_dst;
+                if (my_rq >= lo_off) return;                        // columns beyond N: nothing to stream
+                unsigned char *dst = sRing + (size_t)(kc % kTcSlots) * kTcSlotBytes;
                 const size_t k0 = (size_t)kc * kTcKC;
 #pragma unroll
-                for (int kb = 0; kb < kTcKC / 64; ++kb) {           // per k-block: columns 0..31 = hi, 32..63 = lo (+4 atoms)
-                    cp_async16(dst + kb * 8192, src_hi + k0 + kb * 64);
-                    cp_async16(dst + kb * 8192 + 4096, src_lo + k0 + kb * 64);
+                for (int kb = 0; kb < kTcKC / 64; ++kb) {           // per 64-wide k-block (8 KB apart in the slot)
+                    cp_async16(dst + kb * 8192 + my_dst_hi, src_hi + k0 + kb * 64);
+                    cp_async16(dst + kb * 8192 + my_dst_lo, src_lo + k0 + kb * 64);
                 }
             };
 #pragma unroll 1
@@ -549,11 +557,31 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                 float acc[32], v[32];
 #pragma unroll
                 for (int c = 0; c < 32; ++c) acc[c] = 0.f;
+                // the same association for every N, (hi + lo) per accumulator, so results do not depend on the batch
+                if (ncol == 64) {
+                    float vl[32];
 #pragma unroll
-                for (int q = 0; q < 2 * kTcIssuers; ++q) {       // four accumulators x {hi, lo} column halves
-                    tc::tmem_ld32(tmem + ((uint32_t)(32 * warp) << 16) + 32 * q, v);
+                    for (int q = 0; q < kTcIssuers; ++q) {       // four accumulators x {hi, lo} column halves
+                        tc::tmem_ld32(tmem + ((uint32_t)(32 * warp) << 16) + 64 * q, v);
+                        tc::tmem_ld32(tmem + ((uint32_t)(32 * warp) << 16) + 64 * q + 32, vl);
 #pragma unroll
-                    for (int c = 0; c < 32; ++c) acc[c] += v[c];
+                        for (int c = 0; c < 32; ++c) acc[c] += v[c] + vl[c];
+                    }
+                } else {
+#pragma unroll
+                    for (int q = 0; q < kTcIssuers; ++q) {       // hi and lo halves both sit in the first N <= 32 columns
+                        tc::tmem_ld32(tmem + ((uint32_t)(32 * warp) << 16) + 64 * q, v);
+                        if (ncol == 32) {
+#pragma unroll
+                            for (int c = 0; c < 16; ++c) acc[c] += v[c] + v[16 + c];
+                        } else if (ncol == 16) {
+#pragma unroll
+                            for (int c = 0; c < 8; ++c) acc[c] += v[c] + v[8 + c];
+                        } else {
+#pragma unroll
+                            for (int c = 0; c < 4; ++c) acc[c] += v[c] + v[4 + c];
+                        }
+                    }
                 }
                 if (lane < 16) {
 #pragma unroll
