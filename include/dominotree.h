@@ -146,7 +146,13 @@ int dt_build_trees_host(dt_handle *h, const void *marginal_logits_host, const vo
 int dt_commit_paths(dt_handle *h, const dt_outputs *tree, int32_t batch, int32_t B, const int32_t *target_next,
                     const uint8_t *edge_ok, int32_t *accept_len, int32_t *path_slots, int32_t *bonus_token, void *stream);
 
-/* dt_set_option: tuning knobs for experiments (e.g. "select_chunks"); unknown name -> INVALID_ARG. */
+/* dt_set_option: knobs; unknown name or value -> INVALID_ARG.
+ *   "scorer"        children function of dt_build_trees, the three arms of PAPER.md:553-555 (Appendix D):
+ *                   0 DominoTree (Alg. 1, per-node path-dependent correction; default),
+ *                   1 Marg (base logits alone, one menu per depth, no GRU),
+ *                   2 Cond-static (correction once per depth along Domino's greedy chain, menu shared per depth;
+ *                     bf16 shapes the fused kernel accepts, else dt_build_trees returns DT_ERR_UNSUPPORTED);
+ *   "expand_path", "select_chunks", "select_kernel"   tuning / test switches of the kernels. */
 int dt_set_option(dt_handle *h, const char *name, int64_t value);
 
 /*

@@ -13,6 +13,7 @@
 #include "dt_expand.cuh"
 #include "dt_fused.cuh"
 #include "dt_precompute.cuh"
+#include "dt_scorers.cuh"
 #include "dt_select.cuh"
 
 using namespace dt;
@@ -42,6 +43,8 @@ struct dt_handle {
     // options / bookkeeping
     int64_t opt_select_chunks;
     int64_t opt_select_kernel;      // 0 auto, 1 register-tile kernel only
+    int64_t opt_scorer;             // 0 DominoTree (Alg. 1), 1 Marg, 2 Cond-static
+    int32_t *menu_tok; float *menu_lp;
     int sel_bulk_ok;
     // phase timing (optional): n_slots x kPhaseEvents events, recorded on the caller's stream
     cudaEvent_t *ph_ev; int ph_slots, ph_slot;
@@ -122,6 +125,11 @@ extern "C" int dt_set_option(dt_handle *h, const char *name, int64_t value) {
         h->opt_expand_path = value;
         return DT_OK;
     }
+    if (!strcmp(name, "scorer")) {
+        if (value < 0 || value > 2) return DT_ERR_INVALID_ARG;
+        h->opt_scorer = value;
+        return DT_OK;
+    }
     if (!strcmp(name, "select_kernel")) {
         if (value < 0 || value > 1) return DT_ERR_INVALID_ARG;
         h->opt_select_kernel = value;
@@ -199,7 +207,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     const size_t o_part = carve(rows * kSelMaxChunks * (size_t)max_M * 8);
     const size_t o_cnt = carve(rows * 4), o_tau = carve(rows * 4);
     const size_t o_C = carve(rows * w->r * 4);
-    const size_t slots = (size_t)max_B + 2;                  // fused layout: slot 0 = zeros, node t at t+1
+    const size_t slots = (size_t)(max_B > L ? max_B : L) + 2;  // fused layout: slot 0 = zeros, node t at t+1 (static mode walks L nodes)
     const size_t o_states = carve((size_t)max_batch * slots * w->g * 4);
     // fused path eligibility (shape part; the grid / smem fit is checked per call)
     h->fused_ok = (w->dtype == DT_BF16) && (w->g % 32 == 0) && (w->r % 8 == 0) && max_M <= 256 &&
@@ -221,6 +229,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         o_mpart = carve(mma_tiles * kMmaSplits * (size_t)kMmaBM * kMmaBN * 4);
         o_mtick = carve(mma_tiles * 4);
     }
+    const size_t o_mtok = carve(rows * k * 4), o_mlp = carve(rows * k * 4);
     const size_t o_hg = carve((size_t)max_batch * h->heap_cap * 4);
     const size_t o_htp = carve((size_t)max_batch * h->heap_cap * 8);
     const size_t o_hcnt = carve((size_t)max_batch * 4);
@@ -234,6 +243,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     h->C = (float *)(h->ws + o_C); h->states = (float *)(h->ws + o_states);
     h->heap_g = (float *)(h->ws + o_hg); h->heap_tp = (unsigned long long *)(h->ws + o_htp);
     h->heap_cnt = (int32_t *)(h->ws + o_hcnt);
+    h->menu_tok = (int32_t *)(h->ws + o_mtok); h->menu_lp = (float *)(h->ws + o_mlp);
     if (h->mma_ok) { h->mma_partial = (float *)(h->ws + o_mpart); h->mma_tickets = (unsigned int *)(h->ws + o_mtick); }
     if (cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
@@ -361,7 +371,7 @@ extern "C" int dt_select_topm(dt_handle *h, const void *logits, int32_t rows, in
 
 // Fused persistent expansion (dt_fused.cuh).  Returns 1 if the shape does not fit (caller falls back
 // to the per-step kernels), DT_OK after enqueueing, or a negative error.
-static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st) {
+static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool static_mode = false) {
     if (!h->fused_ok || h->opt_expand_path == 1) return 1;
     int upc = 0;
     bool tcgen = false;
@@ -388,8 +398,9 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st) {
     memset(&f, 0, sizeof(f));
     f.e = p;
     f.upc = upc; f.n_gru = p.g / upc; f.m_tiles = (3 * upc + 15) / 16;
-    f.slot_stride = h->max_B + 2;
+    f.slot_stride = (h->max_B > h->L ? h->max_B : h->L) + 2;
     f.s_hi = h->s_hi; f.s_lo = h->s_lo; f.s32 = h->states; f.partial = h->partial; f.desc = h->desc; f.flags = h->flags;
+    f.static_mode = static_mode ? 1 : 0; f.menu_tok = h->menu_tok; f.menu_lp = h->menu_lp;
     f.w2_smem = 1;
     size_t rs = fused_req_smem(p.r, p.M, p.N, p.k, 1);
     if (rs > (size_t)h->max_smem_optin) { f.w2_smem = 0; rs = fused_req_smem(p.r, p.M, p.N, p.k, 0); }
@@ -407,7 +418,22 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st) {
                                : cudaLaunchCooperativeKernel((const void *)fused_expand_kernel<16>, grid, block, args, dsm, st);
     h->launches++;
     DT_CUDA(h, e);
+    if (static_mode) return DT_OK;
     if ((rc = phase_mark(h, 3, st))) return rc;
+    return phase_mark(h, 4, st);
+}
+
+// Factorized arms (dt_scorers.cuh): best-first over the per-depth menus in h->menu_*, then the emitter.
+static int launch_factorized(dt_handle *h, const ExpandParams &p, cudaStream_t st) {
+    ScorerParams sp;
+    sp.e = p; sp.menu_tok = h->menu_tok; sp.menu_lp = h->menu_lp;
+    const size_t dsm = factorized_smem(p.L, p.k, p.N);
+    if (dsm > 48 * 1024) return DT_ERR_UNSUPPORTED;
+    factorized_expand_kernel<<<p.batch, kFusThreads, dsm, st>>>(sp);
+    h->launches++;
+    DT_CUDA(h, cudaGetLastError());
+    int rc = phase_mark(h, 3, st);
+    if (rc) return rc;
     return phase_mark(h, 4, st);
 }
 
@@ -486,6 +512,24 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
     p.tokens = out->tokens; p.parents = out->parents; p.depths = out->depths; p.positions = out->positions;
     p.n_nodes = out->n_nodes; p.scores = out->scores; p.mask = out->mask;
     p.root_tokens = root_tokens; p.root_positions = root_positions;
+    if (h->opt_scorer == 1) {                       // Marg: menus from the base logits alone, no GRU, no C
+        ScorerParams sp;
+        sp.e = p; sp.menu_tok = h->menu_tok; sp.menu_lp = h->menu_lp;
+        marg_menu_kernel<<<rows, 256, 0, st>>>(sp);
+        h->launches++;
+        DT_CUDA(h, cudaGetLastError());
+        if ((rc = phase_mark(h, 2, st))) return rc;
+        return launch_factorized(h, p, st);
+    }
+    if (h->opt_scorer == 2) {                       // Cond-static: corrected menus along the greedy chain
+        if (w.dtype != DT_BF16) return DT_ERR_UNSUPPORTED;
+        ExpandParams ps = p;
+        ps.B = h->L; ps.N = h->L + 1;               // the chain has L nodes below the root; outputs are not touched
+        rc = launch_fused(h, ps, st, true);
+        if (rc > 0) return DT_ERR_UNSUPPORTED;      // shape the fused kernel rejects
+        if (rc) return rc;
+        return launch_factorized(h, p, st);
+    }
     if (w.dtype == DT_BF16) {
         rc = launch_fused(h, p, st);
         if (rc <= 0) return rc;

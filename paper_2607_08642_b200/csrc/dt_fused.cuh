@@ -53,6 +53,11 @@ struct FusedParams {
     float *partial;                // [n_gru, batch, r]
     unsigned long long *desc;      // [batch]  hand-over word request -> GRU: epoch(16) | state slot + 1 (16) | token (32)
     unsigned int *flags;           // [n_gru]  hand-over word GRU -> request: steps completed by that GRU CTA
+    // Cond-static arm: walk only the greedy chain (the frontier is dropped after every pop) for
+    // B = L steps and record each depth's corrected top-k menu; the tree is then built by dt_scorers.cuh
+    int static_mode;
+    int32_t *menu_tok;             // [batch, L, k]
+    float *menu_lp;                // [batch, L, k]
 };
 
 // Optional in-kernel timeline (compile with -DDT_TRACE; measurement builds only, never the product build):
@@ -883,6 +888,10 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                     nHi[rank] = ord_key(gpar + lpm);
                     nLo[rank] = ((unsigned long long)(0xFFFFFFFFu - (unsigned int)mtok) << 32) |
                                 (unsigned long long)(0xFFFFFFFFu - (unsigned int)t);
+                    if (p.static_mode) {                        // the depth's shared menu (row index = depth of node t)
+                        p.menu_tok[((size_t)b * L + depth) * k + rank] = mtok;
+                        p.menu_lp[((size_t)b * L + depth) * k + rank] = lpm;
+                    }
                 }
             }
             n_new = k;
@@ -904,7 +913,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                 const int dep = nDep[par] + 1;
                 if (t + 1 < B) st_relaxed_u64(p.desc + b, fused_desc_pack(t + 2, dep < L ? par + 1 : -1, tok));
                 nTok[t + 1] = tok; nPar[t + 1] = par; nDep[t + 1] = dep; nSco[t + 1] = ord_key_inv(h);
-                sm.n_valid = t + 2; sm.n_front = min(tot, cap) - 1; sm.cur = cur ^ 1;
+                sm.n_valid = t + 2; sm.n_front = p.static_mode ? 0 : min(tot, cap) - 1; sm.cur = cur ^ 1;
             } else {
                 sm.n_front = 0;
                 if (t + 1 < B) st_relaxed_u64(p.desc + b, fused_desc_pack(t + 2, -1, 0));
@@ -944,6 +953,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     }
     __syncthreads();
 
+    if (p.static_mode) return;                                  // menus are out; dt_scorers.cuh builds and emits the tree
     // emitter (a9): dead-leaf padding (reading A10), positions, ancestor-or-self mask
     const int n = sm.n_valid;
     const int rpos = e.root_positions ? e.root_positions[b] : 0;

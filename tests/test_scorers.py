@@ -136,3 +136,77 @@ def test_factorized_tree_invariants_and_closed_form():
     rec(0.0, 0)
     want = sorted(allg, reverse=True)[:n - 1]
     assert np.allclose(sorted(scores[1:n], reverse=True), want, atol=1e-12)
+
+
+# ------------------------------------------------------------------------------------------- GPU parity
+class _Ref:
+    def __init__(self, t):
+        self.tokens, self.parents, self.depths, self.positions, self.scores, self.mask, self.n_nodes = t
+
+
+def _gpu_tree(out, b):
+    n = int(out.n_nodes[b])
+    return (out.tokens[b].cpu().numpy().astype(np.int64), out.parents[b].cpu().numpy().astype(np.int64),
+            out.depths[b].cpu().numpy().astype(np.int64), out.positions[b].cpu().numpy().astype(np.int64),
+            out.scores[b].cpu().numpy().astype(np.float64), out.mask[b].cpu().numpy(), n)
+
+
+def _run_scorer(case, inp, M, B, T, scorer):
+    case.builder.set_option("scorer", scorer)
+    try:
+        out = case.run_gpu(inp, M, B, T)
+        torch.cuda.synchronize()
+        launches = case.builder.kernel_launches
+    finally:
+        case.builder.set_option("scorer", 0)
+    return out, launches
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfgname,dtype_kw", [("tiny", {}), ("tiny", {"dtype": "bf16", "V": 2000})])
+def test_gpu_marg_matches_oracle(cfgname, dtype_kw):
+    import gpu_util as gu
+    case = gu.tiny_case(**dtype_kw) if dtype_kw else gu.tiny_case()
+    for batch, M, B, T, regime in ((5, 8, 8, 0.0, "flat"), (32, 8, 31, 0.6, "peaked"), (3, 9, 64, 1.0, "flat")):
+        inp = wl.make_inputs(case.cfg, batch=batch, seed=6000 + B, regime=regime)
+        out, launches = _run_scorer(case, inp, M, B, T, 1)
+        assert launches <= 4
+        for b in range(batch):
+            menus = scorers.marg_menus(inp["logits"][b], M, case.k, T)
+            ref = _Ref(scorers.factorized_tree(menus, int(inp["root_tokens"][b]), int(inp["root_positions"][b]), B))
+            _same_tree(_gpu_tree(out, b), ref, tol=1e-4)
+            n = ref.n_nodes
+            assert np.max(np.abs(_gpu_tree(out, b)[4][:n] - ref.scores[:n])) < 2e-3
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("g,path", [(256, 0), (64, 0)])
+def test_gpu_cond_static_matches_oracle(g, path):
+    """Cond-static through the fused kernel in static mode (tcgen05 GRU role at g = 256, mma.sync at g = 64)."""
+    import gpu_util as gu
+    cfg = wl.CONFIGS["tiny"].replace(dtype="bf16", g=g, r=40, d=96, V=2000, L=5, embed_std=1.0)
+    case = gu.get_case(f"cs-{g}", cfg, max_batch=40, max_M=32, max_B=48, k=4)
+    worc = oracle.Weights.from_dict(case.w_cpu) if hasattr(case, "w_cpu") else case.w_orc
+    for batch, M, B, T in ((1, 8, 8, 0.0), (7, 20, 17, 0.6), (33, 24, 40, 1.0)):
+        inp = wl.make_inputs(case.cfg, batch=batch, seed=7000 + B)
+        out, launches = _run_scorer(case, inp, M, B, T, 2)
+        assert launches <= 6
+        for b in range(batch):
+            root, rp = int(inp["root_tokens"][b]), int(inp["root_positions"][b])
+            menus = scorers.cond_static_menus(worc, inp["logits"][b], inp["hidden"][b], root, M, case.k, T)
+            ref = _Ref(scorers.factorized_tree(menus, root, rp, B))
+            _same_tree(_gpu_tree(out, b), ref, tol=1e-4)
+        # and it is a different tree from DominoTree's on this path-sensitive config for at least one request
+        dt_out = case.run_gpu(inp, M, B, T)
+        if batch >= 7:
+            assert not (torch.equal(dt_out.tokens, out.tokens) and torch.equal(dt_out.parents, out.parents))
+
+
+@pytest.mark.gpu
+def test_gpu_cond_static_unsupported_for_fp32():
+    import gpu_util as gu
+    import paper_2607_08642_b200 as dtb
+    case = gu.tiny_case()
+    inp = wl.make_inputs(case.cfg, batch=1)
+    with pytest.raises(dtb.DominoTreeError):
+        _run_scorer(case, inp, 8, 8, 0.0, 2)
