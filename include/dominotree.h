@@ -146,6 +146,18 @@ int dt_build_trees_host(dt_handle *h, const void *marginal_logits_host, const vo
 int dt_commit_paths(dt_handle *h, const dt_outputs *tree, int32_t batch, int32_t B, const int32_t *target_next,
                     const uint8_t *edge_ok, int32_t *accept_len, int32_t *path_slots, int32_t *bonus_token, void *stream);
 
+/*
+ * dt_adaptive_budget: CaDDTree's cost-aware stopping rule on the pop order of the built trees (PAPER.md:97-101,
+ * 161-165): theta(n) = (1 + Phi(n)) / (C_d + C_v(n)), Phi(n) = sum over slots 1..n of exp(scores); n_star is the
+ * first n with theta(n + 1) <= theta(n) (or every valid draft node).  `tree` = DEVICE outputs of dt_build_trees for
+ * the same batch and B (scores, n_nodes are read); cv [B + 1] float device = verification cost of an n-node tree,
+ * C_d = draft cost (same unit).  Outputs (device): n_star [batch] int32 draft nodes to keep (slots 1..n_star),
+ * phi [batch] float or NULL = Phi(n_star).  The paper reports the rule as a negative result on the corrected tree
+ * (it runs to the cap); it is provided as the measurement device of that claim.  Asynchronous, capture-safe.
+ */
+int dt_adaptive_budget(dt_handle *h, const dt_outputs *tree, int32_t batch, int32_t B, double C_d, const float *cv,
+                       int32_t *n_star, float *phi, void *stream);
+
 /* dt_set_option: knobs; unknown name or value -> INVALID_ARG.
  *   "scorer"        children function of dt_build_trees, the three arms of PAPER.md:553-555 (Appendix D):
  *                   0 DominoTree (Alg. 1, per-node path-dependent correction; default),

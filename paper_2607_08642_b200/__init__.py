@@ -17,7 +17,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libdominotree.so")
 
 DT_BF16, DT_F32 = 0, 1
-EXPORTS = ("dt_create", "dt_build_trees", "dt_select_topm", "dt_build_trees_host", "dt_commit_paths", "dt_set_option",
+EXPORTS = ("dt_create", "dt_build_trees", "dt_select_topm", "dt_build_trees_host", "dt_commit_paths", "dt_adaptive_budget", "dt_set_option",
            "dt_kernel_launches", "dt_destroy", "dt_error_string", "dt_version", "dt_workspace_bytes",
            "dt_last_cuda_error", "dt_phase_timing", "dt_phase_slot", "dt_phase_elapsed_ms")
 PHASES = ("select", "precompute", "expand", "emit")
@@ -60,6 +60,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.dt_build_trees.restype = ctypes.c_int
     lib.dt_build_trees_host.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, f32, ctypes.POINTER(_Outputs), vp]
     lib.dt_build_trees_host.restype = ctypes.c_int
+    lib.dt_adaptive_budget.argtypes = [vp, ctypes.POINTER(_Outputs), i32, i32, ctypes.c_double, vp, vp, vp, vp]
+    lib.dt_adaptive_budget.restype = ctypes.c_int
     lib.dt_commit_paths.argtypes = [vp, ctypes.POINTER(_Outputs), i32, i32, vp, vp, vp, vp, vp, vp]
     lib.dt_commit_paths.restype = ctypes.c_int
     lib.dt_select_topm.argtypes = [vp, vp, i32, i32, vp, vp, vp]
@@ -199,6 +201,20 @@ class DominoTreeBuilder:
         st = stream if stream is not None else torch.cuda.current_stream()
         rc = self.lib.dt_select_topm(self._h, lg.data_ptr(), lg.shape[0], M, ids.data_ptr(), vals.data_ptr(), st.cuda_stream)
         _check(self.lib, rc, "dt_select_topm", self._h)
+
+    def adaptive_budget(self, tree: TreeBatch, B: int, C_d: float, cv, stream=None):
+        """dt_adaptive_budget: (n_star [batch] int32, phi [batch] float32) on the device; cv = float32 [B+1] costs."""
+        import torch
+        batch = tree.tokens.shape[0]
+        self._check_in(cv, (B + 1,), torch.float32, True)
+        n_star = torch.empty((batch,), dtype=torch.int32, device=cv.device)
+        phi = torch.empty((batch,), dtype=torch.float32, device=cv.device)
+        st = stream if stream is not None else torch.cuda.current_stream()
+        os_ = tree._struct()
+        rc = self.lib.dt_adaptive_budget(self._h, ctypes.byref(os_), batch, B, float(C_d), cv.data_ptr(),
+                                         n_star.data_ptr(), phi.data_ptr(), st.cuda_stream)
+        _check(self.lib, rc, "dt_adaptive_budget", self._h)
+        return n_star, phi
 
     def commit_paths(self, tree: TreeBatch, B: int, target_next=None, edge_ok=None, stream=None):
         """dt_commit_paths: longest accepted path of every tree -> (accept_len [batch], path_slots [batch, L+1],

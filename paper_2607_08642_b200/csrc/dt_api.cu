@@ -9,6 +9,7 @@
 #include <string.h>
 
 #include "../../include/dominotree.h"
+#include "dt_budget.cuh"
 #include "dt_commit.cuh"
 #include "dt_expand.cuh"
 #include "dt_fused.cuh"
@@ -536,6 +537,20 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
         return launch_expansion<__nv_bfloat16>(h, p, st);
     }
     return launch_expansion<float>(h, p, st);
+}
+
+extern "C" int dt_adaptive_budget(dt_handle *h, const dt_outputs *tree, int32_t batch, int32_t B, double C_d, const float *cv,
+                                  int32_t *n_star, float *phi, void *stream) {
+    if (!h || !tree) return DT_ERR_INVALID_ARG;
+    if (batch < 0 || batch > h->max_batch || B < 1 || B > h->max_B || !(C_d >= 0.0) || isinf(C_d)) return DT_ERR_INVALID_ARG;
+    h->launches = 0;
+    if (batch == 0) return DT_OK;
+    if (!tree->scores || !tree->n_nodes || !cv || !n_star) return DT_ERR_INVALID_ARG;
+    adaptive_budget_kernel<<<(batch + 63) / 64, 64, 0, (cudaStream_t)stream>>>(tree->scores, tree->n_nodes, B + 1, batch, C_d, cv,
+                                                                               n_star, phi);
+    h->launches++;
+    DT_CUDA(h, cudaGetLastError());
+    return DT_OK;
 }
 
 extern "C" int dt_commit_paths(dt_handle *h, const dt_outputs *tree, int32_t batch, int32_t B, const int32_t *target_next,
