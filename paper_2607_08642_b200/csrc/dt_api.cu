@@ -156,7 +156,7 @@ static int launch_gemm_nt(dt_handle *h, const void *A, long long lda, const void
 }
 
 // C = H W1[:, 0:d]^T on the tensor cores (dt_gemm_mma.cuh), split-K kMmaSplits ways.
-constexpr int kMmaSplits = 8;
+constexpr int kMmaSplits = 16;
 static int launch_gemm_mma(dt_handle *h, const void *A, long long lda, const void *Bm, long long ldb,
                            float *out, long long ldo, int Mr, int Nc, int K, cudaStream_t st) {
     GemmMmaParams g;
@@ -218,8 +218,8 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         o_shi = carve((size_t)max_batch * slots * w->g * 2);
         o_slo = carve((size_t)max_batch * slots * w->g * 2);
         o_partial = carve((size_t)(w->g / 8) * max_batch * w->r * 4);
-        o_desc = carve((size_t)max_batch * 8);
-        o_sync = carve(256 * 4);
+        o_desc = carve((size_t)max_batch * 8 * kFusDescStride);
+        o_sync = carve((size_t)256 * 4 * kFusFlagStride);
     }
     // MMA GEMM eligibility: bf16, 16-byte aligned rows of H and W1
     h->mma_ok = (w->dtype == DT_BF16) && (w->d % 8 == 0) && ((w->d + w->g) % 8 == 0) &&

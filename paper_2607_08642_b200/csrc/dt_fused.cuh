@@ -42,6 +42,8 @@ constexpr int kFusKB = 32;        // k per MMA block (two k16 steps)
 constexpr int kFusRing = 3;       // state blocks in flight per warp (cp.async ring)
 constexpr int kFusW2Pad = 32;     // bf16 elements of padding per staged W2 row (row stride = 16 banks mod 32)
 constexpr int kFusMaxFront = 256; // frontier entries kept (>= DT_MAX_B)
+constexpr int kFusDescStride = 16; // u64 words between two requests' descriptors (one 128-byte line each: concurrent
+constexpr int kFusFlagStride = 32; // u32 words between two GRU CTAs' flags         partial writes to one line serialise in L2)
 
 struct FusedParams {
     ExpandParams e;
@@ -106,11 +108,11 @@ __device__ __forceinline__ unsigned long long fused_desc_pack(int epoch, int sid
 // Zero the GRU flags and write the step-0 descriptor (the root: parent state = zeros, reading A4).
 __global__ void fused_init_kernel(FusedParams p) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < p.n_gru) p.flags[i] = 0u;
+    if (i < p.n_gru) p.flags[(size_t)i * kFusFlagStride] = 0u;
     if (i < p.e.batch) {
         int tok = p.e.root_tokens[i];
         tok = min(max(tok, 0), p.e.V - 1);
-        p.desc[i] = fused_desc_pack(1, 0, tok);
+        p.desc[(size_t)i * kFusDescStride] = fused_desc_pack(1, 0, tok);
     }
 }
 
@@ -196,7 +198,7 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
                 int sidx = -1, tok = 0;
                 if (lane < nb) {
                     unsigned long long dsc;
-                    do { dsc = ld_relaxed_u64(p.desc + c0 + lane); } while ((int)(dsc >> 48) != t + 1);
+                    do { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride); } while ((int)(dsc >> 48) != t + 1);
                     sidx = (int)((dsc >> 32) & 0xFFFFu) - 1;
                     tok = (int)(dsc & 0xFFFFFFFFull);
                 }
@@ -367,7 +369,7 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
             __syncthreads();
         }
         DT_TR(0, 0, t, 4);
-        if (tid == 0) { __threadfence(); st_relaxed_u32(p.flags + cta, (unsigned int)(t + 1)); }
+        if (tid == 0) { __threadfence(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, (unsigned int)(t + 1)); }
         DT_TR(0, 0, t, 5);
     }
 }
@@ -475,7 +477,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                 int sidx = -1, tok = 0;
                 if (lane < nb) {
                     unsigned long long dsc;
-                    do { dsc = ld_relaxed_u64(p.desc + c0 + lane); } while ((int)(dsc >> 48) != t + 1);
+                    do { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride); } while ((int)(dsc >> 48) != t + 1);
                     sidx = (int)((dsc >> 32) & 0xFFFFu) - 1;
                     tok = (int)(dsc & 0xFFFFFFFFull);
                 }
@@ -651,7 +653,10 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             __syncthreads();
         }
         DT_TR(0, 0, t, 4);
-        if (tid == 0) { __threadfence(); st_relaxed_u32(p.flags + cta, (unsigned int)(t + 1)); }
+        if (tid == 0) { __threadfence(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, (unsigned int)(t + 1)); }
+#ifdef DT_TRACE
+        if (tid == 0 && t == 5 && cta < 64) g_dt_trace[0][210 + cta / 8][cta % 8] = dt_globaltimer();
+#endif
         DT_TR(0, 0, t, 5);
     }
     __syncthreads();
@@ -740,7 +745,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         if (expand && tid < r) cpre = e.C[((size_t)b * L + depth) * r + tid];
         if (warp == 0) {
             for (int q = lane; q < p.n_gru; q += 32)
-                while (ld_relaxed_u32(p.flags + q) < (unsigned int)(t + 1)) { }
+                while (ld_relaxed_u32(p.flags + (size_t)q * kFusFlagStride) < (unsigned int)(t + 1)) { }
         }
         __syncthreads();
         DT_TR(1, p.n_gru, t, 0);
@@ -911,12 +916,15 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                 const int tok = (int)(0xFFFFFFFFu - (unsigned int)(l >> 32));
                 const int par = (int)(0xFFFFFFFFu - (unsigned int)(l & 0xFFFFFFFFull));
                 const int dep = nDep[par] + 1;
-                if (t + 1 < B) st_relaxed_u64(p.desc + b, fused_desc_pack(t + 2, dep < L ? par + 1 : -1, tok));
+                if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(t + 2, dep < L ? par + 1 : -1, tok));
+#ifdef DT_TRACE
+                if (t == 5 && b < 64) g_dt_trace[1][200 + b / 8][b % 8] = dt_globaltimer();
+#endif
                 nTok[t + 1] = tok; nPar[t + 1] = par; nDep[t + 1] = dep; nSco[t + 1] = ord_key_inv(h);
                 sm.n_valid = t + 2; sm.n_front = p.static_mode ? 0 : min(tot, cap) - 1; sm.cur = cur ^ 1;
             } else {
                 sm.n_front = 0;
-                if (t + 1 < B) st_relaxed_u64(p.desc + b, fused_desc_pack(t + 2, -1, 0));
+                if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(t + 2, -1, 0));
             }
         }
         DT_TR(1, p.n_gru, t, 4);

@@ -21,7 +21,7 @@
 
 namespace dt {
 
-constexpr int kMmaBM = 64, kMmaBN = 64, kMmaBK = 32, kMmaStages = 3, kMmaThreads = 128;
+constexpr int kMmaBM = 64, kMmaBN = 64, kMmaBK = 32, kMmaStages = 4, kMmaThreads = 128;
 constexpr int kMmaLd = kMmaBK + 8;      // padded row (80 B): ldmatrix rows land in distinct banks
 
 struct GemmMmaParams {
