@@ -444,7 +444,7 @@ def main():
     exp_tflops = exp_flops / (ph["expand"] * 1e-6) / 1e12
     roof_expand = {"kernel": "expansion phase (GRU step + correction/log-softmax/top-k + heap)", "bound": "alu",
                    "achieved": exp_tflops, "peak": fma_peak_tflops, "unit": "TFLOP/s", "frac": exp_tflops / fma_peak_tflops,
-                   "traffic": 19.18e6 if c5 else None, "peak_source": "148 SMs x 128 fp32 FMA lanes x 2 x sm_max_mhz (DESIGN.md)",
+                   "traffic": 19.15e6 if c5 else None, "peak_source": "148 SMs x 128 fp32 FMA lanes x 2 x sm_max_mhz (DESIGN.md)",
                    "algorithmic_flops": exp_flops, "us_per_round": ph["expand"],
                    "share_of_step": ph["expand"] / ctx["phase_round_us"],
                    "note": "a chain of B dependent steps: latency-bound, not throughput-bound"}
