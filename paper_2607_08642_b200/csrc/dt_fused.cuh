@@ -84,6 +84,9 @@ __device__ __forceinline__ unsigned long long dt_globaltimer() {
 // poll with relaxed gpu-scope loads and read ALL hand-over data with L1-bypassing loads (ld.global.cg,
 // cp.async.cg), i.e. from L2, the single point of coherence, after the control dependency on the polled
 // word; they need no fence of their own.  Request -> GRU: the descriptor word is the whole payload.
+// Release fence at gpu scope (MEMBAR.ALL.GPU): lighter than __threadfence(), which is sequentially consistent
+// (MEMBAR.SC.GPU) and also invalidates L1.
+__device__ __forceinline__ void fence_release_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
 __device__ __forceinline__ unsigned int ld_relaxed_u32(const unsigned int *p) {
     unsigned int v;
     asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -369,7 +372,7 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
             __syncthreads();
         }
         DT_TR(0, 0, t, 4);
-        if (tid == 0) { __threadfence(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, (unsigned int)(t + 1)); }
+        if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, (unsigned int)(t + 1)); }
         DT_TR(0, 0, t, 5);
     }
 }
@@ -653,7 +656,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             __syncthreads();
         }
         DT_TR(0, 0, t, 4);
-        if (tid == 0) { __threadfence(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, (unsigned int)(t + 1)); }
+        if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, (unsigned int)(t + 1)); }
 #ifdef DT_TRACE
         if (tid == 0 && t == 5 && cta < 64) g_dt_trace[0][210 + cta / 8][cta % 8] = dt_globaltimer();
 #endif
