@@ -13,6 +13,7 @@
 #include "dt_commit.cuh"
 #include "dt_expand.cuh"
 #include "dt_fused.cuh"
+#include "dt_gemm_tc.cuh"
 #include "dt_precompute.cuh"
 #include "dt_scorers.cuh"
 #include "dt_select.cuh"
@@ -34,6 +35,7 @@ struct dt_handle {
     // tensor-core precompute GEMM (bf16): split-K partials + tile tickets; side stream + fork/join events so the
     // GEMM overlaps the HBM-bound select inside the same round (and the same captured graph)
     float *mma_partial; unsigned int *mma_tickets; int mma_ok;
+    float *tcg_partial; int tcg_ok;     // tcgen05 precompute GEMM: [kTcgSplits, rows_pad, r] partials
     cudaStream_t side; cudaEvent_t ev_fork, ev_join;
     // fused persistent expansion (bf16): state copies, split-K partials, hand-over words
     __nv_bfloat16 *s_hi, *s_lo; float *partial; unsigned long long *desc; unsigned int *flags;
@@ -44,6 +46,7 @@ struct dt_handle {
     // options / bookkeeping
     int64_t opt_select_chunks;
     int64_t opt_select_kernel;      // 0 auto, 1 register-tile kernel only
+    int64_t opt_gemm;               // 0 auto (tcgen05 when the shape allows), 1 legacy mma.sync kernel
     int64_t opt_scorer;             // 0 DominoTree (Alg. 1), 1 Marg, 2 Cond-static
     int32_t *menu_tok; float *menu_lp;
     int sel_bulk_ok;
@@ -126,6 +129,11 @@ extern "C" int dt_set_option(dt_handle *h, const char *name, int64_t value) {
         h->opt_expand_path = value;
         return DT_OK;
     }
+    if (!strcmp(name, "precompute_gemm")) {
+        if (value < 0 || value > 1) return DT_ERR_INVALID_ARG;
+        h->opt_gemm = value;
+        return DT_OK;
+    }
     if (!strcmp(name, "scorer")) {
         if (value < 0 || value > 2) return DT_ERR_INVALID_ARG;
         h->opt_scorer = value;
@@ -174,6 +182,22 @@ static int launch_gemm_mma(dt_handle *h, const void *A, long long lda, const voi
     dim3 grid(tn, tm, splits);
     gemm_nt_bf16_mma_kernel<<<grid, kMmaThreads, 0, st>>>(g);
     h->launches++;
+    DT_CUDA(h, cudaGetLastError());
+    return DT_OK;
+}
+
+// C = H W1[:, 0:d]^T on tcgen05 (dt_gemm_tc.cuh): split-K partials, then the fixed-order reduction.
+static int launch_gemm_tc(dt_handle *h, const void *A, long long lda, const void *Bm, long long ldb,
+                          float *out, long long ldo, int Mr, int Nc, int K, cudaStream_t st) {
+    GemmTcParams g;
+    g.A = reinterpret_cast<const __nv_bfloat16 *>(A); g.lda = lda;
+    g.Bm = reinterpret_cast<const __nv_bfloat16 *>(Bm); g.ldb = ldb;
+    g.partial = h->tcg_partial; g.out = out; g.ldo = ldo;
+    g.Mr = Mr; g.Nc = Nc; g.K = K; g.Mr_pad = (Mr + 127) / 128 * 128;
+    gemm_c_tc_kernel<<<dim3(g.Mr_pad / 128, kTcgSplits), kTcgThreads, gemm_tc_smem(), st>>>(g);
+    const long long n = (long long)Mr * (Nc / 4);
+    gemm_c_reduce_kernel<<<(unsigned int)((n + 255) / 256), 256, 0, st>>>(g);
+    h->launches += 2;
     DT_CUDA(h, cudaGetLastError());
     return DT_OK;
 }
@@ -231,6 +255,9 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         o_mtick = carve(mma_tiles * 4);
     }
     const size_t o_mtok = carve(rows * k * 4), o_mlp = carve(rows * k * 4);
+    const size_t rows_pad = (rows + 127) / 128 * 128;
+    h->tcg_ok = h->mma_ok && (w->d % (64 * kTcgSplits) == 0) && (w->r % 16 == 0) && w->r <= 256 && h->opt_gemm != 1;
+    const size_t o_tcg = h->tcg_ok ? carve((size_t)kTcgSplits * rows_pad * w->r * 4) : 0;
     const size_t o_hg = carve((size_t)max_batch * h->heap_cap * 4);
     const size_t o_htp = carve((size_t)max_batch * h->heap_cap * 8);
     const size_t o_hcnt = carve((size_t)max_batch * 4);
@@ -245,6 +272,10 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     h->heap_g = (float *)(h->ws + o_hg); h->heap_tp = (unsigned long long *)(h->ws + o_htp);
     h->heap_cnt = (int32_t *)(h->ws + o_hcnt);
     h->menu_tok = (int32_t *)(h->ws + o_mtok); h->menu_lp = (float *)(h->ws + o_mlp);
+    if (h->tcg_ok) {
+        h->tcg_partial = (float *)(h->ws + o_tcg);
+        if (cudaFuncSetAttribute(gemm_c_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_tc_smem()) != cudaSuccess) { cudaGetLastError(); h->tcg_ok = 0; }
+    }
     if (h->mma_ok) { h->mma_partial = (float *)(h->ws + o_mpart); h->mma_tickets = (unsigned int *)(h->ws + o_mtick); }
     if (cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
@@ -487,7 +518,9 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
     if (mma) {
         DT_CUDA(h, cudaEventRecord(h->ev_fork, st));
         DT_CUDA(h, cudaStreamWaitEvent(h->side, h->ev_fork, 0));
-        rc = launch_gemm_mma(h, backbone_hidden, w.d, w.corr_w1, (long long)w.d + w.g, h->C, w.r, rows, w.r, w.d, h->side);
+        rc = (h->tcg_ok && h->opt_gemm != 1)
+            ? launch_gemm_tc(h, backbone_hidden, w.d, w.corr_w1, (long long)w.d + w.g, h->C, w.r, rows, w.r, w.d, h->side)
+            : launch_gemm_mma(h, backbone_hidden, w.d, w.corr_w1, (long long)w.d + w.g, h->C, w.r, rows, w.r, w.d, h->side);
         if (rc) return rc;
         DT_CUDA(h, cudaEventRecord(h->ev_join, h->side));
     }
