@@ -38,7 +38,7 @@ struct dt_handle {
     float *tcg_partial; int tcg_ok;     // tcgen05 precompute GEMM: [kTcgSplits, rows_pad, r] partials
     cudaStream_t side; cudaEvent_t ev_fork, ev_join;
     // fused persistent expansion (bf16): state copies, split-K partials, hand-over words
-    __nv_bfloat16 *s_hi, *s_lo; float *partial; unsigned long long *desc; unsigned int *flags;
+    __nv_bfloat16 *s_hi, *s_lo; float *partial; unsigned long long *desc; unsigned int *flags, *round_ctr;
     int fused_ok, max_smem_optin;
     int64_t opt_expand_path;        // 0 auto, 1 per-step kernels, 2 fused mma.sync upc=8, 3 fused mma.sync upc=16, 4 fused tcgen05
     // host-call staging (lazy)
@@ -243,7 +243,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         o_slo = carve((size_t)max_batch * slots * w->g * 2);
         o_partial = carve((size_t)(w->g / 8) * max_batch * w->r * 4);
         o_desc = carve((size_t)max_batch * 8 * kFusDescStride);
-        o_sync = carve((size_t)256 * 4 * kFusFlagStride);
+        o_sync = carve((size_t)256 * 4 * kFusFlagStride + 256);
     }
     // MMA GEMM eligibility: bf16, 16-byte aligned rows of H and W1
     h->mma_ok = (w->dtype == DT_BF16) && (w->d % 8 == 0) && ((w->d + w->g) % 8 == 0) &&
@@ -286,6 +286,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         h->s_hi = (__nv_bfloat16 *)(h->ws + o_shi); h->s_lo = (__nv_bfloat16 *)(h->ws + o_slo);
         h->partial = (float *)(h->ws + o_partial); h->desc = (unsigned long long *)(h->ws + o_desc);
         h->flags = (unsigned int *)(h->ws + o_sync);
+        h->round_ctr = h->flags + (size_t)256 * kFusFlagStride;
         bool ok = cudaDeviceGetAttribute(&h->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess;
         h->max_smem_optin -= 1024;                  // room for the kernels' static shared memory
         if (!ok ||
@@ -431,7 +432,7 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
     f.e = p;
     f.upc = upc; f.n_gru = p.g / upc; f.m_tiles = (3 * upc + 15) / 16;
     f.slot_stride = (h->max_B > h->L ? h->max_B : h->L) + 2;
-    f.s_hi = h->s_hi; f.s_lo = h->s_lo; f.s32 = h->states; f.partial = h->partial; f.desc = h->desc; f.flags = h->flags;
+    f.s_hi = h->s_hi; f.s_lo = h->s_lo; f.s32 = h->states; f.partial = h->partial; f.desc = h->desc; f.flags = h->flags; f.round_ctr = h->round_ctr;
     f.static_mode = static_mode ? 1 : 0; f.menu_tok = h->menu_tok; f.menu_lp = h->menu_lp;
     f.w2_smem = 1;
     size_t rs = fused_req_smem(p.r, p.M, p.N, p.k, 1);
@@ -439,8 +440,6 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
     if (rs > (size_t)h->max_smem_optin) return 1;
     const size_t gs = tcgen ? fused_tc_smem(p.g, p.r) : fused_gru_smem(p.g, p.r, upc, f.m_tiles);
     const size_t dsm = gs > rs ? gs : rs;
-    fused_init_kernel<<<((p.batch > f.n_gru ? p.batch : f.n_gru) + 127) / 128, 128, 0, st>>>(f);
-    h->launches++;
     int rc = phase_mark(h, 2, st);
     if (rc) return rc;
     void *args[] = {&f};

@@ -54,7 +54,8 @@ struct FusedParams {
     float *s32;                    // [batch, slot_stride, g]
     float *partial;                // [n_gru, batch, r]
     unsigned long long *desc;      // [batch]  hand-over word request -> GRU: epoch(16) | state slot + 1 (16) | token (32)
-    unsigned int *flags;           // [n_gru]  hand-over word GRU -> request: steps completed by that GRU CTA
+    unsigned int *flags;           // [n_gru]  hand-over word GRU -> request: round base + steps completed by that GRU CTA
+    unsigned int *round_ctr;       // rounds this handle has run: tags every hand-over word, so nothing needs zeroing
     // Cond-static arm: walk only the greedy chain (the frontier is dropped after every pop) for
     // B = L steps and record each depth's corrected top-k menu; the tree is then built by dt_scorers.cuh
     int static_mode;
@@ -103,22 +104,19 @@ __device__ __forceinline__ void st_relaxed_u32(unsigned int *p, unsigned int v) 
 __device__ __forceinline__ void st_relaxed_u64(unsigned long long *p, unsigned long long v) {
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
-__device__ __forceinline__ unsigned long long fused_desc_pack(int epoch, int sidx, int tok) {
-    return ((unsigned long long)(unsigned int)epoch << 48) | ((unsigned long long)(unsigned int)(sidx + 1) << 32) |
-           (unsigned long long)(unsigned int)tok;
+// descriptor word: step epoch (12 bits) | round tag (8) | parent state slot + 1 (12) | token (32)
+__device__ __forceinline__ unsigned long long fused_desc_pack(int epoch, unsigned int tag, int sidx, int tok) {
+    return ((unsigned long long)(unsigned int)epoch << 52) | ((unsigned long long)(tag & 0xFFu) << 44) |
+           ((unsigned long long)(unsigned int)(sidx + 1) << 32) | (unsigned long long)(unsigned int)tok;
 }
-
-// Zero the GRU flags and write the step-0 descriptor (the root: parent state = zeros, reading A4).
-__global__ void fused_init_kernel(FusedParams p) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < p.n_gru) p.flags[(size_t)i * kFusFlagStride] = 0u;
-    if (i < p.e.batch) {
-        int tok = p.e.root_tokens[i];
-        tok = min(max(tok, 0), p.e.V - 1);
-        p.desc[(size_t)i * kFusDescStride] = fused_desc_pack(1, 0, tok);
-    }
+__device__ __forceinline__ bool fused_desc_is(unsigned long long d, int epoch, unsigned int tag) {
+    return (unsigned int)(d >> 44) == (((unsigned int)epoch << 8) | (tag & 0xFFu));
 }
+__device__ __forceinline__ int fused_desc_sidx(unsigned long long d) { return (int)((d >> 32) & 0xFFFu) - 1; }
 
+// No initialisation kernel: the hand-over words carry the handle's round counter (flags: round * 256 + steps done,
+// compared as a signed difference; descriptors: an 8-bit round tag), each request CTA publishes its own root
+// descriptor (parent state = the zero slot, reading A4), and GRU CTA 0 bumps the counter when it leaves.
 // shared-memory footprints (bytes) of the two roles
 __host__ __device__ inline size_t fused_gru_smem(int g, int r, int upc, int m_tiles) {
     size_t w = (size_t)3 * upc * (g + kFusWPad) * 2;
@@ -192,6 +190,7 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
     const int nblk = g / kFusKB;
     const int blk0 = warp * nblk / kFusWarps, blk1 = (warp + 1) * nblk / kFusWarps;
 
+    const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 8;   // this round's tag / flag base
     for (int t = 0; t < e.B; ++t) {
         for (int c0 = 0; c0 < batch; c0 += kFusChunk) {
             const int nb = min(kFusChunk, batch - c0);
@@ -201,8 +200,8 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
                 int sidx = -1, tok = 0;
                 if (lane < nb) {
                     unsigned long long dsc;
-                    do { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride); } while ((int)(dsc >> 48) != t + 1);
-                    sidx = (int)((dsc >> 32) & 0xFFFFu) - 1;
+                    do { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride); } while (!fused_desc_is(dsc, t + 1, rnd));
+                    sidx = fused_desc_sidx(dsc);
                     tok = (int)(dsc & 0xFFFFFFFFull);
                 }
                 sIdx[lane] = sidx; sTok[lane] = tok;
@@ -372,9 +371,10 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
             __syncthreads();
         }
         DT_TR(0, 0, t, 4);
-        if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, (unsigned int)(t + 1)); }
+        if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, fbase + (unsigned int)(t + 1)); }
         DT_TR(0, 0, t, 5);
     }
+    if (cta == 0 && tid == 0) st_relaxed_u32(p.round_ctr, rnd + 1u);      // every CTA read it long ago
 }
 
 // ------------------------------------------------------------------------- GRU role, tcgen05 + TMEM
@@ -465,6 +465,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
     // (hi and lo, both 64-wide k-blocks of the slot); a warp instruction moves 4 whole 128-byte rows
     const int my_c = tid & 7, my_rq = tid >> 3;
 
+    const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 8;   // this round's tag / flag base
     for (int t = 0; t < e.B; ++t) {
         for (int c0 = 0; c0 < batch; c0 += kFusChunk) {
             const int nb = min(kFusChunk, batch - c0);
@@ -480,8 +481,8 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                 int sidx = -1, tok = 0;
                 if (lane < nb) {
                     unsigned long long dsc;
-                    do { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride); } while ((int)(dsc >> 48) != t + 1);
-                    sidx = (int)((dsc >> 32) & 0xFFFFu) - 1;
+                    do { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride); } while (!fused_desc_is(dsc, t + 1, rnd));
+                    sidx = fused_desc_sidx(dsc);
                     tok = (int)(dsc & 0xFFFFFFFFull);
                 }
                 sIdx[lane] = sidx; sTok[lane] = tok;
@@ -656,7 +657,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             __syncthreads();
         }
         DT_TR(0, 0, t, 4);
-        if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, (unsigned int)(t + 1)); }
+        if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, fbase + (unsigned int)(t + 1)); }
 #ifdef DT_TRACE
         if (tid == 0 && t == 5 && cta < 64) g_dt_trace[0][210 + cta / 8][cta % 8] = dt_globaltimer();
 #endif
@@ -664,6 +665,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
     }
     __syncthreads();
     if (warp == 0) tc::tmem_free<kTcCols>(tmem);
+    if (cta == 0 && tid == 0) st_relaxed_u32(p.round_ctr, rnd + 1u);      // every CTA read it long ago
 }
 
 // -------------------------------------------------------------------------------------- request role
@@ -686,6 +688,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     const int b = blockIdx.x - p.n_gru;
     const int r = e.r, M = e.M, k = e.k, N = e.N, L = e.L, batch = e.batch, B = e.B;
     const int ldw2 = r + kFusW2Pad;
+    const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 8;   // this round's tag / flag base
 
     // carve, every array 16-byte aligned: [W2 rows bf16] [frontier lo u64 x2] [new lo] [rank keys] [frontier hi u32 x2]
     // [new hi] [a] [z] [base] [cand tok] [tree tok / par / dep / score]
@@ -730,6 +733,8 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
 
     if (tid == 0) {
         nTok[0] = e.root_tokens[b]; nPar[0] = -1; nDep[0] = 0; nSco[0] = 0.f;
+        // step-0 descriptor: the root, whose parent state is the zero slot (reading A4)
+        st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(1, rnd, 0, min(max(e.root_tokens[b], 0), e.V - 1)));
         sm.n_valid = 1; sm.n_front = 0; sm.cur = 0;
     }
     __syncthreads();
@@ -748,7 +753,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         if (expand && tid < r) cpre = e.C[((size_t)b * L + depth) * r + tid];
         if (warp == 0) {
             for (int q = lane; q < p.n_gru; q += 32)
-                while (ld_relaxed_u32(p.flags + (size_t)q * kFusFlagStride) < (unsigned int)(t + 1)) { }
+                while ((int)(ld_relaxed_u32(p.flags + (size_t)q * kFusFlagStride) - (fbase + (unsigned int)(t + 1))) < 0) { }
         }
         __syncthreads();
         DT_TR(1, p.n_gru, t, 0);
@@ -919,7 +924,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                 const int tok = (int)(0xFFFFFFFFu - (unsigned int)(l >> 32));
                 const int par = (int)(0xFFFFFFFFu - (unsigned int)(l & 0xFFFFFFFFull));
                 const int dep = nDep[par] + 1;
-                if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(t + 2, dep < L ? par + 1 : -1, tok));
+                if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(t + 2, rnd, dep < L ? par + 1 : -1, tok));
 #ifdef DT_TRACE
                 if (t == 5 && b < 64) g_dt_trace[1][200 + b / 8][b % 8] = dt_globaltimer();
 #endif
@@ -927,7 +932,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                 sm.n_valid = t + 2; sm.n_front = p.static_mode ? 0 : min(tot, cap) - 1; sm.cur = cur ^ 1;
             } else {
                 sm.n_front = 0;
-                if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(t + 2, -1, 0));
+                if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(t + 2, rnd, -1, 0));
             }
         }
         DT_TR(1, p.n_gru, t, 4);
