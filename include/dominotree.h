@@ -164,7 +164,9 @@ int dt_adaptive_budget(dt_handle *h, const dt_outputs *tree, int32_t batch, int3
  *                   1 Marg (base logits alone, one menu per depth, no GRU),
  *                   2 Cond-static (correction once per depth along Domino's greedy chain, menu shared per depth;
  *                     bf16 shapes the fused kernel accepts, else dt_build_trees returns DT_ERR_UNSUPPORTED);
- *   "expand_path", "select_chunks", "select_kernel"   tuning / test switches of the kernels. */
+ *   "schedule"      0 best-first heap (Algorithm 1; default), 1 the depth-synchronous frontier builder of the paper's
+ *                   serving path with W = B lanes: the same tree on tie-free inputs;
+ *   "expand_path", "select_chunks", "select_kernel", "precompute_gemm"   tuning / test switches of the kernels. */
 int dt_set_option(dt_handle *h, const char *name, int64_t value);
 
 /*

@@ -12,6 +12,7 @@
 #include "dt_budget.cuh"
 #include "dt_commit.cuh"
 #include "dt_expand.cuh"
+#include "dt_frontier.cuh"
 #include "dt_fused.cuh"
 #include "dt_gemm_tc.cuh"
 #include "dt_precompute.cuh"
@@ -46,6 +47,8 @@ struct dt_handle {
     // options / bookkeeping
     int64_t opt_select_chunks;
     int64_t opt_select_kernel;      // 0 auto, 1 register-tile kernel only
+    int64_t opt_schedule;           // 0 best-first heap (Alg. 1), 1 depth-synchronous frontier builder
+    float *fr_state; int32_t *led_tok, *led_par, *led_cnt, *led_slot, *fr_ref, *fr_plane, *fr_n; float *led_g;
     int64_t opt_gemm;               // 0 auto (tcgen05 when the shape allows), 1 legacy mma.sync kernel
     int64_t opt_scorer;             // 0 DominoTree (Alg. 1), 1 Marg, 2 Cond-static
     int32_t *menu_tok; float *menu_lp;
@@ -127,6 +130,11 @@ extern "C" int dt_set_option(dt_handle *h, const char *name, int64_t value) {
     if (!strcmp(name, "expand_path")) {
         if (value < 0 || value > 4) return DT_ERR_INVALID_ARG;
         h->opt_expand_path = value;
+        return DT_OK;
+    }
+    if (!strcmp(name, "schedule")) {
+        if (value < 0 || value > 1) return DT_ERR_INVALID_ARG;
+        h->opt_schedule = value;
         return DT_OK;
     }
     if (!strcmp(name, "precompute_gemm")) {
@@ -258,6 +266,12 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     const size_t rows_pad = (rows + 127) / 128 * 128;
     h->tcg_ok = h->mma_ok && (w->d % (64 * kTcgSplits) == 0) && (w->r % 16 == 0) && w->r <= 256 && h->opt_gemm != 1;
     const size_t o_tcg = h->tcg_ok ? carve((size_t)kTcgSplits * rows_pad * w->r * 4) : 0;
+    // frontier schedule: lane states (ping-pong), ledger, frontier lists
+    const size_t led_n = (size_t)max_batch * L * max_B * k;
+    const size_t o_fst = carve((size_t)2 * max_batch * max_B * w->g * 4);
+    const size_t o_ltok = carve(led_n * 4), o_lpar = carve(led_n * 4), o_lg = carve(led_n * 4), o_lslot = carve(led_n * 4);
+    const size_t o_lcnt = carve(rows * 4), o_fref = carve((size_t)2 * max_batch * max_B * 4), o_fpl = carve((size_t)2 * max_batch * max_B * 4);
+    const size_t o_fn = carve((size_t)2 * max_batch * 4);
     const size_t o_hg = carve((size_t)max_batch * h->heap_cap * 4);
     const size_t o_htp = carve((size_t)max_batch * h->heap_cap * 8);
     const size_t o_hcnt = carve((size_t)max_batch * 4);
@@ -272,6 +286,9 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     h->heap_g = (float *)(h->ws + o_hg); h->heap_tp = (unsigned long long *)(h->ws + o_htp);
     h->heap_cnt = (int32_t *)(h->ws + o_hcnt);
     h->menu_tok = (int32_t *)(h->ws + o_mtok); h->menu_lp = (float *)(h->ws + o_mlp);
+    h->fr_state = (float *)(h->ws + o_fst); h->led_tok = (int32_t *)(h->ws + o_ltok); h->led_par = (int32_t *)(h->ws + o_lpar);
+    h->led_g = (float *)(h->ws + o_lg); h->led_slot = (int32_t *)(h->ws + o_lslot); h->led_cnt = (int32_t *)(h->ws + o_lcnt);
+    h->fr_ref = (int32_t *)(h->ws + o_fref); h->fr_plane = (int32_t *)(h->ws + o_fpl); h->fr_n = (int32_t *)(h->ws + o_fn);
     if (h->tcg_ok) {
         h->tcg_partial = (float *)(h->ws + o_tcg);
         if (cudaFuncSetAttribute(gemm_c_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_tc_smem()) != cudaSuccess) { cudaGetLastError(); h->tcg_ok = 0; }
@@ -454,6 +471,29 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
     return phase_mark(h, 4, st);
 }
 
+// Depth-synchronous frontier schedule (dt_frontier.cuh): L per-depth launches + the ledger selection / emitter.
+template <typename T>
+static int launch_frontier(dt_handle *h, const ExpandParams &p, cudaStream_t st) {
+    FrontierParams f;
+    f.e = p; f.W = p.B;                              // W = B: the same node set as the heap
+    f.fstate = h->fr_state; f.led_tok = h->led_tok; f.led_par = h->led_par; f.led_g = h->led_g;
+    f.led_cnt = h->led_cnt; f.led_slot = h->led_slot; f.fr_ref = h->fr_ref; f.fr_plane = h->fr_plane; f.n_fr = h->fr_n;
+    const size_t dsm = (size_t)(p.g + p.r + 2 * p.M) * 4 + (size_t)p.M * 4;
+    if (dsm > 48 * 1024) return DT_ERR_UNSUPPORTED;
+    int rc = phase_mark(h, 2, st);
+    if (rc) return rc;
+    for (int d = 0; d < p.L; ++d) {
+        frontier_depth_kernel<T><<<p.batch, kExpThreads, dsm, st>>>(f, d);
+        h->launches++;
+    }
+    DT_CUDA(h, cudaGetLastError());
+    if ((rc = phase_mark(h, 3, st))) return rc;
+    frontier_finalize_kernel<<<p.batch, kExpThreads, (size_t)4 * p.N * 4, st>>>(f);
+    h->launches++;
+    DT_CUDA(h, cudaGetLastError());
+    return phase_mark(h, 4, st);
+}
+
 // Factorized arms (dt_scorers.cuh): best-first over the per-depth menus in h->menu_*, then the emitter.
 static int launch_factorized(dt_handle *h, const ExpandParams &p, cudaStream_t st) {
     ScorerParams sp;
@@ -545,6 +585,8 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
     p.tokens = out->tokens; p.parents = out->parents; p.depths = out->depths; p.positions = out->positions;
     p.n_nodes = out->n_nodes; p.scores = out->scores; p.mask = out->mask;
     p.root_tokens = root_tokens; p.root_positions = root_positions;
+    if (h->opt_schedule == 1 && h->opt_scorer == 0)  // frontier schedule of the DominoTree scorer
+        return (w.dtype == DT_BF16) ? launch_frontier<__nv_bfloat16>(h, p, st) : launch_frontier<float>(h, p, st);
     if (h->opt_scorer == 1) {                       // Marg: menus from the base logits alone, no GRU, no C
         ScorerParams sp;
         sp.e = p; sp.menu_tok = h->menu_tok; sp.menu_lp = h->menu_lp;
