@@ -4,28 +4,33 @@
 //
 // Two CTA roles, co-resident on the chip (cooperative launch), in lock-step over t = 0 .. B-1:
 //
-//  * GRU CTAs (n_gru of them) are weight-stationary: CTA j keeps the 3*upc rows of W_hh that
-//    produce GRU units [j*upc, (j+1)*upc) and the matching columns of W1[:, d:] in shared memory for
+//  * GRU CTAs (n_gru = g / 16 of them) are weight-stationary: CTA j keeps the 48 rows of W_hh that
+//    produce GRU units [16 j, 16 j + 16) and the matching columns of W1[:, d:] in shared memory for
 //    the whole round.  Step t: for the node every request popped t-th, hidden half W_hh S_parent on
-//    the tensor cores (mma.sync m16n8k16, states split bf16 hi + lo so the bf16 x bf16 products are
-//    exact and the state is carried to ~2^-17 relative; split-K over the warps, each warp streaming
-//    its k-blocks of the parents' states from L2 through a private cp.async ring), gates with the input half gathered from the
-//    table P = E W_ih^T, new state S_t, and this CTA's split-K share of
-//    W1[:, d:] S_t written as a partial [batch, r].
+//    the 5th-generation tensor cores (fused_gru_role_tc: tcgen05.mma M = 64, N = hi|lo columns of up
+//    to 32 requests, accumulators in TMEM; the parents' states, split bf16 hi + lo so that every
+//    bf16 x bf16 product is exact and the state is carried to ~2^-17 relative, stream from L2 through
+//    a cp.async ring in the 128-byte-swizzled operand layout), gates with the input half gathered
+//    from the table P = E W_ih^T, new state S_t, and this CTA's split-K share of
+//    W1[:, d:] S_t, a second small tcgen05 GEMM, written as a partial [batch, r].
+//    fused_gru_role<UPC> is the same role on legacy mma.sync for shapes tcgen05 path rejects
+//    (g not a multiple of 256, r > 256): ~256 MAC/clk/SM on B200, kept as the fallback.
 //  * Request CTAs (one per request) own that request's heap in shared memory.  Step t: sum the
-//    partials in CTA order (fixed order => deterministic, batch-invariant), a = SiLU(C + .),
+//    partials in a fixed order (deterministic, batch-invariant), a = SiLU(C + .),
 //    z_m = (base_m + W2[cand_m, :] a) / T_eff over the M candidate rows of the node's depth
 //    (rows staged into shared memory by cp.async while the GRU CTAs work),
-//    slice log-softmax (reading A1), top-k, merge into the sorted frontier, pop entry 0 (reading A8)
-//    into slot t+1.
+//    slice log-softmax (reading A1), top-k, publish the next node's descriptor, merge the children
+//    into the sorted frontier, pop entry 0 (reading A8) into slot t+1.
 //    After the last pop the same CTA emits positions, padding and the ancestor mask (a9).
 //
-// The two roles hand over through self-describing words in global memory, one per producer, so no
-// shared counter is contended: request b publishes {epoch, parent state slot, token} in desc[b] and
-// GRU CTA c publishes its completed step count in flags[c]; consumers poll with L1-bypassing loads
-// (one lane per producer), fence, and release the CTA through one barrier.
+// The two roles hand over through self-describing words in global memory, one per producer and one
+// 128-byte line each, so nothing is contended: request b publishes {step, round tag, parent state
+// slot, token} in its descriptor word and GRU CTA c publishes round * 256 + its completed step count
+// in its flag word; consumers poll with L1-bypassing loads (one lane per producer) and release the
+// CTA through one barrier.  The round counter lives on the device, so no kernel has to reset anything.
 // The request CTA keeps its frontier as a SORTED array (one entry per thread, truncated to the pops
 // that remain), so a pop is "take entry 0" and a push is a rank-and-scatter merge of the k children.
+// Static mode (Cond-static arm) walks only the greedy chain and records per-depth menus.
 #pragma once
 #include "dt_expand.cuh"
 #include "dt_gemm_mma.cuh"
@@ -690,14 +695,13 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     const int ldw2 = r + kFusW2Pad;
     const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 8;   // this round's tag / flag base
 
-    // carve, every array 16-byte aligned: [W2 rows bf16] [frontier lo u64 x2] [new lo] [rank keys] [frontier hi u32 x2]
+    // carve, every array 16-byte aligned: [W2 rows bf16] [frontier lo u64 x2] [new lo] [frontier hi u32 x2]
     // [new hi] [a] [z] [base] [cand tok] [tree tok / par / dep / score]
     size_t off = 0;
     auto carve = [&](size_t bytes) { unsigned char *q = smem_raw + off; off += (bytes + 15) / 16 * 16; return q; };
     __nv_bfloat16 *sW2 = reinterpret_cast<__nv_bfloat16 *>(carve(p.w2_smem ? (size_t)M * ldw2 * 2 : 0));
     unsigned long long *fLo = reinterpret_cast<unsigned long long *>(carve((size_t)2 * kFusMaxFront * 8));
     unsigned long long *nLo = reinterpret_cast<unsigned long long *>(carve((size_t)k * 8));
-    unsigned long long *sKey = reinterpret_cast<unsigned long long *>(carve((size_t)M * 8));
     unsigned int *fHi = reinterpret_cast<unsigned int *>(carve((size_t)2 * kFusMaxFront * 4));
     unsigned int *nHi = reinterpret_cast<unsigned int *>(carve((size_t)k * 4));
     float *sA = reinterpret_cast<float *>(carve((size_t)r * 4));
