@@ -409,6 +409,55 @@ def measure_batch1(ctx):
     return out
 
 
+def _time_graphs(torch, dtb, builder, st, lg, hd, rt, rp, M, B, T):
+    """us per round of batch-1 rounds, one CUDA graph per input, inputs rotated (working set > L2)."""
+    n_in = lg.shape[0]
+    o = dtb.alloc_outputs(1, B)
+    graphs = []
+    with torch.cuda.stream(st):
+        builder.build_trees(lg[0:1], hd[0:1], rt[0:1], rp[0:1], M, B, T, out=o, stream=st)
+        st.synchronize()
+        for i in range(n_in):
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=st):
+                builder.build_trees(lg[i:i + 1], hd[i:i + 1], rt[i:i + 1], rp[i:i + 1], M, B, T, out=o, stream=st)
+            graphs.append(g)
+        for g in graphs:
+            g.replay()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        for i in range(2 * n_in):
+            graphs[i % n_in].replay()
+        e1.record(st)
+        st.synchronize()
+    return 1e3 * e0.elapsed_time(e1) / (2 * n_in)
+
+
+def measure_sweep_and_arms(ctx):
+    """--sweep: BASELINE configs[3] (batch 1, B in {16,32,64,128} x M in {32,64,128}, T = 0) and the three scorer
+    arms of PAPER.md:553-555 at batch 1, B = 16, M = 64, on the bench's weights; 64 rotating inputs per point."""
+    torch, dtb, wl, cfg, st = ctx["torch"], ctx["dtb"], ctx["wl"], ctx["cfg"], ctx["st"]
+    w_gpu = {n: t.cuda() for n, t in ctx["w_cpu"].items()}
+    builder = dtb.DominoTreeBuilder(w_gpu, max_batch=1, L=cfg.L, max_M=128, max_B=128, k=cfg.k)
+    n_in = 64
+    lg = torch.cat([s["logits"] for s in ctx["sets"]])[:n_in]
+    hd = torch.cat([s["hidden"] for s in ctx["sets"]])[:n_in]
+    rt = torch.cat([s["root_tokens"] for s in ctx["sets"]])[:n_in]
+    rp = torch.cat([s["root_positions"] for s in ctx["sets"]])[:n_in]
+    sweep = {}
+    for M in (32, 64, 128):
+        for B in (16, 32, 64, 128):
+            sweep[f"M{M}_B{B}"] = _time_graphs(torch, dtb, builder, st, lg, hd, rt, rp, M, B, 0.0)
+    arms = {}
+    for scorer, name in ((0, "dominotree"), (1, "marg"), (2, "cond_static")):
+        builder.set_option("scorer", scorer)
+        arms[name] = _time_graphs(torch, dtb, builder, st, lg, hd, rt, rp, 64, 16, 0.0)
+    builder.set_option("scorer", 0)
+    builder.close()
+    return {"us_per_round": sweep, "note": "batch 1, flat / peaked inputs mixed, one CUDA graph per round"}, \
+           {"us_per_round_batch1_B16_M64": arms}
+
+
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--gpus", type=int, default=1)
@@ -418,6 +467,7 @@ def main():
     ap.add_argument("--workload", default="concurrent8b")
     ap.add_argument("--rotate", type=int, default=4, help="distinct input sets rotated through the timed region")
     ap.add_argument("--no-extras", action="store_true", help="skip the e2e / cpu_baseline / batch-1 legs")
+    ap.add_argument("--sweep", action="store_true", help="also time the batch-1 B x M sweep and the three scorer arms")
     args = ap.parse_args()
     if args.impl == "reference":
         if args.steps == 200 and args.warmup == 20:      # defaults: keep the CPU run within minutes
@@ -471,6 +521,8 @@ def main():
         if rank == 0 and world == 1:
             line["cpu_baseline"], line["parity_sample"] = measure_cpu_baseline(ctx)
             line["batch1"] = measure_batch1(ctx)
+            if args.sweep:
+                line["sweep"], line["arms"] = measure_sweep_and_arms(ctx)
     if rank == 0:
         print(json.dumps(line), flush=True)
     ctx["builder"].close()
