@@ -478,7 +478,7 @@ static int launch_frontier(dt_handle *h, const ExpandParams &p, cudaStream_t st)
     f.e = p; f.W = p.B;                              // W = B: the same node set as the heap
     f.fstate = h->fr_state; f.led_tok = h->led_tok; f.led_par = h->led_par; f.led_g = h->led_g;
     f.led_cnt = h->led_cnt; f.led_slot = h->led_slot; f.fr_ref = h->fr_ref; f.fr_plane = h->fr_plane; f.n_fr = h->fr_n;
-    const size_t dsm = (size_t)(p.g + p.r + 2 * p.M) * 4 + (size_t)p.M * 4;
+    const size_t dsm = (size_t)(p.g + p.r + 2 * p.M + kFrLanes * p.g) * 4 + (size_t)p.M * 4;
     if (dsm > 48 * 1024) return DT_ERR_UNSUPPORTED;
     int rc = phase_mark(h, 2, st);
     if (rc) return rc;

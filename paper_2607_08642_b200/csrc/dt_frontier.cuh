@@ -29,13 +29,15 @@ struct FrontierParams {
     int32_t *led_slot;              // [batch, L, W k]  tree slot of a selected entry, -1 otherwise
 };
 
+constexpr int kFrLanes = 4;          // frontier lanes advanced together in the GRU phase
+
 // key order of the heap (reading A8): larger pops first
 __device__ __forceinline__ bool led_before(float ga, int ta, int pa, float gb, int tb, int pb) {
     return ga > gb || (ga == gb && (ta < tb || (ta == tb && pa < pb)));
 }
 
 // One depth for one request: states of the frontier lanes, CHILDREN of every lane into the ledger, next frontier.
-// grid = batch, block = 256, dynamic smem = (g + r + 2 M) floats + M ints.
+// grid = batch, block = 256, dynamic smem = (g + r + 2 M + kFrLanes g) floats + M ints.
 template <typename T>
 __global__ void __launch_bounds__(kExpThreads) frontier_depth_kernel(FrontierParams p, int d) {
     extern __shared__ float fsm_[];
@@ -46,6 +48,7 @@ __global__ void __launch_bounds__(kExpThreads) frontier_depth_kernel(FrontierPar
     const int g = e.g, r = e.r, M = e.M, k = e.k, L = e.L, W = p.W;
     float *sS = fsm_, *sA = sS + g, *sZ = sA + r, *sLp = sZ + M;
     int *sTok = reinterpret_cast<int *>(sLp + M);
+    float *sSp = reinterpret_cast<float *>(sTok + M);           // [kFrLanes][g] parent states of one lane group
     const int cur = d & 1, nxt = cur ^ 1;
     const size_t WK = (size_t)W * k;
     const int nl = (d == 0) ? 1 : p.n_fr[(size_t)cur * e.batch + b];
@@ -56,36 +59,61 @@ __global__ void __launch_bounds__(kExpThreads) frontier_depth_kernel(FrontierPar
     for (int m = tid; m < M; m += kExpThreads) sTok[m] = e.cand_id[row * M + m];
     const float base0 = e.cand_val[row * M];
 
-    for (int l = 0; l < nl; ++l) {
-        // (1) lane state: root S_0 = GRUcell(0, E[root]) (A4), else GRUcell(S_parent-lane, E[token])
-        const int ref = (d == 0) ? -1 : p.fr_ref[((size_t)cur * e.batch + b) * W + l];
-        float gpar = 0.f;
-        int tok;
-        const float *Sp = nullptr;
-        if (d == 0) { tok = min(max(e.root_tokens[b], 0), e.V - 1); }
-        else {
-            const size_t li = ((size_t)b * L + (d - 1)) * WK + ref;
-            tok = p.led_tok[li]; gpar = p.led_g[li];
-            Sp = p.fstate + (((size_t)nxt * e.batch + b) * W + p.fr_plane[((size_t)cur * e.batch + b) * W + l]) * g;
+    // (1) lane states, kFrLanes lanes at a time so that every W_hh row is read once per group, not once per lane:
+    //     root S_0 = GRUcell(0, E[root]) (A4), else GRUcell(S_parent-lane, E[token])
+    for (int l0 = 0; l0 < nl; l0 += kFrLanes) {
+        const int ng = min(kFrLanes, nl - l0);
+        __syncthreads();
+        for (int i = tid; i < ng * g; i += kExpThreads) {
+            const int q = i / g, u = i - q * g;
+            float v = 0.f;
+            if (d > 0) v = p.fstate[(((size_t)nxt * e.batch + b) * W + p.fr_plane[((size_t)cur * e.batch + b) * W + l0 + q]) * g + u];
+            sSp[q * g + u] = v;
         }
-        float *Sn = p.fstate + (((size_t)cur * e.batch + b) * W + l) * g;
-        const float *pr = e.P + (size_t)tok * 3 * g;
         __syncthreads();
         for (int u = warp; u < g; u += kExpThreads / 32) {
-            float hr = 0.f, hz = 0.f, hn = 0.f, hp = 0.f;
-            if (Sp) {
-                hr = warp_dot(whh + (size_t)u * g, Sp, g, lane);
-                hz = warp_dot(whh + (size_t)(g + u) * g, Sp, g, lane);
-                hn = warp_dot(whh + (size_t)(2 * g + u) * g, Sp, g, lane);
-                hp = Sp[u];
+            float acc[3][kFrLanes];
+#pragma unroll
+            for (int gt = 0; gt < 3; ++gt)
+#pragma unroll
+                for (int q = 0; q < kFrLanes; ++q) acc[gt][q] = 0.f;
+            if (d > 0) {
+                for (int i = lane; i < g; i += 32) {
+#pragma unroll
+                    for (int gt = 0; gt < 3; ++gt) {
+                        const float wv = ldf(whh, ((size_t)gt * g + u) * g + i);
+#pragma unroll
+                        for (int q = 0; q < kFrLanes; ++q) acc[gt][q] = fmaf(wv, sSp[q * g + i], acc[gt][q]);
+                    }
+                }
+#pragma unroll
+                for (int gt = 0; gt < 3; ++gt)
+#pragma unroll
+                    for (int q = 0; q < kFrLanes; ++q) acc[gt][q] = warp_sum(acc[gt][q]);
             }
-            if (lane == 0) {
+            if (lane < ng) {                                   // lane q finishes unit u of frontier lane l0 + q
+                float hr = 0.f, hz = 0.f, hn = 0.f;
+#pragma unroll
+                for (int q = 0; q < kFrLanes; ++q) if (q == lane) { hr = acc[0][q]; hz = acc[1][q]; hn = acc[2][q]; }
+                int tok;
+                if (d == 0) tok = min(max(e.root_tokens[b], 0), e.V - 1);
+                else tok = p.led_tok[((size_t)b * L + (d - 1)) * WK + p.fr_ref[((size_t)cur * e.batch + b) * W + l0 + lane]];
+                const float *pr = e.P + (size_t)tok * 3 * g;
                 const float rg = sigmoidf_acc(pr[u] + hr), zg = sigmoidf_acc(pr[g + u] + hz);
-                const float ng = tanhf(pr[2 * g + u] + rg * hn);
-                const float h = (1.0f - zg) * ng + zg * hp;
-                Sn[u] = h; sS[u] = h;
+                const float ng2 = tanhf(pr[2 * g + u] + rg * hn);
+                p.fstate[(((size_t)cur * e.batch + b) * W + l0 + lane) * g + u] = (1.0f - zg) * ng2 + zg * sSp[lane * g + u];
             }
         }
+    }
+    __threadfence_block();
+    __syncthreads();
+
+    for (int l = 0; l < nl; ++l) {
+        const int ref = (d == 0) ? -1 : p.fr_ref[((size_t)cur * e.batch + b) * W + l];
+        const float gpar = (d == 0) ? 0.f : p.led_g[((size_t)b * L + (d - 1)) * WK + ref];
+        const float *Sn = p.fstate + (((size_t)cur * e.batch + b) * W + l) * g;
+        __syncthreads();
+        for (int u = tid; u < g; u += kExpThreads) sS[u] = Sn[u];
         __syncthreads();
         // (2) a = SiLU(C + W1[:, d:] S)
         for (int j = warp; j < r; j += kExpThreads / 32) {
