@@ -166,8 +166,19 @@ int dt_adaptive_budget(dt_handle *h, const dt_outputs *tree, int32_t batch, int3
  *                     bf16 shapes the fused kernel accepts, else dt_build_trees returns DT_ERR_UNSUPPORTED);
  *   "schedule"      0 best-first heap (Algorithm 1; default), 1 the depth-synchronous frontier builder of the paper's
  *                   serving path with W = B lanes: the same tree on tie-free inputs;
+ *   "wave_width"    nodes a request may expand per dependent step of the wavefront kernel (0 = auto, 1 = the plain heap
+ *                   schedule, up to 15); any value gives the same tree;
  *   "expand_path", "select_chunks", "select_kernel", "precompute_gemm"   tuning / test switches of the kernels. */
 int dt_set_option(dt_handle *h, const char *name, int64_t value);
+
+/* dt_get_option: read-back values; unknown name -> INVALID_ARG.  The device-side words synchronise the device first
+ * (not capture-safe).
+ *   "expand_path_taken"  expansion path the last dt_build_trees enqueued: 1 per-step kernels, 2 / 3 lock-step fused kernel
+ *                        on mma.sync, 4 lock-step fused kernel on tcgen05, 5 wavefront kernel (dt_wave.cuh);
+ *   "state_slots"        GRU state slots per request in the workspace;
+ *   "device_error"       1 after a hand-over wait inside a persistent kernel timed out (the round's outputs are invalid);
+ *   "wave_steps", "wave_expansions"   dependent steps and CHILDREN evaluations request 0 needed in the last wavefront round. */
+int dt_get_option(dt_handle *h, const char *name, int64_t *value);
 
 /*
  * Phase timing (measurement aid, off by default).  dt_phase_timing(h, n_slots) creates n_slots

@@ -17,7 +17,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libdominotree.so")
 
 DT_BF16, DT_F32 = 0, 1
-EXPORTS = ("dt_create", "dt_build_trees", "dt_select_topm", "dt_build_trees_host", "dt_commit_paths", "dt_adaptive_budget", "dt_set_option",
+EXPORTS = ("dt_create", "dt_build_trees", "dt_select_topm", "dt_build_trees_host", "dt_commit_paths", "dt_adaptive_budget", "dt_set_option", "dt_get_option",
            "dt_kernel_launches", "dt_destroy", "dt_error_string", "dt_version", "dt_workspace_bytes",
            "dt_last_cuda_error", "dt_phase_timing", "dt_phase_slot", "dt_phase_elapsed_ms")
 PHASES = ("select", "precompute", "expand", "emit")
@@ -68,6 +68,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.dt_select_topm.restype = ctypes.c_int
     lib.dt_set_option.argtypes = [vp, ctypes.c_char_p, i64]
     lib.dt_set_option.restype = ctypes.c_int
+    lib.dt_get_option.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(i64)]
+    lib.dt_get_option.restype = ctypes.c_int
     lib.dt_kernel_launches.argtypes = [vp]
     lib.dt_kernel_launches.restype = i64
     lib.dt_destroy.argtypes = [vp]
@@ -263,6 +265,11 @@ class DominoTreeBuilder:
     # -- misc -------------------------------------------------------------------------------------
     def set_option(self, name: str, value: int):
         _check(self.lib, self.lib.dt_set_option(self._h, name.encode(), int(value)), f"dt_set_option({name})")
+
+    def get_option(self, name: str) -> int:
+        v = ctypes.c_int64()
+        _check(self.lib, self.lib.dt_get_option(self._h, name.encode(), ctypes.byref(v)), f"dt_get_option({name})", self._h)
+        return int(v.value)
 
     def phase_timing(self, n_slots: int):
         """dt_phase_timing: create (or with 0 free) n_slots sets of phase-boundary CUDA events."""

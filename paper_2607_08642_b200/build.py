@@ -15,7 +15,7 @@ CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libdominotree.so")
 SOURCES = ["dt_api.cu"]
 HEADERS = ["dt_common.cuh", "dt_select.cuh", "dt_precompute.cuh", "dt_expand.cuh", "dt_fused.cuh", "dt_gemm_mma.cuh",
-           "dt_tcgen05.cuh", "dt_commit.cuh", "dt_scorers.cuh", "dt_budget.cuh", "dt_gemm_tc.cuh", "dt_frontier.cuh"]
+           "dt_tcgen05.cuh", "dt_commit.cuh", "dt_scorers.cuh", "dt_budget.cuh", "dt_gemm_tc.cuh", "dt_frontier.cuh", "dt_wave.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]
 

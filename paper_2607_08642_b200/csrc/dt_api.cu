@@ -18,6 +18,7 @@
 #include "dt_precompute.cuh"
 #include "dt_scorers.cuh"
 #include "dt_select.cuh"
+#include "dt_wave.cuh"
 
 using namespace dt;
 
@@ -41,6 +42,10 @@ struct dt_handle {
     // fused persistent expansion (bf16): state copies, split-K partials, hand-over words
     __nv_bfloat16 *s_hi, *s_lo; float *partial; unsigned long long *desc; unsigned int *flags, *round_ctr;
     int fused_ok, max_smem_optin;
+    // wavefront expansion (dt_wave.cuh): per-item partials, multi-item descriptors, device error word, counters
+    float *wv_partial; unsigned long long *wv_desc; unsigned int *wv_err, *wv_stats; int wave_ok, slot_stride;
+    int64_t opt_wave_width;         // items per request per step (0 = auto)
+    int path_taken;                 // expansion path of the last dt_build_trees: 1 per-step, 2/3 fused mma.sync, 4 fused tcgen05, 5 wavefront
     int64_t opt_expand_path;        // 0 auto, 1 per-step kernels, 2 fused mma.sync upc=8, 3 fused mma.sync upc=16, 4 fused tcgen05
     // host-call staging (lazy)
     char *stage; size_t stage_bytes;
@@ -127,8 +132,13 @@ extern "C" int64_t dt_kernel_launches(const dt_handle *h) { return h ? h->launch
 
 extern "C" int dt_set_option(dt_handle *h, const char *name, int64_t value) {
     if (!h || !name) return DT_ERR_INVALID_ARG;
+    if (!strcmp(name, "wave_width")) {
+        if (value < 0 || value > kWvMaxW) return DT_ERR_INVALID_ARG;
+        h->opt_wave_width = value;
+        return DT_OK;
+    }
     if (!strcmp(name, "expand_path")) {
-        if (value < 0 || value > 4) return DT_ERR_INVALID_ARG;
+        if (value < 0 || value > 5) return DT_ERR_INVALID_ARG;
         h->opt_expand_path = value;
         return DT_OK;
     }
@@ -158,6 +168,22 @@ extern "C" int dt_set_option(dt_handle *h, const char *name, int64_t value) {
         return DT_OK;
     }
     return DT_ERR_INVALID_ARG;
+}
+
+// Read-back knobs (synchronise the device for the device-side words; not capture-safe).
+extern "C" int dt_get_option(dt_handle *h, const char *name, int64_t *value) {
+    if (!h || !name || !value) return DT_ERR_INVALID_ARG;
+    if (!strcmp(name, "expand_path_taken")) { *value = h->path_taken; return DT_OK; }
+    if (!strcmp(name, "state_slots")) { *value = h->slot_stride; return DT_OK; }
+    const bool dev_word = !strcmp(name, "device_error") || !strcmp(name, "wave_steps") || !strcmp(name, "wave_expansions");
+    if (!dev_word) return DT_ERR_INVALID_ARG;
+    *value = 0;
+    if (!h->wv_err) return DT_OK;
+    unsigned int w[12];
+    DT_CUDA(h, cudaDeviceSynchronize());
+    DT_CUDA(h, cudaMemcpy(w, h->wv_err, sizeof(w), cudaMemcpyDeviceToHost));
+    *value = !strcmp(name, "device_error") ? w[0] : !strcmp(name, "wave_steps") ? w[8] : w[9];
+    return DT_OK;
 }
 
 template <typename T>
@@ -240,18 +266,24 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     const size_t o_part = carve(rows * kSelMaxChunks * (size_t)max_M * 8);
     const size_t o_cnt = carve(rows * 4), o_tau = carve(rows * 4);
     const size_t o_C = carve(rows * w->r * 4);
-    const size_t slots = (size_t)(max_B > L ? max_B : L) + 2;  // fused layout: slot 0 = zeros, node t at t+1 (static mode walks L nodes)
+    // state slots per request: slot 0 = zeros, expansion x at x + 1; the wavefront schedule may expand up to 2 max_B + 1
+    // nodes (speculative picks included), static mode walks L nodes
+    const size_t slots = (size_t)((2 * max_B > L) ? 2 * max_B : L) + 2;
+    h->slot_stride = (int)slots;
     const size_t o_states = carve((size_t)max_batch * slots * w->g * 4);
     // fused path eligibility (shape part; the grid / smem fit is checked per call)
     h->fused_ok = (w->dtype == DT_BF16) && (w->g % 32 == 0) && (w->r % 8 == 0) && max_M <= 256 &&
                   ((reinterpret_cast<uintptr_t>(w->gru_w_hh) & 15u) == 0) && ((reinterpret_cast<uintptr_t>(w->corr_w2) & 15u) == 0);
-    size_t o_shi = 0, o_slo = 0, o_partial = 0, o_desc = 0, o_sync = 0;
+    size_t o_shi = 0, o_slo = 0, o_partial = 0, o_desc = 0, o_sync = 0, o_wpart = 0, o_wdesc = 0, o_werr = 0;
     if (h->fused_ok) {
         o_shi = carve((size_t)max_batch * slots * w->g * 2);
         o_slo = carve((size_t)max_batch * slots * w->g * 2);
         o_partial = carve((size_t)(w->g / 8) * max_batch * w->r * 4);
         o_desc = carve((size_t)max_batch * 8 * kFusDescStride);
         o_sync = carve((size_t)256 * 4 * kFusFlagStride + 256);
+        o_wpart = carve((size_t)max_batch * kWvMaxW * (w->g / 16 + 1) * w->r * 4);
+        o_wdesc = carve((size_t)max_batch * kWvDescWords * 8);
+        o_werr = carve(256);
     }
     // MMA GEMM eligibility: bf16, 16-byte aligned rows of H and W1
     h->mma_ok = (w->dtype == DT_BF16) && (w->d % 8 == 0) && ((w->d + w->g) % 8 == 0) &&
@@ -304,13 +336,19 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         h->partial = (float *)(h->ws + o_partial); h->desc = (unsigned long long *)(h->ws + o_desc);
         h->flags = (unsigned int *)(h->ws + o_sync);
         h->round_ctr = h->flags + (size_t)256 * kFusFlagStride;
+        h->wv_partial = (float *)(h->ws + o_wpart); h->wv_desc = (unsigned long long *)(h->ws + o_wdesc);
+        h->wv_err = (unsigned int *)(h->ws + o_werr); h->wv_stats = h->wv_err + 8;
+        h->wave_ok = (slots <= 1023);
         bool ok = cudaDeviceGetAttribute(&h->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess;
         h->max_smem_optin -= 1024;                  // room for the kernels' static shared memory
         if (!ok ||
             cudaFuncSetAttribute(fused_expand_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->max_smem_optin) != cudaSuccess ||
             cudaFuncSetAttribute(fused_expand_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->max_smem_optin) != cudaSuccess ||
             cudaFuncSetAttribute(fused_expand_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->max_smem_optin) != cudaSuccess) {
-            cudaGetLastError(); h->fused_ok = 0;
+            cudaGetLastError(); h->fused_ok = 0; h->wave_ok = 0;
+        }
+        if (h->wave_ok && cudaFuncSetAttribute(wave_expand_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, h->max_smem_optin) != cudaSuccess) {
+            cudaGetLastError(); h->wave_ok = 0;
         }
     }
 
@@ -448,7 +486,7 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
     memset(&f, 0, sizeof(f));
     f.e = p;
     f.upc = upc; f.n_gru = p.g / upc; f.m_tiles = (3 * upc + 15) / 16;
-    f.slot_stride = (h->max_B > h->L ? h->max_B : h->L) + 2;
+    f.slot_stride = h->slot_stride;
     f.s_hi = h->s_hi; f.s_lo = h->s_lo; f.s32 = h->states; f.partial = h->partial; f.desc = h->desc; f.flags = h->flags; f.round_ctr = h->round_ctr;
     f.static_mode = static_mode ? 1 : 0; f.menu_tok = h->menu_tok; f.menu_lp = h->menu_lp;
     f.w2_smem = 1;
@@ -466,7 +504,65 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
                                : cudaLaunchCooperativeKernel((const void *)fused_expand_kernel<16>, grid, block, args, dsm, st);
     h->launches++;
     DT_CUDA(h, e);
+    h->path_taken = tcgen ? 4 : (upc == 8 ? 2 : 3);
     if (static_mode) return DT_OK;
+    if ((rc = phase_mark(h, 3, st))) return rc;
+    return phase_mark(h, 4, st);
+}
+
+// Wavefront expansion (dt_wave.cuh).  Returns 1 if the shape does not fit (caller falls back to the lock-step fused
+// kernel), DT_OK after enqueueing, or a negative error.  Batches beyond what one cooperative launch holds (one request
+// CTA per request beside the g / 16 GRU CTAs) are split into consecutive launches: no cliff, requests are independent.
+static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st) {
+    if (!h->fused_ok || !h->wave_ok || (h->opt_expand_path != 0 && h->opt_expand_path != 5)) return 1;
+    if (p.g % kWvKC || p.g / 16 > 256 || p.r % 8 || p.r > 256 || p.k > 32 || p.M > 256 || p.L > DT_MAX_L) return 1;
+    const int n_gru = p.g / 16;
+    int cap = h->num_sms - n_gru;
+    if (cap > kWvMaxBatch) cap = kWvMaxBatch;
+    if (cap < 1) return 1;
+    const size_t gs = wave_gru_smem(p.g, p.r);
+    if (gs > (size_t)h->max_smem_optin) return 1;
+    int W = (int)h->opt_wave_width;
+    if (W <= 0) { W = 96 / (p.batch < cap ? p.batch : cap); }
+    if (W < 1) W = 1;
+    if (W > kWvMaxW) W = kWvMaxW;
+    const int e_max = h->slot_stride - 1;
+    int nsl = W < kWvMaxSlices ? W : kWvMaxSlices;
+    if (nsl > p.L) nsl = p.L;
+    size_t rs = 0;
+    for (; nsl >= 1; --nsl) {
+        rs = wave_req_smem(p.r, p.M, p.N, p.k, W, e_max, nsl);
+        if (rs <= (size_t)h->max_smem_optin) break;
+    }
+    if (nsl < 1) return 1;
+    const size_t dsm = gs > rs ? gs : rs;
+    int rc = phase_mark(h, 2, st);
+    if (rc) return rc;
+    for (int b0 = 0; b0 < p.batch; b0 += cap) {
+        const int nb = (p.batch - b0 < cap) ? (p.batch - b0) : cap;
+        WaveParams f;
+        memset(&f, 0, sizeof(f));
+        f.e = p;
+        f.e.batch = nb;
+        f.e.C = p.C + (size_t)b0 * p.L * p.r;
+        f.e.cand_id = p.cand_id + (size_t)b0 * p.L * p.M; f.e.cand_val = p.cand_val + (size_t)b0 * p.L * p.M;
+        f.e.tokens = p.tokens + (size_t)b0 * p.N; f.e.parents = p.parents + (size_t)b0 * p.N; f.e.depths = p.depths + (size_t)b0 * p.N;
+        f.e.positions = p.positions + (size_t)b0 * p.N; f.e.scores = p.scores + (size_t)b0 * p.N;
+        f.e.mask = p.mask + (size_t)b0 * p.N * p.N; f.e.n_nodes = p.n_nodes + b0;
+        f.e.root_tokens = p.root_tokens + b0; f.e.root_positions = p.root_positions ? p.root_positions + b0 : nullptr;
+        f.n_gru = n_gru; f.slot_stride = h->slot_stride; f.W = W; f.n_slices = nsl; f.e_max = e_max; f.P = n_gru;
+        const size_t so = (size_t)b0 * h->slot_stride * p.g;
+        f.s_hi = h->s_hi + so; f.s_lo = h->s_lo + so; f.s32 = h->states + so;
+        f.partial = h->wv_partial + (size_t)b0 * kWvMaxW * n_gru * p.r;
+        f.desc = h->wv_desc + (size_t)b0 * kWvDescWords;
+        f.flags = h->flags; f.round_ctr = h->round_ctr; f.err = h->wv_err; f.stats = (b0 == 0) ? h->wv_stats : nullptr;
+        void *args[] = {&f};
+        const dim3 grid(n_gru + nb), block(kWvThreads);
+        cudaError_t e = cudaLaunchCooperativeKernel((const void *)wave_expand_kernel, grid, block, args, dsm, st);
+        h->launches++;
+        DT_CUDA(h, e);
+    }
+    h->path_taken = 5;
     if ((rc = phase_mark(h, 3, st))) return rc;
     return phase_mark(h, 4, st);
 }
@@ -605,7 +701,10 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
         if (rc) return rc;
         return launch_factorized(h, p, st);
     }
+    h->path_taken = 1;
     if (w.dtype == DT_BF16) {
+        rc = launch_wave(h, p, st);
+        if (rc <= 0) return rc;
         rc = launch_fused(h, p, st);
         if (rc <= 0) return rc;
         return launch_expansion<__nv_bfloat16>(h, p, st);

@@ -1,0 +1,783 @@
+// dt_wave.cuh -- steps (a4)-(a9) as ONE persistent kernel with an exact WAVEFRONT schedule (bf16 weights).
+//
+// Algorithm 1 pops one node per step, so a round is a chain of B dependent
+// GRU -> correction -> pop steps.  By the equivalence lemma of Appendix B (scores are
+// monotone along a path, so best-first returns exactly the B best nodes of the candidate tree, an
+// ancestor-closed set) the ORDER in which CHILDREN(.) is evaluated does not matter, only that every
+// node the heap would expand has been expanded before the heap run is replayed.  This kernel therefore
+// lets every request expand up to W nodes per step:
+//
+//   repeat   replay the best-first heap on what is known (children lists of the nodes expanded so far);
+//            the first popped node whose children are unknown is exactly the node Algorithm 1 would
+//            expand next (NEEDED); the next W-1 unexpanded nodes the replay pops are SPECULATIVE picks
+//            (each lies in the top-B of the known scores, a necessary condition for being in the tree);
+//            expand all of them in one batched GRU step;
+//   until    a replay pops B nodes (or runs dry) without meeting an unexpanded node among its first B-1
+//            pops: that replay IS Algorithm 1's run, pop for pop, ties included (reading A8).
+//
+// W = 1 is the plain heap schedule (B steps); a bushy tree of depth D finishes in about D + 1 steps.
+// Speculative expansions that turn out useless cost GRU columns, never correctness.
+//
+// Two CTA roles, co-resident (cooperative launch), hand-over through self-describing words in L2 as in
+// dt_fused.cuh:
+//  * GRU CTAs (g / 16 of them, weight-stationary: 48 rows of W_hh + 16 columns of W1[:, d:] in shared
+//    memory).  Step s: gather the items {request, parent state slot, token} every request published,
+//    and for passes of up to 64 items run D1[node, row] = S_parent[node, :] . W_hh[row, :]^T on
+//    tcgen05 with the NODES as the M dimension (M = 128 rows = 64 nodes x {bf16 hi, bf16 lo}, N = 48,
+//    accumulators in TMEM; states stream from L2 through a cp.async ring in the 128-byte-swizzled
+//    K-major layout), gates with the input half gathered from P = E W_ih^T, new
+//    state to L2, and D2[node, j] = S_new[node, my 16 units] . W1[j, d + my units]^T, this CTA's
+//    split-K share of W1[:, d:] S_new, one M = 128, N = r MMA.
+//  * Request CTAs (one per request) keep the children lists, replay the heap, nominate, and for every
+//    expanded node compute a = SiLU(C + sum of partials), z = (base + W2[cand] a) / T_eff over the M
+//    candidate rows of the node's depth (rows staged per depth in shared memory "slices"), slice
+//    log-softmax (reading A1) and top-k; at the end they emit (a9).
+#pragma once
+#include "dt_fused.cuh"
+
+namespace dt {
+
+constexpr int kWvThreads = 256;
+constexpr int kWvNP = 64;                       // items per GRU pass (M = 128 operand rows: hi | lo)
+constexpr int kWvKC = 128;                      // k per ring slot (two 64-wide swizzle blocks)
+constexpr int kWvSlots = 3;
+constexpr int kWvSlotBytes = 128 * kWvKC * 2;   // 128 rows x 128 k bf16 = 32 KB
+constexpr int kWvDescWords = 16;                // u64 words per request descriptor: header + 15 items, one 128-byte line
+constexpr int kWvMaxW = kWvDescWords - 1;
+constexpr int kWvMaxBatch = 128;                // requests per launch (headers are polled by four warps)
+constexpr int kWvTmemCols = 512;                // D1[w] at 64 w (48 columns each, w < 4), D2 at 256 (r <= 256 columns)
+constexpr int kWvMaxSlices = 8;
+constexpr unsigned int kWvAct = 0x100u;         // replay word: cursor (8) | active (1) | pop slot (16, from bit 16)
+
+struct WaveParams {
+    ExpandParams e;
+    int n_gru;                     // GRU CTAs = g / 16
+    int slot_stride;               // state slots per request (slot 0 = zeros, expansion x lives in slot x + 1)
+    int W;                         // items a request may publish per step (1 .. kWvMaxW)
+    int n_slices;                  // W2 slices in a request CTA's shared memory
+    int e_max;                     // expansions per request = slot_stride - 1
+    int P;                         // partial vectors per item = n_gru
+    __nv_bfloat16 *s_hi, *s_lo;    // [batch, slot_stride, g]
+    float *s32;                    // [batch, slot_stride, g]
+    float *partial;                // [batch, kWvMaxW, P, r]
+    unsigned long long *desc;      // [batch, kWvDescWords]
+    unsigned int *flags;           // [n_gru] one 128-byte line each
+    unsigned int *round_ctr;       // rounds this handle has run (tags every hand-over word)
+    unsigned int *err;             // set to 1 when a hand-over wait timed out (protocol slip: fail, do not hang)
+    unsigned int *stats;           // [4] optional counters of request 0: steps, expansions (measurement aid)
+};
+
+// ---- hand-over words ---------------------------------------------------------------------------------
+// header: round (24) | epoch (12) | first new state slot (12) | done (1) | count (15)
+// item:   token (32) | parent state slot (10) | epoch (10) | round (12)
+// Every word is self-validating (relaxed stores need no ordering between them); epoch = step + 1, so
+// zero-initialised memory never matches.
+__device__ __forceinline__ unsigned long long wave_hdr_pack(unsigned int rnd, int epoch, int first, int done, int count) {
+    return ((unsigned long long)(rnd & 0xFFFFFFu) << 40) | ((unsigned long long)(epoch & 0xFFF) << 28) |
+           ((unsigned long long)(first & 0xFFF) << 16) | ((unsigned long long)(done & 1) << 15) | (unsigned long long)(count & 0x7FFF);
+}
+__device__ __forceinline__ bool wave_hdr_ok(unsigned long long h, unsigned int rnd, int epoch) {
+    if ((unsigned int)(h >> 40) != (rnd & 0xFFFFFFu)) return false;
+    return ((h >> 15) & 1ull) || (int)((h >> 28) & 0xFFFu) == (epoch & 0xFFF);
+}
+__device__ __forceinline__ unsigned long long wave_item_pack(unsigned int rnd, int epoch, int pslot, int tok) {
+    return ((unsigned long long)(unsigned int)tok << 32) | ((unsigned long long)(pslot & 0x3FF) << 22) |
+           ((unsigned long long)(epoch & 0x3FF) << 12) | (unsigned long long)(rnd & 0xFFFu);
+}
+__device__ __forceinline__ bool wave_item_ok(unsigned long long w, unsigned int rnd, int epoch) {
+    return (unsigned int)(w & 0x3FFFFFull) == ((((unsigned int)epoch & 0x3FFu) << 12) | (rnd & 0xFFFu));
+}
+
+__device__ __forceinline__ unsigned long long wave_timer() {
+    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
+}
+constexpr unsigned long long kWvTimeoutNs = 4000000000ull;     // 4 s: far beyond any round; a slip fails instead of hanging
+
+// TMEM -> registers: 8 consecutive fp32 columns of this thread's lane
+__device__ __forceinline__ void wave_tmem_ld8(uint32_t taddr, float (&v)[8]) {
+    uint32_t r[8];
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+// shared-memory footprints (bytes)
+__host__ __device__ inline size_t wave_gru_smem(int g, int r) {
+    const size_t r16 = (size_t)((r + 15) & ~15);
+    return (size_t)48 * g * 2 + (size_t)kWvSlots * kWvSlotBytes + r16 * 32 + 4096 +
+           (size_t)(5 * kWvNP + 3 * kWvMaxBatch + 8) * 4 + 8 * 8 + 64 + 1024;
+}
+__host__ __device__ inline size_t wave_slice_bytes(int r, int M) {
+    return (size_t)((M + 7) / 8) * (size_t)((r + 63) / 64) * 1024;
+}
+__host__ __device__ inline size_t wave_req_smem(int r, int M, int N, int k, int W, int e_max, int n_slices) {
+    auto al = [](size_t x) { return (x + 15) / 16 * 16; };
+    size_t s = (size_t)n_slices * wave_slice_bytes(r, M) + 2 * al((size_t)n_slices * M * 4);
+    s += al((size_t)e_max * k * 8) + al((size_t)e_max * k * 2) + 4 * al((size_t)e_max * 4) + 2 * al((size_t)e_max * 4);
+    s += 4 * al((size_t)N * 4);
+    s += al((size_t)W * r * 4) + al((size_t)W * M * 4) + al((size_t)8 * r * 4);
+    s += al((size_t)4 * kWvMaxW * 4) + al(256);
+    return s + 1024;
+}
+
+// bounded spin on a hand-over word; returns false on timeout (and raises *err)
+template <typename F>
+__device__ __forceinline__ bool wave_spin(F ready, unsigned int *err) {
+    if (ready()) return true;
+    const unsigned long long t0 = wave_timer();
+    unsigned int n = 0;
+    while (!ready()) {
+        if (((++n) & 1023u) == 0u) {
+            if (ld_relaxed_u32(err) != 0u) return false;
+            if (wave_timer() - t0 > kWvTimeoutNs) { atomicExch(err, 1u); return false; }
+        }
+    }
+    return true;
+}
+
+// ------------------------------------------------------------------------------------------ GRU role
+__device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char *smem_raw) {
+    const ExpandParams &e = p.e;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int g = e.g, r = e.r, batch = e.batch;
+    const int cta = blockIdx.x, u0 = cta * 16;
+    const size_t stride = (size_t)p.slot_stride;
+    const int n_kc = g / kWvKC;
+    const int r16 = (r + 15) & ~15;
+
+    // carve (smem_raw is 1024-byte aligned by the kernel)
+    unsigned char *sW = smem_raw;                                     // W_hh slice, K-major sw128: [6 row groups][g/64 atoms][1 KB]
+    const uint32_t sboW = (uint32_t)g * 16;                           // bytes between 8-row groups
+    unsigned char *sRing = sW + (size_t)48 * g * 2;                   // [slot][2 k-blocks][16 row groups][1 KB]
+    unsigned char *sW1 = sRing + (size_t)kWvSlots * kWvSlotBytes;     // W1[:, d + u0 ..] as [r16/8 groups][2 k-halves][8 rows][16 B]
+    unsigned char *sS2 = sW1 + (size_t)r16 * 32;                      // new states [16 groups][2 k-halves][8 rows][16 B]
+    int *sRow = reinterpret_cast<int *>(sS2 + 4096);                  // [64] request * stride + parent slot  (state row)
+    int *sNew = sRow + kWvNP;                                         // [64] request * stride + new slot
+    int *sTok = sNew + kWvNP;                                         // [64]
+    int *sIt = sTok + kWvNP;                                          // [64] request * kWvMaxW + item index (partial row)
+    int *sPz = sIt + kWvNP;                                           // [64] parent slot is the zero slot
+    int *sCnt = sPz + kWvNP;                                          // [128] items per request this step
+    int *sOff = sCnt + kWvMaxBatch;                                   // [129] exclusive prefix
+    int *sFirst = sOff + kWvMaxBatch + 4;                             // [128] first new state slot per request
+    unsigned long long *mbar = reinterpret_cast<unsigned long long *>(sFirst + kWvMaxBatch);   // [0..2] slot free, [3] D1, [4] D2
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(mbar + 8);
+    int *sCtl = reinterpret_cast<int *>(tmem_slot + 2);               // [0] items this step, [1] requests not done, [2] abort, [4..7] live masks
+
+    {   // resident weights
+        const __nv_bfloat16 *whh = reinterpret_cast<const __nv_bfloat16 *>(e.w_hh);
+        const int vpr = g / 8;
+        for (int i = tid; i < 48 * vpr; i += kWvThreads) {
+            const int m = i / vpr, c = i - m * vpr;                // local row m = gate * 16 + unit, 16-byte piece c
+            const int gate = m >> 4, ul = m & 15;
+            const uint4 q = ld_ro_v4(whh + ((size_t)gate * g + u0 + ul) * g + (size_t)c * 8);
+            *reinterpret_cast<uint4 *>(sW + (size_t)(m >> 3) * sboW + (size_t)(c >> 3) * 1024 + (m & 7) * 128 + (((c & 7) ^ (m & 7)) << 4)) = q;
+        }
+        const __nv_bfloat16 *w1 = reinterpret_cast<const __nv_bfloat16 *>(e.w1);
+        for (int i = tid; i < r16 * 16; i += kWvThreads) {
+            const int j = i >> 4, ul = i & 15;
+            const __nv_bfloat16 v = (j < r) ? w1[(size_t)j * (e.d + g) + e.d + u0 + ul] : __float2bfloat16_rn(0.f);
+            *reinterpret_cast<__nv_bfloat16 *>(sW1 + (size_t)(j >> 3) * 256 + (ul >> 3) * 128 + (j & 7) * 16 + (ul & 7) * 2) = v;
+        }
+        for (int i = tid; i < 1024; i += kWvThreads) reinterpret_cast<uint32_t *>(sS2)[i] = 0u;
+        if (tid == 0) {
+            for (int i = 0; i < kWvSlots; ++i) tc::mbar_init(tc::smem_u32(mbar + i), 4);
+            tc::mbar_init(tc::smem_u32(mbar + 3), 4);
+            tc::mbar_init(tc::smem_u32(mbar + 4), 1);
+            tc::mbar_init_fence();
+            sCtl[2] = 0;
+        }
+        if (warp == 0) tc::tmem_alloc<kWvTmemCols>(tmem_slot);
+    }
+    tc::fence_proxy_async();
+    tc::fence_before_sync();
+    __syncthreads();
+    tc::fence_after_sync();
+    const uint32_t tmem = *tmem_slot;
+    const uint32_t idesc1 = tc::make_idesc_bf16(128, 48), idesc2 = tc::make_idesc_bf16(128, r16);
+    const uint32_t mb0 = tc::smem_u32(mbar);
+    const uint64_t descW0 = tc::make_desc_sw128(tc::smem_u32(sW), sboW), descR0 = tc::make_desc_sw128(tc::smem_u32(sRing), 1024);
+    const uint64_t descS2 = tc::make_desc(tc::smem_u32(sS2), 128, 256), descW1 = tc::make_desc(tc::smem_u32(sW1), 128, 256);
+    uint32_t ph_free = 0, ph_d1 = 0, ph_d2 = 0;                    // mbarrier phases (uniform across the CTA)
+
+    // epilogue geometry: TMEM lane quadrant q4, unit half hsel; lanes 0..15 hold the hi rows of nodes 16 q4 + lane,
+    // lanes 16..31 the lo rows of the same nodes; after the hi + lo exchange lane < 16 finishes units 8 hsel + 0..3,
+    // lane >= 16 units 8 hsel + 4..7
+    const int q4 = warp & 3, hsel = warp >> 2, il = lane & 15, uh = lane >> 4;
+    const int my_node = 16 * q4 + il;
+    const int my_u = 8 * hsel + 4 * uh;                              // first of this thread's 4 local units
+    const uint32_t tlane = (uint32_t)(32 * q4) << 16;
+
+    const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 10;
+    for (int s = 0;; ++s) {
+        // ---- headers of step s: one lane per request
+        if (warp < 4) {
+            const int b = warp * 32 + lane;
+            int cnt = 0, first = 0, live = 0;
+            if (b < batch) {
+                unsigned long long hdr = 0ull;
+                const unsigned long long *hp = p.desc + (size_t)b * kWvDescWords;
+                const bool ok = wave_spin([&] { hdr = ld_relaxed_u64(hp); return wave_hdr_ok(hdr, rnd, s + 1); }, p.err);
+                if (!ok) sCtl[2] = 1;
+                else if (!((hdr >> 15) & 1ull)) { cnt = (int)(hdr & 0x7FFFull); first = (int)((hdr >> 16) & 0xFFFull); live = 1; }
+            }
+            sCnt[b] = cnt; sFirst[b] = first;
+            const unsigned int lv = __ballot_sync(0xffffffffu, live != 0);
+            if (lane == 0) sCtl[4 + warp] = (int)lv;
+        }
+        __syncthreads();
+        if (warp == 0) {                                            // exclusive prefix of the counts (4 per lane)
+            int c[4], sum = 0;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) { c[i] = sCnt[lane * 4 + i]; sum += c[i]; }
+            int inc = sum;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+            int run = inc - sum;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) { sOff[lane * 4 + i] = run; run += c[i]; }
+            if (lane == 31) { sOff[kWvMaxBatch] = inc; sCtl[0] = inc; }
+            if (lane == 0) sCtl[1] = (sCtl[4] | sCtl[5] | sCtl[6] | sCtl[7]) != 0;
+        }
+        __syncthreads();
+        const int total = sCtl[0];
+        if (sCtl[2] || !sCtl[1]) break;                              // abort, or every request is done
+
+        for (int p0 = 0; p0 < total; p0 += kWvNP) {
+            const int n = min(kWvNP, total - p0);
+            // ---- items of this pass: thread i < n fetches item p0 + i
+            if (tid < kWvNP) {
+                int row = 0, nw = 0, tok = 0, it = 0, pz = 1;
+                if (tid < n) {
+                    const int qi = p0 + tid;
+                    int lo = 0, hi = kWvMaxBatch - 1;                // last b with sOff[b] <= qi and a non-empty list
+                    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (sOff[mid] <= qi) lo = mid; else hi = mid - 1; }
+                    const int b = lo, j = qi - sOff[b];
+                    unsigned long long w = 0ull;
+                    const unsigned long long *ip = p.desc + (size_t)b * kWvDescWords + 1 + j;
+                    const bool ok = wave_spin([&] { w = ld_relaxed_u64(ip); return wave_item_ok(w, rnd, s + 1); }, p.err);
+                    if (!ok) sCtl[2] = 1;
+                    const int ps = (int)((w >> 22) & 0x3FFull);
+                    tok = (int)(w >> 32);
+                    tok = min(max(tok, 0), e.V - 1);
+                    row = b * (int)stride + ps; nw = b * (int)stride + sFirst[b] + j; it = b * kWvMaxW + j; pz = (ps == 0);
+                }
+                sRow[tid] = row; sNew[tid] = nw; sTok[tid] = tok; sIt[tid] = it; sPz[tid] = pz;
+            }
+            __syncthreads();
+
+            // ---- this thread's share of a ring slot: 8 operand rows (rho = (tid >> 4) + 16 i), 16-byte piece tid & 15
+            const int piece = tid & 15, kb = piece >> 3, pc = piece & 7;
+            const __nv_bfloat16 *src[8];
+            uint32_t dsto[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int rho = (tid >> 4) + 16 * i;
+                const int node = 16 * (rho >> 5) + (rho & 15), hl = (rho >> 4) & 1;
+                src[i] = nullptr;
+                if (node < n) src[i] = (hl ? p.s_lo : p.s_hi) + (size_t)sRow[node] * g + (size_t)piece * 8;
+                dsto[i] = (uint32_t)(kb * 16384 + (rho >> 3) * 1024 + (rho & 7) * 128 + ((pc ^ (rho & 7)) << 4));
+            }
+            auto issue_chunk = [&](int kc) {
+                unsigned char *dst = sRing + (size_t)(kc % kWvSlots) * kWvSlotBytes;
+                const size_t k0 = (size_t)kc * kWvKC;
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+                    if (src[i]) cp_async16(dst + dsto[i], src[i] + k0);
+            };
+#pragma unroll 1
+            for (int kc = 0; kc < kWvSlots; ++kc) { if (kc < n_kc) issue_chunk(kc); cp_async_commit(); }
+
+            // ---- epilogue operands (input half from P, previous state): issued now, consumed after the MMAs
+            float4 pr = make_float4(0.f, 0.f, 0.f, 0.f), pz4 = pr, pn = pr, hp = pr;
+            const bool mine = (my_node < n);
+            if (mine) {
+                const float *prow = e.P + (size_t)sTok[my_node] * 3 * g + u0 + my_u;
+                pr = __ldg(reinterpret_cast<const float4 *>(prow));
+                pz4 = __ldg(reinterpret_cast<const float4 *>(prow + g));
+                pn = __ldg(reinterpret_cast<const float4 *>(prow + 2 * g));
+                if (!sPz[my_node]) hp = __ldcg(reinterpret_cast<const float4 *>(p.s32 + (size_t)sRow[my_node] * g + u0 + my_u));
+            }
+
+            // ---- D1[128 x 48] = [S_hi | S_lo rows] . W_hh slice^T, K streamed through the ring
+#pragma unroll 1
+            for (int kc = 0; kc < n_kc; ++kc) {
+                cp_async_wait<kWvSlots - 1>();
+                tc::fence_proxy_async();
+                __syncthreads();
+                const int sl = kc % kWvSlots;
+                if (warp < 4 && lane == 0) {
+                    // warp w issues K = 16 steps 2 w and 2 w + 1 of the slot's eight into its own accumulator D1[w]
+                    tc::fence_after_sync();
+#pragma unroll
+                    for (int jj = 0; jj < 2; ++jj) {
+                        const int j8 = 2 * warp + jj, kbj = j8 >> 2, s4 = j8 & 3;
+                        const uint64_t da = descR0 + (uint64_t)((sl * kWvSlotBytes + kbj * 16384) / 16 + s4 * 2);
+                        const uint64_t db = descW0 + (uint64_t)((kc * 2 + kbj) * 64 + s4 * 2);
+                        tc::mma_bf16(tmem + 64 * warp, da, db, idesc1, (kc | jj) ? 1u : 0u);
+                    }
+                    if (kc + kWvSlots < n_kc) tc::commit(mb0 + 8 * sl);          // this slot is refilled below
+                    if (kc == n_kc - 1) tc::commit(mb0 + 24);
+                }
+                if (kc + kWvSlots < n_kc) {                  // refill the slot once its MMAs have read it
+                    tc::mbar_wait(mb0 + 8 * sl, (ph_free >> sl) & 1u);
+                    ph_free ^= 1u << sl;
+                    issue_chunk(kc + kWvSlots);
+                }
+                cp_async_commit();
+            }
+            cp_async_wait<0>();
+            tc::mbar_wait(mb0 + 24, ph_d1); ph_d1 ^= 1u;
+            tc::fence_after_sync();
+            __syncwarp();
+
+            // ---- gates (reading A2): columns gate * 16 + unit of the four accumulators, hi + lo rows added
+            float acc[24];
+#pragma unroll
+            for (int c = 0; c < 24; ++c) acc[c] = 0.f;
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                for (int gate = 0; gate < 3; ++gate) {
+                    float v[8];
+                    wave_tmem_ld8(tmem + tlane + 64 * a + gate * 16 + 8 * hsel, v);
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) acc[gate * 8 + c] += v[c];
+                }
+#pragma unroll
+            for (int c = 0; c < 24; ++c) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 16);
+            {
+                const float prv[4] = {pr.x, pr.y, pr.z, pr.w}, pzv[4] = {pz4.x, pz4.y, pz4.z, pz4.w};
+                const float pnv[4] = {pn.x, pn.y, pn.z, pn.w}, hpv[4] = {hp.x, hp.y, hp.z, hp.w};
+                float hn[4];
+                __nv_bfloat16 bh[4], bl[4];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const float rg = sigmoidf_fast(prv[c] + acc[4 * uh + c]);
+                    const float zg = sigmoidf_fast(pzv[c] + acc[8 + 4 * uh + c]);
+                    const float ng = tanhf_fast(pnv[c] + rg * acc[16 + 4 * uh + c]);
+                    hn[c] = mine ? ((1.0f - zg) * ng + zg * hpv[c]) : 0.f;
+                    bh[c] = __float2bfloat16_rn(hn[c]);
+                    bl[c] = __float2bfloat16_rn(hn[c] - __bfloat162float(bh[c]));
+                }
+                uint2 ph, pl;
+                ph.x = (uint32_t)__bfloat16_as_ushort(bh[0]) | ((uint32_t)__bfloat16_as_ushort(bh[1]) << 16);
+                ph.y = (uint32_t)__bfloat16_as_ushort(bh[2]) | ((uint32_t)__bfloat16_as_ushort(bh[3]) << 16);
+                pl.x = (uint32_t)__bfloat16_as_ushort(bl[0]) | ((uint32_t)__bfloat16_as_ushort(bl[1]) << 16);
+                pl.y = (uint32_t)__bfloat16_as_ushort(bl[2]) | ((uint32_t)__bfloat16_as_ushort(bl[3]) << 16);
+                if (mine) {                                          // publish S_new: fp32 and the bf16 hi/lo split
+                    const size_t o = (size_t)sNew[my_node] * g + u0 + my_u;
+                    __stcg(reinterpret_cast<float4 *>(p.s32 + o), make_float4(hn[0], hn[1], hn[2], hn[3]));
+                    __stcg(reinterpret_cast<uint2 *>(p.s_hi + o), ph);
+                    __stcg(reinterpret_cast<uint2 *>(p.s_lo + o), pl);
+                }
+                // operand A of the W1 GEMM: rows 32 q4 + il (hi) and + 16 (lo), k = local unit
+                const int rh = 32 * q4 + il, rl = rh + 16;
+                *reinterpret_cast<uint2 *>(sS2 + (size_t)(rh >> 3) * 256 + hsel * 128 + (rh & 7) * 16 + uh * 8) = ph;
+                *reinterpret_cast<uint2 *>(sS2 + (size_t)(rl >> 3) * 256 + hsel * 128 + (rl & 7) * 16 + uh * 8) = pl;
+            }
+            tc::fence_proxy_async();
+            tc::fence_before_sync();
+            __syncthreads();
+            // ---- D2[128 x r] = S_new[rows, my 16 units] . W1[:, d + my units]^T : this CTA's split-K share
+            if (tid == 0) {
+                tc::fence_after_sync();
+                tc::mma_bf16(tmem + 256, descS2, descW1, idesc2, 0u);
+                tc::commit(mb0 + 32);
+            }
+            tc::mbar_wait(mb0 + 32, ph_d2); ph_d2 ^= 1u;
+            tc::fence_after_sync();
+            __syncwarp();
+            {
+                float *prow = p.partial + ((size_t)(mine ? sIt[my_node] : 0) * p.P + cta) * r;
+#pragma unroll 1
+                for (int blk = 0; blk < 4; ++blk) {
+                    const int col0 = 128 * hsel + 32 * blk;
+                    if (col0 >= r16) break;                          // warp-uniform
+                    float v[32];
+                    tc::tmem_ld32(tmem + tlane + 256 + col0, v);
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) v[c] += __shfl_xor_sync(0xffffffffu, v[c], 16);
+                    if (mine) {
+#pragma unroll
+                        for (int c4 = 0; c4 < 4; ++c4) {
+                            const int col = col0 + 16 * uh + 4 * c4;
+                            // the uh half selects which 16 of the 32 columns this lane stores
+                            const float4 o = uh ? make_float4(v[16 + 4 * c4], v[17 + 4 * c4], v[18 + 4 * c4], v[19 + 4 * c4])
+                                                : make_float4(v[4 * c4], v[4 * c4 + 1], v[4 * c4 + 2], v[4 * c4 + 3]);
+                            if (col + 3 < r) __stcg(reinterpret_cast<float4 *>(prow + col), o);
+                        }
+                    }
+                }
+            }
+            tc::fence_before_sync();
+            __syncthreads();
+        }
+        if (sCtl[2]) break;
+        if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, fbase + (unsigned int)(s + 1)); }
+    }
+    __syncthreads();
+    if (warp == 0) tc::tmem_free<kWvTmemCols>(tmem);
+    // every CTA of the grid has read the counter: a request is done only after all GRU CTAs finished step 0
+    if (cta == 0 && tid == 0) st_relaxed_u32(p.round_ctr, rnd + 1u);
+}
+
+// -------------------------------------------------------------------------------------- request role
+struct WaveCtl {
+    int n_exp;          // expansions allocated so far (expansion 0 = the root)
+    int c;              // committed pops: slots 1 .. c are final
+    int n_items;        // items published for the coming step
+    int done, n_valid, n_stage, abort_, pad;
+    int slDepth[kWvMaxSlices];      // depth whose candidate rows a slice holds (-1 = empty)
+    int slUsed[kWvMaxSlices];       // last step that needs the slice
+    int stage[kWvMaxSlices];        // slices to fill before the coming step
+    signed char d2s[DT_MAX_L];      // depth -> slice (-1 = not resident)
+};
+
+__device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char *smem_raw) {
+    const ExpandParams &e = p.e;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int b = blockIdx.x - p.n_gru;
+    const int r = e.r, M = e.M, k = e.k, N = e.N, L = e.L, B = e.B;
+    const int W = p.W, nsl = p.n_slices, e_max = p.e_max, P = p.P;
+    const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 10;
+    const size_t slice_bytes = wave_slice_bytes(r, M);
+    const int Ka = (r + 63) / 64, nvec = r / 8;
+
+    size_t off = 0;
+    auto carve = [&](size_t bytes) { unsigned char *q = smem_raw + off; off += (bytes + 15) / 16 * 16; return q; };
+    unsigned char *sW2 = carve((size_t)nsl * slice_bytes);
+    int *slTok = reinterpret_cast<int *>(carve((size_t)nsl * M * 4));
+    float *slBase = reinterpret_cast<float *>(carve((size_t)nsl * M * 4));
+    unsigned long long *cKey = reinterpret_cast<unsigned long long *>(carve((size_t)e_max * k * 8));   // children of expansion x, best first
+    short *cExp = reinterpret_cast<short *>(carve((size_t)e_max * k * 2));                             // expansion of that child, -1 = none
+    int *eTok = reinterpret_cast<int *>(carve((size_t)e_max * 4));
+    int *ePar = reinterpret_cast<int *>(carve((size_t)e_max * 4));
+    int *eDep = reinterpret_cast<int *>(carve((size_t)e_max * 4));
+    float *eSco = reinterpret_cast<float *>(carve((size_t)e_max * 4));
+    unsigned int *simC = reinterpret_cast<unsigned int *>(carve((size_t)e_max * 4));   // replay state at the commit point
+    unsigned int *simT = reinterpret_cast<unsigned int *>(carve((size_t)e_max * 4));   // ... of the running replay
+    int *nTok = reinterpret_cast<int *>(carve((size_t)N * 4));
+    int *nPar = reinterpret_cast<int *>(carve((size_t)N * 4));
+    int *nDep = reinterpret_cast<int *>(carve((size_t)N * 4));
+    float *nSco = reinterpret_cast<float *>(carve((size_t)N * 4));
+    float *sA = reinterpret_cast<float *>(carve((size_t)W * r * 4));
+    float *sZ = reinterpret_cast<float *>(carve((size_t)W * M * 4));
+    float *sPg = reinterpret_cast<float *>(carve((size_t)8 * r * 4));
+    int *itE = reinterpret_cast<int *>(carve((size_t)4 * kWvMaxW * 4));
+    int *itTok = itE + kWvMaxW, *itPs = itTok + kWvMaxW;
+    WaveCtl &ctl = *reinterpret_cast<WaveCtl *>(carve(256));
+
+    const __nv_bfloat16 *w2 = reinterpret_cast<const __nv_bfloat16 *>(e.w2);
+    unsigned long long *my_desc = p.desc + (size_t)b * kWvDescWords;
+
+    // fill the slices listed in ctl.stage with the candidate table of their depth: ids, base logits, the M rows of W2
+    auto stage_slices = [&]() {
+        const int ns = ctl.n_stage;
+        for (int q = 0; q < ns; ++q) {
+            const int si = ctl.stage[q];
+            const size_t row = (size_t)b * L + ctl.slDepth[si];
+            for (int m = tid; m < M; m += kWvThreads) {
+                slTok[si * M + m] = e.cand_id[row * M + m];
+                slBase[si * M + m] = e.cand_val[row * M + m];
+            }
+        }
+        __syncthreads();
+        for (int q = 0; q < ns; ++q) {
+            const int si = ctl.stage[q];
+            unsigned char *dst = sW2 + (size_t)si * slice_bytes;
+            for (int i = tid; i < M * nvec; i += kWvThreads) {
+                const int m = i / nvec, v = i - m * nvec;
+                cp_async16(dst + (size_t)(m >> 3) * Ka * 1024 + (size_t)(v >> 3) * 1024 + (m & 7) * 128 + (((v & 7) ^ (m & 7)) << 4),
+                           w2 + (size_t)slTok[si * M + m] * r + (size_t)v * 8);
+            }
+        }
+        cp_async_commit();
+    };
+
+    if (tid == 0) {
+        const int root = e.root_tokens[b];
+        ctl.n_exp = 1; ctl.c = 0; ctl.n_items = 1; ctl.done = 0; ctl.n_valid = 1; ctl.abort_ = 0;
+        for (int i = 0; i < kWvMaxSlices; ++i) { ctl.slDepth[i] = -1; ctl.slUsed[i] = -1; }
+        for (int i = 0; i < DT_MAX_L; ++i) ctl.d2s[i] = -1;
+        ctl.slDepth[0] = 0; ctl.slUsed[0] = 0; ctl.d2s[0] = 0; ctl.stage[0] = 0; ctl.n_stage = 1;
+        eTok[0] = root; ePar[0] = -1; eDep[0] = 0; eSco[0] = 0.f; simC[0] = 0u; simT[0] = 0u;
+        nTok[0] = root; nPar[0] = -1; nDep[0] = 0; nSco[0] = 0.f;
+        itE[0] = 0;
+        // step 0: the root, whose parent state is the zero slot (reading A4)
+        st_relaxed_u64(my_desc + 1, wave_item_pack(rnd, 1, 0, min(max(root, 0), e.V - 1)));
+        st_relaxed_u64(my_desc, wave_hdr_pack(rnd, 1, 1, 0, 1));
+    }
+    __syncthreads();
+    stage_slices();
+    if (tid == 0) ctl.n_stage = 0;                               // every thread read the list before the barrier inside
+
+    for (int s = 0;; ++s) {
+        const int n_it = ctl.n_items;
+        if (warp == 0) {
+            bool ok = true;
+            for (int q = lane; q < p.n_gru; q += 32) {
+                const unsigned int *fp = p.flags + (size_t)q * kFusFlagStride;
+                ok = wave_spin([&] { return (int)(ld_relaxed_u32(fp) - (fbase + (unsigned int)(s + 1))) >= 0; }, p.err) && ok;
+            }
+            if (!ok) ctl.abort_ = 1;
+        }
+        __syncthreads();
+        if (ctl.abort_) break;
+
+        // ---- a_j = SiLU(C + W1[:, d:] S_j): the P split-K partials are summed in a fixed order (batch-invariant)
+        for (int j = 0; j < n_it; ++j) {
+            const int x = itE[j];
+            const size_t row = (size_t)b * L + eDep[x];             // H_{depth+1} <-> row index depth (A12)
+            const int r4 = r >> 2;
+            const int G = min(8, kWvThreads / r4);
+            const int per = (P + G - 1) / G;
+            const int jq = tid % r4, qg = tid / r4;
+            if (qg < G) {
+                const float4 *pp = reinterpret_cast<const float4 *>(p.partial + ((size_t)(b * kWvMaxW + j) * P) * r) + jq;
+                const int q0 = qg * per, q1 = min(P, q0 + per);
+                float4 s0 = make_float4(0.f, 0.f, 0.f, 0.f), s1 = s0;
+                int q = q0;
+                for (; q + 8 <= q1; q += 8) {
+                    float4 v[8];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) v[i] = __ldcg(pp + (size_t)(q + i) * r4);
+#pragma unroll
+                    for (int i = 0; i < 8; i += 2) {
+                        s0.x += v[i].x; s0.y += v[i].y; s0.z += v[i].z; s0.w += v[i].w;
+                        s1.x += v[i + 1].x; s1.y += v[i + 1].y; s1.z += v[i + 1].z; s1.w += v[i + 1].w;
+                    }
+                }
+                for (; q < q1; ++q) {
+                    const float4 v = __ldcg(pp + (size_t)q * r4);
+                    s0.x += v.x; s0.y += v.y; s0.z += v.z; s0.w += v.w;
+                }
+                *reinterpret_cast<float4 *>(sPg + (size_t)qg * r + 4 * jq) = make_float4(s0.x + s1.x, s0.y + s1.y, s0.z + s1.z, s0.w + s1.w);
+            }
+            __syncthreads();
+            for (int jj = tid; jj < r; jj += kWvThreads) {
+                float acc = sPg[jj];
+                for (int gq = 1; gq < G; ++gq) acc += sPg[(size_t)gq * r + jj];
+                const float xx = e.C[row * r + jj] + acc;
+                sA[(size_t)j * r + jj] = xx * sigmoidf_acc(xx);
+            }
+            __syncthreads();
+        }
+        cp_async_wait<0>();
+        __syncthreads();
+
+        // ---- z_m = ((base_m - base_0) + W2[cand_m, :] a) / T_eff   PAPER.md:143-144 (shift-invariant)
+        // a warp takes 8 candidate rows (one swizzle row group), four lanes per row
+        for (int j = 0; j < n_it; ++j) {
+            const int si = ctl.d2s[eDep[itE[j]]];
+            const unsigned char *sl = sW2 + (size_t)si * slice_bytes;
+            const float *bs = slBase + si * M;
+            const float base0 = bs[0];
+            const float *aj = sA + (size_t)j * r;
+            const int rw = lane & 7, qq = lane >> 3;
+            for (int rg = warp; rg < (M + 7) / 8; rg += kWvThreads / 32) {
+                const unsigned char *rowp = sl + (size_t)rg * Ka * 1024 + rw * 128;
+                float acc = 0.f;
+                for (int v = qq; v < nvec; v += 4) {
+                    const uint4 q = *reinterpret_cast<const uint4 *>(rowp + (size_t)(v >> 3) * 1024 + (((v & 7) ^ rw) << 4));
+                    const float4 a0 = *reinterpret_cast<const float4 *>(aj + (size_t)v * 8);
+                    const float4 a1 = *reinterpret_cast<const float4 *>(aj + (size_t)v * 8 + 4);
+                    float f[8];
+                    unpack8(q, f);
+                    acc = fmaf(f[0], a0.x, acc); acc = fmaf(f[1], a0.y, acc); acc = fmaf(f[2], a0.z, acc); acc = fmaf(f[3], a0.w, acc);
+                    acc = fmaf(f[4], a1.x, acc); acc = fmaf(f[5], a1.y, acc); acc = fmaf(f[6], a1.z, acc); acc = fmaf(f[7], a1.w, acc);
+                }
+                acc += __shfl_xor_sync(0xffffffffu, acc, 8);
+                acc += __shfl_xor_sync(0xffffffffu, acc, 16);
+                const int m = 8 * rg + rw;
+                if (qq == 0 && m < M) sZ[(size_t)j * M + m] = __fdiv_rn((bs[m] - base0) + acc, e.T_eff);
+            }
+        }
+        __syncthreads();
+
+        // ---- slice log-softmax (reading A1) and top-k by (logp desc, token asc): one warp per node
+        for (int j = warp; j < n_it; j += kWvThreads / 32) {
+            const int x = itE[j];
+            const int si = ctl.d2s[eDep[x]];
+            const float *zj = sZ + (size_t)j * M;
+            const int *tk = slTok + si * M;
+            float zmax = -INFINITY;
+            for (int m = lane; m < M; m += 32) zmax = fmaxf(zmax, zj[m]);
+            zmax = warp_max(zmax);
+            float ssum = 0.f;
+            for (int m = lane; m < M; m += 32) ssum += expf(zj[m] - zmax);
+            ssum = warp_sum(ssum);
+            const float lse = logf(ssum);
+            const float gpar = eSco[x];
+            unsigned long long *ck = cKey + (size_t)x * k;
+            for (int m = lane; m < M; m += 32) {
+                const float mz = zj[m];
+                const int mtok = tk[m];
+                int rank = 0;
+                for (int q = 0; q < M; ++q) {
+                    const float oz = zj[q];
+                    rank += (oz > mz) || (oz == mz && tk[q] < mtok);
+                }
+                if (rank < k) {
+                    const float lpm = (mz - zmax) - lse;
+                    ck[rank] = ((unsigned long long)ord_key(gpar + lpm) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned int)mtok);
+                }
+            }
+            __syncwarp();
+            // the list is kept sorted by the pop comparator itself (fp32 rounding of g + logp may merge two scores)
+            unsigned long long mk = 0ull;
+            int rk = 0;
+            if (lane < k) {
+                mk = ck[lane];
+                for (int q = 0; q < k; ++q) rk += (ck[q] > mk);
+            }
+            __syncwarp();
+            if (lane < k) { ck[rk] = mk; cExp[(size_t)x * k + lane] = -1; }
+        }
+        __syncthreads();
+
+        // ---- replay the heap from the commit point, nominate, publish (warp 0)
+        if (warp == 0) {
+            const int n_exp = ctl.n_exp;
+            int t = ctl.c;
+            if (s == 0 && lane == 0) { simC[0] = kWvAct; }          // the root is slot 0; its children are known now
+            __syncwarp();
+            for (int x = lane; x < n_exp; x += 32) simT[x] = simC[x];
+            __syncwarp();
+            bool committing = true, finished = false;
+            int found = 0;
+            const int step_next = s + 1;
+            while (true) {
+                if (t >= B) { finished = committing; break; }
+                unsigned long long bk = 0ull;
+                unsigned int bps = 0xFFFFFFFFu;
+                int be = -1;
+                for (int x = lane; x < n_exp; x += 32) {
+                    const unsigned int w = simT[x];
+                    const int cur = (int)(w & 0xFFu);
+                    if (!(w & kWvAct) || cur >= k) continue;
+                    const unsigned long long key = cKey[(size_t)x * k + cur];
+                    const unsigned int ps = w >> 16;
+                    if (be < 0 || key > bk || (key == bk && ps < bps)) { bk = key; bps = ps; be = x; }
+                }
+                if (__ballot_sync(0xffffffffu, be >= 0) == 0u) { finished = committing; break; }   // the candidate tree ran dry
+                // pop comparator of reading A8: score desc, token asc, parent slot asc
+                const unsigned int hi = (be >= 0) ? (unsigned int)(bk >> 32) : 0u;
+                const unsigned int mh = __reduce_max_sync(0xffffffffu, hi);
+                bool el = (be >= 0) && hi == mh;
+                const unsigned int lo = el ? (unsigned int)(bk & 0xFFFFFFFFull) : 0u;
+                const unsigned int ml = __reduce_max_sync(0xffffffffu, lo);
+                el = el && lo == ml;
+                const unsigned int mp = __reduce_min_sync(0xffffffffu, el ? bps : 0xFFFFFFFFu);
+                el = el && bps == mp;
+                const int wl = __ffs(__ballot_sync(0xffffffffu, el)) - 1;
+                const int es = __shfl_sync(0xffffffffu, be, wl);
+                const unsigned int wv = simT[es];
+                const int jc = (int)(wv & 0xFFu);
+                const int tok = (int)(0xFFFFFFFFu - ml);
+                const int dep = eDep[es] + 1;
+                const int x = cExp[(size_t)es * k + jc];
+                const bool needs = (x < 0) && dep < L && (t + 1 < B);
+                if (committing && needs) {                          // everything before this pop is final
+                    for (int y = lane; y < n_exp; y += 32) simC[y] = simT[y];
+                    if (lane == 0) ctl.c = t;
+                    committing = false;
+                    __syncwarp();
+                }
+                t += 1;
+                if (lane == 0) {
+                    simT[es] = wv + 1u;
+                    nTok[t] = tok; nPar[t] = (int)(wv >> 16); nDep[t] = dep; nSco[t] = ord_key_inv(mh);
+                    if (x >= 0) simT[x] = kWvAct | ((unsigned int)t << 16);
+                }
+                if (needs && found < W) {                           // warp-uniform; lane 0 decides, the count is broadcast
+                    // resources: a state slot (speculative picks leave room for the expansions Algorithm 1 still needs)
+                    // and a W2 slice for the node's depth
+                    int add = 0;
+                    if (lane == 0) {
+                        const int xn = n_exp + found;
+                        bool can = (xn < e_max) && (found == 0 || xn + 1 + (B - ctl.c) <= e_max);
+                        int si = -1;
+                        if (can) {
+                            si = ctl.d2s[dep];
+                            if (si < 0) {
+                                int best = -1, bu = 0x7FFFFFFF;
+                                for (int q = 0; q < nsl; ++q)
+                                    if (ctl.slUsed[q] != step_next && ctl.slUsed[q] < bu) { bu = ctl.slUsed[q]; best = q; }
+                                si = best;
+                                if (si >= 0) {
+                                    if (ctl.slDepth[si] >= 0) ctl.d2s[ctl.slDepth[si]] = -1;
+                                    ctl.slDepth[si] = dep; ctl.d2s[dep] = (signed char)si;
+                                    ctl.stage[ctl.n_stage] = si; ctl.n_stage += 1;
+                                }
+                            }
+                            can = (si >= 0);
+                        }
+                        if (can) {
+                            ctl.slUsed[si] = step_next;
+                            cExp[(size_t)es * k + jc] = (short)xn;
+                            eTok[xn] = tok; ePar[xn] = es; eDep[xn] = dep; eSco[xn] = ord_key_inv(mh);
+                            simC[xn] = 0u; simT[xn] = 0u;
+                            itE[found] = xn; itTok[found] = tok; itPs[found] = es + 1;
+                            add = 1;
+                        }
+                    }
+                    found += __shfl_sync(0xffffffffu, add, 0);
+                }
+                __syncwarp();
+                if (!committing && found >= W) break;
+            }
+            if (finished) {
+                if (lane == 0) {
+                    ctl.done = 1; ctl.n_valid = t + 1; ctl.n_items = 0;
+                    st_relaxed_u64(my_desc, wave_hdr_pack(rnd, s + 2, 0, 1, 0));
+                    if (p.stats && b == 0) { p.stats[0] = (unsigned int)(s + 1); p.stats[1] = (unsigned int)n_exp; }
+                }
+            } else {
+                if (lane < found) st_relaxed_u64(my_desc + 1 + lane, wave_item_pack(rnd, s + 2, itPs[lane], min(max(itTok[lane], 0), e.V - 1)));
+                if (lane == 0) {
+                    st_relaxed_u64(my_desc, wave_hdr_pack(rnd, s + 2, n_exp + 1, 0, found));
+                    ctl.n_items = found; ctl.n_exp = n_exp + found;
+                }
+            }
+        }
+        __syncthreads();
+        if (ctl.done) break;
+        stage_slices();
+        if (tid == 0) ctl.n_stage = 0;
+    }
+    __syncthreads();
+
+    // emitter (a9): dead-leaf padding (reading A10), positions, ancestor-or-self mask
+    const int n = ctl.abort_ ? 1 : ctl.n_valid;
+    const int rpos = e.root_positions ? e.root_positions[b] : 0;
+    for (int i = tid; i < N; i += kWvThreads) {
+        const size_t so = (size_t)b * N + i;
+        const bool dead = (i >= n);
+        const int dep = dead ? 1 : nDep[i];
+        e.tokens[so] = dead ? 0 : nTok[i];
+        e.parents[so] = dead ? 0 : nPar[i];
+        e.depths[so] = dep;
+        e.scores[so] = dead ? -INFINITY : nSco[i];
+        e.positions[so] = rpos + dep;
+        if (dead) nPar[i] = 0;
+    }
+    if (tid == 0) e.n_nodes[b] = n;
+    uint8_t *mk = e.mask + (size_t)b * N * N;
+    for (int i = tid; i < N * N; i += kWvThreads) mk[i] = 0;
+    __syncthreads();
+    for (int i = tid; i < N; i += kWvThreads) {
+        int a = i;
+        while (a >= 0) { mk[(size_t)i * N + a] = 1; a = nPar[a]; }
+    }
+}
+
+__global__ void __launch_bounds__(kWvThreads, 1) wave_expand_kernel(WaveParams p) {
+    extern __shared__ __align__(1024) unsigned char wave_smem[];
+    if ((int)blockIdx.x < p.n_gru) wave_gru_role(p, wave_smem);
+    else wave_req_role(p, wave_smem);
+}
+
+}  // namespace dt
