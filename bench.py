@@ -458,6 +458,74 @@ def measure_sweep_and_arms(ctx):
            {"us_per_round_batch1_B16_M64": arms}
 
 
+
+# ----------------------------------------------------------------------------------- in-kernel timeline
+GRU_STAMPS = ("headers seen", "item list built", "ring + P loads issued", "D1 in TMEM", "gates + states stored",
+              "D2 in TMEM", "partials stored", "flag released")
+REQ_STAMPS = ("flags seen", "a = SiLU(C + partials)", "W2 slice dots", "softmax + top-k", "replay + publish",
+              "slices staged (issue)")
+
+
+def run_trace(args):
+    """--trace: the measurement build libdominotree_trace.so (-DDT_TRACE) stamps %globaltimer inside the wavefront
+    kernel (GRU CTA 0, request CTA 0); prints the median time between consecutive stamps per regime as one JSON line.
+    Never a bench value: the stamps perturb the kernel slightly."""
+    import ctypes
+    import numpy as np
+    import torch
+    import paper_2607_08642_b200 as dtb
+    from paper_2607_08642_b200 import build as dtbuild
+    from paper_2607_08642_b200 import workloads as wl
+    lib_path = dtbuild.build(trace=True)
+    cfg = wl.CONFIGS[args.workload]
+    batch = args.trace_batch or cfg.batch
+    w_gpu = {n: t.cuda() for n, t in wl.make_weights(cfg).items()}
+    builder = dtb.DominoTreeBuilder(w_gpu, max_batch=batch, L=cfg.L, max_M=cfg.M, max_B=cfg.B, k=cfg.k, lib_path=lib_path)
+    if args.wave_width:
+        builder.set_option("wave_width", args.wave_width)
+    lib = builder.lib
+    lib.dt_trace_read.argtypes = [ctypes.c_void_p]
+    lib.dt_trace_read.restype = ctypes.c_int
+    S, K = 64, 16
+    buf = np.zeros((2, S, K), dtype=np.uint64)
+    out = {"workload": cfg.name, "batch": batch, "wave_width": args.wave_width or "auto", "unit": "ns (median over steps)"}
+    for regime in ("flat", "peaked"):
+        inp = wl.make_inputs(cfg, batch=batch, regime=regime)
+        dev = {k_: inp[k_].cuda() for k_ in ("logits", "hidden", "root_tokens", "root_positions")}
+        o = dtb.alloc_outputs(batch, cfg.B)
+        for _ in range(3):
+            builder.build_trees(dev["logits"], dev["hidden"], dev["root_tokens"], dev["root_positions"], cfg.M, cfg.B, cfg.T, out=o)
+        torch.cuda.synchronize()
+        assert lib.dt_trace_read(buf.ctypes.data) == 0
+        builder.build_trees(dev["logits"], dev["hidden"], dev["root_tokens"], dev["root_positions"], cfg.M, cfg.B, cfg.T, out=o)
+        torch.cuda.synchronize()
+        assert lib.dt_trace_read(buf.ctypes.data) == 0
+        t = buf.astype(np.int64)
+        steps = int((t[0, :, 0] > 0).sum())
+        rows = {}
+        g = t[0, 1:max(steps - 1, 2)]          # skip step 0 (weight load) and the last
+        q = t[1, 1:max(steps - 1, 2)]
+        for i in range(1, len(GRU_STAMPS)):
+            d = g[:, i] - g[:, i - 1]
+            rows["gru: " + GRU_STAMPS[i]] = float(np.median(d[(g[:, i] > 0) & (g[:, i - 1] > 0)])) if len(d) else None
+        for i in range(1, len(REQ_STAMPS)):
+            d = q[:, i] - q[:, i - 1]
+            ok = (q[:, i] > 0) & (q[:, i - 1] > 0)
+            rows["req: " + REQ_STAMPS[i]] = float(np.median(d[ok])) if ok.any() else None
+        ok = (q[:, 0] > 0) & (g[:, 7] > 0)
+        rows["hop: flag released -> request sees flags"] = float(np.median((q[:, 0] - g[:, 7])[ok])) if ok.any() else None
+        gn = t[0, 2:max(steps, 3)]
+        ok = (gn[:, 0] > 0) & (q[:len(gn), 4] > 0)
+        rows["hop: request published -> GRU sees headers"] = float(np.median((gn[:, 0] - q[:len(gn), 4])[ok])) if ok.any() else None
+        period = np.diff(t[0, 1:steps, 0])
+        rows["step period"] = float(np.median(period)) if len(period) else None
+        rows["steps"] = steps
+        rows["expansions_request0"] = builder.get_option("wave_expansions")
+        out[regime] = rows
+    print(json.dumps({"trace": out}), flush=True)
+    builder.close()
+
+
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--gpus", type=int, default=1)
@@ -468,11 +536,16 @@ def main():
     ap.add_argument("--rotate", type=int, default=4, help="distinct input sets rotated through the timed region")
     ap.add_argument("--no-extras", action="store_true", help="skip the e2e / cpu_baseline / batch-1 legs")
     ap.add_argument("--sweep", action="store_true", help="also time the batch-1 B x M sweep and the three scorer arms")
+    ap.add_argument("--trace", action="store_true", help="in-kernel timeline of the wavefront kernel (measurement build, not a bench value)")
+    ap.add_argument("--trace-batch", type=int, default=0, help="batch of the --trace leg (default: the workload's)")
+    ap.add_argument("--wave-width", type=int, default=0, help="nodes a request may expand per step (0 = auto)")
     args = ap.parse_args()
     if args.impl == "reference":
         if args.steps == 200 and args.warmup == 20:      # defaults: keep the CPU run within minutes
             args.steps, args.warmup = 10, 3
         return run_reference(args)
+    if args.trace:
+        return run_trace(args)
 
     ctx = run_ours(args)
     cfg, peaks, world, rank = ctx["cfg"], ctx["peaks"], ctx["world"], ctx["rank"]

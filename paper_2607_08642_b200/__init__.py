@@ -133,9 +133,10 @@ class DominoTreeBuilder:
     gru_w_hh, corr_w1, corr_w2 to contiguous CUDA tensors of one dtype (bf16 or fp32); they are
     borrowed for the lifetime of the builder."""
 
-    def __init__(self, weights: Dict[str, "object"], max_batch: int, L: int, max_M: int, max_B: int, k: int = 8):
+    def __init__(self, weights: Dict[str, "object"], max_batch: int, L: int, max_M: int, max_B: int, k: int = 8,
+                 lib_path: Optional[str] = None):
         import torch
-        self.lib = load_library()
+        self.lib = load_library(lib_path)
         self._h = ctypes.c_void_p()
         ws = [weights[n] for n in ("embed", "gru_w_ih", "gru_w_hh", "corr_w1", "corr_w2")]
         for t in ws:

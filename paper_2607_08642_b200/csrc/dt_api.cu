@@ -45,6 +45,7 @@ struct dt_handle {
     // wavefront expansion (dt_wave.cuh): per-item partials, multi-item descriptors, device error word, counters
     float *wv_partial; unsigned long long *wv_desc; unsigned int *wv_err, *wv_stats; int wave_ok, slot_stride;
     int64_t opt_wave_width;         // items per request per step (0 = auto)
+    int wave_clusters;              // co-resident clusters of kWvCS CTAs (0 = not queried yet, -1 = unavailable)
     int path_taken;                 // expansion path of the last dt_build_trees: 1 per-step, 2/3 fused mma.sync, 4 fused tcgen05, 5 wavefront
     int64_t opt_expand_path;        // 0 auto, 1 per-step kernels, 2 fused mma.sync upc=8, 3 fused mma.sync upc=16, 4 fused tcgen05
     // host-call staging (lazy)
@@ -516,12 +517,25 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
 static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st) {
     if (!h->fused_ok || !h->wave_ok || (h->opt_expand_path != 0 && h->opt_expand_path != 5)) return 1;
     if (p.g % kWvKC || p.g / 16 > 256 || p.r % 8 || p.r > 256 || p.k > 32 || p.M > 256 || p.L > DT_MAX_L) return 1;
-    const int n_gru = p.g / 16;
-    int cap = h->num_sms - n_gru;
-    if (cap > kWvMaxBatch) cap = kWvMaxBatch;
-    if (cap < 1) return 1;
+    const int n_gru = p.g / 16;                          // a multiple of kWvCS (g is a multiple of 128)
     const size_t gs = wave_gru_smem(p.g, p.r);
     if (gs > (size_t)h->max_smem_optin) return 1;
+    // co-resident clusters of kWvCS CTAs at one CTA per SM (queried once per handle)
+    if (h->wave_clusters == 0) {
+        cudaLaunchConfig_t qc;
+        memset(&qc, 0, sizeof(qc));
+        qc.gridDim = dim3(h->num_sms / kWvCS * kWvCS); qc.blockDim = dim3(kWvThreads); qc.dynamicSmemBytes = (size_t)h->max_smem_optin;
+        cudaLaunchAttribute qa[1];
+        qa[0].id = cudaLaunchAttributeClusterDimension; qa[0].val.clusterDim.x = kWvCS; qa[0].val.clusterDim.y = 1; qa[0].val.clusterDim.z = 1;
+        qc.attrs = qa; qc.numAttrs = 1;
+        int nc = 0;
+        if (cudaOccupancyMaxActiveClusters(&nc, (const void *)wave_expand_kernel, &qc) != cudaSuccess) { cudaGetLastError(); nc = -1; }
+        h->wave_clusters = nc > 0 ? nc : -1;
+    }
+    if (h->wave_clusters < 0) return 1;
+    int cap = (h->wave_clusters - n_gru / kWvCS) * kWvCS;
+    if (cap > kWvMaxBatch) cap = kWvMaxBatch;
+    if (cap < 1) return 1;
     int W = (int)h->opt_wave_width;
     if (W <= 0) { W = 96 / (p.batch < cap ? p.batch : cap); }
     if (W < 1) W = 1;
@@ -550,15 +564,22 @@ static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st) {
         f.e.positions = p.positions + (size_t)b0 * p.N; f.e.scores = p.scores + (size_t)b0 * p.N;
         f.e.mask = p.mask + (size_t)b0 * p.N * p.N; f.e.n_nodes = p.n_nodes + b0;
         f.e.root_tokens = p.root_tokens + b0; f.e.root_positions = p.root_positions ? p.root_positions + b0 : nullptr;
-        f.n_gru = n_gru; f.slot_stride = h->slot_stride; f.W = W; f.n_slices = nsl; f.e_max = e_max; f.P = n_gru;
+        f.n_gru = n_gru; f.slot_stride = h->slot_stride; f.W = W; f.n_slices = nsl; f.e_max = e_max;
+        f.P = n_gru / kWvCS; f.rpc = 16 * ((p.r + 16 * kWvCS - 1) / (16 * kWvCS));
         const size_t so = (size_t)b0 * h->slot_stride * p.g;
         f.s_hi = h->s_hi + so; f.s_lo = h->s_lo + so; f.s32 = h->states + so;
-        f.partial = h->wv_partial + (size_t)b0 * kWvMaxW * n_gru * p.r;
+        f.partial = h->wv_partial + (size_t)b0 * kWvMaxW * f.P * p.r;
         f.desc = h->wv_desc + (size_t)b0 * kWvDescWords;
         f.flags = h->flags; f.round_ctr = h->round_ctr; f.err = h->wv_err; f.stats = (b0 == 0) ? h->wv_stats : nullptr;
-        void *args[] = {&f};
-        const dim3 grid(n_gru + nb), block(kWvThreads);
-        cudaError_t e = cudaLaunchCooperativeKernel((const void *)wave_expand_kernel, grid, block, args, dsm, st);
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = dim3(n_gru + (nb + kWvCS - 1) / kWvCS * kWvCS); cfg.blockDim = dim3(kWvThreads);
+        cfg.dynamicSmemBytes = dsm; cfg.stream = st;
+        cudaLaunchAttribute at[2];
+        at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = kWvCS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        at[1].id = cudaLaunchAttributeCooperative; at[1].val.cooperative = 1;
+        cfg.attrs = at; cfg.numAttrs = 2;
+        cudaError_t e = cudaLaunchKernelEx(&cfg, wave_expand_kernel, f);
         h->launches++;
         DT_CUDA(h, e);
     }
@@ -801,8 +822,14 @@ extern "C" int dt_build_trees_host(dt_handle *h, const void *logits_h, const voi
 }
 
 #ifdef DT_TRACE
-// measurement builds only (-DDT_TRACE): copy the in-kernel timeline of the last fused round to `host` (2*256*8 u64)
+// measurement builds only (libdominotree_trace.so, -DDT_TRACE): copy the in-kernel timeline of the last wavefront round
+// to `host` (2 roles x kWvTraceSteps x kWvTraceStamps u64 of %globaltimer, zero = not reached) and clear it
 extern "C" int dt_trace_read(unsigned long long *host) {
-    return cudaMemcpyFromSymbol(host, dt::g_dt_trace, sizeof(unsigned long long) * 2 * 256 * 8) == cudaSuccess ? 0 : -3;
+    const size_t n = sizeof(unsigned long long) * 2 * dt::kWvTraceSteps * dt::kWvTraceStamps;
+    if (cudaDeviceSynchronize() != cudaSuccess) return DT_ERR_CUDA;
+    if (cudaMemcpyFromSymbol(host, dt::g_wv_trace, n) != cudaSuccess) return DT_ERR_CUDA;
+    void *sym = nullptr;
+    if (cudaGetSymbolAddress(&sym, dt::g_wv_trace) != cudaSuccess || cudaMemset(sym, 0, n) != cudaSuccess) return DT_ERR_CUDA;
+    return DT_OK;
 }
 #endif

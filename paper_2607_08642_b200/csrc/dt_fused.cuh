@@ -68,21 +68,6 @@ struct FusedParams {
     float *menu_lp;                // [batch, L, k]
 };
 
-// Optional in-kernel timeline (compile with -DDT_TRACE; measurement builds only, never the product build):
-// thread 0 of GRU CTA 0 (role 0) and of request CTA 0 (role 1) stamp %globaltimer at fixed points of every step.
-#ifdef DT_TRACE
-__device__ unsigned long long g_dt_trace[2][256][8];
-__device__ __forceinline__ unsigned long long dt_globaltimer() {
-    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
-}
-#define DT_TR(role, first_cta, t, i) do { if (threadIdx.x == 0 && (int)blockIdx.x == (first_cta)) g_dt_trace[role][t][i] = dt_globaltimer(); } while (0)
-// fine-grained stamps of GRU CTA 0 at step 5: rows 200.. of role 0
-#define DT_TRF(t, i) do { if (threadIdx.x == 0 && blockIdx.x == 0 && (t) == 5) g_dt_trace[0][200 + (i) / 8][(i) % 8] = dt_globaltimer(); } while (0)
-#else
-#define DT_TRF(t, i) do { } while (0)
-#define DT_TR(role, first_cta, t, i) do { } while (0)
-#endif
-
 // ---- hand-over words -------------------------------------------------------------------------------
 // Both directions use one self-describing word per producer (no shared counter, so no serialised
 // atomics).  GRU -> request: the GRU CTA's threads store states / partials, a CTA barrier, then thread 0
@@ -212,7 +197,6 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
                 sIdx[lane] = sidx; sTok[lane] = tok;
             }
             __syncthreads();
-            if (c0 == 0) DT_TR(0, 0, t, 0);
 
             // stream this warp's k-blocks of the parents' states (bf16 hi | lo) into its ring
             auto issue_block = [&](int blk) {
@@ -303,7 +287,6 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
             }
             cp_async_wait<0>();
             __syncthreads();                                    // every warp is done with its ring: reuse it as sRed
-            if (c0 == 0) DT_TR(0, 0, t, 1);
             {
                 float *red = sRed + (size_t)warp * MT * 16 * kFusRedLd;
 #pragma unroll
@@ -316,7 +299,6 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
                     }
             }
             __syncthreads();
-            if (c0 == 0) DT_TR(0, 0, t, 2);
             // gates (reading A2): r, z, n rows of unit ul are local rows ul, UPC + ul, 2 UPC + ul
 #pragma unroll
             for (int i = 0; i < PP; ++i) {
@@ -348,7 +330,6 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
                 sNewL[bl * 16 + ul] = lo;
             }
             __syncthreads();
-            if (c0 == 0) DT_TR(0, 0, t, 3);
             // this CTA's split-K share of W1[:, d:] S_t on the tensor cores:
             // [r x 16] (bf16 weights, exact) x [16 x 32] (new states, bf16 hi + lo)
             for (int mt = warp; mt < (r + 15) / 16; mt += kFusWarps) {
@@ -375,9 +356,7 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
             }
             __syncthreads();
         }
-        DT_TR(0, 0, t, 4);
         if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, fbase + (unsigned int)(t + 1)); }
-        DT_TR(0, 0, t, 5);
     }
     if (cta == 0 && tid == 0) st_relaxed_u32(p.round_ctr, rnd + 1u);      // every CTA read it long ago
 }
@@ -493,13 +472,11 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                 sIdx[lane] = sidx; sTok[lane] = tok;
             }
             __syncthreads();
-            if (c0 == 0) DT_TR(0, 0, t, 0);
 
             // source rows of this thread's ring pieces (column n < 32: hi of request n, else lo of request n - 32)
             const int my_sidx = sIdx[my_rq];
             const size_t my_off = (my_sidx > 0) ? ((size_t)(c0 + my_rq) * stride + my_sidx) * g : 0;   // 0 = zero slot
             const __nv_bfloat16 *src_hi = p.s_hi + my_off + (size_t)my_c * 8, *src_lo = p.s_lo + my_off + (size_t)my_c * 8;
-            DT_TRF(t, 40);
             auto issue_chunk = [&](int kc) {
                 if (my_rq >= lo_off) return;                        // columns beyond N: nothing to stream
                 unsigned char *dst = sRing + (size_t)(kc % kTcSlots) * kTcSlotBytes;
@@ -512,7 +489,6 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             };
 #pragma unroll 1
             for (int kc = 0; kc < kTcSlots; ++kc) { if (kc < n_kc) issue_chunk(kc); cp_async_commit(); }
-            DT_TRF(t, 41);
 
             // epilogue operands (input half from P, previous state): issued now, consumed after the MMAs
             float pr[PP], pz[PP], pn[PP], hp[PP];
@@ -521,26 +497,19 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                 const int idx = tid + i * kFusThreads, ul = idx & 15, bl = idx >> 4;   // lanes along the units: 64 B per row
                 const int sidx = sIdx[bl];
                 pr[i] = pz[i] = pn[i] = hp[i] = 0.f;
-#ifndef DT_EXP_NOP
                 if (sidx >= 0) {
                     const float *prow = e.P + (size_t)sTok[bl] * 3 * g + u0 + ul;
                     pr[i] = __ldg(prow); pz[i] = __ldg(prow + g); pn[i] = __ldg(prow + 2 * g);
                     if (sidx > 0) hp[i] = __ldcg(p.s32 + ((size_t)(c0 + bl) * stride + sidx) * g + u0 + ul);
                 }
-#endif
             }
 
-            DT_TRF(t, 42);
             // hidden half: D1[64 x 64] = W_hh slice [64 x g] . [S_hi | S_lo]^T, K streamed through the ring
 #pragma unroll 1
             for (int kc = 0; kc < n_kc; ++kc) {
-                DT_TRF(t, kc * 5 + 0);
                 cp_async_wait<kTcSlots - 1>();
-                DT_TRF(t, kc * 5 + 1);
                 tc::fence_proxy_async();
-                DT_TRF(t, kc * 5 + 2);
                 __syncthreads();
-                DT_TRF(t, kc * 5 + 3);
                 if (warp < kTcIssuers && lane == 0) {
                     // warp w issues k-block w of the slot (A: +1 KB per block, B: +8 KB) as four K = 16 steps (+32 B)
                     // into its own accumulator D1[w]; the epilogue adds the four
@@ -553,7 +522,6 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                     if (kc + kTcSlots < n_kc) tc::commit(mb0 + 8 * (kc & 1));       // this slot is refilled below
                     if (kc == n_kc - 1) tc::commit(mb0 + 16);
                 }
-                DT_TRF(t, kc * 5 + 4);
                 if (kc + kTcSlots < n_kc) {                  // refill the slot once its MMAs have read it
                     tc::mbar_wait(mb0 + 8 * (kc & 1), (ph_free >> (kc & 1)) & 1u);
                     ph_free ^= 1u << (kc & 1);
@@ -562,11 +530,8 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                 cp_async_commit();
             }
             cp_async_wait<0>();
-            DT_TRF(t, 43);
             tc::mbar_wait(mb0 + 16, ph_d1); ph_d1 ^= 1u;
-            DT_TRF(t, 44);
             tc::fence_after_sync();
-            if (c0 == 0) DT_TR(0, 0, t, 1);
             // TMEM -> shared: row m = 16 w + i sits in lane 32 w + i (i < 16) for an M = 64 accumulator
             __syncwarp();
             if (warp < 3) {
@@ -606,7 +571,6 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             }
             tc::fence_before_sync();
             __syncthreads();
-            if (c0 == 0) DT_TR(0, 0, t, 2);
             // gates (reading A2): rows ul, 16 + ul, 32 + ul are the r, z, n pre-activations of unit ul
 #pragma unroll
             for (int i = 0; i < PP; ++i) {
@@ -633,7 +597,6 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             }
             tc::fence_proxy_async();
             __syncthreads();
-            if (c0 == 0) DT_TR(0, 0, t, 3);
             // this CTA's split-K share of W1[:, d:] S_t: D2[r x 64] = W1 slice [r x 16] . [S_hi | S_lo]^T
             if (tid == 0) {
                 tc::fence_after_sync();
@@ -661,12 +624,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             tc::fence_before_sync();
             __syncthreads();
         }
-        DT_TR(0, 0, t, 4);
         if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, fbase + (unsigned int)(t + 1)); }
-#ifdef DT_TRACE
-        if (tid == 0 && t == 5 && cta < 64) g_dt_trace[0][210 + cta / 8][cta % 8] = dt_globaltimer();
-#endif
-        DT_TR(0, 0, t, 5);
     }
     __syncthreads();
     if (warp == 0) tc::tmem_free<kTcCols>(tmem);
@@ -760,7 +718,6 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                 while ((int)(ld_relaxed_u32(p.flags + (size_t)q * kFusFlagStride) - (fbase + (unsigned int)(t + 1))) < 0) { }
         }
         __syncthreads();
-        DT_TR(1, p.n_gru, t, 0);
         // the live frontier is entries 1 .. n_front of buffer `cur` (entry 0 was popped by the previous step)
         const unsigned int *oHi = fHi + cur * kFusMaxFront + 1;
         const unsigned long long *oLo = fLo + cur * kFusMaxFront + 1;
@@ -808,7 +765,6 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             }
             cp_async_wait<0>();
             __syncthreads();
-            DT_TR(1, p.n_gru, t, 1);
             // z_m = ((base_m - base_0) + W2[cand_m, :] a) / T_eff     PAPER.md:143-144 (shift-invariant)
             // four lanes per candidate row, interleaved 16-byte pieces
             const float base0 = sBase[0];
@@ -859,7 +815,6 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                 if (lane == 0) { sWst[2 * warp] = wmx; sWst[2 * warp + 1] = wsm; }
             }
             __syncthreads();
-            DT_TR(1, p.n_gru, t, 2);
             // ... then every thread merges the 8 warps' (max, sum) pairs in warp order
             float zmax = -INFINITY;
 #pragma unroll
@@ -913,7 +868,6 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             }
             n_new = k;
             __syncthreads();
-            DT_TR(1, p.n_gru, t, 3);
         }
         // The node popped now is the better of the old frontier head and the best new entry: thread 0 publishes its
         // descriptor BEFORE the merge, so the GRU CTAs start step t+1 while this CTA is still merging.
@@ -929,9 +883,6 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                 const int par = (int)(0xFFFFFFFFu - (unsigned int)(l & 0xFFFFFFFFull));
                 const int dep = nDep[par] + 1;
                 if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(t + 2, rnd, dep < L ? par + 1 : -1, tok));
-#ifdef DT_TRACE
-                if (t == 5 && b < 64) g_dt_trace[1][200 + b / 8][b % 8] = dt_globaltimer();
-#endif
                 nTok[t + 1] = tok; nPar[t + 1] = par; nDep[t + 1] = dep; nSco[t + 1] = ord_key_inv(h);
                 sm.n_valid = t + 2; sm.n_front = p.static_mode ? 0 : min(tot, cap) - 1; sm.cur = cur ^ 1;
             } else {
@@ -939,7 +890,6 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                 if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(t + 2, rnd, -1, 0));
             }
         }
-        DT_TR(1, p.n_gru, t, 4);
         // merge the new entries into the sorted frontier (other buffer), truncated to the pops that remain
         if (tot > 0) {
             if (tid < n_front) {
@@ -969,7 +919,6 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         int next_dep = L;                                       // depth of the node popped now (L = none / leaf)
         if (tot > 0) next_dep = nDep[t + 1];
         if (t + 1 < B && next_dep < L) stage_depth(next_dep);   // overlaps the GRU CTAs' step t+1
-        DT_TR(1, p.n_gru, t, 5);
     }
     __syncthreads();
 

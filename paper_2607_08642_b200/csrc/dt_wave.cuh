@@ -40,12 +40,12 @@ namespace dt {
 constexpr int kWvThreads = 256;
 constexpr int kWvNP = 64;                       // items per GRU pass (M = 128 operand rows: hi | lo)
 constexpr int kWvKC = 128;                      // k per ring slot (two 64-wide swizzle blocks)
-constexpr int kWvSlots = 3;
-constexpr int kWvSlotBytes = 128 * kWvKC * 2;   // 128 rows x 128 k bf16 = 32 KB
+constexpr int kWvRingBytes = 96 * 1024;         // state ring: three 128-row chunks, or more slots of fewer rows
+constexpr int kWvCS = 4;                        // GRU CTAs per thread-block cluster
 constexpr int kWvDescWords = 16;                // u64 words per request descriptor: header + 15 items, one 128-byte line
 constexpr int kWvMaxW = kWvDescWords - 1;
 constexpr int kWvMaxBatch = 128;                // requests per launch (headers are polled by four warps)
-constexpr int kWvTmemCols = 512;                // D1[w] at 64 w (48 columns each, w < 4), D2 at 256 (r <= 256 columns)
+constexpr int kWvTmemCols = 512;                // D1[w] at 64 w (48 columns each, w < 2), D2 at 256 (rpc <= 64 columns)
 constexpr int kWvMaxSlices = 8;
 constexpr unsigned int kWvAct = 0x100u;         // replay word: cursor (8) | active (1) | pop slot (16, from bit 16)
 
@@ -56,7 +56,8 @@ struct WaveParams {
     int W;                         // items a request may publish per step (1 .. kWvMaxW)
     int n_slices;                  // W2 slices in a request CTA's shared memory
     int e_max;                     // expansions per request = slot_stride - 1
-    int P;                         // partial vectors per item = n_gru
+    int P;                         // partial vectors per item = n_gru / kWvCS (one per cluster of GRU CTAs)
+    int rpc;                       // rows of W1 each CTA of a cluster reduces: 16 ceil(r / (16 kWvCS))
     __nv_bfloat16 *s_hi, *s_lo;    // [batch, slot_stride, g]
     float *s32;                    // [batch, slot_stride, g]
     float *partial;                // [batch, kWvMaxW, P, r]
@@ -91,6 +92,16 @@ __device__ __forceinline__ bool wave_item_ok(unsigned long long w, unsigned int 
 __device__ __forceinline__ unsigned long long wave_timer() {
     unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
 }
+// In-kernel timeline (measurement builds only: `python -m paper_2607_08642_b200.build --trace` compiles the separate
+// libdominotree_trace.so with -DDT_TRACE, read by `bench.py --trace`): thread 0 of GRU CTA 0 (role 0) and of request
+// CTA 0 (role 1) stamp %globaltimer at fixed points of the first kWvTraceSteps steps.
+constexpr int kWvTraceSteps = 64, kWvTraceStamps = 16;
+#ifdef DT_TRACE
+__device__ unsigned long long g_wv_trace[2][kWvTraceSteps][kWvTraceStamps];
+#define WV_TR(role, cond, step, i) do { if (threadIdx.x == 0 && (cond) && (step) < kWvTraceSteps) g_wv_trace[role][step][i] = wave_timer(); } while (0)
+#else
+#define WV_TR(role, cond, step, i) do { } while (0)
+#endif
 constexpr unsigned long long kWvTimeoutNs = 4000000000ull;     // 4 s: far beyond any round; a slip fails instead of hanging
 
 // TMEM -> registers: 8 consecutive fp32 columns of this thread's lane
@@ -107,8 +118,10 @@ __device__ __forceinline__ void wave_tmem_ld8(uint32_t taddr, float (&v)[8]) {
 // shared-memory footprints (bytes)
 __host__ __device__ inline size_t wave_gru_smem(int g, int r) {
     const size_t r16 = (size_t)((r + 15) & ~15);
-    return (size_t)48 * g * 2 + (size_t)kWvSlots * kWvSlotBytes + r16 * 32 + 4096 +
-           (size_t)(5 * kWvNP + 3 * kWvMaxBatch + 8) * 4 + 8 * 8 + 64 + 1024;
+    (void)r16;
+    const size_t rpc = (size_t)16 * ((r + 16 * kWvCS - 1) / (16 * kWvCS));
+    return (size_t)48 * g * 2 + (size_t)kWvRingBytes + (size_t)kWvCS * 4096 + (size_t)kWvCS * rpc * 32 +
+           (size_t)(5 * kWvNP + 3 * kWvMaxBatch + 8) * 4 + 12 * 8 + 64 + 1024;
 }
 __host__ __device__ inline size_t wave_slice_bytes(int r, int M) {
     return (size_t)((M + 7) / 8) * (size_t)((r + 63) / 64) * 1024;
@@ -116,9 +129,9 @@ __host__ __device__ inline size_t wave_slice_bytes(int r, int M) {
 __host__ __device__ inline size_t wave_req_smem(int r, int M, int N, int k, int W, int e_max, int n_slices) {
     auto al = [](size_t x) { return (x + 15) / 16 * 16; };
     size_t s = (size_t)n_slices * wave_slice_bytes(r, M) + 2 * al((size_t)n_slices * M * 4);
-    s += al((size_t)e_max * k * 8) + al((size_t)e_max * k * 2) + 4 * al((size_t)e_max * 4) + 2 * al((size_t)e_max * 4);
+    s += al((size_t)e_max * k * 8) + al((size_t)e_max * k * 2) + 4 * al((size_t)e_max * 4) + 2 * al((size_t)e_max * 4) + al((size_t)e_max * 8);
     s += 4 * al((size_t)N * 4);
-    s += al((size_t)W * r * 4) + al((size_t)W * M * 4) + al((size_t)8 * r * 4);
+    s += al((size_t)W * r * 4) + al((size_t)W * M * 4);
     s += al((size_t)4 * kWvMaxW * 4) + al(256);
     return s + 1024;
 }
@@ -139,22 +152,67 @@ __device__ __forceinline__ bool wave_spin(F ready, unsigned int *err) {
 }
 
 // ------------------------------------------------------------------------------------------ GRU role
+// thread-block cluster helpers (the GRU CTAs run in clusters of kWvCS: the W1 partial is reduced over the cluster's
+// 16 kWvCS units inside the tensor core after an all-gather of the new states through distributed shared memory)
+__device__ __forceinline__ uint32_t wave_cluster_rank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t wave_mapa(uint32_t saddr, uint32_t rank) {
+    uint32_t r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank)); return r;
+}
+__device__ __forceinline__ void wave_st_cluster_v2(uint32_t addr, uint2 v) {
+    asm volatile("st.shared::cluster.v2.b32 [%0], {%1, %2};" ::"r"(addr), "r"(v.x), "r"(v.y) : "memory");
+}
+__device__ __forceinline__ void wave_cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void wave_cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
+// six 8-column TMEM loads (three gates x two accumulators) and one wait
+__device__ __forceinline__ void wave_tmem_ld_gates(uint32_t t0, uint32_t t1, float (&v)[48]) {
+    uint32_t r[48];
+#define WV_LD8(base, off, i)                                                                                   \
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"              \
+                 : "=r"(r[i]), "=r"(r[i + 1]), "=r"(r[i + 2]), "=r"(r[i + 3]), "=r"(r[i + 4]), "=r"(r[i + 5]), \
+                   "=r"(r[i + 6]), "=r"(r[i + 7]) : "r"((base) + (off)) : "memory")
+    WV_LD8(t0, 0, 0); WV_LD8(t0, 16, 8); WV_LD8(t0, 32, 16);
+    WV_LD8(t1, 0, 24); WV_LD8(t1, 16, 32); WV_LD8(t1, 32, 40);
+#undef WV_LD8
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 48; ++i) v[i] = __uint_as_float(r[i]);
+}
+__device__ __forceinline__ void wave_tmem_ld16(uint32_t taddr, float (&v)[16]) {
+    uint32_t r[16];
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                 : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
+template <int N> __device__ __forceinline__ void wave_cp_wait_n(int n) {
+    if (n >= N) cp_async_wait<N>();
+    else if constexpr (N > 0) wave_cp_wait_n<N - 1>(n);
+}
+
 __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char *smem_raw) {
     const ExpandParams &e = p.e;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g = e.g, r = e.r, batch = e.batch;
     const int cta = blockIdx.x, u0 = cta * 16;
+    const int crank = (int)wave_cluster_rank(), cbase = cta - crank;   // rank in the cluster, first CTA of the cluster
     const size_t stride = (size_t)p.slot_stride;
     const int n_kc = g / kWvKC;
-    const int r16 = (r + 15) & ~15;
+    const int rpc = p.rpc;                                             // rows of W1 this CTA reduces (multiple of 16)
 
-    // carve (smem_raw is 1024-byte aligned by the kernel)
+    // carve (smem_raw is 1024-byte aligned by the kernel).  The M = 128 MMA always reads 16 row groups per k-block; when a
+    // pass has fewer rows the ring is packed tighter and those phantom reads run past the k-block, at the end of the ring
+    // into sS2 (valid memory, results of phantom rows are never used).
     unsigned char *sW = smem_raw;                                     // W_hh slice, K-major sw128: [6 row groups][g/64 atoms][1 KB]
     const uint32_t sboW = (uint32_t)g * 16;                           // bytes between 8-row groups
-    unsigned char *sRing = sW + (size_t)48 * g * 2;                   // [slot][2 k-blocks][16 row groups][1 KB]
-    unsigned char *sW1 = sRing + (size_t)kWvSlots * kWvSlotBytes;     // W1[:, d + u0 ..] as [r16/8 groups][2 k-halves][8 rows][16 B]
-    unsigned char *sS2 = sW1 + (size_t)r16 * 32;                      // new states [16 groups][2 k-halves][8 rows][16 B]
-    int *sRow = reinterpret_cast<int *>(sS2 + 4096);                  // [64] request * stride + parent slot  (state row)
+    unsigned char *sRing = sW + (size_t)48 * g * 2;                   // [slot][2 k-blocks][G row groups][1 KB]
+    unsigned char *sS2 = sRing + kWvRingBytes;                        // [kWvCS][16 groups][2 k-halves][8 rows][16 B]: new states of
+                                                                      // the cluster's 16 kWvCS units (block c written by rank c)
+    unsigned char *sW1 = sS2 + (size_t)kWvCS * 4096;                  // [kWvCS][rpc/8 groups][2 k-halves][8 rows][16 B]
+    int *sRow = reinterpret_cast<int *>(sW1 + (size_t)kWvCS * rpc * 32);   // [64] request * stride + parent slot  (state row)
     int *sNew = sRow + kWvNP;                                         // [64] request * stride + new slot
     int *sTok = sNew + kWvNP;                                         // [64]
     int *sIt = sTok + kWvNP;                                          // [64] request * kWvMaxW + item index (partial row)
@@ -162,8 +220,8 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
     int *sCnt = sPz + kWvNP;                                          // [128] items per request this step
     int *sOff = sCnt + kWvMaxBatch;                                   // [129] exclusive prefix
     int *sFirst = sOff + kWvMaxBatch + 4;                             // [128] first new state slot per request
-    unsigned long long *mbar = reinterpret_cast<unsigned long long *>(sFirst + kWvMaxBatch);   // [0..2] slot free, [3] D1, [4] D2
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(mbar + 8);
+    unsigned long long *mbar = reinterpret_cast<unsigned long long *>(sFirst + kWvMaxBatch);   // [0..7] slot free, [8] D1, [9] D2
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(mbar + 12);
     int *sCtl = reinterpret_cast<int *>(tmem_slot + 2);               // [0] items this step, [1] requests not done, [2] abort, [4..7] live masks
 
     {   // resident weights
@@ -175,17 +233,19 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
             const uint4 q = ld_ro_v4(whh + ((size_t)gate * g + u0 + ul) * g + (size_t)c * 8);
             *reinterpret_cast<uint4 *>(sW + (size_t)(m >> 3) * sboW + (size_t)(c >> 3) * 1024 + (m & 7) * 128 + (((c & 7) ^ (m & 7)) << 4)) = q;
         }
+        // W1 rows [crank * rpc, crank * rpc + rpc) x the 16 units of every CTA of the cluster (one K = 16 step each)
         const __nv_bfloat16 *w1 = reinterpret_cast<const __nv_bfloat16 *>(e.w1);
-        for (int i = tid; i < r16 * 16; i += kWvThreads) {
-            const int j = i >> 4, ul = i & 15;
-            const __nv_bfloat16 v = (j < r) ? w1[(size_t)j * (e.d + g) + e.d + u0 + ul] : __float2bfloat16_rn(0.f);
-            *reinterpret_cast<__nv_bfloat16 *>(sW1 + (size_t)(j >> 3) * 256 + (ul >> 3) * 128 + (j & 7) * 16 + (ul & 7) * 2) = v;
+        for (int i = tid; i < kWvCS * rpc * 16; i += kWvThreads) {
+            const int c = i / (rpc * 16), rem = i - c * rpc * 16;
+            const int jl = rem >> 4, ul = rem & 15, j = crank * rpc + jl;
+            const __nv_bfloat16 v = (j < r) ? w1[(size_t)j * (e.d + g) + e.d + (cbase + c) * 16 + ul] : __float2bfloat16_rn(0.f);
+            *reinterpret_cast<__nv_bfloat16 *>(sW1 + (size_t)c * rpc * 32 + (size_t)(jl >> 3) * 256 + (ul >> 3) * 128 + (jl & 7) * 16 + (ul & 7) * 2) = v;
         }
-        for (int i = tid; i < 1024; i += kWvThreads) reinterpret_cast<uint32_t *>(sS2)[i] = 0u;
+        for (int i = tid; i < kWvCS * 1024; i += kWvThreads) reinterpret_cast<uint32_t *>(sS2)[i] = 0u;
         if (tid == 0) {
-            for (int i = 0; i < kWvSlots; ++i) tc::mbar_init(tc::smem_u32(mbar + i), 4);
-            tc::mbar_init(tc::smem_u32(mbar + 3), 4);
-            tc::mbar_init(tc::smem_u32(mbar + 4), 1);
+            for (int i = 0; i < 8; ++i) tc::mbar_init(tc::smem_u32(mbar + i), 2);
+            tc::mbar_init(tc::smem_u32(mbar + 8), 2);
+            tc::mbar_init(tc::smem_u32(mbar + 9), 1);
             tc::mbar_init_fence();
             sCtl[2] = 0;
         }
@@ -195,12 +255,15 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
     tc::fence_before_sync();
     __syncthreads();
     tc::fence_after_sync();
+    wave_cluster_arrive();                                            // peers' sS2 is zeroed before anyone stores into it
+    wave_cluster_wait();
     const uint32_t tmem = *tmem_slot;
-    const uint32_t idesc1 = tc::make_idesc_bf16(128, 48), idesc2 = tc::make_idesc_bf16(128, r16);
+    const uint32_t idesc1 = tc::make_idesc_bf16(128, 48), idesc2 = tc::make_idesc_bf16(128, rpc);
     const uint32_t mb0 = tc::smem_u32(mbar);
     const uint64_t descW0 = tc::make_desc_sw128(tc::smem_u32(sW), sboW), descR0 = tc::make_desc_sw128(tc::smem_u32(sRing), 1024);
     const uint64_t descS2 = tc::make_desc(tc::smem_u32(sS2), 128, 256), descW1 = tc::make_desc(tc::smem_u32(sW1), 128, 256);
     uint32_t ph_free = 0, ph_d1 = 0, ph_d2 = 0;                    // mbarrier phases (uniform across the CTA)
+    bool pend2 = false;                                             // a cluster arrive (sS2 consumed) awaits its wait
 
     // epilogue geometry: TMEM lane quadrant q4, unit half hsel; lanes 0..15 hold the hi rows of nodes 16 q4 + lane,
     // lanes 16..31 the lo rows of the same nodes; after the hi + lo exchange lane < 16 finishes units 8 hsel + 0..3,
@@ -209,6 +272,18 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
     const int my_node = 16 * q4 + il;
     const int my_u = 8 * hsel + 4 * uh;                              // first of this thread's 4 local units
     const uint32_t tlane = (uint32_t)(32 * q4) << 16;
+    // where this thread's new states go in every cluster CTA's sS2 (block crank): rows 32 q4 + il (hi) and + 16 (lo)
+    uint32_t s2_hi[kWvCS], s2_lo[kWvCS];
+    {
+        const int rh = 32 * q4 + il, rl = rh + 16;
+        const uint32_t oh = (uint32_t)(crank * 4096 + (rh >> 3) * 256 + hsel * 128 + (rh & 7) * 16 + uh * 8);
+        const uint32_t ol = (uint32_t)(crank * 4096 + (rl >> 3) * 256 + hsel * 128 + (rl & 7) * 16 + uh * 8);
+#pragma unroll
+        for (int c = 0; c < kWvCS; ++c) {
+            s2_hi[c] = wave_mapa(tc::smem_u32(sS2) + oh, (uint32_t)c);
+            s2_lo[c] = wave_mapa(tc::smem_u32(sS2) + ol, (uint32_t)c);
+        }
+    }
 
     const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 10;
     for (int s = 0;; ++s) {
@@ -244,6 +319,7 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
         __syncthreads();
         const int total = sCtl[0];
         if (sCtl[2] || !sCtl[1]) break;                              // abort, or every request is done
+        WV_TR(0, cta == 0, s, 0);
 
         for (int p0 = 0; p0 < total; p0 += kWvNP) {
             const int n = min(kWvNP, total - p0);
@@ -252,7 +328,7 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                 int row = 0, nw = 0, tok = 0, it = 0, pz = 1;
                 if (tid < n) {
                     const int qi = p0 + tid;
-                    int lo = 0, hi = kWvMaxBatch - 1;                // last b with sOff[b] <= qi and a non-empty list
+                    int lo = 0, hi = kWvMaxBatch - 1;                // last b with sOff[b] <= qi: its list is not empty
                     while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (sOff[mid] <= qi) lo = mid; else hi = mid - 1; }
                     const int b = lo, j = qi - sOff[b];
                     unsigned long long w = 0ull;
@@ -267,8 +343,13 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                 sRow[tid] = row; sNew[tid] = nw; sTok[tid] = tok; sIt[tid] = it; sPz[tid] = pz;
             }
             __syncthreads();
+            WV_TR(0, cta == 0 && p0 == 0, s, 1);
 
-            // ---- this thread's share of a ring slot: 8 operand rows (rho = (tid >> 4) + 16 i), 16-byte piece tid & 15
+            // ---- ring geometry of this pass: G row groups per k-block (16 nodes fill 4), as many slots as fit
+            const int G = 4 * ((n + 15) >> 4);
+            const int kb_bytes = G * 1024, slot_bytes = 2 * kb_bytes;
+            const int nslot = min(min(n_kc, 8), kWvRingBytes / slot_bytes);
+            // this thread's share of a slot: 8 operand rows (rho = (tid >> 4) + 16 i), 16-byte piece tid & 15
             const int piece = tid & 15, kb = piece >> 3, pc = piece & 7;
             const __nv_bfloat16 *src[8];
             uint32_t dsto[8];
@@ -278,17 +359,17 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                 const int node = 16 * (rho >> 5) + (rho & 15), hl = (rho >> 4) & 1;
                 src[i] = nullptr;
                 if (node < n) src[i] = (hl ? p.s_lo : p.s_hi) + (size_t)sRow[node] * g + (size_t)piece * 8;
-                dsto[i] = (uint32_t)(kb * 16384 + (rho >> 3) * 1024 + (rho & 7) * 128 + ((pc ^ (rho & 7)) << 4));
+                dsto[i] = (uint32_t)(kb * kb_bytes + (rho >> 3) * 1024 + (rho & 7) * 128 + ((pc ^ (rho & 7)) << 4));
             }
             auto issue_chunk = [&](int kc) {
-                unsigned char *dst = sRing + (size_t)(kc % kWvSlots) * kWvSlotBytes;
+                unsigned char *dst = sRing + (size_t)(kc % nslot) * slot_bytes;
                 const size_t k0 = (size_t)kc * kWvKC;
 #pragma unroll
                 for (int i = 0; i < 8; ++i)
                     if (src[i]) cp_async16(dst + dsto[i], src[i] + k0);
             };
 #pragma unroll 1
-            for (int kc = 0; kc < kWvSlots; ++kc) { if (kc < n_kc) issue_chunk(kc); cp_async_commit(); }
+            for (int kc = 0; kc < nslot; ++kc) { issue_chunk(kc); cp_async_commit(); }
 
             // ---- epilogue operands (input half from P, previous state): issued now, consumed after the MMAs
             float4 pr = make_float4(0.f, 0.f, 0.f, 0.f), pz4 = pr, pn = pr, hp = pr;
@@ -300,52 +381,52 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                 pn = __ldg(reinterpret_cast<const float4 *>(prow + 2 * g));
                 if (!sPz[my_node]) hp = __ldcg(reinterpret_cast<const float4 *>(p.s32 + (size_t)sRow[my_node] * g + u0 + my_u));
             }
+            WV_TR(0, cta == 0 && p0 == 0, s, 2);
 
-            // ---- D1[128 x 48] = [S_hi | S_lo rows] . W_hh slice^T, K streamed through the ring
+            // ---- D1[128 x 48] = [S_hi | S_lo rows] . W_hh slice^T, K streamed through the ring.  Chunk j sits in cp.async
+            // group j; the slot of chunk kc - 1 is refilled one iteration after its MMAs were issued.
 #pragma unroll 1
             for (int kc = 0; kc < n_kc; ++kc) {
-                cp_async_wait<kWvSlots - 1>();
+                wave_cp_wait_n<7>(kc == 0 ? nslot - 1 : nslot - 2);
                 tc::fence_proxy_async();
                 __syncthreads();
-                const int sl = kc % kWvSlots;
-                if (warp < 4 && lane == 0) {
-                    // warp w issues K = 16 steps 2 w and 2 w + 1 of the slot's eight into its own accumulator D1[w]
+                const int sl = kc % nslot;
+                if (warp < 2 && lane == 0) {
+                    // warp w issues K = 16 steps 4 w .. 4 w + 3 of the chunk's eight (= k-block w) into its own accumulator D1[w]
                     tc::fence_after_sync();
 #pragma unroll
-                    for (int jj = 0; jj < 2; ++jj) {
-                        const int j8 = 2 * warp + jj, kbj = j8 >> 2, s4 = j8 & 3;
-                        const uint64_t da = descR0 + (uint64_t)((sl * kWvSlotBytes + kbj * 16384) / 16 + s4 * 2);
-                        const uint64_t db = descW0 + (uint64_t)((kc * 2 + kbj) * 64 + s4 * 2);
-                        tc::mma_bf16(tmem + 64 * warp, da, db, idesc1, (kc | jj) ? 1u : 0u);
+                    for (int s4 = 0; s4 < 4; ++s4) {
+                        const uint64_t da = descR0 + (uint64_t)((sl * slot_bytes + warp * kb_bytes) / 16 + s4 * 2);
+                        const uint64_t db = descW0 + (uint64_t)((kc * 2 + warp) * 64 + s4 * 2);
+                        tc::mma_bf16(tmem + 64 * warp, da, db, idesc1, (kc | s4) ? 1u : 0u);
                     }
-                    if (kc + kWvSlots < n_kc) tc::commit(mb0 + 8 * sl);          // this slot is refilled below
-                    if (kc == n_kc - 1) tc::commit(mb0 + 24);
+                    if (kc + nslot < n_kc) tc::commit(mb0 + 8 * sl);             // this slot is refilled next iteration
+                    if (kc == n_kc - 1) tc::commit(mb0 + 64);
                 }
-                if (kc + kWvSlots < n_kc) {                  // refill the slot once its MMAs have read it
-                    tc::mbar_wait(mb0 + 8 * sl, (ph_free >> sl) & 1u);
-                    ph_free ^= 1u << sl;
-                    issue_chunk(kc + kWvSlots);
+                if (kc >= 1) {
+                    if (kc - 1 + nslot < n_kc) {                 // refill the previous chunk's slot once its MMAs have read it
+                        const int slp = (kc - 1) % nslot;
+                        tc::mbar_wait(mb0 + 8 * slp, (ph_free >> slp) & 1u);
+                        ph_free ^= 1u << slp;
+                        issue_chunk(kc - 1 + nslot);
+                    }
+                    cp_async_commit();
                 }
-                cp_async_commit();
             }
             cp_async_wait<0>();
-            tc::mbar_wait(mb0 + 24, ph_d1); ph_d1 ^= 1u;
+            tc::mbar_wait(mb0 + 64, ph_d1); ph_d1 ^= 1u;
             tc::fence_after_sync();
             __syncwarp();
+            WV_TR(0, cta == 0 && p0 == 0, s, 3);
 
-            // ---- gates (reading A2): columns gate * 16 + unit of the four accumulators, hi + lo rows added
+            // ---- gates (reading A2): columns gate * 16 + unit of the two accumulators, hi + lo rows added
             float acc[24];
+            {
+                float v[48];
+                wave_tmem_ld_gates(tmem + tlane + 8 * hsel, tmem + tlane + 64 + 8 * hsel, v);
 #pragma unroll
-            for (int c = 0; c < 24; ++c) acc[c] = 0.f;
-#pragma unroll
-            for (int a = 0; a < 4; ++a)
-#pragma unroll
-                for (int gate = 0; gate < 3; ++gate) {
-                    float v[8];
-                    wave_tmem_ld8(tmem + tlane + 64 * a + gate * 16 + 8 * hsel, v);
-#pragma unroll
-                    for (int c = 0; c < 8; ++c) acc[gate * 8 + c] += v[c];
-                }
+                for (int c = 0; c < 24; ++c) acc[c] = v[c] + v[24 + c];
+            }
 #pragma unroll
             for (int c = 0; c < 24; ++c) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 16);
             {
@@ -355,9 +436,9 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                 __nv_bfloat16 bh[4], bl[4];
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
-                    const float rg = sigmoidf_fast(prv[c] + acc[4 * uh + c]);
-                    const float zg = sigmoidf_fast(pzv[c] + acc[8 + 4 * uh + c]);
-                    const float ng = tanhf_fast(pnv[c] + rg * acc[16 + 4 * uh + c]);
+                    const float rg = sigmoidf_fast(prv[c] + (uh ? acc[4 + c] : acc[c]));
+                    const float zg = sigmoidf_fast(pzv[c] + (uh ? acc[12 + c] : acc[8 + c]));
+                    const float ng = tanhf_fast(pnv[c] + rg * (uh ? acc[20 + c] : acc[16 + c]));
                     hn[c] = mine ? ((1.0f - zg) * ng + zg * hpv[c]) : 0.f;
                     bh[c] = __float2bfloat16_rn(hn[c]);
                     bl[c] = __float2bfloat16_rn(hn[c] - __bfloat162float(bh[c]));
@@ -373,52 +454,59 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                     __stcg(reinterpret_cast<uint2 *>(p.s_hi + o), ph);
                     __stcg(reinterpret_cast<uint2 *>(p.s_lo + o), pl);
                 }
-                // operand A of the W1 GEMM: rows 32 q4 + il (hi) and + 16 (lo), k = local unit
-                const int rh = 32 * q4 + il, rl = rh + 16;
-                *reinterpret_cast<uint2 *>(sS2 + (size_t)(rh >> 3) * 256 + hsel * 128 + (rh & 7) * 16 + uh * 8) = ph;
-                *reinterpret_cast<uint2 *>(sS2 + (size_t)(rl >> 3) * 256 + hsel * 128 + (rl & 7) * 16 + uh * 8) = pl;
+                // all-gather over the cluster: block `crank` of every cluster CTA's sS2 (operand A of the W1 GEMM)
+                if (pend2) { wave_cluster_wait(); pend2 = false; }   // every peer's previous W1 GEMM has read its sS2
+#pragma unroll
+                for (int c = 0; c < kWvCS; ++c) { wave_st_cluster_v2(s2_hi[c], ph); wave_st_cluster_v2(s2_lo[c], pl); }
             }
+            wave_cluster_arrive();
+            wave_cluster_wait();
             tc::fence_proxy_async();
             tc::fence_before_sync();
             __syncthreads();
-            // ---- D2[128 x r] = S_new[rows, my 16 units] . W1[:, d + my units]^T : this CTA's split-K share
+            WV_TR(0, cta == 0 && p0 == 0, s, 4);
+            // ---- D2[128 x rpc] = S_new[rows, the cluster's 16 kWvCS units] . W1[my rpc rows, d + those units]^T:
+            // one K = 16 step per cluster CTA, accumulated in rank order
             if (tid == 0) {
                 tc::fence_after_sync();
-                tc::mma_bf16(tmem + 256, descS2, descW1, idesc2, 0u);
-                tc::commit(mb0 + 32);
+#pragma unroll
+                for (int c = 0; c < kWvCS; ++c)
+                    tc::mma_bf16(tmem + 256, descS2 + (uint64_t)(c * 256), descW1 + (uint64_t)(c * rpc * 2), idesc2, c ? 1u : 0u);
+                tc::commit(mb0 + 72);
             }
-            tc::mbar_wait(mb0 + 32, ph_d2); ph_d2 ^= 1u;
+            tc::mbar_wait(mb0 + 72, ph_d2); ph_d2 ^= 1u;
             tc::fence_after_sync();
             __syncwarp();
+            wave_cluster_arrive(); pend2 = true;                     // my sS2 may be overwritten by the next pass
+            WV_TR(0, cta == 0 && p0 == 0, s, 5);
             {
-                float *prow = p.partial + ((size_t)(mine ? sIt[my_node] : 0) * p.P + cta) * r;
+                // partial[item][cluster][crank * rpc + col]: lanes < 16 store columns 0..7 of a 16-column block, lanes >= 16 8..15
+                float *prow = p.partial + ((size_t)(mine ? sIt[my_node] : 0) * p.P + (cta / kWvCS)) * r + crank * rpc;
 #pragma unroll 1
-                for (int blk = 0; blk < 4; ++blk) {
-                    const int col0 = 128 * hsel + 32 * blk;
-                    if (col0 >= r16) break;                          // warp-uniform
-                    float v[32];
-                    tc::tmem_ld32(tmem + tlane + 256 + col0, v);
+                for (int blk = hsel; blk < rpc / 16; blk += 2) {
+                    float v[16];
+                    wave_tmem_ld16(tmem + tlane + 256 + 16 * blk, v);
 #pragma unroll
-                    for (int c = 0; c < 32; ++c) v[c] += __shfl_xor_sync(0xffffffffu, v[c], 16);
+                    for (int c = 0; c < 16; ++c) v[c] += __shfl_xor_sync(0xffffffffu, v[c], 16);
                     if (mine) {
-#pragma unroll
-                        for (int c4 = 0; c4 < 4; ++c4) {
-                            const int col = col0 + 16 * uh + 4 * c4;
-                            // the uh half selects which 16 of the 32 columns this lane stores
-                            const float4 o = uh ? make_float4(v[16 + 4 * c4], v[17 + 4 * c4], v[18 + 4 * c4], v[19 + 4 * c4])
-                                                : make_float4(v[4 * c4], v[4 * c4 + 1], v[4 * c4 + 2], v[4 * c4 + 3]);
-                            if (col + 3 < r) __stcg(reinterpret_cast<float4 *>(prow + col), o);
-                        }
+                        const int col = 16 * blk + 8 * uh;
+                        const float4 o0 = uh ? make_float4(v[8], v[9], v[10], v[11]) : make_float4(v[0], v[1], v[2], v[3]);
+                        const float4 o1 = uh ? make_float4(v[12], v[13], v[14], v[15]) : make_float4(v[4], v[5], v[6], v[7]);
+                        if (crank * rpc + col + 3 < r) __stcg(reinterpret_cast<float4 *>(prow + col), o0);
+                        if (crank * rpc + col + 7 < r) __stcg(reinterpret_cast<float4 *>(prow + col + 4), o1);
                     }
                 }
             }
             tc::fence_before_sync();
             __syncthreads();
+            WV_TR(0, cta == 0 && p0 == 0, s, 6);
         }
         if (sCtl[2]) break;
         if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, fbase + (unsigned int)(s + 1)); }
+        WV_TR(0, cta == 0, s, 7);
     }
     __syncthreads();
+    if (pend2) wave_cluster_wait();
     if (warp == 0) tc::tmem_free<kWvTmemCols>(tmem);
     // every CTA of the grid has read the counter: a request is done only after all GRU CTAs finished step 0
     if (cta == 0 && tid == 0) st_relaxed_u32(p.round_ctr, rnd + 1u);
@@ -459,13 +547,13 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
     float *eSco = reinterpret_cast<float *>(carve((size_t)e_max * 4));
     unsigned int *simC = reinterpret_cast<unsigned int *>(carve((size_t)e_max * 4));   // replay state at the commit point
     unsigned int *simT = reinterpret_cast<unsigned int *>(carve((size_t)e_max * 4));   // ... of the running replay
+    unsigned long long *hT = reinterpret_cast<unsigned long long *>(carve((size_t)e_max * 8));   // head key of every active list (0 = none)
     int *nTok = reinterpret_cast<int *>(carve((size_t)N * 4));
     int *nPar = reinterpret_cast<int *>(carve((size_t)N * 4));
     int *nDep = reinterpret_cast<int *>(carve((size_t)N * 4));
     float *nSco = reinterpret_cast<float *>(carve((size_t)N * 4));
     float *sA = reinterpret_cast<float *>(carve((size_t)W * r * 4));
     float *sZ = reinterpret_cast<float *>(carve((size_t)W * M * 4));
-    float *sPg = reinterpret_cast<float *>(carve((size_t)8 * r * 4));
     int *itE = reinterpret_cast<int *>(carve((size_t)4 * kWvMaxW * 4));
     int *itTok = itE + kWvMaxW, *itPs = itTok + kWvMaxW;
     WaveCtl &ctl = *reinterpret_cast<WaveCtl *>(carve(256));
@@ -526,21 +614,20 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
         }
         __syncthreads();
         if (ctl.abort_) break;
+        WV_TR(1, b == 0, s, 0);
 
-        // ---- a_j = SiLU(C + W1[:, d:] S_j): the P split-K partials are summed in a fixed order (batch-invariant)
-        for (int j = 0; j < n_it; ++j) {
-            const int x = itE[j];
-            const size_t row = (size_t)b * L + eDep[x];             // H_{depth+1} <-> row index depth (A12)
+        // ---- a_j = SiLU(C + W1[:, d:] S_j): the P cluster partials are summed in a fixed order (batch-invariant);
+        // one thread per (item, four columns), all loads of a thread in flight at once
+        {
             const int r4 = r >> 2;
-            const int G = min(8, kWvThreads / r4);
-            const int per = (P + G - 1) / G;
-            const int jq = tid % r4, qg = tid / r4;
-            if (qg < G) {
+            for (int pair = tid; pair < n_it * r4; pair += kWvThreads) {
+                const int j = pair / r4, jq = pair - j * r4;
+                const int x = itE[j];
+                const float4 cv = __ldg(reinterpret_cast<const float4 *>(e.C + ((size_t)b * L + eDep[x]) * r) + jq);   // H_{depth+1} <-> row depth (A12)
                 const float4 *pp = reinterpret_cast<const float4 *>(p.partial + ((size_t)(b * kWvMaxW + j) * P) * r) + jq;
-                const int q0 = qg * per, q1 = min(P, q0 + per);
                 float4 s0 = make_float4(0.f, 0.f, 0.f, 0.f), s1 = s0;
-                int q = q0;
-                for (; q + 8 <= q1; q += 8) {
+                int q = 0;
+                for (; q + 8 <= P; q += 8) {
                     float4 v[8];
 #pragma unroll
                     for (int i = 0; i < 8; ++i) v[i] = __ldcg(pp + (size_t)(q + i) * r4);
@@ -550,23 +637,19 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                         s1.x += v[i + 1].x; s1.y += v[i + 1].y; s1.z += v[i + 1].z; s1.w += v[i + 1].w;
                     }
                 }
-                for (; q < q1; ++q) {
+                for (; q < P; ++q) {
                     const float4 v = __ldcg(pp + (size_t)q * r4);
                     s0.x += v.x; s0.y += v.y; s0.z += v.z; s0.w += v.w;
                 }
-                *reinterpret_cast<float4 *>(sPg + (size_t)qg * r + 4 * jq) = make_float4(s0.x + s1.x, s0.y + s1.y, s0.z + s1.z, s0.w + s1.w);
+                float4 o;
+                o.x = cv.x + (s0.x + s1.x); o.y = cv.y + (s0.y + s1.y); o.z = cv.z + (s0.z + s1.z); o.w = cv.w + (s0.w + s1.w);
+                o.x *= sigmoidf_acc(o.x); o.y *= sigmoidf_acc(o.y); o.z *= sigmoidf_acc(o.z); o.w *= sigmoidf_acc(o.w);
+                *reinterpret_cast<float4 *>(sA + (size_t)j * r + 4 * jq) = o;
             }
-            __syncthreads();
-            for (int jj = tid; jj < r; jj += kWvThreads) {
-                float acc = sPg[jj];
-                for (int gq = 1; gq < G; ++gq) acc += sPg[(size_t)gq * r + jj];
-                const float xx = e.C[row * r + jj] + acc;
-                sA[(size_t)j * r + jj] = xx * sigmoidf_acc(xx);
-            }
-            __syncthreads();
         }
         cp_async_wait<0>();
         __syncthreads();
+        WV_TR(1, b == 0, s, 1);
 
         // ---- z_m = ((base_m - base_0) + W2[cand_m, :] a) / T_eff   PAPER.md:143-144 (shift-invariant)
         // a warp takes 8 candidate rows (one swizzle row group), four lanes per row
@@ -596,47 +679,65 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
             }
         }
         __syncthreads();
+        WV_TR(1, b == 0, s, 2);
 
-        // ---- slice log-softmax (reading A1) and top-k by (logp desc, token asc): one warp per node
+        // ---- slice log-softmax (reading A1) and top-k by (logp desc, token asc): one warp per node, candidates in
+        // registers (lane holds m = lane + 32 i), k rounds of a warp-wide arg-max
         for (int j = warp; j < n_it; j += kWvThreads / 32) {
             const int x = itE[j];
             const int si = ctl.d2s[eDep[x]];
             const float *zj = sZ + (size_t)j * M;
             const int *tk = slTok + si * M;
+            float zl[8];
+            unsigned int tl[8];
             float zmax = -INFINITY;
-            for (int m = lane; m < M; m += 32) zmax = fmaxf(zmax, zj[m]);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int m = lane + 32 * i;
+                zl[i] = (m < M) ? zj[m] : -INFINITY;
+                tl[i] = (m < M) ? (unsigned int)tk[m] : 0xFFFFFFFFu;
+                zmax = fmaxf(zmax, zl[i]);
+            }
             zmax = warp_max(zmax);
             float ssum = 0.f;
-            for (int m = lane; m < M; m += 32) ssum += expf(zj[m] - zmax);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) if (lane + 32 * i < M) ssum += expf(zl[i] - zmax);
             ssum = warp_sum(ssum);
             const float lse = logf(ssum);
             const float gpar = eSco[x];
             unsigned long long *ck = cKey + (size_t)x * k;
-            for (int m = lane; m < M; m += 32) {
-                const float mz = zj[m];
-                const int mtok = tk[m];
-                int rank = 0;
-                for (int q = 0; q < M; ++q) {
-                    const float oz = zj[q];
-                    rank += (oz > mz) || (oz == mz && tk[q] < mtok);
+            unsigned int taken = 0u;
+            for (int rk = 0; rk < k; ++rk) {
+                unsigned int bz = 0u, bt = 0xFFFFFFFFu;
+                int bi = -1;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    if (lane + 32 * i >= M || ((taken >> i) & 1u)) continue;
+                    const unsigned int kz = ord_key(zl[i]);
+                    if (bi < 0 || kz > bz || (kz == bz && tl[i] < bt)) { bz = kz; bt = tl[i]; bi = i; }
                 }
-                if (rank < k) {
-                    const float lpm = (mz - zmax) - lse;
-                    ck[rank] = ((unsigned long long)ord_key(gpar + lpm) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned int)mtok);
+                const unsigned int mz = __reduce_max_sync(0xffffffffu, bi >= 0 ? bz : 0u);
+                const bool el = (bi >= 0) && bz == mz;
+                const unsigned int mt = __reduce_min_sync(0xffffffffu, el ? bt : 0xFFFFFFFFu);
+                if (el && bt == mt) {                               // tokens of one slice are distinct: exactly one lane
+                    taken |= 1u << bi;
+                    const float lpm = (zl[bi] - zmax) - lse;
+                    ck[rk] = ((unsigned long long)ord_key(gpar + lpm) << 32) | (unsigned long long)(0xFFFFFFFFu - bt);
                 }
             }
             __syncwarp();
             // the list is kept sorted by the pop comparator itself (fp32 rounding of g + logp may merge two scores)
             unsigned long long mk = 0ull;
-            int rk = 0;
+            int rk2 = 0;
             if (lane < k) {
                 mk = ck[lane];
-                for (int q = 0; q < k; ++q) rk += (ck[q] > mk);
+                for (int q = 0; q < k; ++q) rk2 += (ck[q] > mk);
             }
             __syncwarp();
-            if (lane < k) { ck[rk] = mk; cExp[(size_t)x * k + lane] = -1; }
+            if (lane < k) { ck[rk2] = mk; cExp[(size_t)x * k + lane] = -1; }
         }
         __syncthreads();
+        WV_TR(1, b == 0, s, 3);
 
         // ---- replay the heap from the commit point, nominate, publish (warp 0)
         if (warp == 0) {
@@ -644,7 +745,11 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
             int t = ctl.c;
             if (s == 0 && lane == 0) { simC[0] = kWvAct; }          // the root is slot 0; its children are known now
             __syncwarp();
-            for (int x = lane; x < n_exp; x += 32) simT[x] = simC[x];
+            for (int x = lane; x < n_exp; x += 32) {
+                const unsigned int w = simC[x];
+                simT[x] = w;
+                hT[x] = ((w & kWvAct) && (int)(w & 0xFFu) < k) ? cKey[(size_t)x * k + (w & 0xFFu)] : 0ull;
+            }
             __syncwarp();
             bool committing = true, finished = false;
             int found = 0;
@@ -655,11 +760,9 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                 unsigned int bps = 0xFFFFFFFFu;
                 int be = -1;
                 for (int x = lane; x < n_exp; x += 32) {
-                    const unsigned int w = simT[x];
-                    const int cur = (int)(w & 0xFFu);
-                    if (!(w & kWvAct) || cur >= k) continue;
-                    const unsigned long long key = cKey[(size_t)x * k + cur];
-                    const unsigned int ps = w >> 16;
+                    const unsigned long long key = hT[x];
+                    if (key == 0ull) continue;
+                    const unsigned int ps = simT[x] >> 16;
                     if (be < 0 || key > bk || (key == bk && ps < bps)) { bk = key; bps = ps; be = x; }
                 }
                 if (__ballot_sync(0xffffffffu, be >= 0) == 0u) { finished = committing; break; }   // the candidate tree ran dry
@@ -689,8 +792,9 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                 t += 1;
                 if (lane == 0) {
                     simT[es] = wv + 1u;
+                    hT[es] = (jc + 1 < k) ? cKey[(size_t)es * k + jc + 1] : 0ull;
                     nTok[t] = tok; nPar[t] = (int)(wv >> 16); nDep[t] = dep; nSco[t] = ord_key_inv(mh);
-                    if (x >= 0) simT[x] = kWvAct | ((unsigned int)t << 16);
+                    if (x >= 0) { simT[x] = kWvAct | ((unsigned int)t << 16); hT[x] = cKey[(size_t)x * k]; }
                 }
                 if (needs && found < W) {                           // warp-uniform; lane 0 decides, the count is broadcast
                     // resources: a state slot (speculative picks leave room for the expansions Algorithm 1 still needs)
@@ -719,7 +823,7 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                             ctl.slUsed[si] = step_next;
                             cExp[(size_t)es * k + jc] = (short)xn;
                             eTok[xn] = tok; ePar[xn] = es; eDep[xn] = dep; eSco[xn] = ord_key_inv(mh);
-                            simC[xn] = 0u; simT[xn] = 0u;
+                            simC[xn] = 0u; simT[xn] = 0u; hT[xn] = 0ull;
                             itE[found] = xn; itTok[found] = tok; itPs[found] = es + 1;
                             add = 1;
                         }
@@ -744,8 +848,10 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
             }
         }
         __syncthreads();
+        WV_TR(1, b == 0, s, 4);
         if (ctl.done) break;
         stage_slices();
+        WV_TR(1, b == 0, s, 5);
         if (tid == 0) ctl.n_stage = 0;
     }
     __syncthreads();
@@ -777,7 +883,7 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
 __global__ void __launch_bounds__(kWvThreads, 1) wave_expand_kernel(WaveParams p) {
     extern __shared__ __align__(1024) unsigned char wave_smem[];
     if ((int)blockIdx.x < p.n_gru) wave_gru_role(p, wave_smem);
-    else wave_req_role(p, wave_smem);
+    else if ((int)blockIdx.x - p.n_gru < p.e.batch) wave_req_role(p, wave_smem);   // CTAs padding the last cluster leave
 }
 
 }  // namespace dt
