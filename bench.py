@@ -512,6 +512,14 @@ def run_trace(args):
             d = q[:, i] - q[:, i - 1]
             ok = (q[:, i] > 0) & (q[:, i - 1] > 0)
             rows["req: " + REQ_STAMPS[i]] = float(np.median(d[ok])) if ok.any() else None
+        for a_, b_, name in ((3, 6, "req:   (wait) top-k barrier -> replay starts"), (6, 7, "req:   replay: copy commit state"),
+                             (7, 8, "req:   replay: pops"), (8, 9, "req:   replay: publish")):
+            ok = (q[:, a_] > 0) & (q[:, b_] > 0)
+            rows[name] = float(np.median((q[:, b_] - q[:, a_])[ok])) if ok.any() else None
+        rows["req:   replay: pops per step (median)"] = float(np.median(q[:, 10]))
+        rows["req:   replay: active mask at pop 1"] = hex(int(q[1, 11]))
+        rows["req:   replay: pop 1 arg-max collectives (SM cycles)"] = float(np.median(q[:, 12]))
+        rows["req:   replay: pop 1 whole (SM cycles)"] = float(np.median(q[:, 13]))
         ok = (q[:, 0] > 0) & (g[:, 7] > 0)
         rows["hop: flag released -> request sees flags"] = float(np.median((q[:, 0] - g[:, 7])[ok])) if ok.any() else None
         gn = t[0, 2:max(steps, 3)]

@@ -42,10 +42,11 @@ constexpr int kWvNP = 64;                       // items per GRU pass (M = 128 o
 constexpr int kWvKC = 128;                      // k per ring slot (two 64-wide swizzle blocks)
 constexpr int kWvRingBytes = 96 * 1024;         // state ring: three 128-row chunks, or more slots of fewer rows
 constexpr int kWvCS = 4;                        // GRU CTAs per thread-block cluster
+constexpr int kWvLdH = 68;                      // floats per row of the pre-activation buffer (64 nodes + pad)
 constexpr int kWvDescWords = 16;                // u64 words per request descriptor: header + 15 items, one 128-byte line
 constexpr int kWvMaxW = kWvDescWords - 1;
 constexpr int kWvMaxBatch = 128;                // requests per launch (headers are polled by four warps)
-constexpr int kWvTmemCols = 512;                // D1[w] at 64 w (48 columns each, w < 2), D2 at 256 (rpc <= 64 columns)
+constexpr int kWvTmemCols = 512;                // 4 or 8 independent D1 accumulators of N <= 128 / 64 columns; D2 reuses column 0 ..
 constexpr int kWvMaxSlices = 8;
 constexpr unsigned int kWvAct = 0x100u;         // replay word: cursor (8) | active (1) | pop slot (16, from bit 16)
 
@@ -98,7 +99,12 @@ __device__ __forceinline__ unsigned long long wave_timer() {
 constexpr int kWvTraceSteps = 64, kWvTraceStamps = 16;
 #ifdef DT_TRACE
 __device__ unsigned long long g_wv_trace[2][kWvTraceSteps][kWvTraceStamps];
-#define WV_TR(role, cond, step, i) do { if (threadIdx.x == 0 && (cond) && (step) < kWvTraceSteps) g_wv_trace[role][step][i] = wave_timer(); } while (0)
+__device__ unsigned long long g_wv_trace_sink[kWvThreads];
+// branch-free on purpose: a thread-0-only branch would leave its warp diverged and slow every warp collective after it
+#define WV_TR(role, cond, step, i) do { \
+        const bool wv_on__ = (threadIdx.x == 0) && (cond) && (step) < kWvTraceSteps; \
+        unsigned long long *wv_dst__ = wv_on__ ? &g_wv_trace[role][wv_on__ ? (step) : 0][i] : &g_wv_trace_sink[threadIdx.x]; \
+        *wv_dst__ = wave_timer(); } while (0)
 #else
 #define WV_TR(role, cond, step, i) do { } while (0)
 #endif
@@ -121,7 +127,7 @@ __host__ __device__ inline size_t wave_gru_smem(int g, int r) {
     (void)r16;
     const size_t rpc = (size_t)16 * ((r + 16 * kWvCS - 1) / (16 * kWvCS));
     return (size_t)48 * g * 2 + (size_t)kWvRingBytes + (size_t)kWvCS * 4096 + (size_t)kWvCS * rpc * 32 +
-           (size_t)(5 * kWvNP + 3 * kWvMaxBatch + 8) * 4 + 12 * 8 + 64 + 1024;
+           (size_t)(5 * kWvNP + 3 * kWvMaxBatch + 8) * 4 + 20 * 8 + 64 + 1024;
 }
 __host__ __device__ inline size_t wave_slice_bytes(int r, int M) {
     return (size_t)((M + 7) / 8) * (size_t)((r + 63) / 64) * 1024;
@@ -131,7 +137,7 @@ __host__ __device__ inline size_t wave_req_smem(int r, int M, int N, int k, int 
     size_t s = (size_t)n_slices * wave_slice_bytes(r, M) + 2 * al((size_t)n_slices * M * 4);
     s += al((size_t)e_max * k * 8) + al((size_t)e_max * k * 2) + 4 * al((size_t)e_max * 4) + 2 * al((size_t)e_max * 4) + al((size_t)e_max * 8);
     s += 4 * al((size_t)N * 4);
-    s += al((size_t)W * r * 4) + al((size_t)W * M * 4);
+    s += al((size_t)W * r * 4) + al((size_t)W * M * 4) + al((size_t)W * M * 8) + al((size_t)W * M);
     s += al((size_t)4 * kWvMaxW * 4) + al(256);
     return s + 1024;
 }
@@ -164,20 +170,6 @@ __device__ __forceinline__ void wave_st_cluster_v2(uint32_t addr, uint2 v) {
 __device__ __forceinline__ void wave_cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void wave_cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
-// six 8-column TMEM loads (three gates x two accumulators) and one wait
-__device__ __forceinline__ void wave_tmem_ld_gates(uint32_t t0, uint32_t t1, float (&v)[48]) {
-    uint32_t r[48];
-#define WV_LD8(base, off, i)                                                                                   \
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"              \
-                 : "=r"(r[i]), "=r"(r[i + 1]), "=r"(r[i + 2]), "=r"(r[i + 3]), "=r"(r[i + 4]), "=r"(r[i + 5]), \
-                   "=r"(r[i + 6]), "=r"(r[i + 7]) : "r"((base) + (off)) : "memory")
-    WV_LD8(t0, 0, 0); WV_LD8(t0, 16, 8); WV_LD8(t0, 32, 16);
-    WV_LD8(t1, 0, 24); WV_LD8(t1, 16, 32); WV_LD8(t1, 32, 40);
-#undef WV_LD8
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-    for (int i = 0; i < 48; ++i) v[i] = __uint_as_float(r[i]);
-}
 __device__ __forceinline__ void wave_tmem_ld16(uint32_t taddr, float (&v)[16]) {
     uint32_t r[16];
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
@@ -187,6 +179,25 @@ __device__ __forceinline__ void wave_tmem_ld16(uint32_t taddr, float (&v)[16]) {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
     for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
+// make the mbarrier count this thread's earlier cp.async copies: it arrives once they have landed (the barrier's expected
+// count includes these arrivals)
+__device__ __forceinline__ void wave_cp_async_arrive(uint32_t mbar_addr) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(mbar_addr) : "memory");
+}
+__device__ __forceinline__ void wave_tmem_ld16x2(uint32_t ta, uint32_t tb, float (&va)[16], float (&vb)[16]) {
+    uint32_t r[32];
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                 : "r"(ta) : "memory");
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+                   "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+                 : "r"(tb) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { va[i] = __uint_as_float(r[i]); vb[i] = __uint_as_float(r[16 + i]); }
 }
 template <int N> __device__ __forceinline__ void wave_cp_wait_n(int n) {
     if (n >= N) cp_async_wait<N>();
@@ -203,12 +214,11 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
     const int n_kc = g / kWvKC;
     const int rpc = p.rpc;                                             // rows of W1 this CTA reduces (multiple of 16)
 
-    // carve (smem_raw is 1024-byte aligned by the kernel).  The M = 128 MMA always reads 16 row groups per k-block; when a
-    // pass has fewer rows the ring is packed tighter and those phantom reads run past the k-block, at the end of the ring
-    // into sS2 (valid memory, results of phantom rows are never used).
+    // carve (smem_raw is 1024-byte aligned by the kernel)
     unsigned char *sW = smem_raw;                                     // W_hh slice, K-major sw128: [6 row groups][g/64 atoms][1 KB]
     const uint32_t sboW = (uint32_t)g * 16;                           // bytes between 8-row groups
-    unsigned char *sRing = sW + (size_t)48 * g * 2;                   // [slot][2 k-blocks][G row groups][1 KB]
+    unsigned char *sRing = sW + (size_t)48 * g * 2;                   // [slot][2 k-blocks][N / 8 row groups][1 KB]
+    float *sH = reinterpret_cast<float *>(sRing);                    // [48][kWvLdH] hidden-half pre-activations (aliases the ring after D1)
     unsigned char *sS2 = sRing + kWvRingBytes;                        // [kWvCS][16 groups][2 k-halves][8 rows][16 B]: new states of
                                                                       // the cluster's 16 kWvCS units (block c written by rank c)
     unsigned char *sW1 = sS2 + (size_t)kWvCS * 4096;                  // [kWvCS][rpc/8 groups][2 k-halves][8 rows][16 B]
@@ -220,8 +230,8 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
     int *sCnt = sPz + kWvNP;                                          // [128] items per request this step
     int *sOff = sCnt + kWvMaxBatch;                                   // [129] exclusive prefix
     int *sFirst = sOff + kWvMaxBatch + 4;                             // [128] first new state slot per request
-    unsigned long long *mbar = reinterpret_cast<unsigned long long *>(sFirst + kWvMaxBatch);   // [0..7] slot free, [8] D1, [9] D2
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(mbar + 12);
+    unsigned long long *mbar = reinterpret_cast<unsigned long long *>(sFirst + kWvMaxBatch);   // [0..7] slot full, [8] D1, [9] D2, [10..17] slot empty
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(mbar + 20);
     int *sCtl = reinterpret_cast<int *>(tmem_slot + 2);               // [0] items this step, [1] requests not done, [2] abort, [4..7] live masks
 
     {   // resident weights
@@ -243,8 +253,8 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
         }
         for (int i = tid; i < kWvCS * 1024; i += kWvThreads) reinterpret_cast<uint32_t *>(sS2)[i] = 0u;
         if (tid == 0) {
-            for (int i = 0; i < 8; ++i) tc::mbar_init(tc::smem_u32(mbar + i), 2);
-            tc::mbar_init(tc::smem_u32(mbar + 8), 2);
+            for (int i = 0; i < 8; ++i) { tc::mbar_init(tc::smem_u32(mbar + i), kWvThreads - 128); tc::mbar_init(tc::smem_u32(mbar + 10 + i), 4); }
+            tc::mbar_init(tc::smem_u32(mbar + 8), 4);
             tc::mbar_init(tc::smem_u32(mbar + 9), 1);
             tc::mbar_init_fence();
             sCtl[2] = 0;
@@ -258,11 +268,11 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
     wave_cluster_arrive();                                            // peers' sS2 is zeroed before anyone stores into it
     wave_cluster_wait();
     const uint32_t tmem = *tmem_slot;
-    const uint32_t idesc1 = tc::make_idesc_bf16(128, 48), idesc2 = tc::make_idesc_bf16(128, rpc);
+    const uint32_t idesc2 = tc::make_idesc_bf16(128, rpc);
     const uint32_t mb0 = tc::smem_u32(mbar);
     const uint64_t descW0 = tc::make_desc_sw128(tc::smem_u32(sW), sboW), descR0 = tc::make_desc_sw128(tc::smem_u32(sRing), 1024);
     const uint64_t descS2 = tc::make_desc(tc::smem_u32(sS2), 128, 256), descW1 = tc::make_desc(tc::smem_u32(sW1), 128, 256);
-    uint32_t ph_free = 0, ph_d1 = 0, ph_d2 = 0;                    // mbarrier phases (uniform across the CTA)
+    uint32_t ph_full = 0, ph_empty = 0, ph_d1 = 0, ph_d2 = 0;      // mbarrier phases (each role keeps the bits of the barriers it waits on)
     bool pend2 = false;                                             // a cluster arrive (sS2 consumed) awaits its wait
 
     // epilogue geometry: TMEM lane quadrant q4, unit half hsel; lanes 0..15 hold the hi rows of nodes 16 q4 + lane,
@@ -285,6 +295,9 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
         }
     }
 
+    // every GRU CTA walks the K chunks of a pass in its own rotation: 64 CTAs asking L2 for the same lines at the same
+    // moment is a hot spot; the order depends on the CTA only, never on the batch, so results stay batch-invariant
+    const int kshift = cta % n_kc;
     const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 10;
     for (int s = 0;; ++s) {
         // ---- headers of step s: one lane per request
@@ -345,32 +358,15 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
             __syncthreads();
             WV_TR(0, cta == 0 && p0 == 0, s, 1);
 
-            // ---- ring geometry of this pass: G row groups per k-block (16 nodes fill 4), as many slots as fit
-            const int G = 4 * ((n + 15) >> 4);
-            const int kb_bytes = G * 1024, slot_bytes = 2 * kb_bytes;
+            // ---- this pass: the parents' states are operand B of D1[64 x N] = W_hh slice . [S_hi | S_lo]^T with N = 2 nh columns
+            // (hi halves of the nh = 4 ceil(n / 4) nodes, then their lo halves); ring slots of N / 8 row groups per k-block
+            const int nh = 4 * ((n + 3) >> 2), N = 2 * nh;
+            const int kb_bytes = (N >> 3) * 1024, slot_bytes = 2 * kb_bytes;
             const int nslot = min(min(n_kc, 8), kWvRingBytes / slot_bytes);
-            // this thread's share of a slot: 8 operand rows (rho = (tid >> 4) + 16 i), 16-byte piece tid & 15
-            const int piece = tid & 15, kb = piece >> 3, pc = piece & 7;
-            const __nv_bfloat16 *src[8];
-            uint32_t dsto[8];
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const int rho = (tid >> 4) + 16 * i;
-                const int node = 16 * (rho >> 5) + (rho & 15), hl = (rho >> 4) & 1;
-                src[i] = nullptr;
-                if (node < n) src[i] = (hl ? p.s_lo : p.s_hi) + (size_t)sRow[node] * g + (size_t)piece * 8;
-                dsto[i] = (uint32_t)(kb * kb_bytes + (rho >> 3) * 1024 + (rho & 7) * 128 + ((pc ^ (rho & 7)) << 4));
-            }
-            auto issue_chunk = [&](int kc) {
-                unsigned char *dst = sRing + (size_t)(kc % nslot) * slot_bytes;
-                const size_t k0 = (size_t)kc * kWvKC;
-#pragma unroll
-                for (int i = 0; i < 8; ++i)
-                    if (src[i]) cp_async16(dst + dsto[i], src[i] + k0);
-            };
-#pragma unroll 1
-            for (int kc = 0; kc < nslot; ++kc) { issue_chunk(kc); cp_async_commit(); }
-
+            const uint32_t idesc1 = tc::make_idesc_bf16(64, N);
+            // independent D1 accumulators, npad columns apart; the same four whatever N is, so that the association of the
+            // K sum (and with it every bit of the result) does not depend on how many nodes share the pass
+            constexpr int NA = 4, npad = kWvTmemCols / NA;
             // ---- epilogue operands (input half from P, previous state): issued now, consumed after the MMAs
             float4 pr = make_float4(0.f, 0.f, 0.f, 0.f), pz4 = pr, pn = pr, hp = pr;
             const bool mine = (my_node < n);
@@ -383,52 +379,90 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
             }
             WV_TR(0, cta == 0 && p0 == 0, s, 2);
 
-            // ---- D1[128 x 48] = [S_hi | S_lo rows] . W_hh slice^T, K streamed through the ring.  Chunk j sits in cp.async
-            // group j; the slot of chunk kc - 1 is refilled one iteration after its MMAs were issued.
-#pragma unroll 1
-            for (int kc = 0; kc < n_kc; ++kc) {
-                wave_cp_wait_n<7>(kc == 0 ? nslot - 1 : nslot - 2);
-                tc::fence_proxy_async();
-                __syncthreads();
-                const int sl = kc % nslot;
-                if (warp < 2 && lane == 0) {
-                    // warp w issues K = 16 steps 4 w .. 4 w + 3 of the chunk's eight (= k-block w) into its own accumulator D1[w]
-                    tc::fence_after_sync();
+            // ---- D1[64 x N] = W_hh slice . [S_hi | S_lo]^T, K streamed through the ring by a warp-specialised pipeline with no
+            // CTA barrier inside: warps 2..7 produce (cp.async into the slot, completion tracked by the slot's `full`
+            // mbarrier), lane 0 of warps 0 and 1 consume (tcgen05.mma, tcgen05.commit on the slot's `empty` mbarrier).
+            if (warp >= 4) {
+                // producer: 16-byte piece ptid & 15 of operand rows rho = (ptid >> 4) + 8 i
+                const int ptid = tid - 128, piece = ptid & 15, kb = piece >> 3, pc = piece & 7;
+                const __nv_bfloat16 *src[16];
 #pragma unroll
-                    for (int s4 = 0; s4 < 4; ++s4) {
-                        const uint64_t da = descR0 + (uint64_t)((sl * slot_bytes + warp * kb_bytes) / 16 + s4 * 2);
-                        const uint64_t db = descW0 + (uint64_t)((kc * 2 + warp) * 64 + s4 * 2);
-                        tc::mma_bf16(tmem + 64 * warp, da, db, idesc1, (kc | s4) ? 1u : 0u);
+                for (int i = 0; i < 16; ++i) {
+                    const int rho = (ptid >> 4) + 8 * i;
+                    const int hl = (rho >= nh), node = rho - (hl ? nh : 0);
+                    src[i] = nullptr;
+                    if (rho < N && node < n) src[i] = (hl ? p.s_lo : p.s_hi) + (size_t)sRow[node] * g + (size_t)piece * 8;
+                }
+                const int r7 = (ptid >> 4) & 7;                      // rho & 7 is the same for all 16 rows of a thread
+                const uint32_t doff = (uint32_t)(kb * kb_bytes + r7 * 128 + ((pc ^ r7) << 4));
+#pragma unroll 1
+                for (int kc = 0; kc < n_kc; ++kc) {
+                    const int sl = kc % nslot;
+                    if (kc >= nslot) {                           // the MMAs of the slot's previous chunk have read it
+                        tc::mbar_wait(mb0 + 80 + 8 * sl, (ph_empty >> sl) & 1u);
+                        ph_empty ^= 1u << sl;
                     }
-                    if (kc + nslot < n_kc) tc::commit(mb0 + 8 * sl);             // this slot is refilled next iteration
+                    unsigned char *dst = sRing + (size_t)sl * slot_bytes + doff;
+                    const size_t k0 = (size_t)((kc + kshift) % n_kc) * kWvKC;
+#pragma unroll
+                    for (int i = 0; i < 16; ++i)
+                        if (src[i]) cp_async16(dst + i * 1024, src[i] + k0);   // rho >> 3 = i
+                    wave_cp_async_arrive(mb0 + 8 * sl);
+                }
+            } else if (lane == 0) {
+                // consumer: warp w issues K = 16 steps 2 w, 2 w + 1 of every chunk into its own accumulator D1[w] (a thread needs
+                // ~120 cycles to issue one tcgen05.mma and ~200 for a commit, so four threads share the work)
+                const int kbw = warp >> 1, s40 = (warp & 1) * 2;
+#pragma unroll 1
+                for (int kc = 0; kc < n_kc; ++kc) {
+                    const int sl = kc % nslot;
+                    tc::mbar_wait(mb0 + 8 * sl, (ph_full >> sl) & 1u);
+                    ph_full ^= 1u << sl;
+                    tc::fence_proxy_async();
+                    tc::fence_after_sync();
+                    const uint64_t da = descW0 + (uint64_t)((((kc + kshift) % n_kc) * 2 + kbw) * 64 + s40 * 2);
+                    const uint64_t db = descR0 + (uint64_t)((sl * slot_bytes + kbw * kb_bytes) / 16 + s40 * 2);
+                    tc::mma_bf16(tmem + warp * npad, da, db, idesc1, kc ? 1u : 0u);
+                    tc::mma_bf16(tmem + warp * npad, da + 2, db + 2, idesc1, 1u);
+                    if (kc + nslot < n_kc) tc::commit(mb0 + 80 + 8 * sl);        // this slot will be refilled
                     if (kc == n_kc - 1) tc::commit(mb0 + 64);
                 }
-                if (kc >= 1) {
-                    if (kc - 1 + nslot < n_kc) {                 // refill the previous chunk's slot once its MMAs have read it
-                        const int slp = (kc - 1) % nslot;
-                        tc::mbar_wait(mb0 + 8 * slp, (ph_free >> slp) & 1u);
-                        ph_free ^= 1u << slp;
-                        issue_chunk(kc - 1 + nslot);
-                    }
-                    cp_async_commit();
-                }
             }
-            cp_async_wait<0>();
+            __syncwarp();
             tc::mbar_wait(mb0 + 64, ph_d1); ph_d1 ^= 1u;
             tc::fence_after_sync();
             __syncwarp();
             WV_TR(0, cta == 0 && p0 == 0, s, 3);
 
-            // ---- gates (reading A2): columns gate * 16 + unit of the two accumulators, hi + lo rows added
-            float acc[24];
-            {
-                float v[48];
-                wave_tmem_ld_gates(tmem + tlane + 8 * hsel, tmem + tlane + 64 + 8 * hsel, v);
+            // ---- TMEM -> shared: an M = 64 accumulator keeps row 16 q + i in lane 32 q + i (i < 16), so quadrant q holds gate q
+            // (r, z, n) of the 16 units; the two accumulators and the hi / lo column blocks are added here (fixed order)
+            if (q4 < 3 && 16 * hsel < nh) {
+#pragma unroll 1
+                for (int c16 = hsel; 16 * c16 < nh; c16 += 2) {
+                    float v0[16], v1[16], v2[16];
 #pragma unroll
-                for (int c = 0; c < 24; ++c) acc[c] = v[c] + v[24 + c];
+                    for (int c = 0; c < 16; ++c) v0[c] = 0.f;
+#pragma unroll 1
+                    for (int a = 0; a < NA; ++a) {                   // accumulators in index order, hi then lo column block
+                        wave_tmem_ld16x2(tmem + tlane + a * npad + 16 * c16, tmem + tlane + a * npad + nh + 16 * c16, v1, v2);
+#pragma unroll
+                        for (int c = 0; c < 16; ++c) v0[c] += v1[c] + v2[c];
+                    }
+                    if (lane < 16) {
+                        float4 *dst = reinterpret_cast<float4 *>(sH + (size_t)(16 * q4 + lane) * kWvLdH + 16 * c16);
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) dst[c] = make_float4(v0[4 * c], v0[4 * c + 1], v0[4 * c + 2], v0[4 * c + 3]);
+                    }
+                }
             }
+            tc::fence_before_sync();
+            __syncthreads();
+            // ---- gates (reading A2): thread = (node 16 q4 + il, units 8 hsel + 4 uh ..)
+            float acc[12];
 #pragma unroll
-            for (int c = 0; c < 24; ++c) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 16);
+            for (int gate = 0; gate < 3; ++gate)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) acc[gate * 4 + c] = sH[(size_t)(16 * gate + my_u + c) * kWvLdH + my_node];
             {
                 const float prv[4] = {pr.x, pr.y, pr.z, pr.w}, pzv[4] = {pz4.x, pz4.y, pz4.z, pz4.w};
                 const float pnv[4] = {pn.x, pn.y, pn.z, pn.w}, hpv[4] = {hp.x, hp.y, hp.z, hp.w};
@@ -436,9 +470,9 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                 __nv_bfloat16 bh[4], bl[4];
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
-                    const float rg = sigmoidf_fast(prv[c] + (uh ? acc[4 + c] : acc[c]));
-                    const float zg = sigmoidf_fast(pzv[c] + (uh ? acc[12 + c] : acc[8 + c]));
-                    const float ng = tanhf_fast(pnv[c] + rg * (uh ? acc[20 + c] : acc[16 + c]));
+                    const float rg = sigmoidf_fast(prv[c] + acc[c]);
+                    const float zg = sigmoidf_fast(pzv[c] + acc[4 + c]);
+                    const float ng = tanhf_fast(pnv[c] + rg * acc[8 + c]);
                     hn[c] = mine ? ((1.0f - zg) * ng + zg * hpv[c]) : 0.f;
                     bh[c] = __float2bfloat16_rn(hn[c]);
                     bl[c] = __float2bfloat16_rn(hn[c] - __bfloat162float(bh[c]));
@@ -471,7 +505,7 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                 tc::fence_after_sync();
 #pragma unroll
                 for (int c = 0; c < kWvCS; ++c)
-                    tc::mma_bf16(tmem + 256, descS2 + (uint64_t)(c * 256), descW1 + (uint64_t)(c * rpc * 2), idesc2, c ? 1u : 0u);
+                    tc::mma_bf16(tmem, descS2 + (uint64_t)(c * 256), descW1 + (uint64_t)(c * rpc * 2), idesc2, c ? 1u : 0u);   // D1's columns are dead
                 tc::commit(mb0 + 72);
             }
             tc::mbar_wait(mb0 + 72, ph_d2); ph_d2 ^= 1u;
@@ -485,7 +519,7 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
 #pragma unroll 1
                 for (int blk = hsel; blk < rpc / 16; blk += 2) {
                     float v[16];
-                    wave_tmem_ld16(tmem + tlane + 256 + 16 * blk, v);
+                    wave_tmem_ld16(tmem + tlane + 16 * blk, v);
 #pragma unroll
                     for (int c = 0; c < 16; ++c) v[c] += __shfl_xor_sync(0xffffffffu, v[c], 16);
                     if (mine) {
@@ -554,6 +588,8 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
     float *nSco = reinterpret_cast<float *>(carve((size_t)N * 4));
     float *sA = reinterpret_cast<float *>(carve((size_t)W * r * 4));
     float *sZ = reinterpret_cast<float *>(carve((size_t)W * M * 4));
+    unsigned long long *sKey = reinterpret_cast<unsigned long long *>(carve((size_t)W * M * 8));   // (z, ~token) of every candidate
+    unsigned char *sRank = carve((size_t)W * M);
     int *itE = reinterpret_cast<int *>(carve((size_t)4 * kWvMaxW * 4));
     int *itTok = itE + kWvMaxW, *itPs = itTok + kWvMaxW;
     WaveCtl &ctl = *reinterpret_cast<WaveCtl *>(carve(256));
@@ -562,24 +598,31 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
     unsigned long long *my_desc = p.desc + (size_t)b * kWvDescWords;
 
     // fill the slices listed in ctl.stage with the candidate table of their depth: ids, base logits, the M rows of W2
+    // (compact code on purpose: the step loop has to stay inside the instruction cache)
     auto stage_slices = [&]() {
         const int ns = ctl.n_stage;
+#pragma unroll 1
         for (int q = 0; q < ns; ++q) {
             const int si = ctl.stage[q];
             const size_t row = (size_t)b * L + ctl.slDepth[si];
+#pragma unroll 1
             for (int m = tid; m < M; m += kWvThreads) {
                 slTok[si * M + m] = e.cand_id[row * M + m];
                 slBase[si * M + m] = e.cand_val[row * M + m];
             }
         }
         __syncthreads();
-        for (int q = 0; q < ns; ++q) {
-            const int si = ctl.stage[q];
-            unsigned char *dst = sW2 + (size_t)si * slice_bytes;
-            for (int i = tid; i < M * nvec; i += kWvThreads) {
-                const int m = i / nvec, v = i - m * nvec;
-                cp_async16(dst + (size_t)(m >> 3) * Ka * 1024 + (size_t)(v >> 3) * 1024 + (m & 7) * 128 + (((v & 7) ^ (m & 7)) << 4),
-                           w2 + (size_t)slTok[si * M + m] * r + (size_t)v * 8);
+        const int v = tid % nvec, m0 = tid / nvec, dm = kWvThreads / nvec;   // a thread keeps its 16-byte piece, rows m0, m0 + dm, ..
+        if (m0 < dm) {
+#pragma unroll 1
+            for (int q = 0; q < ns; ++q) {
+                const int si = ctl.stage[q];
+                unsigned char *dst = sW2 + (size_t)si * slice_bytes + (size_t)(v >> 3) * 1024;
+                const int *tk = slTok + si * M;
+#pragma unroll 2
+                for (int m = m0; m < M; m += dm)
+                    cp_async16(dst + (size_t)(m >> 3) * Ka * 1024 + (m & 7) * 128 + (((v & 7) ^ (m & 7)) << 4),
+                               w2 + (size_t)tk[m] * r + (size_t)v * 8);
             }
         }
         cp_async_commit();
@@ -604,6 +647,12 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
 
     for (int s = 0;; ++s) {
         const int n_it = ctl.n_items;
+        // C = H W1h^T of the item's depth does not depend on the GRU CTAs: fetch it while waiting for them (A12: row = depth)
+        float4 cpre = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (tid < n_it * (r >> 2)) {
+            const int j = tid / (r >> 2), jq = tid - j * (r >> 2);
+            cpre = __ldg(reinterpret_cast<const float4 *>(e.C + ((size_t)b * L + eDep[itE[j]]) * r) + jq);
+        }
         if (warp == 0) {
             bool ok = true;
             for (int q = lane; q < p.n_gru; q += 32) {
@@ -620,23 +669,24 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
         // one thread per (item, four columns), all loads of a thread in flight at once
         {
             const int r4 = r >> 2;
+#pragma unroll 1
             for (int pair = tid; pair < n_it * r4; pair += kWvThreads) {
                 const int j = pair / r4, jq = pair - j * r4;
-                const int x = itE[j];
-                const float4 cv = __ldg(reinterpret_cast<const float4 *>(e.C + ((size_t)b * L + eDep[x]) * r) + jq);   // H_{depth+1} <-> row depth (A12)
+                const float4 cv = (pair == tid) ? cpre : __ldg(reinterpret_cast<const float4 *>(e.C + ((size_t)b * L + eDep[itE[j]]) * r) + jq);
                 const float4 *pp = reinterpret_cast<const float4 *>(p.partial + ((size_t)(b * kWvMaxW + j) * P) * r) + jq;
                 float4 s0 = make_float4(0.f, 0.f, 0.f, 0.f), s1 = s0;
                 int q = 0;
-                for (; q + 8 <= P; q += 8) {
-                    float4 v[8];
+                for (; q + 16 <= P; q += 16) {
+                    float4 v[16];
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) v[i] = __ldcg(pp + (size_t)(q + i) * r4);
+                    for (int i = 0; i < 16; ++i) v[i] = __ldcg(pp + (size_t)(q + i) * r4);
 #pragma unroll
-                    for (int i = 0; i < 8; i += 2) {
+                    for (int i = 0; i < 16; i += 2) {
                         s0.x += v[i].x; s0.y += v[i].y; s0.z += v[i].z; s0.w += v[i].w;
                         s1.x += v[i + 1].x; s1.y += v[i + 1].y; s1.z += v[i + 1].z; s1.w += v[i + 1].w;
                     }
                 }
+#pragma unroll 1
                 for (; q < P; ++q) {
                     const float4 v = __ldcg(pp + (size_t)q * r4);
                     s0.x += v.x; s0.y += v.y; s0.z += v.z; s0.w += v.w;
@@ -653,6 +703,7 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
 
         // ---- z_m = ((base_m - base_0) + W2[cand_m, :] a) / T_eff   PAPER.md:143-144 (shift-invariant)
         // a warp takes 8 candidate rows (one swizzle row group), four lanes per row
+#pragma unroll 1
         for (int j = 0; j < n_it; ++j) {
             const int si = ctl.d2s[eDep[itE[j]]];
             const unsigned char *sl = sW2 + (size_t)si * slice_bytes;
@@ -660,9 +711,11 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
             const float base0 = bs[0];
             const float *aj = sA + (size_t)j * r;
             const int rw = lane & 7, qq = lane >> 3;
+#pragma unroll 1
             for (int rg = warp; rg < (M + 7) / 8; rg += kWvThreads / 32) {
                 const unsigned char *rowp = sl + (size_t)rg * Ka * 1024 + rw * 128;
                 float acc = 0.f;
+#pragma unroll 2
                 for (int v = qq; v < nvec; v += 4) {
                     const uint4 q = *reinterpret_cast<const uint4 *>(rowp + (size_t)(v >> 3) * 1024 + (((v & 7) ^ rw) << 4));
                     const float4 a0 = *reinterpret_cast<const float4 *>(aj + (size_t)v * 8);
@@ -675,54 +728,69 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                 acc += __shfl_xor_sync(0xffffffffu, acc, 8);
                 acc += __shfl_xor_sync(0xffffffffu, acc, 16);
                 const int m = 8 * rg + rw;
-                if (qq == 0 && m < M) sZ[(size_t)j * M + m] = __fdiv_rn((bs[m] - base0) + acc, e.T_eff);
+                if (qq == 0 && m < M) {
+                    const float z = __fdiv_rn((bs[m] - base0) + acc, e.T_eff);
+                    sZ[(size_t)j * M + m] = z;
+                    sKey[(size_t)j * M + m] = ((unsigned long long)ord_key(z) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned int)slTok[si * M + m]);
+                }
             }
         }
         __syncthreads();
         WV_TR(1, b == 0, s, 2);
 
-        // ---- slice log-softmax (reading A1) and top-k by (logp desc, token asc): one warp per node, candidates in
-        // registers (lane holds m = lane + 32 i), k rounds of a warp-wide arg-max
+        // ---- top-k by (z desc, token asc): rank by counting over the sortable keys, `tpc` neighbouring lanes per candidate
+        {
+            const int tot = n_it * M;
+            int tpc = 1;
+            while (tpc < 8 && tot * tpc * 2 <= kWvThreads) tpc <<= 1;
+            const int per = (M + tpc - 1) / tpc;
+#pragma unroll 1
+            for (int base = 0; base < tot * tpc; base += kWvThreads) {      // block-uniform trip count
+                const int idx = base + tid, pair = idx / tpc, part = idx - pair * tpc;
+                const bool act = pair < tot;
+                const int j = act ? pair / M : 0, m = act ? pair - j * M : 0;
+                const unsigned long long *kj = sKey + (size_t)j * M;
+                const unsigned long long mk = kj[m];
+                int rank = 0;
+                if (act) {
+                    const int m0 = part * per, m1 = min(M, m0 + per);
+                    int q = m0;
+                    if (!(m0 & 1))
+#pragma unroll 4
+                        for (; q + 2 <= m1; q += 2) {
+                            const ulonglong2 o = *reinterpret_cast<const ulonglong2 *>(kj + q);
+                            rank += (o.x > mk) + (o.y > mk);
+                        }
+#pragma unroll 1
+                    for (; q < m1; ++q) rank += (kj[q] > mk);
+                }
+                for (int o = 1; o < tpc; o <<= 1) rank += __shfl_xor_sync(0xffffffffu, rank, o);
+                if (act && part == 0) sRank[(size_t)j * M + m] = (unsigned char)min(rank, 255);
+            }
+        }
+        __syncthreads();
+        // ---- slice log-softmax (reading A1) and the children list: one warp per node
+#pragma unroll 1
         for (int j = warp; j < n_it; j += kWvThreads / 32) {
             const int x = itE[j];
-            const int si = ctl.d2s[eDep[x]];
             const float *zj = sZ + (size_t)j * M;
-            const int *tk = slTok + si * M;
-            float zl[8];
-            unsigned int tl[8];
             float zmax = -INFINITY;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const int m = lane + 32 * i;
-                zl[i] = (m < M) ? zj[m] : -INFINITY;
-                tl[i] = (m < M) ? (unsigned int)tk[m] : 0xFFFFFFFFu;
-                zmax = fmaxf(zmax, zl[i]);
-            }
+#pragma unroll 1
+            for (int m = lane; m < M; m += 32) zmax = fmaxf(zmax, zj[m]);
             zmax = warp_max(zmax);
             float ssum = 0.f;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) if (lane + 32 * i < M) ssum += expf(zl[i] - zmax);
+#pragma unroll 1
+            for (int m = lane; m < M; m += 32) ssum += expf(zj[m] - zmax);
             ssum = warp_sum(ssum);
             const float lse = logf(ssum);
             const float gpar = eSco[x];
             unsigned long long *ck = cKey + (size_t)x * k;
-            unsigned int taken = 0u;
-            for (int rk = 0; rk < k; ++rk) {
-                unsigned int bz = 0u, bt = 0xFFFFFFFFu;
-                int bi = -1;
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    if (lane + 32 * i >= M || ((taken >> i) & 1u)) continue;
-                    const unsigned int kz = ord_key(zl[i]);
-                    if (bi < 0 || kz > bz || (kz == bz && tl[i] < bt)) { bz = kz; bt = tl[i]; bi = i; }
-                }
-                const unsigned int mz = __reduce_max_sync(0xffffffffu, bi >= 0 ? bz : 0u);
-                const bool el = (bi >= 0) && bz == mz;
-                const unsigned int mt = __reduce_min_sync(0xffffffffu, el ? bt : 0xFFFFFFFFu);
-                if (el && bt == mt) {                               // tokens of one slice are distinct: exactly one lane
-                    taken |= 1u << bi;
-                    const float lpm = (zl[bi] - zmax) - lse;
-                    ck[rk] = ((unsigned long long)ord_key(gpar + lpm) << 32) | (unsigned long long)(0xFFFFFFFFu - bt);
+#pragma unroll 1
+            for (int m = lane; m < M; m += 32) {
+                const int rank = sRank[(size_t)j * M + m];
+                if (rank < k) {
+                    const float lpm = (zj[m] - zmax) - lse;
+                    ck[rank] = ((unsigned long long)ord_key(gpar + lpm) << 32) | (sKey[(size_t)j * M + m] & 0xFFFFFFFFull);
                 }
             }
             __syncwarp();
@@ -731,6 +799,7 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
             int rk2 = 0;
             if (lane < k) {
                 mk = ck[lane];
+#pragma unroll 1
                 for (int q = 0; q < k; ++q) rk2 += (ck[q] > mk);
             }
             __syncwarp();
@@ -741,73 +810,100 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
 
         // ---- replay the heap from the commit point, nominate, publish (warp 0)
         if (warp == 0) {
+            WV_TR(1, b == 0, s, 6);
             const int n_exp = ctl.n_exp;
             int t = ctl.c;
+            int n_pops = 0;
             if (s == 0 && lane == 0) { simC[0] = kWvAct; }          // the root is slot 0; its children are known now
             __syncwarp();
+#pragma unroll 1
             for (int x = lane; x < n_exp; x += 32) {
                 const unsigned int w = simC[x];
                 simT[x] = w;
                 hT[x] = ((w & kWvAct) && (int)(w & 0xFFu) < k) ? cKey[(size_t)x * k + (w & 0xFFu)] : 0ull;
             }
             __syncwarp();
+            WV_TR(1, b == 0, s, 7);
             bool committing = true, finished = false;
-            int found = 0;
+            int found = 0, c_new = t;
             const int step_next = s + 1;
             while (true) {
                 if (t >= B) { finished = committing; break; }
+                // every lane scans the lists it owns and keeps the best head with what the pop needs to know about it
                 unsigned long long bk = 0ull;
-                unsigned int bps = 0xFFFFFFFFu;
+                unsigned int bw = 0u;
                 int be = -1;
+#pragma unroll 1
                 for (int x = lane; x < n_exp; x += 32) {
                     const unsigned long long key = hT[x];
                     if (key == 0ull) continue;
-                    const unsigned int ps = simT[x] >> 16;
-                    if (be < 0 || key > bk || (key == bk && ps < bps)) { bk = key; bps = ps; be = x; }
+                    const unsigned int w = simT[x];
+                    if (be < 0 || key > bk || (key == bk && (w >> 16) < (bw >> 16))) { bk = key; bw = w; be = x; }
                 }
+#ifdef DT_TRACE
+                const unsigned int wv_am = __activemask();
+                const bool wv_pr = (b == 0 && s < kWvTraceSteps && n_pops == 1 && lane == 0);
+                *(wv_pr ? &g_wv_trace[1][wv_pr ? s : 0][11] : &g_wv_trace_sink[threadIdx.x]) = wv_am;
+                const long long ck0 = clock64();
+#endif
                 if (__ballot_sync(0xffffffffu, be >= 0) == 0u) { finished = committing; break; }   // the candidate tree ran dry
                 // pop comparator of reading A8: score desc, token asc, parent slot asc
                 const unsigned int hi = (be >= 0) ? (unsigned int)(bk >> 32) : 0u;
                 const unsigned int mh = __reduce_max_sync(0xffffffffu, hi);
                 bool el = (be >= 0) && hi == mh;
-                const unsigned int lo = el ? (unsigned int)(bk & 0xFFFFFFFFull) : 0u;
-                const unsigned int ml = __reduce_max_sync(0xffffffffu, lo);
-                el = el && lo == ml;
-                const unsigned int mp = __reduce_min_sync(0xffffffffu, el ? bps : 0xFFFFFFFFu);
-                el = el && bps == mp;
-                const int wl = __ffs(__ballot_sync(0xffffffffu, el)) - 1;
+                const unsigned int ml = __reduce_max_sync(0xffffffffu, el ? (unsigned int)(bk & 0xFFFFFFFFull) : 0u);
+                el = el && (unsigned int)(bk & 0xFFFFFFFFull) == ml;
+                unsigned int bal = __ballot_sync(0xffffffffu, el);
+                if (__popc(bal) > 1) {                              // the same token at the same score under two parents
+                    const unsigned int mp = __reduce_min_sync(0xffffffffu, el ? (bw >> 16) : 0xFFFFFFFFu);
+                    bal = __ballot_sync(0xffffffffu, el && (bw >> 16) == mp);
+                }
+                const int wl = __ffs(bal) - 1;
+#ifdef DT_TRACE
+                *(wv_pr ? &g_wv_trace[1][wv_pr ? s : 0][12] : &g_wv_trace_sink[threadIdx.x]) = (unsigned long long)(clock64() - ck0);
+#endif
+                // the winning lane looks up its node; the rest of the warp gets the few words it needs by shuffle
+                int jc = 0, dep = 0, x = -1;
+                if (lane == wl) {
+                    jc = (int)(bw & 0xFFu);
+                    dep = eDep[be] + 1;
+                    x = cExp[(size_t)be * k + jc];
+                }
                 const int es = __shfl_sync(0xffffffffu, be, wl);
-                const unsigned int wv = simT[es];
-                const int jc = (int)(wv & 0xFFu);
+                const unsigned int wv = __shfl_sync(0xffffffffu, bw, wl);
+                jc = __shfl_sync(0xffffffffu, jc, wl);
+                dep = __shfl_sync(0xffffffffu, dep, wl);
+                x = __shfl_sync(0xffffffffu, x, wl);
                 const int tok = (int)(0xFFFFFFFFu - ml);
-                const int dep = eDep[es] + 1;
-                const int x = cExp[(size_t)es * k + jc];
                 const bool needs = (x < 0) && dep < L && (t + 1 < B);
                 if (committing && needs) {                          // everything before this pop is final
+#pragma unroll 1
                     for (int y = lane; y < n_exp; y += 32) simC[y] = simT[y];
-                    if (lane == 0) ctl.c = t;
+                    c_new = t;
                     committing = false;
                     __syncwarp();
                 }
                 t += 1;
-                if (lane == 0) {
+                if (lane == wl) {
                     simT[es] = wv + 1u;
                     hT[es] = (jc + 1 < k) ? cKey[(size_t)es * k + jc + 1] : 0ull;
                     nTok[t] = tok; nPar[t] = (int)(wv >> 16); nDep[t] = dep; nSco[t] = ord_key_inv(mh);
                     if (x >= 0) { simT[x] = kWvAct | ((unsigned int)t << 16); hT[x] = cKey[(size_t)x * k]; }
                 }
-                if (needs && found < W) {                           // warp-uniform; lane 0 decides, the count is broadcast
+                bool stop = false;
+                if (needs) {                                        // warp-uniform; lane 0 decides, the verdict is broadcast
                     // resources: a state slot (speculative picks leave room for the expansions Algorithm 1 still needs)
                     // and a W2 slice for the node's depth
                     int add = 0;
                     if (lane == 0) {
                         const int xn = n_exp + found;
-                        bool can = (xn < e_max) && (found == 0 || xn + 1 + (B - ctl.c) <= e_max);
+                        bool can = (xn < e_max) && (found == 0 || xn + 1 + (B - c_new) <= e_max);
                         int si = -1;
                         if (can) {
                             si = ctl.d2s[dep];
                             if (si < 0) {
                                 int best = -1, bu = 0x7FFFFFFF;
+#pragma unroll 1
                                 for (int q = 0; q < nsl; ++q)
                                     if (ctl.slUsed[q] != step_next && ctl.slUsed[q] < bu) { bu = ctl.slUsed[q]; best = q; }
                                 si = best;
@@ -828,14 +924,24 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                             add = 1;
                         }
                     }
-                    found += __shfl_sync(0xffffffffu, add, 0);
+                    add = __shfl_sync(0xffffffffu, add, 0);
+                    found += add;
+                    stop = (add == 0) || found >= W;                // out of slots / slices, or the step is full
                 }
                 __syncwarp();
-                if (!committing && found >= W) break;
+#ifdef DT_TRACE
+                *(wv_pr ? &g_wv_trace[1][wv_pr ? s : 0][13] : &g_wv_trace_sink[threadIdx.x]) = (unsigned long long)(clock64() - ck0);
+#endif
+                n_pops += 1;
+                if (stop) break;
             }
+            WV_TR(1, b == 0, s, 8);
+#ifdef DT_TRACE
+            { const bool on = (threadIdx.x == 0 && b == 0 && s < kWvTraceSteps); *(on ? &g_wv_trace[1][on ? s : 0][10] : &g_wv_trace_sink[threadIdx.x]) = (unsigned long long)n_pops; }
+#endif
             if (finished) {
                 if (lane == 0) {
-                    ctl.done = 1; ctl.n_valid = t + 1; ctl.n_items = 0;
+                    ctl.done = 1; ctl.n_valid = t + 1; ctl.n_items = 0; ctl.c = t;
                     st_relaxed_u64(my_desc, wave_hdr_pack(rnd, s + 2, 0, 1, 0));
                     if (p.stats && b == 0) { p.stats[0] = (unsigned int)(s + 1); p.stats[1] = (unsigned int)n_exp; }
                 }
@@ -843,9 +949,10 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                 if (lane < found) st_relaxed_u64(my_desc + 1 + lane, wave_item_pack(rnd, s + 2, itPs[lane], min(max(itTok[lane], 0), e.V - 1)));
                 if (lane == 0) {
                     st_relaxed_u64(my_desc, wave_hdr_pack(rnd, s + 2, n_exp + 1, 0, found));
-                    ctl.n_items = found; ctl.n_exp = n_exp + found;
+                    ctl.n_items = found; ctl.n_exp = n_exp + found; ctl.c = c_new;
                 }
             }
+            WV_TR(1, b == 0, s, 9);
         }
         __syncthreads();
         WV_TR(1, b == 0, s, 4);
