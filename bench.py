@@ -460,10 +460,15 @@ def measure_sweep_and_arms(ctx):
 
 
 # ----------------------------------------------------------------------------------- in-kernel timeline
-GRU_STAMPS = ("headers seen", "item list built", "ring + P loads issued", "D1 in TMEM", "gates + states stored",
-              "D2 in TMEM", "partials stored", "flag released")
-REQ_STAMPS = ("flags seen", "a = SiLU(C + partials)", "W2 slice dots", "softmax + top-k", "replay + publish",
-              "slices staged (issue)")
+# (stamp index, what has happened by then), in program order, for GRU CTA 0 / request CTA 0 (dt_wave.cuh WV_TR)
+GRU_STAMPS = ((0, "items polled + compacted"), (1, "pass begins"), (2, "P / previous-state loads issued"),
+              (8, "issuer 0: first K chunk landed"), (9, "issuer 0: all tcgen05.mma + commit issued"), (3, "D1 complete (mbarrier)"),
+              (10, "TMEM loads, hi + lo shuffles, gates"), (11, "global + DSMEM state stores issued"), (12, "cluster barrier"),
+              (4, "proxy fence + CTA barrier"), (13, "thread 0: D2 tcgen05.mma + commit issued"), (5, "D2 complete (mbarrier)"),
+              (6, "partials stored + CTA barrier"), (7, "gpu fence + flag store"))
+REQ_STAMPS = ((0, "flags seen"), (1, "a = SiLU(C + partials)"), (2, "W2 slice dots"), (3, "slice log-softmax + top-k"),
+              (6, "merge into the sorted frontier"), (9, "nominate + publish (warp 0)"), (4, "CTA barrier"),
+              (5, "slices staged (issue)"))
 
 
 def run_trace(args):
@@ -505,26 +510,15 @@ def run_trace(args):
         rows = {}
         g = t[0, 1:max(steps - 1, 2)]          # skip step 0 (weight load) and the last
         q = t[1, 1:max(steps - 1, 2)]
-        for i in range(1, len(GRU_STAMPS)):
-            d = g[:, i] - g[:, i - 1]
-            rows["gru: " + GRU_STAMPS[i]] = float(np.median(d[(g[:, i] > 0) & (g[:, i - 1] > 0)])) if len(d) else None
-        for i in range(1, len(REQ_STAMPS)):
-            d = q[:, i] - q[:, i - 1]
-            ok = (q[:, i] > 0) & (q[:, i - 1] > 0)
-            rows["req: " + REQ_STAMPS[i]] = float(np.median(d[ok])) if ok.any() else None
-        for a_, b_, name in ((3, 6, "req:   (wait) top-k barrier -> replay starts"), (6, 7, "req:   replay: copy commit state"),
-                             (7, 8, "req:   replay: pops"), (8, 9, "req:   replay: publish")):
-            ok = (q[:, a_] > 0) & (q[:, b_] > 0)
-            rows[name] = float(np.median((q[:, b_] - q[:, a_])[ok])) if ok.any() else None
-        rows["req:   replay: pops per step (median)"] = float(np.median(q[:, 10]))
-        rows["req:   replay: active mask at pop 1"] = hex(int(q[1, 11]))
-        rows["req:   replay: pop 1 arg-max collectives (SM cycles)"] = float(np.median(q[:, 12]))
-        rows["req:   replay: pop 1 whole (SM cycles)"] = float(np.median(q[:, 13]))
+        for role, arr, stamps in (("gru", g, GRU_STAMPS), ("req", q, REQ_STAMPS)):
+            for (i0, _), (i1, name) in zip(stamps[:-1], stamps[1:]):
+                ok = (arr[:, i1] > 0) & (arr[:, i0] > 0)
+                rows[f"{role}: {name}"] = float(np.median((arr[:, i1] - arr[:, i0])[ok])) if ok.any() else None
         ok = (q[:, 0] > 0) & (g[:, 7] > 0)
         rows["hop: flag released -> request sees flags"] = float(np.median((q[:, 0] - g[:, 7])[ok])) if ok.any() else None
         gn = t[0, 2:max(steps, 3)]
-        ok = (gn[:, 0] > 0) & (q[:len(gn), 4] > 0)
-        rows["hop: request published -> GRU sees headers"] = float(np.median((gn[:, 0] - q[:len(gn), 4])[ok])) if ok.any() else None
+        ok = (gn[:, 0] > 0) & (q[:len(gn), 9] > 0)
+        rows["hop: request published -> GRU sees headers"] = float(np.median((gn[:, 0] - q[:len(gn), 9])[ok])) if ok.any() else None
         period = np.diff(t[0, 1:steps, 0])
         rows["step period"] = float(np.median(period)) if len(period) else None
         rows["steps"] = steps

@@ -43,7 +43,7 @@ struct dt_handle {
     __nv_bfloat16 *s_hi, *s_lo; float *partial; unsigned long long *desc; unsigned int *flags, *round_ctr;
     int fused_ok, max_smem_optin;
     // wavefront expansion (dt_wave.cuh): per-item partials, multi-item descriptors, device error word, counters
-    float *wv_partial; unsigned long long *wv_desc; unsigned int *wv_err, *wv_stats; int wave_ok, slot_stride;
+    float *wv_partial; unsigned long long *wv_desc; unsigned int *wv_err, *wv_stats, *wv_flags, *wv_round; int wave_ok, slot_stride;
     int64_t opt_wave_width;         // items per request per step (0 = auto)
     int wave_clusters;              // co-resident clusters of kWvCS CTAs (0 = not queried yet, -1 = unavailable)
     int path_taken;                 // expansion path of the last dt_build_trees: 1 per-step, 2/3 fused mma.sync, 4 fused tcgen05, 5 wavefront
@@ -275,7 +275,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     // fused path eligibility (shape part; the grid / smem fit is checked per call)
     h->fused_ok = (w->dtype == DT_BF16) && (w->g % 32 == 0) && (w->r % 8 == 0) && max_M <= 256 &&
                   ((reinterpret_cast<uintptr_t>(w->gru_w_hh) & 15u) == 0) && ((reinterpret_cast<uintptr_t>(w->corr_w2) & 15u) == 0);
-    size_t o_shi = 0, o_slo = 0, o_partial = 0, o_desc = 0, o_sync = 0, o_wpart = 0, o_wdesc = 0, o_werr = 0;
+    size_t o_shi = 0, o_slo = 0, o_partial = 0, o_desc = 0, o_sync = 0, o_wpart = 0, o_wdesc = 0, o_werr = 0, o_wsync = 0;
     if (h->fused_ok) {
         o_shi = carve((size_t)max_batch * slots * w->g * 2);
         o_slo = carve((size_t)max_batch * slots * w->g * 2);
@@ -285,6 +285,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         o_wpart = carve((size_t)max_batch * kWvMaxW * (w->g / 16 + 1) * w->r * 4);
         o_wdesc = carve((size_t)max_batch * kWvDescWords * 8);
         o_werr = carve(256);
+        o_wsync = carve((size_t)256 * 4 * kFusFlagStride + 256);   // the wavefront kernel's own flags + round counter (its tags differ)
     }
     // MMA GEMM eligibility: bf16, 16-byte aligned rows of H and W1
     h->mma_ok = (w->dtype == DT_BF16) && (w->d % 8 == 0) && ((w->d + w->g) % 8 == 0) &&
@@ -339,6 +340,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         h->round_ctr = h->flags + (size_t)256 * kFusFlagStride;
         h->wv_partial = (float *)(h->ws + o_wpart); h->wv_desc = (unsigned long long *)(h->ws + o_wdesc);
         h->wv_err = (unsigned int *)(h->ws + o_werr); h->wv_stats = h->wv_err + 8;
+        h->wv_flags = (unsigned int *)(h->ws + o_wsync); h->wv_round = h->wv_flags + (size_t)256 * kFusFlagStride;
         h->wave_ok = (slots <= 1023);
         bool ok = cudaDeviceGetAttribute(&h->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess;
         h->max_smem_optin -= 1024;                  // room for the kernels' static shared memory
@@ -516,7 +518,7 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
 // CTA per request beside the g / 16 GRU CTAs) are split into consecutive launches: no cliff, requests are independent.
 static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st) {
     if (!h->fused_ok || !h->wave_ok || (h->opt_expand_path != 0 && h->opt_expand_path != 5)) return 1;
-    if (p.g % kWvKC || p.g / 16 > 256 || p.r % 8 || p.r > 256 || p.k > 32 || p.M > 256 || p.L > DT_MAX_L) return 1;
+    if (p.g % kWvKC || p.g / 16 > 256 || p.r % 8 || p.r > 256 || p.k > 32 || p.M > 256 || p.L > DT_MAX_L || p.V > (1 << 20)) return 1;
     const int n_gru = p.g / 16;                          // a multiple of kWvCS (g is a multiple of 128)
     const size_t gs = wave_gru_smem(p.g, p.r);
     if (gs > (size_t)h->max_smem_optin) return 1;
@@ -540,12 +542,17 @@ static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st) {
     if (W <= 0) { W = 96 / (p.batch < cap ? p.batch : cap); }
     if (W < 1) W = 1;
     if (W > kWvMaxW) W = kWvMaxW;
+    {   // a GRU CTA keeps at most kWvMaxItems compacted items per step; a request CTA merges at most 256 new candidates
+        const int nbmax = p.batch < cap ? p.batch : cap;
+        if (W * nbmax > kWvMaxItems) W = kWvMaxItems / nbmax;
+        if (W * p.k > 256) W = 256 / p.k;
+    }
     const int e_max = h->slot_stride - 1;
     int nsl = W < kWvMaxSlices ? W : kWvMaxSlices;
     if (nsl > p.L) nsl = p.L;
     size_t rs = 0;
     for (; nsl >= 1; --nsl) {
-        rs = wave_req_smem(p.r, p.M, p.N, p.k, W, e_max, nsl);
+        rs = wave_req_smem2(p.r, p.M, p.B, p.k, W, e_max, nsl);
         if (rs <= (size_t)h->max_smem_optin) break;
     }
     if (nsl < 1) return 1;
@@ -570,7 +577,7 @@ static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st) {
         f.s_hi = h->s_hi + so; f.s_lo = h->s_lo + so; f.s32 = h->states + so;
         f.partial = h->wv_partial + (size_t)b0 * kWvMaxW * f.P * p.r;
         f.desc = h->wv_desc + (size_t)b0 * kWvDescWords;
-        f.flags = h->flags; f.round_ctr = h->round_ctr; f.err = h->wv_err; f.stats = (b0 == 0) ? h->wv_stats : nullptr;
+        f.flags = h->wv_flags; f.round_ctr = h->wv_round; f.err = h->wv_err; f.stats = (b0 == 0) ? h->wv_stats : nullptr;
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof(cfg));
         cfg.gridDim = dim3(n_gru + (nb + kWvCS - 1) / kWvCS * kWvCS); cfg.blockDim = dim3(kWvThreads);

@@ -16,18 +16,19 @@
 //            pops: that replay IS Algorithm 1's run, pop for pop, ties included (reading A8).
 //
 // W = 1 is the plain heap schedule (B steps); a bushy tree of depth D finishes in about D + 1 steps.
-// Speculative expansions that turn out useless cost GRU columns, never correctness.
+// Speculative expansions that turn out useless cost GRU rows, never correctness.
 //
-// Two CTA roles, co-resident (cooperative launch), hand-over through self-describing words in L2 as in
-// dt_fused.cuh:
-//  * GRU CTAs (g / 16 of them, weight-stationary: 48 rows of W_hh + 16 columns of W1[:, d:] in shared
-//    memory).  Step s: gather the items {request, parent state slot, token} every request published,
-//    and for passes of up to 64 items run D1[node, row] = S_parent[node, :] . W_hh[row, :]^T on
-//    tcgen05 with the NODES as the M dimension (M = 128 rows = 64 nodes x {bf16 hi, bf16 lo}, N = 48,
-//    accumulators in TMEM; states stream from L2 through a cp.async ring in the 128-byte-swizzled
-//    K-major layout), gates with the input half gathered from P = E W_ih^T, new
-//    state to L2, and D2[node, j] = S_new[node, my 16 units] . W1[j, d + my units]^T, this CTA's
-//    split-K share of W1[:, d:] S_new, one M = 128, N = r MMA.
+// Two CTA roles, co-resident (cooperative launch), hand-over through self-describing words in L2:
+//  * GRU CTAs (g / 16 of them, in clusters of 4, weight-stationary: 48 rows of W_hh and the W1[:, d:] block of the
+//    cluster's 64 units in shared memory).  Step s: poll every request's item line (one 128-byte line of up to 15
+//    self-validating words {token, parent state slot, count, epoch, round}), compact the items, and for passes of up
+//    to 64 items run D1[row, gate unit] = S_parent[row, :] . W_hh[gate unit, :]^T on tcgen05 with the NODES as the
+//    M dimension (M = 128 rows = 64 nodes x {bf16 hi, bf16 lo}, N = 48, four accumulators in TMEM, one per issuing
+//    thread; the states stream from L2 through a cp.async ring in the 128-byte-swizzled K-major layout, completion
+//    tracked by mbarriers, no CTA barrier inside), gates in registers with the input half gathered from
+//    P = E W_ih^T, new state to L2 and, over distributed shared memory, to every CTA of the
+//    cluster, then D2[row, j] = S_new[row, the cluster's 64 units] . W1[j, d + those units]^T: the cluster's
+//    split-K share of W1[:, d:] S_new, 16 partial vectors per node.
 //  * Request CTAs (one per request) keep the children lists, replay the heap, nominate, and for every
 //    expanded node compute a = SiLU(C + sum of partials), z = (base + W2[cand] a) / T_eff over the M
 //    candidate rows of the node's depth (rows staged per depth in shared memory "slices"), slice
@@ -38,15 +39,18 @@
 namespace dt {
 
 constexpr int kWvThreads = 256;
-constexpr int kWvNP = 64;                       // items per GRU pass (M = 128 operand rows: hi | lo)
+constexpr int kWvNP = 64;                       // items per GRU pass (N = 128 operand columns: hi and lo of 64 nodes)
 constexpr int kWvKC = 128;                      // k per ring slot (two 64-wide swizzle blocks)
-constexpr int kWvRingBytes = 96 * 1024;         // state ring: three 128-row chunks, or more slots of fewer rows
+constexpr int kWvSlots = 3;
+constexpr int kWvSlotBytes = 32 * 1024;         // 128 rows x 128 k x 2 B
+constexpr int kWvRingBytes = kWvSlots * kWvSlotBytes;
 constexpr int kWvCS = 4;                        // GRU CTAs per thread-block cluster
-constexpr int kWvLdH = 68;                      // floats per row of the pre-activation buffer (64 nodes + pad)
-constexpr int kWvDescWords = 16;                // u64 words per request descriptor: header + 15 items, one 128-byte line
+constexpr int kWvDescWords = 16;                // u64 words per request line: 15 items + one spare, one 128-byte line
 constexpr int kWvMaxW = kWvDescWords - 1;
-constexpr int kWvMaxBatch = 128;                // requests per launch (headers are polled by four warps)
-constexpr int kWvTmemCols = 512;                // 4 or 8 independent D1 accumulators of N <= 128 / 64 columns; D2 reuses column 0 ..
+constexpr int kWvMaxBatch = 64;                 // requests per launch (larger batches run as consecutive launches)
+constexpr int kWvMaxItems = 512;                // items per step over all requests of a launch (W is clamped to this)
+constexpr int kWvTmemCols = 512;                // D1: 4 accumulators of N <= 128 columns; D2 reuses column 0 ..
+constexpr int kWvLdH = 68;                      // floats per row of the pre-activation buffer (64 nodes + pad)
 constexpr int kWvMaxSlices = 8;
 constexpr unsigned int kWvAct = 0x100u;         // replay word: cursor (8) | active (1) | pop slot (16, from bit 16)
 
@@ -63,31 +67,33 @@ struct WaveParams {
     float *s32;                    // [batch, slot_stride, g]
     float *partial;                // [batch, kWvMaxW, P, r]
     unsigned long long *desc;      // [batch, kWvDescWords]
-    unsigned int *flags;           // [n_gru] one 128-byte line each
+    unsigned int *flags;           // [n_gru] one 128-byte line each: steps completed (released: states and partials visible)
     unsigned int *round_ctr;       // rounds this handle has run (tags every hand-over word)
     unsigned int *err;             // set to 1 when a hand-over wait timed out (protocol slip: fail, do not hang)
     unsigned int *stats;           // [4] optional counters of request 0: steps, expansions (measurement aid)
 };
 
 // ---- hand-over words ---------------------------------------------------------------------------------
-// header: round (24) | epoch (12) | first new state slot (12) | done (1) | count (15)
-// item:   token (32) | parent state slot (10) | epoch (10) | round (12)
-// Every word is self-validating (relaxed stores need no ordering between them); epoch = step + 1, so
-// zero-initialised memory never matches.
-__device__ __forceinline__ unsigned long long wave_hdr_pack(unsigned int rnd, int epoch, int first, int done, int count) {
-    return ((unsigned long long)(rnd & 0xFFFFFFu) << 40) | ((unsigned long long)(epoch & 0xFFF) << 28) |
-           ((unsigned long long)(first & 0xFFF) << 16) | ((unsigned long long)(done & 1) << 15) | (unsigned long long)(count & 0x7FFF);
-}
-__device__ __forceinline__ bool wave_hdr_ok(unsigned long long h, unsigned int rnd, int epoch) {
-    if ((unsigned int)(h >> 40) != (rnd & 0xFFFFFFu)) return false;
-    return ((h >> 15) & 1ull) || (int)((h >> 28) & 0xFFFu) == (epoch & 0xFFF);
-}
-__device__ __forceinline__ unsigned long long wave_item_pack(unsigned int rnd, int epoch, int pslot, int tok) {
-    return ((unsigned long long)(unsigned int)tok << 32) | ((unsigned long long)(pslot & 0x3FF) << 22) |
-           ((unsigned long long)(epoch & 0x3FF) << 12) | (unsigned long long)(rnd & 0xFFFu);
+// item word j of a request's line:  token (20) | parent state slot (10) | done (1) | count (4) | epoch (10) | round (19)
+// Every word is self-validating (relaxed stores need no ordering between them) and carries the request's item count
+// of the step, so one poll of the line tells a GRU CTA everything; epoch = step + 1, so zero-initialised memory never
+// matches.  Word 0 is written every step (count 0 .. 15, or `done`, which stays valid for the rest of the round).
+__device__ __forceinline__ unsigned long long wave_item_pack(unsigned int rnd, int epoch, int count, int done, int pslot, int tok) {
+    return ((unsigned long long)((unsigned int)tok & 0xFFFFFu) << 44) | ((unsigned long long)(pslot & 0x3FF) << 34) |
+           ((unsigned long long)(done & 1) << 33) | ((unsigned long long)(count & 0xF) << 29) |
+           ((unsigned long long)(epoch & 0x3FF) << 19) | (unsigned long long)(rnd & 0x7FFFFu);
 }
 __device__ __forceinline__ bool wave_item_ok(unsigned long long w, unsigned int rnd, int epoch) {
-    return (unsigned int)(w & 0x3FFFFFull) == ((((unsigned int)epoch & 0x3FFu) << 12) | (rnd & 0xFFFu));
+    return (unsigned int)(w & 0x1FFFFFFFull) == ((((unsigned int)epoch & 0x3FFu) << 19) | (rnd & 0x7FFFFu));
+}
+__device__ __forceinline__ bool wave_item0_ok(unsigned long long w, unsigned int rnd, int epoch) {
+    if ((unsigned int)(w & 0x7FFFFull) != (rnd & 0x7FFFFu)) return false;
+    return ((w >> 33) & 1ull) || (int)((w >> 19) & 0x3FFu) == (epoch & 0x3FF);
+}
+// compacted item in a GRU CTA's shared memory: token (20) | parent slot (10) | new slot (10) | request (7) | item index (4)
+__device__ __forceinline__ unsigned long long wave_citem_pack(int tok, int ps, int ns, int b, int j) {
+    return (unsigned long long)(unsigned int)tok | ((unsigned long long)ps << 20) | ((unsigned long long)ns << 30) |
+           ((unsigned long long)b << 40) | ((unsigned long long)j << 47);
 }
 
 __device__ __forceinline__ unsigned long long wave_timer() {
@@ -99,49 +105,28 @@ __device__ __forceinline__ unsigned long long wave_timer() {
 constexpr int kWvTraceSteps = 64, kWvTraceStamps = 16;
 #ifdef DT_TRACE
 __device__ unsigned long long g_wv_trace[2][kWvTraceSteps][kWvTraceStamps];
-__device__ unsigned long long g_wv_trace_sink[kWvThreads];
-// branch-free on purpose: a thread-0-only branch would leave its warp diverged and slow every warp collective after it
+// one PREDICATED store by thread 0 (no branch: a thread-0-only branch would leave its warp diverged and slow every warp
+// collective after it; no store at all by the other threads: a release fence waits for every store in flight)
 #define WV_TR(role, cond, step, i) do { \
         const bool wv_on__ = (threadIdx.x == 0) && (cond) && (step) < kWvTraceSteps; \
-        unsigned long long *wv_dst__ = wv_on__ ? &g_wv_trace[role][wv_on__ ? (step) : 0][i] : &g_wv_trace_sink[threadIdx.x]; \
-        *wv_dst__ = wave_timer(); } while (0)
+        unsigned long long *wv_dst__ = &g_wv_trace[role][wv_on__ ? (step) : 0][i]; \
+        const unsigned long long wv_t__ = wave_timer(); \
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.global.u64 [%0], %1;\n\t}\n" \
+                     :: "l"(wv_dst__), "l"(wv_t__), "r"((unsigned int)wv_on__) : "memory"); } while (0)
 #else
 #define WV_TR(role, cond, step, i) do { } while (0)
 #endif
 constexpr unsigned long long kWvTimeoutNs = 4000000000ull;     // 4 s: far beyond any round; a slip fails instead of hanging
 
-// TMEM -> registers: 8 consecutive fp32 columns of this thread's lane
-__device__ __forceinline__ void wave_tmem_ld8(uint32_t taddr, float (&v)[8]) {
-    uint32_t r[8];
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-                 : "r"(taddr) : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-    for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
-}
-
 // shared-memory footprints (bytes)
 __host__ __device__ inline size_t wave_gru_smem(int g, int r) {
-    const size_t r16 = (size_t)((r + 15) & ~15);
-    (void)r16;
     const size_t rpc = (size_t)16 * ((r + 16 * kWvCS - 1) / (16 * kWvCS));
     return (size_t)48 * g * 2 + (size_t)kWvRingBytes + (size_t)kWvCS * 4096 + (size_t)kWvCS * rpc * 32 +
-           (size_t)(5 * kWvNP + 3 * kWvMaxBatch + 8) * 4 + 20 * 8 + 64 + 1024;
+           (size_t)kWvMaxItems * 8 + (size_t)(2 * kWvMaxBatch + 8) * 4 + 24 * 8 + 64 + 1024;
 }
 __host__ __device__ inline size_t wave_slice_bytes(int r, int M) {
     return (size_t)((M + 7) / 8) * (size_t)((r + 63) / 64) * 1024;
 }
-__host__ __device__ inline size_t wave_req_smem(int r, int M, int N, int k, int W, int e_max, int n_slices) {
-    auto al = [](size_t x) { return (x + 15) / 16 * 16; };
-    size_t s = (size_t)n_slices * wave_slice_bytes(r, M) + 2 * al((size_t)n_slices * M * 4);
-    s += al((size_t)e_max * k * 8) + al((size_t)e_max * k * 2) + 4 * al((size_t)e_max * 4) + 2 * al((size_t)e_max * 4) + al((size_t)e_max * 8);
-    s += 4 * al((size_t)N * 4);
-    s += al((size_t)W * r * 4) + al((size_t)W * M * 4) + al((size_t)W * M * 8) + al((size_t)W * M);
-    s += al((size_t)4 * kWvMaxW * 4) + al(256);
-    return s + 1024;
-}
-
 // bounded spin on a hand-over word; returns false on timeout (and raises *err)
 template <typename F>
 __device__ __forceinline__ bool wave_spin(F ready, unsigned int *err) {
@@ -164,44 +149,50 @@ __device__ __forceinline__ uint32_t wave_cluster_rank() { uint32_t r; asm volati
 __device__ __forceinline__ uint32_t wave_mapa(uint32_t saddr, uint32_t rank) {
     uint32_t r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank)); return r;
 }
-__device__ __forceinline__ void wave_st_cluster_v2(uint32_t addr, uint2 v) {
-    asm volatile("st.shared::cluster.v2.b32 [%0], {%1, %2};" ::"r"(addr), "r"(v.x), "r"(v.y) : "memory");
+__device__ __forceinline__ void wave_st_cluster_v4(uint32_t addr, uint4 v) {
+    asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 __device__ __forceinline__ void wave_cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void wave_cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
 __device__ __forceinline__ void wave_cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
-__device__ __forceinline__ void wave_tmem_ld16(uint32_t taddr, float (&v)[16]) {
-    uint32_t r[16];
+__device__ __forceinline__ unsigned int wave_ld_acquire_u32(const unsigned int *p) {
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+// two {value, tag} elements per access; each 64-bit element is read / written as one unit
+__device__ __forceinline__ void wave_st_pair2(uint2 *p, float a, float b, unsigned int tag) {
+    const unsigned long long x = ((unsigned long long)tag << 32) | __float_as_uint(a), y = ((unsigned long long)tag << 32) | __float_as_uint(b);
+    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(x), "l"(y) : "memory");
+}
+__device__ __forceinline__ void wave_ld_pair2(const uint2 *p, unsigned long long &x, unsigned long long &y) {
+    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(x), "=l"(y) : "l"(p) : "memory");
+}
+
+// TMEM -> registers without the wait: 8 / 16 consecutive fp32 columns of this thread's lane
+__device__ __forceinline__ void wave_tmem_ld8_nw(uint32_t taddr, uint32_t (&r)[8]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void wave_tmem_ld16_nw(uint32_t taddr, uint32_t (&r)[16]) {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
                    "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
                  : "r"(taddr) : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-    for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
 }
+__device__ __forceinline__ void wave_tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 // make the mbarrier count this thread's earlier cp.async copies: it arrives once they have landed (the barrier's expected
 // count includes these arrivals)
+__device__ __forceinline__ void wave_mbar_arrive(uint32_t mbar_addr) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar_addr) : "memory");
+}
+__device__ __forceinline__ void wave_cp_async16_s(uint32_t saddr, const void *gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(saddr), "l"(gmem));
+}
 __device__ __forceinline__ void wave_cp_async_arrive(uint32_t mbar_addr) {
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(mbar_addr) : "memory");
-}
-__device__ __forceinline__ void wave_tmem_ld16x2(uint32_t ta, uint32_t tb, float (&va)[16], float (&vb)[16]) {
-    uint32_t r[32];
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-                 : "r"(ta) : "memory");
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-                 : "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
-                   "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-                 : "r"(tb) : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-    for (int i = 0; i < 16; ++i) { va[i] = __uint_as_float(r[i]); vb[i] = __uint_as_float(r[16 + i]); }
-}
-template <int N> __device__ __forceinline__ void wave_cp_wait_n(int n) {
-    if (n >= N) cp_async_wait<N>();
-    else if constexpr (N > 0) wave_cp_wait_n<N - 1>(n);
 }
 
 __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char *smem_raw) {
@@ -210,29 +201,25 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
     const int g = e.g, r = e.r, batch = e.batch;
     const int cta = blockIdx.x, u0 = cta * 16;
     const int crank = (int)wave_cluster_rank(), cbase = cta - crank;   // rank in the cluster, first CTA of the cluster
-    const size_t stride = (size_t)p.slot_stride;
+    const int stride = p.slot_stride;
     const int n_kc = g / kWvKC;
     const int rpc = p.rpc;                                             // rows of W1 this CTA reduces (multiple of 16)
 
     // carve (smem_raw is 1024-byte aligned by the kernel)
     unsigned char *sW = smem_raw;                                     // W_hh slice, K-major sw128: [6 row groups][g/64 atoms][1 KB]
     const uint32_t sboW = (uint32_t)g * 16;                           // bytes between 8-row groups
-    unsigned char *sRing = sW + (size_t)48 * g * 2;                   // [slot][2 k-blocks][N / 8 row groups][1 KB]
+    unsigned char *sRing = sW + (size_t)48 * g * 2;                   // [slot][2 k-blocks][16 row groups][1 KB]
+    unsigned long long *sRaw = reinterpret_cast<unsigned long long *>(sRing);   // [batch][16] polled lines (between steps the ring is idle)
     float *sH = reinterpret_cast<float *>(sRing);                    // [48][kWvLdH] hidden-half pre-activations (aliases the ring after D1)
     unsigned char *sS2 = sRing + kWvRingBytes;                        // [kWvCS][16 groups][2 k-halves][8 rows][16 B]: new states of
                                                                       // the cluster's 16 kWvCS units (block c written by rank c)
     unsigned char *sW1 = sS2 + (size_t)kWvCS * 4096;                  // [kWvCS][rpc/8 groups][2 k-halves][8 rows][16 B]
-    int *sRow = reinterpret_cast<int *>(sW1 + (size_t)kWvCS * rpc * 32);   // [64] request * stride + parent slot  (state row)
-    int *sNew = sRow + kWvNP;                                         // [64] request * stride + new slot
-    int *sTok = sNew + kWvNP;                                         // [64]
-    int *sIt = sTok + kWvNP;                                          // [64] request * kWvMaxW + item index (partial row)
-    int *sPz = sIt + kWvNP;                                           // [64] parent slot is the zero slot
-    int *sCnt = sPz + kWvNP;                                          // [128] items per request this step
-    int *sOff = sCnt + kWvMaxBatch;                                   // [129] exclusive prefix
-    int *sFirst = sOff + kWvMaxBatch + 4;                             // [128] first new state slot per request
-    unsigned long long *mbar = reinterpret_cast<unsigned long long *>(sFirst + kWvMaxBatch);   // [0..7] slot full, [8] D1, [9] D2, [10..17] slot empty
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(mbar + 20);
-    int *sCtl = reinterpret_cast<int *>(tmem_slot + 2);               // [0] items this step, [1] requests not done, [2] abort, [4..7] live masks
+    unsigned long long *sItems = reinterpret_cast<unsigned long long *>(sW1 + (size_t)kWvCS * rpc * 32);   // [kWvMaxItems] compacted items of the step
+    int *sCnt = reinterpret_cast<int *>(sItems + kWvMaxItems);        // [64] items per request this step (-1 = done)
+    int *sCum = sCnt + kWvMaxBatch;                                   // [64] items per request so far = expansions allocated
+    unsigned long long *mbar = reinterpret_cast<unsigned long long *>(sCum + kWvMaxBatch + 8);   // [0..7] slot full, [8..15] slot empty, [16] D1, [17] D2, [18] first group of chunks full
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(mbar + 24);
+    int *sCtl = reinterpret_cast<int *>(tmem_slot + 2);               // [2] abort
 
     {   // resident weights
         const __nv_bfloat16 *whh = reinterpret_cast<const __nv_bfloat16 *>(e.w_hh);
@@ -252,10 +239,12 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
             *reinterpret_cast<__nv_bfloat16 *>(sW1 + (size_t)c * rpc * 32 + (size_t)(jl >> 3) * 256 + (ul >> 3) * 128 + (jl & 7) * 16 + (ul & 7) * 2) = v;
         }
         for (int i = tid; i < kWvCS * 1024; i += kWvThreads) reinterpret_cast<uint32_t *>(sS2)[i] = 0u;
+        for (int i = tid; i < kWvMaxBatch; i += kWvThreads) sCum[i] = 0;
         if (tid == 0) {
-            for (int i = 0; i < 8; ++i) { tc::mbar_init(tc::smem_u32(mbar + i), kWvThreads - 128); tc::mbar_init(tc::smem_u32(mbar + 10 + i), 4); }
-            tc::mbar_init(tc::smem_u32(mbar + 8), 4);
-            tc::mbar_init(tc::smem_u32(mbar + 9), 1);
+            for (int i = 0; i < 8; ++i) { tc::mbar_init(tc::smem_u32(mbar + i), kWvThreads - 128); tc::mbar_init(tc::smem_u32(mbar + 8 + i), 4); }
+            tc::mbar_init(tc::smem_u32(mbar + 16), 4);
+            tc::mbar_init(tc::smem_u32(mbar + 17), 1);
+            tc::mbar_init(tc::smem_u32(mbar + 18), kWvThreads - 128);
             tc::mbar_init_fence();
             sCtl[2] = 0;
         }
@@ -270,29 +259,27 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
     const uint32_t tmem = *tmem_slot;
     const uint32_t idesc2 = tc::make_idesc_bf16(128, rpc);
     const uint32_t mb0 = tc::smem_u32(mbar);
+    const uint32_t mbFull = mb0, mbEmpty = mb0 + 64, mbD1 = mb0 + 128, mbD2 = mb0 + 136, mbGrp = mb0 + 144;
     const uint64_t descW0 = tc::make_desc_sw128(tc::smem_u32(sW), sboW), descR0 = tc::make_desc_sw128(tc::smem_u32(sRing), 1024);
     const uint64_t descS2 = tc::make_desc(tc::smem_u32(sS2), 128, 256), descW1 = tc::make_desc(tc::smem_u32(sW1), 128, 256);
-    uint32_t ph_full = 0, ph_empty = 0, ph_d1 = 0, ph_d2 = 0;      // mbarrier phases (each role keeps the bits of the barriers it waits on)
+    uint32_t ph_full = 0, ph_empty = 0, ph_d1 = 0, ph_d2 = 0, ph_grp = 0;      // mbarrier phases (each role keeps the bits of the barriers it waits on)
     bool pend2 = false;                                             // a cluster arrive (sS2 consumed) awaits its wait
 
     // epilogue geometry: TMEM lane quadrant q4, unit half hsel; lanes 0..15 hold the hi rows of nodes 16 q4 + lane,
-    // lanes 16..31 the lo rows of the same nodes; after the hi + lo exchange lane < 16 finishes units 8 hsel + 0..3,
-    // lane >= 16 units 8 hsel + 4..7
+    // lanes 16..31 the lo rows of the same nodes (operand row rho = 32 q4 + lane); after the hi + lo exchange lane < 16
+    // finishes units 8 hsel + 0..3, lane >= 16 units 8 hsel + 4..7
     const int q4 = warp & 3, hsel = warp >> 2, il = lane & 15, uh = lane >> 4;
     const int my_node = 16 * q4 + il;
     const int my_u = 8 * hsel + 4 * uh;                              // first of this thread's 4 local units
     const uint32_t tlane = (uint32_t)(32 * q4) << 16;
-    // where this thread's new states go in every cluster CTA's sS2 (block crank): rows 32 q4 + il (hi) and + 16 (lo)
-    uint32_t s2_hi[kWvCS], s2_lo[kWvCS];
+    // where this thread's 16-byte piece of the new states (8 units, hi for lanes < 16, lo for the others) goes in every
+    // cluster CTA's sS2 (block crank): row rho, k-half hsel
+    uint32_t s2_dst[kWvCS];
     {
-        const int rh = 32 * q4 + il, rl = rh + 16;
-        const uint32_t oh = (uint32_t)(crank * 4096 + (rh >> 3) * 256 + hsel * 128 + (rh & 7) * 16 + uh * 8);
-        const uint32_t ol = (uint32_t)(crank * 4096 + (rl >> 3) * 256 + hsel * 128 + (rl & 7) * 16 + uh * 8);
+        const int rho = 32 * q4 + lane;
+        const uint32_t o = (uint32_t)(crank * 4096 + (rho >> 3) * 256 + hsel * 128 + (rho & 7) * 16);
 #pragma unroll
-        for (int c = 0; c < kWvCS; ++c) {
-            s2_hi[c] = wave_mapa(tc::smem_u32(sS2) + oh, (uint32_t)c);
-            s2_lo[c] = wave_mapa(tc::smem_u32(sS2) + ol, (uint32_t)c);
-        }
+        for (int c = 0; c < kWvCS; ++c) s2_dst[c] = wave_mapa(tc::smem_u32(sS2) + o, (uint32_t)c);
     }
 
     // every GRU CTA walks the K chunks of a pass in its own rotation: 64 CTAs asking L2 for the same lines at the same
@@ -300,66 +287,87 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
     const int kshift = cta % n_kc;
     const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 10;
     for (int s = 0;; ++s) {
-        // ---- headers of step s: one lane per request
-        if (warp < 4) {
-            const int b = warp * 32 + lane;
-            int cnt = 0, first = 0, live = 0;
-            if (b < batch) {
-                unsigned long long hdr = 0ull;
-                const unsigned long long *hp = p.desc + (size_t)b * kWvDescWords;
-                const bool ok = wave_spin([&] { hdr = ld_relaxed_u64(hp); return wave_hdr_ok(hdr, rnd, s + 1); }, p.err);
-                if (!ok) sCtl[2] = 1;
-                else if (!((hdr >> 15) & 1ull)) { cnt = (int)(hdr & 0x7FFFull); first = (int)((hdr >> 16) & 0xFFFull); live = 1; }
+        // ---- item lines of step s: a half-warp per request, a lane per word of its 128-byte line
+        for (int b0 = 2 * warp; b0 < batch; b0 += 2 * (kWvThreads / 32)) {
+            const int b = b0 + (lane >> 4), j = lane & 15;
+            const bool have = b < batch;
+            const unsigned long long *wp = p.desc + (size_t)(have ? b : 0) * kWvDescWords + j;
+            unsigned long long w = 0ull, t0 = 0ull;
+            bool v = false, ok = !have;
+            int cnt = 0, dn = 0;
+            unsigned int n = 0;
+            while (true) {
+                if (have && !v) {
+                    w = ld_relaxed_u64(wp);
+                    v = (j == 0) ? wave_item0_ok(w, rnd, s + 1) : wave_item_ok(w, rnd, s + 1);
+                }
+                const unsigned long long w0 = __shfl_sync(0xffffffffu, w, lane & 16);
+                const int v0 = __shfl_sync(0xffffffffu, (int)v, lane & 16);
+                if (v0) { cnt = (int)((w0 >> 29) & 0xFull); dn = (int)((w0 >> 33) & 1ull); }
+                ok = !have || (v0 && (dn || j >= cnt || v));
+                if (__all_sync(0xffffffffu, ok)) break;
+                bool to = false;
+                if (((++n) & 1023u) == 0u) {
+                    if (n == 1024u) t0 = wave_timer();
+                    to = (ld_relaxed_u32(p.err) != 0u) || (wave_timer() - t0 > kWvTimeoutNs);
+                }
+                if (__any_sync(0xffffffffu, to)) { if (lane == 0) { atomicExch(p.err, 1u); sCtl[2] = 1; } break; }
             }
-            sCnt[b] = cnt; sFirst[b] = first;
-            const unsigned int lv = __ballot_sync(0xffffffffu, live != 0);
-            if (lane == 0) sCtl[4 + warp] = (int)lv;
+            if (have) {
+                if (j == 0) sCnt[b] = dn ? -1 : cnt;
+                if (!dn && j < cnt) sRaw[b * kWvDescWords + j] = w;
+            }
+        }
+        if (s > 0 && warp == 7) {
+            // the parents' states were written by other GRU CTAs in earlier steps: acquire their `states visible` words (they
+            // were set long ago: a request only nominates after it has seen the partials of that step)
+            const unsigned int want = fbase + (unsigned int)s;
+            const bool ok = wave_spin([&] {
+                bool all = true;
+                for (int q = lane; q < p.n_gru; q += 32)
+                    all = all && ((int)(wave_ld_acquire_u32(p.flags + (size_t)q * kFusFlagStride) - want) >= 0);
+                return all; }, p.err);
+            if (!ok) sCtl[2] = 1;
         }
         __syncthreads();
-        if (warp == 0) {                                            // exclusive prefix of the counts (4 per lane)
-            int c[4], sum = 0;
+        // ---- compaction: every warp scans the counts (two requests per lane), warp w packs requests w, w + 8, ..
+        int total;
+        {
+            const int r0 = (lane < batch) ? sCnt[lane] : -1, r1 = (lane + 32 < batch) ? sCnt[lane + 32] : -1;
+            const int c0 = max(r0, 0), c1 = max(r1, 0);
+            int i0 = c0, i1 = c1;
 #pragma unroll
-            for (int i = 0; i < 4; ++i) { c[i] = sCnt[lane * 4 + i]; sum += c[i]; }
-            int inc = sum;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-            int run = inc - sum;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) { sOff[lane * 4 + i] = run; run += c[i]; }
-            if (lane == 31) { sOff[kWvMaxBatch] = inc; sCtl[0] = inc; }
-            if (lane == 0) sCtl[1] = (sCtl[4] | sCtl[5] | sCtl[6] | sCtl[7]) != 0;
+            for (int o = 1; o < 32; o <<= 1) {
+                const int a0 = __shfl_up_sync(0xffffffffu, i0, o), a1 = __shfl_up_sync(0xffffffffu, i1, o);
+                if (lane >= o) { i0 += a0; i1 += a1; }
+            }
+            const int tot0 = __shfl_sync(0xffffffffu, i0, 31);
+            total = tot0 + __shfl_sync(0xffffffffu, i1, 31);
+            const int ex0 = i0 - c0, ex1 = tot0 + i1 - c1;
+            const bool live = __any_sync(0xffffffffu, r0 >= 0 || r1 >= 0);
+            if (sCtl[2] || !live) break;                             // abort, or every request is done (block-uniform)
+            for (int b = warp; b < batch; b += kWvThreads / 32) {
+                const int off = __shfl_sync(0xffffffffu, (b < 32) ? ex0 : ex1, b & 31);
+                const int cb = __shfl_sync(0xffffffffu, (b < 32) ? c0 : c1, b & 31);
+                const int first = 1 + sCum[b];
+                if (lane < cb) {
+                    const unsigned long long w = sRaw[b * kWvDescWords + lane];
+                    const int tok = min((int)(w >> 44), e.V - 1), ps = (int)((w >> 34) & 0x3FFull);
+                    sItems[off + lane] = wave_citem_pack(tok, ps, first + lane, b, lane);
+                }
+                __syncwarp();
+                if (lane == 0) sCum[b] = first - 1 + cb;
+            }
         }
         __syncthreads();
-        const int total = sCtl[0];
-        if (sCtl[2] || !sCtl[1]) break;                              // abort, or every request is done
         WV_TR(0, cta == 0, s, 0);
 
         for (int p0 = 0; p0 < total; p0 += kWvNP) {
             const int n = min(kWvNP, total - p0);
-            // ---- items of this pass: thread i < n fetches item p0 + i
-            if (tid < kWvNP) {
-                int row = 0, nw = 0, tok = 0, it = 0, pz = 1;
-                if (tid < n) {
-                    const int qi = p0 + tid;
-                    int lo = 0, hi = kWvMaxBatch - 1;                // last b with sOff[b] <= qi: its list is not empty
-                    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (sOff[mid] <= qi) lo = mid; else hi = mid - 1; }
-                    const int b = lo, j = qi - sOff[b];
-                    unsigned long long w = 0ull;
-                    const unsigned long long *ip = p.desc + (size_t)b * kWvDescWords + 1 + j;
-                    const bool ok = wave_spin([&] { w = ld_relaxed_u64(ip); return wave_item_ok(w, rnd, s + 1); }, p.err);
-                    if (!ok) sCtl[2] = 1;
-                    const int ps = (int)((w >> 22) & 0x3FFull);
-                    tok = (int)(w >> 32);
-                    tok = min(max(tok, 0), e.V - 1);
-                    row = b * (int)stride + ps; nw = b * (int)stride + sFirst[b] + j; it = b * kWvMaxW + j; pz = (ps == 0);
-                }
-                sRow[tid] = row; sNew[tid] = nw; sTok[tid] = tok; sIt[tid] = it; sPz[tid] = pz;
-            }
-            __syncthreads();
-            WV_TR(0, cta == 0 && p0 == 0, s, 1);
-
-            // ---- this pass: the parents' states are operand B of D1[64 x N] = W_hh slice . [S_hi | S_lo]^T with N = 2 nh columns
-            // (hi halves of the nh = 4 ceil(n / 4) nodes, then their lo halves); ring slots of N / 8 row groups per k-block
+            // this pass: the parents' states are operand B of D1[64 x N] = W_hh slice . [S_hi | S_lo]^T with N = 2 nh columns (hi halves
+            // of the nh = 4 ceil(n / 4) nodes, then their lo halves): the tensor core fetches (64 + N) x 32 bytes of operands per
+            // K = 16 step at ~64 B/clk, so a pass of few nodes is short.  A ring slot holds two k-blocks of N rows, so such a pass
+            // also keeps every K chunk in flight at once and a full pass streams through 3 slots
             const int nh = 4 * ((n + 3) >> 2), N = 2 * nh;
             const int kb_bytes = (N >> 3) * 1024, slot_bytes = 2 * kb_bytes;
             const int nslot = min(min(n_kc, 8), kWvRingBytes / slot_bytes);
@@ -367,86 +375,143 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
             // independent D1 accumulators, npad columns apart; the same four whatever N is, so that the association of the
             // K sum (and with it every bit of the result) does not depend on how many nodes share the pass
             constexpr int NA = 4, npad = kWvTmemCols / NA;
+            WV_TR(0, cta == 0 && p0 == 0, s, 1);
             // ---- epilogue operands (input half from P, previous state): issued now, consumed after the MMAs
             float4 pr = make_float4(0.f, 0.f, 0.f, 0.f), pz4 = pr, pn = pr, hp = pr;
             const bool mine = (my_node < n);
+            int my_new = 0, my_it = 0;
             if (mine) {
-                const float *prow = e.P + (size_t)sTok[my_node] * 3 * g + u0 + my_u;
+                const unsigned long long it = sItems[p0 + my_node];
+                const int tok = (int)(it & 0xFFFFFull), ps = (int)((it >> 20) & 0x3FFull), bq = (int)((it >> 40) & 0x7Full);
+                my_new = bq * stride + (int)((it >> 30) & 0x3FFull);
+                my_it = bq * kWvMaxW + (int)((it >> 47) & 0xFull);
+                const float *prow = e.P + (size_t)tok * 3 * g + u0 + my_u;
                 pr = __ldg(reinterpret_cast<const float4 *>(prow));
                 pz4 = __ldg(reinterpret_cast<const float4 *>(prow + g));
                 pn = __ldg(reinterpret_cast<const float4 *>(prow + 2 * g));
-                if (!sPz[my_node]) hp = __ldcg(reinterpret_cast<const float4 *>(p.s32 + (size_t)sRow[my_node] * g + u0 + my_u));
+                if (ps) hp = __ldcg(reinterpret_cast<const float4 *>(p.s32 + ((size_t)bq * stride + ps) * g + u0 + my_u));
             }
             WV_TR(0, cta == 0 && p0 == 0, s, 2);
 
-            // ---- D1[64 x N] = W_hh slice . [S_hi | S_lo]^T, K streamed through the ring by a warp-specialised pipeline with no
-            // CTA barrier inside: warps 2..7 produce (cp.async into the slot, completion tracked by the slot's `full`
-            // mbarrier), lane 0 of warps 0 and 1 consume (tcgen05.mma, tcgen05.commit on the slot's `empty` mbarrier).
+            // ---- D1[64 x N] = W_hh slice . [S_hi | S_lo]^T, K streamed through the ring by a warp-specialised pipeline
+            // with no CTA barrier inside: warps 4..7 produce (cp.async into the slot, completion tracked by the slot's `full`
+            // mbarrier), lane 0 of warps 0..3 consume (tcgen05.mma, tcgen05.commit on the slot's `empty` mbarrier).
             if (warp >= 4) {
-                // producer: 16-byte piece ptid & 15 of operand rows rho = (ptid >> 4) + 8 i
+                // producer: 16-byte piece ptid & 15 of operand rows rho = (ptid >> 4) + 8 i (row rho < nh: hi half of node rho)
                 const int ptid = tid - 128, piece = ptid & 15, kb = piece >> 3, pc = piece & 7;
-                const __nv_bfloat16 *src[16];
-#pragma unroll
-                for (int i = 0; i < 16; ++i) {
-                    const int rho = (ptid >> 4) + 8 * i;
+                const int r7 = ptid >> 4;                            // rho & 7, the same for all rows of a thread
+                const uint32_t doff = tc::smem_u32(sRing) + (uint32_t)(kb * kb_bytes + r7 * 128 + ((pc ^ r7) << 4));
+                const int nfirst = min(nslot, n_kc), ngrp = N >> 3;
+                // source of this thread's piece of row group i (null: the row is not in use)
+                auto src_of = [&](int i) -> const __nv_bfloat16 * {
+                    const int rho = r7 + 8 * i;
                     const int hl = (rho >= nh), node = rho - (hl ? nh : 0);
-                    src[i] = nullptr;
-                    if (rho < N && node < n) src[i] = (hl ? p.s_lo : p.s_hi) + (size_t)sRow[node] * g + (size_t)piece * 8;
-                }
-                const int r7 = (ptid >> 4) & 7;                      // rho & 7 is the same for all 16 rows of a thread
-                const uint32_t doff = (uint32_t)(kb * kb_bytes + r7 * 128 + ((pc ^ r7) << 4));
-#pragma unroll 1
-                for (int kc = 0; kc < n_kc; ++kc) {
-                    const int sl = kc % nslot;
-                    if (kc >= nslot) {                           // the MMAs of the slot's previous chunk have read it
-                        tc::mbar_wait(mb0 + 80 + 8 * sl, (ph_empty >> sl) & 1u);
-                        ph_empty ^= 1u << sl;
+                    if (node >= n) return nullptr;
+                    const unsigned long long it = sItems[p0 + node];
+                    const size_t row = (size_t)((unsigned int)(it >> 40) & 0x7Fu) * stride + (size_t)((unsigned int)(it >> 20) & 0x3FFu);
+                    return (hl ? p.s_lo : p.s_hi) + row * g + (size_t)piece * 8;
+                };
+                // A copy instruction occupies the LSU for ~14 cycles even with every lane predicated off, divisions and address
+                // conversions cost hundreds of cycles with one warp per scheduler: real (uniform) branches around unused row
+                // groups, no division, shared-space addresses.  The chunks that fit the ring at once go row group by row group
+                // and share ONE arrive-on-completion (it sits in the copy queue: later copies would wait behind it).
+                if (nfirst == n_kc) {
+#pragma unroll 2
+                    for (int i = 0; i < ngrp; ++i) {
+                        const __nv_bfloat16 *sp = src_of(i);
+                        if (__ballot_sync(0xffffffffu, sp != nullptr) == 0u) continue;     // nobody in the warp has this row group
+                        if (sp) {
+                            int kcs = kshift;
+#pragma unroll 4
+                            for (int kc = 0; kc < nfirst; ++kc) {
+                                wave_cp_async16_s(doff + (uint32_t)(kc * slot_bytes + i * 1024), sp + (size_t)kcs * kWvKC);
+                                if (++kcs == n_kc) kcs = 0;
+                            }
+                        }
                     }
-                    unsigned char *dst = sRing + (size_t)sl * slot_bytes + doff;
-                    const size_t k0 = (size_t)((kc + kshift) % n_kc) * kWvKC;
+                    wave_cp_async_arrive(mbGrp);
+                } else {
+                    // a large pass streams through the ring: chunk by chunk, a slot refilled once the MMAs of its previous chunk
+                    // have read it (at least 7 of the 16 row groups are in use, so the sources live in registers)
+                    const __nv_bfloat16 *src[16];
 #pragma unroll
-                    for (int i = 0; i < 16; ++i)
-                        if (src[i]) cp_async16(dst + i * 1024, src[i] + k0);   // rho >> 3 = i
-                    wave_cp_async_arrive(mb0 + 8 * sl);
+                    for (int i = 0; i < 16; ++i) src[i] = (i < ngrp) ? src_of(i) : nullptr;
+                    int sl = 0, kcs = kshift;
+#pragma unroll 1
+                    for (int kc = 0; kc < n_kc; ++kc) {
+                        if (kc >= nslot) {
+                            tc::mbar_wait(mbEmpty + 8 * sl, (ph_empty >> sl) & 1u);
+                            ph_empty ^= 1u << sl;
+                        }
+                        const uint32_t dst = doff + (uint32_t)(sl * slot_bytes);
+                        const size_t k0 = (size_t)kcs * kWvKC;
+#pragma unroll
+                        for (int i = 0; i < 16; ++i)
+                            if (src[i]) wave_cp_async16_s(dst + i * 1024, src[i] + k0);
+                        if (kc == nfirst - 1) wave_cp_async_arrive(mbGrp);
+                        else if (kc >= nfirst) wave_cp_async_arrive(mbFull + 8 * sl);
+                        if (++sl == nslot) sl = 0;
+                        if (++kcs == n_kc) kcs = 0;
+                    }
                 }
             } else if (lane == 0) {
-                // consumer: warp w issues K = 16 steps 2 w, 2 w + 1 of every chunk into its own accumulator D1[w] (a thread needs
-                // ~120 cycles to issue one tcgen05.mma and ~200 for a commit, so four threads share the work)
+                // consumer: warp w issues K = 16 steps 2 w, 2 w + 1 of every chunk into its own accumulator D1[w].  MMAs are issued
+                // in bursts: every wait -> proxy fence -> issue round costs a few hundred ns, the MMAs themselves tens, so the
+                // first burst takes every chunk the ring holds (all of K when the pass is small), the rest follow chunk by chunk
                 const int kbw = warp >> 1, s40 = (warp & 1) * 2;
+                tc::fence_after_sync();
+                int kc = 0, sl = 0, kcs = kshift;
+                const uint64_t daw = descW0 + (uint64_t)(kbw * 64 + s40 * 2);
+                const uint64_t dbw = descR0 + (uint64_t)((kbw * kb_bytes) / 16 + s40 * 2);
 #pragma unroll 1
-                for (int kc = 0; kc < n_kc; ++kc) {
-                    const int sl = kc % nslot;
-                    tc::mbar_wait(mb0 + 8 * sl, (ph_full >> sl) & 1u);
-                    ph_full ^= 1u << sl;
+                while (kc < n_kc) {
+                    const int k1 = (kc == 0) ? min(nslot, n_kc) : kc + 1;
+                    if (kc == 0) { tc::mbar_wait(mbGrp, ph_grp); ph_grp ^= 1u; }
+                    else { tc::mbar_wait(mbFull + 8 * sl, (ph_full >> sl) & 1u); ph_full ^= 1u << sl; }
+                    WV_TR(0, cta == 0 && p0 == 0 && kc == 0, s, 8);
                     tc::fence_proxy_async();
-                    tc::fence_after_sync();
-                    const uint64_t da = descW0 + (uint64_t)((((kc + kshift) % n_kc) * 2 + kbw) * 64 + s40 * 2);
-                    const uint64_t db = descR0 + (uint64_t)((sl * slot_bytes + kbw * kb_bytes) / 16 + s40 * 2);
-                    tc::mma_bf16(tmem + warp * npad, da, db, idesc1, kc ? 1u : 0u);
-                    tc::mma_bf16(tmem + warp * npad, da + 2, db + 2, idesc1, 1u);
-                    if (kc + nslot < n_kc) tc::commit(mb0 + 80 + 8 * sl);        // this slot will be refilled
-                    if (kc == n_kc - 1) tc::commit(mb0 + 64);
+#pragma unroll 1
+                    for (int q = kc; q < k1; ++q) {
+                        const uint64_t da = daw + (uint64_t)(kcs * 128);
+                        const uint64_t db = dbw + (uint64_t)((sl * slot_bytes) >> 4);
+                        tc::mma_bf16(tmem + warp * npad, da, db, idesc1, q ? 1u : 0u);
+                        tc::mma_bf16(tmem + warp * npad, da + 2, db + 2, idesc1, 1u);
+                        if (q + nslot < n_kc) tc::commit(mbEmpty + 8 * sl);      // this slot will be refilled
+                        if (++sl == nslot) sl = 0;
+                        if (++kcs == n_kc) kcs = 0;
+                    }
+                    kc = k1;
                 }
+                tc::commit(mbD1);
+                WV_TR(0, cta == 0 && p0 == 0, s, 9);
             }
             __syncwarp();
-            tc::mbar_wait(mb0 + 64, ph_d1); ph_d1 ^= 1u;
+            tc::mbar_wait(mbD1, ph_d1); ph_d1 ^= 1u;
             tc::fence_after_sync();
             __syncwarp();
             WV_TR(0, cta == 0 && p0 == 0, s, 3);
 
             // ---- TMEM -> shared: an M = 64 accumulator keeps row 16 q + i in lane 32 q + i (i < 16), so quadrant q holds gate q
-            // (r, z, n) of the 16 units; the two accumulators and the hi / lo column blocks are added here (fixed order)
+            // (r, z, n) of the 16 units; the four accumulators and the hi / lo column blocks are added here (fixed order)
             if (q4 < 3 && 16 * hsel < nh) {
 #pragma unroll 1
                 for (int c16 = hsel; 16 * c16 < nh; c16 += 2) {
-                    float v0[16], v1[16], v2[16];
+                    float v0[16];
 #pragma unroll
                     for (int c = 0; c < 16; ++c) v0[c] = 0.f;
-#pragma unroll 1
-                    for (int a = 0; a < NA; ++a) {                   // accumulators in index order, hi then lo column block
-                        wave_tmem_ld16x2(tmem + tlane + a * npad + 16 * c16, tmem + tlane + a * npad + nh + 16 * c16, v1, v2);
 #pragma unroll
-                        for (int c = 0; c < 16; ++c) v0[c] += v1[c] + v2[c];
+                    for (int a2 = 0; a2 < NA; a2 += 2) {             // accumulators in index order, hi then lo column block
+                        uint32_t u[4][16];
+                        wave_tmem_ld16_nw(tmem + tlane + a2 * npad + 16 * c16, u[0]);
+                        wave_tmem_ld16_nw(tmem + tlane + a2 * npad + nh + 16 * c16, u[1]);
+                        wave_tmem_ld16_nw(tmem + tlane + (a2 + 1) * npad + 16 * c16, u[2]);
+                        wave_tmem_ld16_nw(tmem + tlane + (a2 + 1) * npad + nh + 16 * c16, u[3]);
+                        wave_tmem_wait_ld();
+#pragma unroll
+                        for (int c = 0; c < 16; ++c) {
+                            v0[c] += __uint_as_float(u[0][c]) + __uint_as_float(u[1][c]);
+                            v0[c] += __uint_as_float(u[2][c]) + __uint_as_float(u[3][c]);
+                        }
                     }
                     if (lane < 16) {
                         float4 *dst = reinterpret_cast<float4 *>(sH + (size_t)(16 * q4 + lane) * kWvLdH + 16 * c16);
@@ -458,11 +523,11 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
             tc::fence_before_sync();
             __syncthreads();
             // ---- gates (reading A2): thread = (node 16 q4 + il, units 8 hsel + 4 uh ..)
-            float acc[12];
+            float acc[24];
 #pragma unroll
             for (int gate = 0; gate < 3; ++gate)
 #pragma unroll
-                for (int c = 0; c < 4; ++c) acc[gate * 4 + c] = sH[(size_t)(16 * gate + my_u + c) * kWvLdH + my_node];
+                for (int c = 0; c < 4; ++c) acc[gate * 8 + c] = sH[(size_t)(16 * gate + my_u + c) * kWvLdH + my_node];
             {
                 const float prv[4] = {pr.x, pr.y, pr.z, pr.w}, pzv[4] = {pz4.x, pz4.y, pz4.z, pz4.w};
                 const float pnv[4] = {pn.x, pn.y, pn.z, pn.w}, hpv[4] = {hp.x, hp.y, hp.z, hp.w};
@@ -471,8 +536,8 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     const float rg = sigmoidf_fast(prv[c] + acc[c]);
-                    const float zg = sigmoidf_fast(pzv[c] + acc[4 + c]);
-                    const float ng = tanhf_fast(pnv[c] + rg * acc[8 + c]);
+                    const float zg = sigmoidf_fast(pzv[c] + acc[8 + c]);
+                    const float ng = tanhf_fast(pnv[c] + rg * acc[16 + c]);
                     hn[c] = mine ? ((1.0f - zg) * ng + zg * hpv[c]) : 0.f;
                     bh[c] = __float2bfloat16_rn(hn[c]);
                     bl[c] = __float2bfloat16_rn(hn[c] - __bfloat162float(bh[c]));
@@ -482,19 +547,30 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                 ph.y = (uint32_t)__bfloat16_as_ushort(bh[2]) | ((uint32_t)__bfloat16_as_ushort(bh[3]) << 16);
                 pl.x = (uint32_t)__bfloat16_as_ushort(bl[0]) | ((uint32_t)__bfloat16_as_ushort(bl[1]) << 16);
                 pl.y = (uint32_t)__bfloat16_as_ushort(bl[2]) | ((uint32_t)__bfloat16_as_ushort(bl[3]) << 16);
-                if (mine) {                                          // publish S_new: fp32 and the bf16 hi/lo split
-                    const size_t o = (size_t)sNew[my_node] * g + u0 + my_u;
-                    __stcg(reinterpret_cast<float4 *>(p.s32 + o), make_float4(hn[0], hn[1], hn[2], hn[3]));
-                    __stcg(reinterpret_cast<uint2 *>(p.s_hi + o), ph);
-                    __stcg(reinterpret_cast<uint2 *>(p.s_lo + o), pl);
-                }
+                // lane < 16 (hi row) collects the hi halves of units 8 hsel .. + 8, its partner (lo row) the lo halves
+                const uint2 snd = uh ? ph : pl;
+                uint2 rcv;
+                rcv.x = __shfl_xor_sync(0xffffffffu, snd.x, 16);
+                rcv.y = __shfl_xor_sync(0xffffffffu, snd.y, 16);
+                const uint4 piece = uh ? make_uint4(rcv.x, rcv.y, pl.x, pl.y) : make_uint4(ph.x, ph.y, rcv.x, rcv.y);
+                WV_TR(0, cta == 0 && p0 == 0, s, 10);
                 // all-gather over the cluster: block `crank` of every cluster CTA's sS2 (operand A of the W1 GEMM)
                 if (pend2) { wave_cluster_wait(); pend2 = false; }   // every peer's previous W1 GEMM has read its sS2
+                if (mine) {
 #pragma unroll
-                for (int c = 0; c < kWvCS; ++c) { wave_st_cluster_v2(s2_hi[c], ph); wave_st_cluster_v2(s2_lo[c], pl); }
+                    for (int c = 0; c < kWvCS; ++c) wave_st_cluster_v4(s2_dst[c], piece);
+                }
+                // the release of the arrive covers what was stored BEFORE it: the global stores come after, so the cluster
+                // does not wait for their round trip to L2 (the gpu fence in front of the flag does)
+                wave_cluster_arrive();
+                WV_TR(0, cta == 0 && p0 == 0, s, 11);
+                if (mine) {                                          // publish S_new: fp32 and the bf16 hi / lo split
+                    __stcg(reinterpret_cast<float4 *>(p.s32 + (size_t)my_new * g + u0 + my_u), make_float4(hn[0], hn[1], hn[2], hn[3]));
+                    __stcg(reinterpret_cast<uint4 *>((uh ? p.s_lo : p.s_hi) + (size_t)my_new * g + u0 + 8 * hsel), piece);
+                }
             }
-            wave_cluster_arrive();
             wave_cluster_wait();
+            WV_TR(0, cta == 0 && p0 == 0, s, 12);
             tc::fence_proxy_async();
             tc::fence_before_sync();
             __syncthreads();
@@ -506,22 +582,25 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
 #pragma unroll
                 for (int c = 0; c < kWvCS; ++c)
                     tc::mma_bf16(tmem, descS2 + (uint64_t)(c * 256), descW1 + (uint64_t)(c * rpc * 2), idesc2, c ? 1u : 0u);   // D1's columns are dead
-                tc::commit(mb0 + 72);
+                tc::commit(mbD2);
             }
-            tc::mbar_wait(mb0 + 72, ph_d2); ph_d2 ^= 1u;
+            WV_TR(0, cta == 0 && p0 == 0, s, 13);
+            tc::mbar_wait(mbD2, ph_d2); ph_d2 ^= 1u;
             tc::fence_after_sync();
             __syncwarp();
-            wave_cluster_arrive(); pend2 = true;                     // my sS2 may be overwritten by the next pass
             WV_TR(0, cta == 0 && p0 == 0, s, 5);
+            wave_cluster_arrive_relaxed(); pend2 = true;             // my sS2 may be overwritten by the next pass (no data to release)
             {
                 // partial[item][cluster][crank * rpc + col]: lanes < 16 store columns 0..7 of a 16-column block, lanes >= 16 8..15
-                float *prow = p.partial + ((size_t)(mine ? sIt[my_node] : 0) * p.P + (cta / kWvCS)) * r + crank * rpc;
+                float *prow = p.partial + ((size_t)my_it * p.P + (cta / kWvCS)) * r + crank * rpc;
 #pragma unroll 1
                 for (int blk = hsel; blk < rpc / 16; blk += 2) {
+                    uint32_t u[16];
+                    wave_tmem_ld16_nw(tmem + tlane + 16 * blk, u);
+                    wave_tmem_wait_ld();
                     float v[16];
-                    wave_tmem_ld16(tmem + tlane + 16 * blk, v);
 #pragma unroll
-                    for (int c = 0; c < 16; ++c) v[c] += __shfl_xor_sync(0xffffffffu, v[c], 16);
+                    for (int c = 0; c < 16; ++c) { v[c] = __uint_as_float(u[c]); v[c] += __shfl_xor_sync(0xffffffffu, v[c], 16); }
                     if (mine) {
                         const int col = 16 * blk + 8 * uh;
                         const float4 o0 = uh ? make_float4(v[8], v[9], v[10], v[11]) : make_float4(v[0], v[1], v[2], v[3]);
@@ -536,7 +615,10 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
             WV_TR(0, cta == 0 && p0 == 0, s, 6);
         }
         if (sCtl[2]) break;
-        if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, fbase + (unsigned int)(s + 1)); }
+        if (tid == 0) {
+            fence_release_gpu();                                     // states and partials of this step are visible before the flag
+            st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, fbase + (unsigned int)(s + 1));
+        }
         WV_TR(0, cta == 0, s, 7);
     }
     __syncthreads();
@@ -547,16 +629,42 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
 }
 
 // -------------------------------------------------------------------------------------- request role
+// The frontier is kept as a SORTED list G of the best known nodes (children of the nodes expanded so far), cut at B
+// entries: the known set only grows, so a node ranked beyond B can never enter the tree.  Sort key (larger = earlier):
+//     score desc, depth asc, token asc        [then parent position asc, then arrival order: never equal]
+// `depth asc` keeps a parent in front of a child whose fp32 score rounds to the parent's (g + logp == g happens for
+// saturated slices); everything else is the pop comparator of reading A8.  The first B - 1 entries are exactly the
+// nodes Algorithm 1 expands, so a step nominates the first W of them that are not expanded yet
+// (the first one is the node Algorithm 1 needs next, the others are speculative) and the round ends when there is none.
 struct WaveCtl {
     int n_exp;          // expansions allocated so far (expansion 0 = the root)
-    int c;              // committed pops: slots 1 .. c are final
     int n_items;        // items published for the coming step
-    int done, n_valid, n_stage, abort_, pad;
+    int nG;             // entries of the sorted frontier
+    int cur;            // which of the two frontier buffers is current
+    int done, n_stage, abort_, pad;
     int slDepth[kWvMaxSlices];      // depth whose candidate rows a slice holds (-1 = empty)
     int slUsed[kWvMaxSlices];       // last step that needs the slice
     int stage[kWvMaxSlices];        // slices to fill before the coming step
     signed char d2s[DT_MAX_L];      // depth -> slice (-1 = not resident)
 };
+// frontier entry: key = ord(score) (32) | 63 - depth (6, from bit 20) | 0xFFFFF - token (20);
+//                 meta = depth (6) | own expansion + 1 (10, from bit 6; 0 = not expanded) | parent expansion (10, from bit 16)
+__device__ __forceinline__ unsigned long long wave_gkey(float score, int depth, int tok) {
+    return ((unsigned long long)ord_key(score) << 32) | ((unsigned long long)(63 - min(depth, 63)) << 20) |
+           (unsigned long long)(0xFFFFFu - ((unsigned int)tok & 0xFFFFFu));
+}
+constexpr int kWvDropped = 0x3FFFFFFF;
+
+__host__ __device__ inline size_t wave_req_smem2(int r, int M, int B, int k, int W, int e_max, int n_slices) {
+    auto al = [](size_t x) { return (x + 15) / 16 * 16; };
+    size_t s = (size_t)n_slices * wave_slice_bytes(r, M) + 2 * al((size_t)n_slices * M * 4);
+    s += 2 * al((size_t)B * 8) + 2 * al((size_t)B * 4);                     // frontier, two buffers
+    s += al((size_t)W * k * 8) + al((size_t)W * k * 4);                     // new children
+    s += 3 * al((size_t)e_max * 4);                                         // eDep, eSco, ePos
+    s += al((size_t)W * r * 4) + al((size_t)W * M * 4) + al((size_t)W * M * 8);
+    s += al((size_t)4 * kWvMaxW * 4) + al(256);
+    return s + 1024;
+}
 
 __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char *smem_raw) {
     const ExpandParams &e = p.e;
@@ -573,23 +681,20 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
     unsigned char *sW2 = carve((size_t)nsl * slice_bytes);
     int *slTok = reinterpret_cast<int *>(carve((size_t)nsl * M * 4));
     float *slBase = reinterpret_cast<float *>(carve((size_t)nsl * M * 4));
-    unsigned long long *cKey = reinterpret_cast<unsigned long long *>(carve((size_t)e_max * k * 8));   // children of expansion x, best first
-    short *cExp = reinterpret_cast<short *>(carve((size_t)e_max * k * 2));                             // expansion of that child, -1 = none
-    int *eTok = reinterpret_cast<int *>(carve((size_t)e_max * 4));
-    int *ePar = reinterpret_cast<int *>(carve((size_t)e_max * 4));
-    int *eDep = reinterpret_cast<int *>(carve((size_t)e_max * 4));
-    float *eSco = reinterpret_cast<float *>(carve((size_t)e_max * 4));
-    unsigned int *simC = reinterpret_cast<unsigned int *>(carve((size_t)e_max * 4));   // replay state at the commit point
-    unsigned int *simT = reinterpret_cast<unsigned int *>(carve((size_t)e_max * 4));   // ... of the running replay
-    unsigned long long *hT = reinterpret_cast<unsigned long long *>(carve((size_t)e_max * 8));   // head key of every active list (0 = none)
-    int *nTok = reinterpret_cast<int *>(carve((size_t)N * 4));
-    int *nPar = reinterpret_cast<int *>(carve((size_t)N * 4));
-    int *nDep = reinterpret_cast<int *>(carve((size_t)N * 4));
-    float *nSco = reinterpret_cast<float *>(carve((size_t)N * 4));
+    unsigned long long *gKey[2];
+    unsigned int *gMeta[2];
+    gKey[0] = reinterpret_cast<unsigned long long *>(carve((size_t)B * 8));
+    gKey[1] = reinterpret_cast<unsigned long long *>(carve((size_t)B * 8));
+    gMeta[0] = reinterpret_cast<unsigned int *>(carve((size_t)B * 4));
+    gMeta[1] = reinterpret_cast<unsigned int *>(carve((size_t)B * 4));
+    unsigned long long *nKey = reinterpret_cast<unsigned long long *>(carve((size_t)W * k * 8));   // children of this step's items
+    unsigned int *nMeta = reinterpret_cast<unsigned int *>(carve((size_t)W * k * 4));
+    int *eDep = reinterpret_cast<int *>(carve((size_t)e_max * 4));                 // depth of expansion x's node
+    float *eSco = reinterpret_cast<float *>(carve((size_t)e_max * 4));             // its score
+    int *ePos = reinterpret_cast<int *>(carve((size_t)e_max * 4));                 // its position in the frontier (-1 root)
     float *sA = reinterpret_cast<float *>(carve((size_t)W * r * 4));
     float *sZ = reinterpret_cast<float *>(carve((size_t)W * M * 4));
     unsigned long long *sKey = reinterpret_cast<unsigned long long *>(carve((size_t)W * M * 8));   // (z, ~token) of every candidate
-    unsigned char *sRank = carve((size_t)W * M);
     int *itE = reinterpret_cast<int *>(carve((size_t)4 * kWvMaxW * 4));
     int *itTok = itE + kWvMaxW, *itPs = itTok + kWvMaxW;
     WaveCtl &ctl = *reinterpret_cast<WaveCtl *>(carve(256));
@@ -598,7 +703,6 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
     unsigned long long *my_desc = p.desc + (size_t)b * kWvDescWords;
 
     // fill the slices listed in ctl.stage with the candidate table of their depth: ids, base logits, the M rows of W2
-    // (compact code on purpose: the step loop has to stay inside the instruction cache)
     auto stage_slices = [&]() {
         const int ns = ctl.n_stage;
 #pragma unroll 1
@@ -630,16 +734,14 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
 
     if (tid == 0) {
         const int root = e.root_tokens[b];
-        ctl.n_exp = 1; ctl.c = 0; ctl.n_items = 1; ctl.done = 0; ctl.n_valid = 1; ctl.abort_ = 0;
+        ctl.n_exp = 1; ctl.n_items = 1; ctl.nG = 0; ctl.cur = 0; ctl.done = 0; ctl.abort_ = 0;
         for (int i = 0; i < kWvMaxSlices; ++i) { ctl.slDepth[i] = -1; ctl.slUsed[i] = -1; }
         for (int i = 0; i < DT_MAX_L; ++i) ctl.d2s[i] = -1;
         ctl.slDepth[0] = 0; ctl.slUsed[0] = 0; ctl.d2s[0] = 0; ctl.stage[0] = 0; ctl.n_stage = 1;
-        eTok[0] = root; ePar[0] = -1; eDep[0] = 0; eSco[0] = 0.f; simC[0] = 0u; simT[0] = 0u;
-        nTok[0] = root; nPar[0] = -1; nDep[0] = 0; nSco[0] = 0.f;
+        eDep[0] = 0; eSco[0] = 0.f; ePos[0] = -1;
         itE[0] = 0;
         // step 0: the root, whose parent state is the zero slot (reading A4)
-        st_relaxed_u64(my_desc + 1, wave_item_pack(rnd, 1, 0, min(max(root, 0), e.V - 1)));
-        st_relaxed_u64(my_desc, wave_hdr_pack(rnd, 1, 1, 0, 1));
+        st_relaxed_u64(my_desc, wave_item_pack(rnd, 1, 1, 0, 0, min(max(root, 0), e.V - 1)));
     }
     __syncthreads();
     stage_slices();
@@ -647,54 +749,57 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
 
     for (int s = 0;; ++s) {
         const int n_it = ctl.n_items;
-        // C = H W1h^T of the item's depth does not depend on the GRU CTAs: fetch it while waiting for them (A12: row = depth)
-        float4 cpre = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (tid < n_it * (r >> 2)) {
-            const int j = tid / (r >> 2), jq = tid - j * (r >> 2);
-            cpre = __ldg(reinterpret_cast<const float4 *>(e.C + ((size_t)b * L + eDep[itE[j]]) * r) + jq);
-        }
+        // the first round of the partial sums: who am I, where are my partials, and C = H W1h^T of the node's depth (A12: row =
+        // depth), which does not depend on the GRU CTAs: all of it while they work
+        const int r4 = r >> 2;
+        const int pair0 = tid >> 1, j0 = pair0 / r4, jq0 = pair0 - j0 * r4;
+        const bool act0 = pair0 < n_it * r4;
+        float4 cv0 = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (act0 && !(tid & 1)) cv0 = __ldg(reinterpret_cast<const float4 *>(e.C + ((size_t)b * L + eDep[itE[j0]]) * r) + jq0);
         if (warp == 0) {
-            bool ok = true;
-            for (int q = lane; q < p.n_gru; q += 32) {
-                const unsigned int *fp = p.flags + (size_t)q * kFusFlagStride;
-                ok = wave_spin([&] { return (int)(ld_relaxed_u32(fp) - (fbase + (unsigned int)(s + 1))) >= 0; }, p.err) && ok;
-            }
+            // all of a lane's flags are polled in one round trip per iteration
+            const unsigned int want = fbase + (unsigned int)(s + 1);
+            const bool ok = wave_spin([&] {
+                bool all = true;
+                for (int q = lane; q < p.n_gru; q += 32)
+                    all = all && ((int)(wave_ld_acquire_u32(p.flags + (size_t)q * kFusFlagStride) - want) >= 0);
+                return all; }, p.err);
             if (!ok) ctl.abort_ = 1;
         }
         __syncthreads();
         if (ctl.abort_) break;
         WV_TR(1, b == 0, s, 0);
 
-        // ---- a_j = SiLU(C + W1[:, d:] S_j): the P cluster partials are summed in a fixed order (batch-invariant);
-        // one thread per (item, four columns), all loads of a thread in flight at once
+        // ---- a_j = SiLU(C + W1[:, d:] S_j): the P cluster partials are summed in a fixed order (batch-invariant): two
+        // neighbouring lanes per (node, four columns) take the even / the odd clusters, all loads of a lane in flight at once
         {
-            const int r4 = r >> 2;
 #pragma unroll 1
-            for (int pair = tid; pair < n_it * r4; pair += kWvThreads) {
-                const int j = pair / r4, jq = pair - j * r4;
-                const float4 cv = (pair == tid) ? cpre : __ldg(reinterpret_cast<const float4 *>(e.C + ((size_t)b * L + eDep[itE[j]]) * r) + jq);
-                const float4 *pp = reinterpret_cast<const float4 *>(p.partial + ((size_t)(b * kWvMaxW + j) * P) * r) + jq;
-                float4 s0 = make_float4(0.f, 0.f, 0.f, 0.f), s1 = s0;
-                int q = 0;
-                for (; q + 16 <= P; q += 16) {
-                    float4 v[16];
+            for (int base = 0; base < 2 * n_it * r4; base += kWvThreads) {          // block-uniform trip count
+                const int idx = base + tid, pair = idx >> 1, h = idx & 1;
+                const bool act = base ? (pair < n_it * r4) : act0;
+                const int j = base ? (act ? pair / r4 : 0) : j0, jq = base ? (act ? pair - j * r4 : 0) : jq0;
+                float4 acc = make_float4(0.f, 0.f, 0.f, 0.f), cv = cv0;
+                if (act) {
+                    if (base && h == 0) cv = __ldg(reinterpret_cast<const float4 *>(e.C + ((size_t)b * L + eDep[itE[j]]) * r) + jq);
+                    const float4 *pp = reinterpret_cast<const float4 *>(p.partial + ((size_t)(b * kWvMaxW + j) * P) * r) + jq;
+#pragma unroll 1
+                    for (int q0 = h; q0 < P; q0 += 16) {
+                        float4 v[8];
 #pragma unroll
-                    for (int i = 0; i < 16; ++i) v[i] = __ldcg(pp + (size_t)(q + i) * r4);
+                        for (int i = 0; i < 8; ++i) v[i] = (q0 + 2 * i < P) ? __ldcg(pp + (size_t)(q0 + 2 * i) * r4) : make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-                    for (int i = 0; i < 16; i += 2) {
-                        s0.x += v[i].x; s0.y += v[i].y; s0.z += v[i].z; s0.w += v[i].w;
-                        s1.x += v[i + 1].x; s1.y += v[i + 1].y; s1.z += v[i + 1].z; s1.w += v[i + 1].w;
+                        for (int i = 0; i < 8; ++i) { acc.x += v[i].x; acc.y += v[i].y; acc.z += v[i].z; acc.w += v[i].w; }
                     }
                 }
-#pragma unroll 1
-                for (; q < P; ++q) {
-                    const float4 v = __ldcg(pp + (size_t)q * r4);
-                    s0.x += v.x; s0.y += v.y; s0.z += v.z; s0.w += v.w;
+                // even clusters + odd clusters, then C
+                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 1); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 1);
+                acc.z += __shfl_xor_sync(0xffffffffu, acc.z, 1); acc.w += __shfl_xor_sync(0xffffffffu, acc.w, 1);
+                if (act && h == 0) {
+                    float4 o;
+                    o.x = cv.x + acc.x; o.y = cv.y + acc.y; o.z = cv.z + acc.z; o.w = cv.w + acc.w;
+                    o.x *= sigmoidf_acc(o.x); o.y *= sigmoidf_acc(o.y); o.z *= sigmoidf_acc(o.z); o.w *= sigmoidf_acc(o.w);
+                    *reinterpret_cast<float4 *>(sA + (size_t)j * r + 4 * jq) = o;
                 }
-                float4 o;
-                o.x = cv.x + (s0.x + s1.x); o.y = cv.y + (s0.y + s1.y); o.z = cv.z + (s0.z + s1.z); o.w = cv.w + (s0.w + s1.w);
-                o.x *= sigmoidf_acc(o.x); o.y *= sigmoidf_acc(o.y); o.z *= sigmoidf_acc(o.z); o.w *= sigmoidf_acc(o.w);
-                *reinterpret_cast<float4 *>(sA + (size_t)j * r + 4 * jq) = o;
             }
         }
         cp_async_wait<0>();
@@ -702,7 +807,7 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
         WV_TR(1, b == 0, s, 1);
 
         // ---- z_m = ((base_m - base_0) + W2[cand_m, :] a) / T_eff   PAPER.md:143-144 (shift-invariant)
-        // a warp takes 8 candidate rows (one swizzle row group), four lanes per row
+        // a warp takes 8 candidate rows (one swizzle row group), four lanes per row; two accumulation chains per lane
 #pragma unroll 1
         for (int j = 0; j < n_it; ++j) {
             const int si = ctl.d2s[eDep[itE[j]]];
@@ -714,17 +819,18 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
 #pragma unroll 1
             for (int rg = warp; rg < (M + 7) / 8; rg += kWvThreads / 32) {
                 const unsigned char *rowp = sl + (size_t)rg * Ka * 1024 + rw * 128;
-                float acc = 0.f;
-#pragma unroll 2
+                float acc0 = 0.f, acc1 = 0.f;
+#pragma unroll 4
                 for (int v = qq; v < nvec; v += 4) {
                     const uint4 q = *reinterpret_cast<const uint4 *>(rowp + (size_t)(v >> 3) * 1024 + (((v & 7) ^ rw) << 4));
                     const float4 a0 = *reinterpret_cast<const float4 *>(aj + (size_t)v * 8);
                     const float4 a1 = *reinterpret_cast<const float4 *>(aj + (size_t)v * 8 + 4);
                     float f[8];
                     unpack8(q, f);
-                    acc = fmaf(f[0], a0.x, acc); acc = fmaf(f[1], a0.y, acc); acc = fmaf(f[2], a0.z, acc); acc = fmaf(f[3], a0.w, acc);
-                    acc = fmaf(f[4], a1.x, acc); acc = fmaf(f[5], a1.y, acc); acc = fmaf(f[6], a1.z, acc); acc = fmaf(f[7], a1.w, acc);
+                    acc0 = fmaf(f[0], a0.x, acc0); acc1 = fmaf(f[1], a0.y, acc1); acc0 = fmaf(f[2], a0.z, acc0); acc1 = fmaf(f[3], a0.w, acc1);
+                    acc0 = fmaf(f[4], a1.x, acc0); acc1 = fmaf(f[5], a1.y, acc1); acc0 = fmaf(f[6], a1.z, acc0); acc1 = fmaf(f[7], a1.w, acc1);
                 }
+                float acc = acc0 + acc1;
                 acc += __shfl_xor_sync(0xffffffffu, acc, 8);
                 acc += __shfl_xor_sync(0xffffffffu, acc, 16);
                 const int m = 8 * rg + rw;
@@ -738,19 +844,39 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
         __syncthreads();
         WV_TR(1, b == 0, s, 2);
 
-        // ---- top-k by (z desc, token asc): rank by counting over the sortable keys, `tpc` neighbouring lanes per candidate
+        // ---- slice log-softmax (reading A1) and top-k by (z desc, token asc): rank by counting over the sortable keys, `tpc`
+        // neighbouring lanes per candidate, every warp working for ONE node (it computes that node's max and log-sum-exp
+        // itself); the k best become frontier candidates with score g_parent + logp
         {
-            const int tot = n_it * M;
-            int tpc = 1;
-            while (tpc < 8 && tot * tpc * 2 <= kWvThreads) tpc <<= 1;
-            const int per = (M + tpc - 1) / tpc;
+            int ltpc = 3;                                            // log2 of the lanes per candidate
+            while (ltpc > 0 && n_it * ((M << ltpc) + 31 >> 5) > kWvThreads / 32) --ltpc;
+            const int tpc = 1 << ltpc;
+            const int wpi = ((M << ltpc) + 31) >> 5;                 // warps per node
+            const int per = (M + tpc - 1) >> ltpc;
+            int jw = 0, wl = warp;                                   // node of this warp within a round, warp within the node
+            while (wl >= wpi) { wl -= wpi; ++jw; }
+            int ipr = 0;                                             // nodes per round
+            for (int w = wpi; w <= kWvThreads / 32; w += wpi) ++ipr;
+            if (ipr < 1) ipr = 1;
 #pragma unroll 1
-            for (int base = 0; base < tot * tpc; base += kWvThreads) {      // block-uniform trip count
-                const int idx = base + tid, pair = idx / tpc, part = idx - pair * tpc;
-                const bool act = pair < tot;
-                const int j = act ? pair / M : 0, m = act ? pair - j * M : 0;
+            for (int j0s = 0; j0s < n_it; j0s += ipr) {
+                const int j = j0s + jw;
+                if (j >= n_it || jw >= ipr) continue;                // warp-uniform
+                const int x = itE[j];
+                const float *zj = sZ + (size_t)j * M;
                 const unsigned long long *kj = sKey + (size_t)j * M;
-                const unsigned long long mk = kj[m];
+                float zmax = -INFINITY;
+#pragma unroll 1
+                for (int m = lane; m < M; m += 32) zmax = fmaxf(zmax, zj[m]);
+                zmax = ord_key_inv(__reduce_max_sync(0xffffffffu, ord_key(zmax)));
+                float ssum = 0.f;
+#pragma unroll 1
+                for (int m = lane; m < M; m += 32) ssum += __expf(zj[m] - zmax);
+                ssum = warp_sum(ssum);
+                const float lse = __logf(ssum);
+                const int t = (wl * 32 + lane) >> ltpc, part = lane & (tpc - 1);   // candidate and the share of the keys it counts
+                const bool act = t < M;
+                const unsigned long long mk = act ? kj[t] : 0ull;
                 int rank = 0;
                 if (act) {
                     const int m0 = part * per, m1 = min(M, m0 + per);
@@ -765,139 +891,99 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                     for (; q < m1; ++q) rank += (kj[q] > mk);
                 }
                 for (int o = 1; o < tpc; o <<= 1) rank += __shfl_xor_sync(0xffffffffu, rank, o);
-                if (act && part == 0) sRank[(size_t)j * M + m] = (unsigned char)min(rank, 255);
-            }
-        }
-        __syncthreads();
-        // ---- slice log-softmax (reading A1) and the children list: one warp per node
-#pragma unroll 1
-        for (int j = warp; j < n_it; j += kWvThreads / 32) {
-            const int x = itE[j];
-            const float *zj = sZ + (size_t)j * M;
-            float zmax = -INFINITY;
-#pragma unroll 1
-            for (int m = lane; m < M; m += 32) zmax = fmaxf(zmax, zj[m]);
-            zmax = warp_max(zmax);
-            float ssum = 0.f;
-#pragma unroll 1
-            for (int m = lane; m < M; m += 32) ssum += expf(zj[m] - zmax);
-            ssum = warp_sum(ssum);
-            const float lse = logf(ssum);
-            const float gpar = eSco[x];
-            unsigned long long *ck = cKey + (size_t)x * k;
-#pragma unroll 1
-            for (int m = lane; m < M; m += 32) {
-                const int rank = sRank[(size_t)j * M + m];
-                if (rank < k) {
-                    const float lpm = (zj[m] - zmax) - lse;
-                    ck[rank] = ((unsigned long long)ord_key(gpar + lpm) << 32) | (sKey[(size_t)j * M + m] & 0xFFFFFFFFull);
+                if (act && part == 0 && rank < k) {
+                    const float lpm = (zj[t] - zmax) - lse;
+                    const int tok = (int)(0xFFFFFFFFu - (unsigned int)(mk & 0xFFFFFFFFull));
+                    const int cdep = eDep[x] + 1;
+                    nKey[j * k + rank] = wave_gkey(eSco[x] + lpm, cdep, tok);
+                    nMeta[j * k + rank] = (unsigned int)cdep | ((unsigned int)x << 16);
                 }
             }
-            __syncwarp();
-            // the list is kept sorted by the pop comparator itself (fp32 rounding of g + logp may merge two scores)
-            unsigned long long mk = 0ull;
-            int rk2 = 0;
-            if (lane < k) {
-                mk = ck[lane];
-#pragma unroll 1
-                for (int q = 0; q < k; ++q) rk2 += (ck[q] > mk);
-            }
-            __syncwarp();
-            if (lane < k) { ck[rk2] = mk; cExp[(size_t)x * k + lane] = -1; }
         }
         __syncthreads();
         WV_TR(1, b == 0, s, 3);
 
-        // ---- replay the heap from the commit point, nominate, publish (warp 0)
-        if (warp == 0) {
-            WV_TR(1, b == 0, s, 6);
-            const int n_exp = ctl.n_exp;
-            int t = ctl.c;
-            int n_pops = 0;
-            if (s == 0 && lane == 0) { simC[0] = kWvAct; }          // the root is slot 0; its children are known now
-            __syncwarp();
+        // ---- merge the n_it k new candidates into the sorted frontier (rank by counting, cut at B)
+        {
+            const int cur = ctl.cur, n_old = ctl.nG, n_new = n_it * k, tot = n_old + n_new;
+            const unsigned long long *oK = gKey[cur];
+            const unsigned int *oM = gMeta[cur];
+            unsigned long long *dK = gKey[cur ^ 1];
+            unsigned int *dM = gMeta[cur ^ 1];
+            // strict total order: key desc, then parent position asc, then index asc (old entries before new ones)
+            auto prec = [&](unsigned long long ka, unsigned int ma, int ia, unsigned long long kb, unsigned int mb, int ib) {
+                if (ka != kb) return ka > kb;
+                const int pa = ePos[(ma >> 16) & 0x3FFu], pb = ePos[(mb >> 16) & 0x3FFu];
+                if (pa != pb) return pa < pb;
+                return ia < ib;
+            };
+            int rk[2] = {0, 0};
+            unsigned long long mk[2] = {0ull, 0ull};
+            unsigned int mm[2] = {0u, 0u};
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int i = tid + h * kWvThreads;
+                if (i >= tot) continue;
+                const bool is_old = i < n_old;
+                mk[h] = is_old ? oK[i] : nKey[i - n_old];
+                mm[h] = is_old ? oM[i] : nMeta[i - n_old];
+                int rank = 0;
+                if (is_old) rank = i;
+                else {                                               // old entries in front of it: the list is sorted
+                    int lo = 0, hi = n_old;
+                    while (lo < hi) { const int mid = (lo + hi) >> 1; if (prec(oK[mid], oM[mid], mid, mk[h], mm[h], i)) lo = mid + 1; else hi = mid; }
+                    rank = lo;
+                }
 #pragma unroll 1
-            for (int x = lane; x < n_exp; x += 32) {
-                const unsigned int w = simC[x];
-                simT[x] = w;
-                hT[x] = ((w & kWvAct) && (int)(w & 0xFFu) < k) ? cKey[(size_t)x * k + (w & 0xFFu)] : 0ull;
+                for (int q = 0; q < n_new; ++q) {
+                    if (n_old + q == i) continue;
+                    rank += prec(nKey[q], nMeta[q], n_old + q, mk[h], mm[h], i) ? 1 : 0;
+                }
+                rk[h] = rank;
             }
-            __syncwarp();
-            WV_TR(1, b == 0, s, 7);
-            bool committing = true, finished = false;
-            int found = 0, c_new = t;
-            const int step_next = s + 1;
-            while (true) {
-                if (t >= B) { finished = committing; break; }
-                // every lane scans the lists it owns and keeps the best head with what the pop needs to know about it
-                unsigned long long bk = 0ull;
-                unsigned int bw = 0u;
-                int be = -1;
+            __syncthreads();                                         // every rank is computed from the old positions
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int i = tid + h * kWvThreads;
+                if (i >= tot) continue;
+                const int own = (int)((mm[h] >> 6) & 0x3FFu);
+                if (rk[h] < B) { dK[rk[h]] = mk[h]; dM[rk[h]] = mm[h]; if (own) ePos[own - 1] = rk[h]; }
+                else if (own) ePos[own - 1] = kWvDropped;
+            }
+            if (tid == 0) { ctl.cur = cur ^ 1; ctl.nG = min(tot, B); }
+        }
+        __syncthreads();
+        WV_TR(1, b == 0, s, 6);
+
+        // ---- nominate (warp 0): the first W frontier entries among the first B - 1 that have depth < L and no expansion yet
+        if (warp == 0) {
+            const int cur = ctl.cur, nG = ctl.nG, n_exp = ctl.n_exp;
+            unsigned long long *cK = gKey[cur];
+            unsigned int *cM = gMeta[cur];
+            const int lim = min(nG, B - 1), step_next = s + 1;
+            int found = 0, c_first = -1;
+            bool stop = false;
 #pragma unroll 1
-                for (int x = lane; x < n_exp; x += 32) {
-                    const unsigned long long key = hT[x];
-                    if (key == 0ull) continue;
-                    const unsigned int w = simT[x];
-                    if (be < 0 || key > bk || (key == bk && (w >> 16) < (bw >> 16))) { bk = key; bw = w; be = x; }
-                }
-#ifdef DT_TRACE
-                const unsigned int wv_am = __activemask();
-                const bool wv_pr = (b == 0 && s < kWvTraceSteps && n_pops == 1 && lane == 0);
-                *(wv_pr ? &g_wv_trace[1][wv_pr ? s : 0][11] : &g_wv_trace_sink[threadIdx.x]) = wv_am;
-                const long long ck0 = clock64();
-#endif
-                if (__ballot_sync(0xffffffffu, be >= 0) == 0u) { finished = committing; break; }   // the candidate tree ran dry
-                // pop comparator of reading A8: score desc, token asc, parent slot asc
-                const unsigned int hi = (be >= 0) ? (unsigned int)(bk >> 32) : 0u;
-                const unsigned int mh = __reduce_max_sync(0xffffffffu, hi);
-                bool el = (be >= 0) && hi == mh;
-                const unsigned int ml = __reduce_max_sync(0xffffffffu, el ? (unsigned int)(bk & 0xFFFFFFFFull) : 0u);
-                el = el && (unsigned int)(bk & 0xFFFFFFFFull) == ml;
-                unsigned int bal = __ballot_sync(0xffffffffu, el);
-                if (__popc(bal) > 1) {                              // the same token at the same score under two parents
-                    const unsigned int mp = __reduce_min_sync(0xffffffffu, el ? (bw >> 16) : 0xFFFFFFFFu);
-                    bal = __ballot_sync(0xffffffffu, el && (bw >> 16) == mp);
-                }
-                const int wl = __ffs(bal) - 1;
-#ifdef DT_TRACE
-                *(wv_pr ? &g_wv_trace[1][wv_pr ? s : 0][12] : &g_wv_trace_sink[threadIdx.x]) = (unsigned long long)(clock64() - ck0);
-#endif
-                // the winning lane looks up its node; the rest of the warp gets the few words it needs by shuffle
-                int jc = 0, dep = 0, x = -1;
-                if (lane == wl) {
-                    jc = (int)(bw & 0xFFu);
-                    dep = eDep[be] + 1;
-                    x = cExp[(size_t)be * k + jc];
-                }
-                const int es = __shfl_sync(0xffffffffu, be, wl);
-                const unsigned int wv = __shfl_sync(0xffffffffu, bw, wl);
-                jc = __shfl_sync(0xffffffffu, jc, wl);
-                dep = __shfl_sync(0xffffffffu, dep, wl);
-                x = __shfl_sync(0xffffffffu, x, wl);
-                const int tok = (int)(0xFFFFFFFFu - ml);
-                const bool needs = (x < 0) && dep < L && (t + 1 < B);
-                if (committing && needs) {                          // everything before this pop is final
-#pragma unroll 1
-                    for (int y = lane; y < n_exp; y += 32) simC[y] = simT[y];
-                    c_new = t;
-                    committing = false;
-                    __syncwarp();
-                }
-                t += 1;
-                if (lane == wl) {
-                    simT[es] = wv + 1u;
-                    hT[es] = (jc + 1 < k) ? cKey[(size_t)es * k + jc + 1] : 0ull;
-                    nTok[t] = tok; nPar[t] = (int)(wv >> 16); nDep[t] = dep; nSco[t] = ord_key_inv(mh);
-                    if (x >= 0) { simT[x] = kWvAct | ((unsigned int)t << 16); hT[x] = cKey[(size_t)x * k]; }
-                }
-                bool stop = false;
-                if (needs) {                                        // warp-uniform; lane 0 decides, the verdict is broadcast
-                    // resources: a state slot (speculative picks leave room for the expansions Algorithm 1 still needs)
-                    // and a W2 slice for the node's depth
+            for (int i0 = 0; i0 < lim && !stop; i0 += 32) {
+                const int i = i0 + lane;
+                unsigned int m = 0u;
+                bool want = false;
+                if (i < lim) { m = cM[i]; want = ((m >> 6) & 0x3FFu) == 0u && (int)(m & 0x3Fu) < L; }
+                unsigned int bal = __ballot_sync(0xffffffffu, want);
+                while (bal && !stop) {
+                    const int ln = __ffs(bal) - 1;
+                    bal &= bal - 1;
+                    const int idx = i0 + ln;
+                    if (c_first < 0) c_first = idx;
                     int add = 0;
                     if (lane == 0) {
+                        const unsigned int mt = cM[idx];
+                        const unsigned long long ky = cK[idx];
+                        const int dep = (int)(mt & 0x3Fu), par = (int)((mt >> 16) & 0x3FFu);
                         const int xn = n_exp + found;
-                        bool can = (xn < e_max) && (found == 0 || xn + 1 + (B - c_new) <= e_max);
+                        // resources: a state slot (speculative picks leave room for the expansions Algorithm 1 still needs)
+                        // and a W2 slice for the node's depth
+                        bool can = (xn < e_max) && (found == 0 || xn + 1 + (B - c_first) <= e_max);
                         int si = -1;
                         if (can) {
                             si = ctl.d2s[dep];
@@ -917,10 +1003,9 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                         }
                         if (can) {
                             ctl.slUsed[si] = step_next;
-                            cExp[(size_t)es * k + jc] = (short)xn;
-                            eTok[xn] = tok; ePar[xn] = es; eDep[xn] = dep; eSco[xn] = ord_key_inv(mh);
-                            simC[xn] = 0u; simT[xn] = 0u; hT[xn] = 0ull;
-                            itE[found] = xn; itTok[found] = tok; itPs[found] = es + 1;
+                            cM[idx] = mt | ((unsigned int)(xn + 1) << 6);
+                            eDep[xn] = dep; eSco[xn] = ord_key_inv((unsigned int)(ky >> 32)); ePos[xn] = idx;
+                            itE[found] = xn; itTok[found] = (int)(0xFFFFFu - (unsigned int)(ky & 0xFFFFFull)); itPs[found] = par + 1;
                             add = 1;
                         }
                     }
@@ -928,29 +1013,20 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                     found += add;
                     stop = (add == 0) || found >= W;                // out of slots / slices, or the step is full
                 }
-                __syncwarp();
-#ifdef DT_TRACE
-                *(wv_pr ? &g_wv_trace[1][wv_pr ? s : 0][13] : &g_wv_trace_sink[threadIdx.x]) = (unsigned long long)(clock64() - ck0);
-#endif
-                n_pops += 1;
-                if (stop) break;
             }
-            WV_TR(1, b == 0, s, 8);
-#ifdef DT_TRACE
-            { const bool on = (threadIdx.x == 0 && b == 0 && s < kWvTraceSteps); *(on ? &g_wv_trace[1][on ? s : 0][10] : &g_wv_trace_sink[threadIdx.x]) = (unsigned long long)n_pops; }
-#endif
-            if (finished) {
+            __syncwarp();
+            if (c_first < 0) {                                       // nothing left to expand: the frontier is Algorithm 1's tree
                 if (lane == 0) {
-                    ctl.done = 1; ctl.n_valid = t + 1; ctl.n_items = 0; ctl.c = t;
-                    st_relaxed_u64(my_desc, wave_hdr_pack(rnd, s + 2, 0, 1, 0));
+                    ctl.done = 1; ctl.n_items = 0;
+                    st_relaxed_u64(my_desc, wave_item_pack(rnd, s + 2, 0, 1, 0, 0));
                     if (p.stats && b == 0) { p.stats[0] = (unsigned int)(s + 1); p.stats[1] = (unsigned int)n_exp; }
                 }
             } else {
-                if (lane < found) st_relaxed_u64(my_desc + 1 + lane, wave_item_pack(rnd, s + 2, itPs[lane], min(max(itTok[lane], 0), e.V - 1)));
-                if (lane == 0) {
-                    st_relaxed_u64(my_desc, wave_hdr_pack(rnd, s + 2, n_exp + 1, 0, found));
-                    ctl.n_items = found; ctl.n_exp = n_exp + found; ctl.c = c_new;
-                }
+                // every word carries the count; word 0 is written even when nothing could be nominated
+                if (lane < max(found, 1))
+                    st_relaxed_u64(my_desc + lane, wave_item_pack(rnd, s + 2, found, 0, lane < found ? itPs[lane] : 0,
+                                                                  lane < found ? itTok[lane] : 0));
+                if (lane == 0) { ctl.n_items = found; ctl.n_exp = n_exp + found; }
             }
             WV_TR(1, b == 0, s, 9);
         }
@@ -963,19 +1039,27 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
     }
     __syncthreads();
 
-    // emitter (a9): dead-leaf padding (reading A10), positions, ancestor-or-self mask
-    const int n = ctl.abort_ ? 1 : ctl.n_valid;
+    // emitter (a9): slots in frontier order, dead-leaf padding (reading A10), positions, ancestor-or-self mask
+    const int n = ctl.abort_ ? 1 : ctl.nG + 1;
+    const unsigned long long *fK = gKey[ctl.cur];
+    const unsigned int *fM = gMeta[ctl.cur];
+    int *nPar = reinterpret_cast<int *>(gKey[ctl.cur ^ 1]);         // parent slot of every output slot (the spare frontier buffer: 8 B >= 4 (B + 1))
     const int rpos = e.root_positions ? e.root_positions[b] : 0;
     for (int i = tid; i < N; i += kWvThreads) {
         const size_t so = (size_t)b * N + i;
-        const bool dead = (i >= n);
-        const int dep = dead ? 1 : nDep[i];
-        e.tokens[so] = dead ? 0 : nTok[i];
-        e.parents[so] = dead ? 0 : nPar[i];
-        e.depths[so] = dep;
-        e.scores[so] = dead ? -INFINITY : nSco[i];
-        e.positions[so] = rpos + dep;
-        if (dead) nPar[i] = 0;
+        int tok = 0, par = 0, dep = 1;
+        float sc = -INFINITY;
+        if (i == 0) { tok = e.root_tokens[b]; par = -1; dep = 0; sc = 0.f; }
+        else if (i < n) {
+            const unsigned long long ky = fK[i - 1];
+            const unsigned int mt = fM[i - 1];
+            tok = (int)(0xFFFFFu - (unsigned int)(ky & 0xFFFFFull));
+            par = ePos[(mt >> 16) & 0x3FFu] + 1;
+            dep = (int)(mt & 0x3Fu);
+            sc = ord_key_inv((unsigned int)(ky >> 32));
+        }
+        e.tokens[so] = tok; e.parents[so] = par; e.depths[so] = dep; e.scores[so] = sc; e.positions[so] = rpos + dep;
+        nPar[i] = (i < n) ? par : 0;
     }
     if (tid == 0) e.n_nodes[b] = n;
     uint8_t *mk = e.mask + (size_t)b * N * N;
