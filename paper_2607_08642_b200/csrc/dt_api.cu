@@ -45,8 +45,12 @@ struct dt_handle {
     // wavefront expansion (dt_wave.cuh): per-item partials, multi-item descriptors, device error word, counters
     float *wv_partial; unsigned long long *wv_desc; unsigned int *wv_err, *wv_stats, *wv_flags, *wv_round; int wave_ok, slot_stride;
     int64_t opt_wave_width;         // items per request per step (0 = auto)
+    int64_t opt_adaptive;           // 1 (default): the device picks wavefront or lock-step per round (wave_regime_kernel)
+    unsigned int *sched_sel;        // device word: sum over the rows of p1 in 16-bit fixed point (wave_regime_kernel)
+    unsigned int sched_thr;         // wavefront schedule when the sum is below this
     int wave_clusters;              // co-resident clusters of kWvCS CTAs (0 = not queried yet, -1 = unavailable)
-    int path_taken;                 // expansion path of the last dt_build_trees: 1 per-step, 2/3 fused mma.sync, 4 fused tcgen05, 5 wavefront
+    int path_taken;                 // expansion path of the last dt_build_trees: 1 per-step, 2/3 fused mma.sync, 4 fused tcgen05, 5 wavefront,
+                                    // 6 adaptive (wavefront or fused tcgen05 / mma.sync, chosen on the device per round)
     int64_t opt_expand_path;        // 0 auto, 1 per-step kernels, 2 fused mma.sync upc=8, 3 fused mma.sync upc=16, 4 fused tcgen05
     // host-call staging (lazy)
     char *stage; size_t stage_bytes;
@@ -138,6 +142,11 @@ extern "C" int dt_set_option(dt_handle *h, const char *name, int64_t value) {
         h->opt_wave_width = value;
         return DT_OK;
     }
+    if (!strcmp(name, "adaptive_schedule")) {
+        if (value < 0 || value > 1) return DT_ERR_INVALID_ARG;
+        h->opt_adaptive = value;
+        return DT_OK;
+    }
     if (!strcmp(name, "expand_path")) {
         if (value < 0 || value > 5) return DT_ERR_INVALID_ARG;
         h->opt_expand_path = value;
@@ -176,14 +185,15 @@ extern "C" int dt_get_option(dt_handle *h, const char *name, int64_t *value) {
     if (!h || !name || !value) return DT_ERR_INVALID_ARG;
     if (!strcmp(name, "expand_path_taken")) { *value = h->path_taken; return DT_OK; }
     if (!strcmp(name, "state_slots")) { *value = h->slot_stride; return DT_OK; }
-    const bool dev_word = !strcmp(name, "device_error") || !strcmp(name, "wave_steps") || !strcmp(name, "wave_expansions");
+    const bool dev_word = !strcmp(name, "device_error") || !strcmp(name, "wave_steps") || !strcmp(name, "wave_expansions") ||
+                          !strcmp(name, "schedule_chosen");
     if (!dev_word) return DT_ERR_INVALID_ARG;
     *value = 0;
     if (!h->wv_err) return DT_OK;
-    unsigned int w[12];
+    unsigned int w[20];
     DT_CUDA(h, cudaDeviceSynchronize());
     DT_CUDA(h, cudaMemcpy(w, h->wv_err, sizeof(w), cudaMemcpyDeviceToHost));
-    *value = !strcmp(name, "device_error") ? w[0] : !strcmp(name, "wave_steps") ? w[8] : w[9];
+    *value = !strcmp(name, "device_error") ? w[0] : !strcmp(name, "wave_steps") ? w[8] : !strcmp(name, "wave_expansions") ? w[9] : (w[16] < h->sched_thr ? 1 : 0);
     return DT_OK;
 }
 
@@ -253,6 +263,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     h->w = *w;
     h->max_batch = max_batch; h->L = L; h->max_M = max_M; h->max_B = max_B; h->k = k;
     h->heap_cap = max_B * k + k;
+    h->opt_adaptive = 1;
     h->esize = (w->dtype == DT_BF16) ? 2 : 4;
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess ||
@@ -339,7 +350,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         h->flags = (unsigned int *)(h->ws + o_sync);
         h->round_ctr = h->flags + (size_t)256 * kFusFlagStride;
         h->wv_partial = (float *)(h->ws + o_wpart); h->wv_desc = (unsigned long long *)(h->ws + o_wdesc);
-        h->wv_err = (unsigned int *)(h->ws + o_werr); h->wv_stats = h->wv_err + 8;
+        h->wv_err = (unsigned int *)(h->ws + o_werr); h->wv_stats = h->wv_err + 8; h->sched_sel = h->wv_err + 16;
         h->wv_flags = (unsigned int *)(h->ws + o_wsync); h->wv_round = h->wv_flags + (size_t)256 * kFusFlagStride;
         h->wave_ok = (slots <= 1023);
         bool ok = cudaDeviceGetAttribute(&h->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess;
@@ -462,7 +473,10 @@ extern "C" int dt_select_topm(dt_handle *h, const void *logits, int32_t rows, in
 
 // Fused persistent expansion (dt_fused.cuh).  Returns 1 if the shape does not fit (caller falls back
 // to the per-step kernels), DT_OK after enqueueing, or a negative error.
-static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool static_mode = false) {
+// `sel` >= 0: adaptive round, the kernel runs only when the device's schedule word equals it; `probe`: only report the fit;
+// `m_begin` / `m_end`: record the phase marks in front of / behind the launch
+static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool static_mode = false, int sel = -1, bool probe = false,
+                        bool m_begin = true, bool m_end = true) {
     if (!h->fused_ok || h->opt_expand_path == 1) return 1;
     int upc = 0;
     bool tcgen = false;
@@ -498,7 +512,9 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
     if (rs > (size_t)h->max_smem_optin) return 1;
     const size_t gs = tcgen ? fused_tc_smem(p.g, p.r) : fused_gru_smem(p.g, p.r, upc, f.m_tiles);
     const size_t dsm = gs > rs ? gs : rs;
-    int rc = phase_mark(h, 2, st);
+    if (probe) return DT_OK;
+    if (sel >= 0) { f.sched_sel = h->sched_sel; f.sched_want = (unsigned int)sel; f.sched_thr = h->sched_thr; }
+    int rc = m_begin ? phase_mark(h, 2, st) : DT_OK;
     if (rc) return rc;
     void *args[] = {&f};
     const dim3 grid(f.n_gru + p.batch), block(kFusThreads);
@@ -508,7 +524,7 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
     h->launches++;
     DT_CUDA(h, e);
     h->path_taken = tcgen ? 4 : (upc == 8 ? 2 : 3);
-    if (static_mode) return DT_OK;
+    if (static_mode || !m_end) return DT_OK;
     if ((rc = phase_mark(h, 3, st))) return rc;
     return phase_mark(h, 4, st);
 }
@@ -516,7 +532,8 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
 // Wavefront expansion (dt_wave.cuh).  Returns 1 if the shape does not fit (caller falls back to the lock-step fused
 // kernel), DT_OK after enqueueing, or a negative error.  Batches beyond what one cooperative launch holds (one request
 // CTA per request beside the g / 16 GRU CTAs) are split into consecutive launches: no cliff, requests are independent.
-static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st) {
+static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st, int sel = -1, bool probe = false, bool m_begin = true,
+                       bool m_end = true) {
     if (!h->fused_ok || !h->wave_ok || (h->opt_expand_path != 0 && h->opt_expand_path != 5)) return 1;
     if (p.g % kWvKC || p.g / 16 > 256 || p.r % 8 || p.r > 256 || p.k > 32 || p.M > 256 || p.L > DT_MAX_L || p.V > (1 << 20)) return 1;
     const int n_gru = p.g / 16;                          // a multiple of kWvCS (g is a multiple of 128)
@@ -539,7 +556,7 @@ static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st) {
     if (cap > kWvMaxBatch) cap = kWvMaxBatch;
     if (cap < 1) return 1;
     int W = (int)h->opt_wave_width;
-    if (W <= 0) { W = 96 / (p.batch < cap ? p.batch : cap); }
+    if (W <= 0) { W = 128 / (p.batch < cap ? p.batch : cap); }     // ~128 nodes per step over the batch: two GRU passes
     if (W < 1) W = 1;
     if (W > kWvMaxW) W = kWvMaxW;
     {   // a GRU CTA keeps at most kWvMaxItems compacted items per step; a request CTA merges at most 256 new candidates
@@ -557,7 +574,8 @@ static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st) {
     }
     if (nsl < 1) return 1;
     const size_t dsm = gs > rs ? gs : rs;
-    int rc = phase_mark(h, 2, st);
+    if (probe) return DT_OK;
+    int rc = m_begin ? phase_mark(h, 2, st) : DT_OK;
     if (rc) return rc;
     for (int b0 = 0; b0 < p.batch; b0 += cap) {
         const int nb = (p.batch - b0 < cap) ? (p.batch - b0) : cap;
@@ -578,6 +596,7 @@ static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st) {
         f.partial = h->wv_partial + (size_t)b0 * kWvMaxW * f.P * p.r;
         f.desc = h->wv_desc + (size_t)b0 * kWvDescWords;
         f.flags = h->wv_flags; f.round_ctr = h->wv_round; f.err = h->wv_err; f.stats = (b0 == 0) ? h->wv_stats : nullptr;
+        if (sel >= 0) { f.sched_sel = h->sched_sel; f.sched_want = (unsigned int)sel; f.sched_thr = h->sched_thr; }
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof(cfg));
         cfg.gridDim = dim3(n_gru + (nb + kWvCS - 1) / kWvCS * kWvCS); cfg.blockDim = dim3(kWvThreads);
@@ -591,6 +610,7 @@ static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st) {
         DT_CUDA(h, e);
     }
     h->path_taken = 5;
+    if (!m_end) return DT_OK;
     if ((rc = phase_mark(h, 3, st))) return rc;
     return phase_mark(h, 4, st);
 }
@@ -731,6 +751,22 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
     }
     h->path_taken = 1;
     if (w.dtype == DT_BF16) {
+        // adaptive round: both persistent kernels are enqueued, the device's schedule word lets one of them run
+        if (h->opt_expand_path == 0 && h->opt_adaptive && launch_wave(h, p, st, -1, true) == DT_OK &&
+            launch_fused(h, p, st, false, -1, true) == DT_OK) {
+            DT_CUDA(h, cudaMemsetAsync(h->sched_sel, 0, 4, st));
+            h->sched_thr = (unsigned int)(0.6 * 65536.0 * rows);
+            wave_regime_kernel<<<(rows + 7) / 8, 256, 0, st>>>(h->cand_val, rows, M, 1.0f / p.T_eff, h->sched_sel);
+            h->launches++;
+            DT_CUDA(h, cudaGetLastError());
+            rc = launch_wave(h, p, st, 1, false, true, false);
+            if (rc) return rc < 0 ? rc : DT_ERR_CUDA;
+            const int64_t n = h->launches;
+            rc = launch_fused(h, p, st, false, 0, false, false, true);
+            h->launches = n + 1;
+            h->path_taken = 6;
+            return rc < 0 ? rc : (rc ? DT_ERR_CUDA : DT_OK);
+        }
         rc = launch_wave(h, p, st);
         if (rc <= 0) return rc;
         rc = launch_fused(h, p, st);

@@ -64,6 +64,8 @@ struct FusedParams {
     // Cond-static arm: walk only the greedy chain (the frontier is dropped after every pop) for
     // B = L steps and record each depth's corrected top-k menu; the tree is then built by dt_scorers.cuh
     int static_mode;
+    // adaptive schedule (dt_api.cu): the kernel runs only when (*sched_sel < sched_thr) == sched_want (null: always)
+    const unsigned int *sched_sel; unsigned int sched_want, sched_thr;
     int32_t *menu_tok;             // [batch, L, k]
     float *menu_lp;                // [batch, L, k]
 };
@@ -950,6 +952,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
 template <int UPC>
 __global__ void __launch_bounds__(kFusThreads, 1) fused_expand_kernel(FusedParams p) {
     extern __shared__ __align__(1024) unsigned char fused_smem[];
+    if (p.sched_sel && (unsigned int)(*p.sched_sel < p.sched_thr) != p.sched_want) return;   // the other schedule was chosen (grid-uniform)
     if ((int)blockIdx.x < p.n_gru) {
         if constexpr (UPC == 0) fused_gru_role_tc(p, fused_smem);
         else fused_gru_role<UPC>(p, fused_smem);

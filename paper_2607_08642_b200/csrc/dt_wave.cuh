@@ -71,6 +71,7 @@ struct WaveParams {
     unsigned int *round_ctr;       // rounds this handle has run (tags every hand-over word)
     unsigned int *err;             // set to 1 when a hand-over wait timed out (protocol slip: fail, do not hang)
     unsigned int *stats;           // [4] optional counters of request 0: steps, expansions (measurement aid)
+    const unsigned int *sched_sel; unsigned int sched_want, sched_thr;   // run only when (*sched_sel < sched_thr) == sched_want (null: always)
 };
 
 // ---- hand-over words ---------------------------------------------------------------------------------
@@ -1071,8 +1072,26 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
     }
 }
 
+// Which schedule pays is a property of the round's candidate tables: bushy trees (flat slices) finish in a few wide
+// wavefront steps, chains (peaked slices) need one dependent step per node whatever the width, and there the lock-step
+// kernel's shorter step wins.  The decision is taken for the whole batch from the a1 output: the mean top-1 probability
+// of the base slices, p1 = 1 / sum_m exp((v_m - v_0) / T_eff) (reading A1 without the correction), against a threshold.
+// A warp per row adds its p1 in 16-bit fixed point to one device word (integer adds: the sum does not depend on their order);
+// the word is cleared by a memset node at the start of the round and compared with `sched_thr` by the expansion kernels.
+__global__ void __launch_bounds__(256) wave_regime_kernel(const float *cand_val, int rows, int M, float inv_T, unsigned int *acc) {
+    const int row = blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (row >= rows) return;
+    const float *v = cand_val + (size_t)row * M;
+    const float v0 = v[0];
+    float ssum = 0.f;
+    for (int m = threadIdx.x & 31; m < M; m += 32) ssum += __expf((v[m] - v0) * inv_T);
+    ssum = warp_sum(ssum);
+    if ((threadIdx.x & 31) == 0) atomicAdd(acc, (unsigned int)(65536.0f / ssum + 0.5f));
+}
+
 __global__ void __launch_bounds__(kWvThreads, 1) wave_expand_kernel(WaveParams p) {
     extern __shared__ __align__(1024) unsigned char wave_smem[];
+    if (p.sched_sel && (unsigned int)(*p.sched_sel < p.sched_thr) != p.sched_want) return;   // the other schedule was chosen (grid-uniform)
     if ((int)blockIdx.x < p.n_gru) wave_gru_role(p, wave_smem);
     else if ((int)blockIdx.x - p.n_gru < p.e.batch) wave_req_role(p, wave_smem);   // CTAs padding the last cluster leave
 }
