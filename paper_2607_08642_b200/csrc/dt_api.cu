@@ -55,6 +55,9 @@ struct dt_handle {
     // host-call staging (lazy)
     char *stage; size_t stage_bytes;
     // options / bookkeeping
+    int64_t opt_sel_span;           // 1: the bulk select kernel records its device-side span (first CTA start .. last CTA end)
+    unsigned long long *sel_span;
+    int64_t opt_gemm_serial;        // 1: the precompute GEMM runs after the select on the caller's stream (no overlap)
     int64_t opt_select_chunks;
     int64_t opt_select_kernel;      // 0 auto, 1 register-tile kernel only
     int64_t opt_schedule;           // 0 best-first heap (Alg. 1), 1 depth-synchronous frontier builder
@@ -167,6 +170,8 @@ extern "C" int dt_set_option(dt_handle *h, const char *name, int64_t value) {
         h->opt_scorer = value;
         return DT_OK;
     }
+    if (!strcmp(name, "select_span")) { h->opt_sel_span = value; return DT_OK; }
+    if (!strcmp(name, "precompute_serial")) { h->opt_gemm_serial = value; return DT_OK; }
     if (!strcmp(name, "select_kernel")) {
         if (value < 0 || value > 1) return DT_ERR_INVALID_ARG;
         h->opt_select_kernel = value;
@@ -186,13 +191,18 @@ extern "C" int dt_get_option(dt_handle *h, const char *name, int64_t *value) {
     if (!strcmp(name, "expand_path_taken")) { *value = h->path_taken; return DT_OK; }
     if (!strcmp(name, "state_slots")) { *value = h->slot_stride; return DT_OK; }
     const bool dev_word = !strcmp(name, "device_error") || !strcmp(name, "wave_steps") || !strcmp(name, "wave_expansions") ||
-                          !strcmp(name, "schedule_chosen");
+                          !strcmp(name, "schedule_chosen") || !strcmp(name, "select_span_ns");
     if (!dev_word) return DT_ERR_INVALID_ARG;
     *value = 0;
     if (!h->wv_err) return DT_OK;
-    unsigned int w[20];
+    unsigned int w[40];
     DT_CUDA(h, cudaDeviceSynchronize());
     DT_CUDA(h, cudaMemcpy(w, h->wv_err, sizeof(w), cudaMemcpyDeviceToHost));
+    if (!strcmp(name, "select_span_ns")) {
+        const unsigned long long t0 = ((unsigned long long)w[33] << 32) | w[32], t1 = ((unsigned long long)w[35] << 32) | w[34];
+        *value = (t1 > t0) ? (int64_t)(t1 - t0) : 0;
+        return DT_OK;
+    }
     *value = !strcmp(name, "device_error") ? w[0] : !strcmp(name, "wave_steps") ? w[8] : !strcmp(name, "wave_expansions") ? w[9] : (w[16] < h->sched_thr ? 1 : 0);
     return DT_OK;
 }
@@ -350,7 +360,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         h->flags = (unsigned int *)(h->ws + o_sync);
         h->round_ctr = h->flags + (size_t)256 * kFusFlagStride;
         h->wv_partial = (float *)(h->ws + o_wpart); h->wv_desc = (unsigned long long *)(h->ws + o_wdesc);
-        h->wv_err = (unsigned int *)(h->ws + o_werr); h->wv_stats = h->wv_err + 8; h->sched_sel = h->wv_err + 16;
+        h->wv_err = (unsigned int *)(h->ws + o_werr); h->wv_stats = h->wv_err + 8; h->sched_sel = h->wv_err + 16; h->sel_span = reinterpret_cast<unsigned long long *>(h->wv_err + 32);
         h->wv_flags = (unsigned int *)(h->ws + o_wsync); h->wv_round = h->wv_flags + (size_t)256 * kFusFlagStride;
         h->wave_ok = (slots <= 1023);
         bool ok = cudaDeviceGetAttribute(&h->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess;
@@ -367,8 +377,10 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     }
 
     h->sel_bulk_ok =
-        cudaFuncSetAttribute(select_topm_bulk_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSelBulkDynSmem) == cudaSuccess &&
-        cudaFuncSetAttribute(select_topm_bulk_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSelBulkDynSmem) == cudaSuccess;
+        cudaFuncSetAttribute(select_topm_bulk_kernel<__nv_bfloat16, SelectSmemBig>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_bulk_dyn_smem<SelectSmemBig>()) == cudaSuccess &&
+        cudaFuncSetAttribute(select_topm_bulk_kernel<float, SelectSmemBig>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_bulk_dyn_smem<SelectSmemBig>()) == cudaSuccess &&
+        cudaFuncSetAttribute(select_topm_bulk_kernel<__nv_bfloat16, SelectSmemW4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_bulk_dyn_smem<SelectSmemW4>()) == cudaSuccess &&
+        cudaFuncSetAttribute(select_topm_bulk_kernel<float, SelectSmemW4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_bulk_dyn_smem<SelectSmemW4>()) == cudaSuccess;
     if (!h->sel_bulk_ok) cudaGetLastError();
     int rc = DT_OK;
     if (cudaMemset(h->ws, 0, h->ws_bytes) != cudaSuccess) rc = DT_ERR_CUDA;
@@ -438,17 +450,29 @@ static int launch_select(dt_handle *h, const void *logits, int rows, int M, int3
     SelectParams p;
     p.logits = logits; p.rows = rows; p.V = V; p.M = M;
     p.row_vecs = (V + kvec - 1) / kvec;
-    int S = pick_chunks(h, rows, M, SelectSmemBig::kCap, p.row_vecs);
+    const bool w4 = false;                       // (4-warp CTAs, four per SM: measured slower, looser threshold claims)
+    int S = pick_chunks(h, rows, M, w4 ? SelectSmemW4::kCap : SelectSmemBig::kCap, p.row_vecs);
     if (S > p.row_vecs) S = p.row_vecs;
     p.S = S;
     p.chunk_vecs = (p.row_vecs + S - 1) / S;
     if (bulk) p.chunk_vecs = (p.chunk_vecs + kSelTileVecs - 1) / kSelTileVecs * kSelTileVecs;   // chunks start on tile boundaries
     p.cand_id = cand_id; p.cand_val = cand_val;
     p.part = h->sel_part; p.row_counter = h->sel_counter; p.row_tau = h->sel_tau;
+    p.span = nullptr;
+    if (h->opt_sel_span && bulk && h->sel_span) {
+        p.span = h->sel_span;
+        DT_CUDA(h, cudaMemsetAsync(h->sel_span, 0xFF, 8, st));
+        DT_CUDA(h, cudaMemsetAsync(h->sel_span + 1, 0, 8, st));
+    }
     dim3 grid(S, rows);
     if (bulk) {
-        if (h->w.dtype == DT_BF16) select_topm_bulk_kernel<__nv_bfloat16><<<grid, kSelThreads, kSelBulkDynSmem, st>>>(p);
-        else select_topm_bulk_kernel<float><<<grid, kSelThreads, kSelBulkDynSmem, st>>>(p);
+        if (h->w.dtype == DT_BF16) {
+            if (w4) select_topm_bulk_kernel<__nv_bfloat16, SelectSmemW4><<<grid, 128, sel_bulk_dyn_smem<SelectSmemW4>(), st>>>(p);
+            else select_topm_bulk_kernel<__nv_bfloat16, SelectSmemBig><<<grid, 256, sel_bulk_dyn_smem<SelectSmemBig>(), st>>>(p);
+        } else {
+            if (w4) select_topm_bulk_kernel<float, SelectSmemW4><<<grid, 128, sel_bulk_dyn_smem<SelectSmemW4>(), st>>>(p);
+            else select_topm_bulk_kernel<float, SelectSmemBig><<<grid, 256, sel_bulk_dyn_smem<SelectSmemBig>(), st>>>(p);
+        }
     } else if (h->w.dtype == DT_BF16) {
         if (aligned) select_topm_kernel<__nv_bfloat16, true><<<grid, kSelThreads, 0, st>>>(p);
         else select_topm_kernel<__nv_bfloat16, false><<<grid, kSelThreads, 0, st>>>(p);
@@ -698,7 +722,8 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
     // bf16: tensor cores, forked onto the handle's side stream so it overlaps the HBM-bound select (fork/join by
     // events: capture-safe, becomes a parallel graph branch).  Measured at C5: overlapped select + GEMM 64 us,
     // back to back 51 + 35 us.
-    if (mma) {
+    const bool serial = mma && h->opt_gemm_serial;
+    if (mma && !serial) {
         DT_CUDA(h, cudaEventRecord(h->ev_fork, st));
         DT_CUDA(h, cudaStreamWaitEvent(h->side, h->ev_fork, 0));
         rc = (h->tcg_ok && h->opt_gemm != 1)
@@ -710,7 +735,11 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
     rc = launch_select(h, marginal_logits, rows, M, h->cand_id, h->cand_val, st);
     if (rc) return rc;
     if ((rc = phase_mark(h, 1, st))) return rc;
-    if (mma) DT_CUDA(h, cudaStreamWaitEvent(st, h->ev_join, 0));
+    if (serial) {
+        rc = (h->tcg_ok && h->opt_gemm != 1)
+            ? launch_gemm_tc(h, backbone_hidden, w.d, w.corr_w1, (long long)w.d + w.g, h->C, w.r, rows, w.r, w.d, st)
+            : launch_gemm_mma(h, backbone_hidden, w.d, w.corr_w1, (long long)w.d + w.g, h->C, w.r, rows, w.r, w.d, st);
+    } else if (mma) DT_CUDA(h, cudaStreamWaitEvent(st, h->ev_join, 0));
     else if (w.dtype == DT_BF16)
         rc = launch_gemm_nt<__nv_bfloat16>(h, backbone_hidden, w.d, w.corr_w1, (long long)w.d + w.g, h->C, w.r, rows, w.r, w.d, st);
     else

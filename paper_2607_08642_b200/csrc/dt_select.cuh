@@ -44,6 +44,7 @@ struct SelectParams {
     unsigned long long *part;       // [rows, S, M] per-chunk sorted keys (S > 1)
     unsigned int *row_counter;      // [rows] arrival tickets, self-resetting
     unsigned int *row_tau;          // [rows] shared lower bound (ordered key), self-resetting
+    unsigned long long *span;       // optional measurement aid: [0] min %globaltimer at CTA start, [1] max at CTA end
 };
 
 template <typename T> struct SelOps;
@@ -125,27 +126,30 @@ template <> struct SelOps<float> {
 
 // Shared-memory state of one CTA.  SEG = keys per warp-private candidate segment (M <= SEG / 2),
 // FIN = survivors the epilogue ranks by counting, QCAP = per-warp queue of vectors awaiting the element filter.
-template <int SEG, int FIN, int QCAP>
+template <int SEG, int FIN, int QCAP, int NW>
 struct SelectSmemT {
-    static constexpr int kSeg = SEG, kCap = SEG * kSelWarps, kFin = FIN, kQ = QCAP;
-    unsigned long long cand[SEG * kSelWarps];   // 8 warp-private segments; reused for sorting / merging
+    static constexpr int kSeg = SEG, kCap = SEG * NW, kFin = FIN, kQ = QCAP, kWarps = NW;
+    unsigned long long cand[SEG * NW];          // NW warp-private segments; reused for sorting / merging
     unsigned long long fin[FIN];                // survivors of the final prune
-    uint4 qv[kSelWarps][QCAP];                  // per-warp queue: vectors that hold an element >= tau ...
-    int qi[kSelWarps][QCAP];                    // ... and their vector index in the row
-    unsigned int wcnt[kSelWarps];               // keys in each warp's segment
-    unsigned int claim[kSelWarps];              // c_w: >= q lanes of warp w have seen an element with ordered key >= c_w
-    unsigned int claimM[kSelWarps];             // >= M elements of warp w have ordered key >= claimM[w] (after a compaction)
+    int qi[NW][QCAP];                    // per-warp queue: row index of every vector that held an element >= tau when it
+                                                // streamed by; the vectors are read again (from L2) when the queue is filtered,
+                                                // normally once, after the chunk, against the FINAL threshold
+    unsigned int wcnt[NW];                      // keys in each warp's segment
+    unsigned int claim[NW];              // c_w: >= q lanes of warp w have seen an element with ordered key >= c_w
+    unsigned int claimM[NW];             // >= M elements of warp w have ordered key >= claimM[w] (after a compaction)
     unsigned int cnt2;
     unsigned int is_last;
 };
-using SelectSmemBig = SelectSmemT<512, 512, 64>;      // any M <= 256 (47 KB static)
+using SelectSmemBig = SelectSmemT<512, 512, 256, 8>;  // 8 warps, any M <= 256 (44 KB static)
+using SelectSmemW4 = SelectSmemT<512, 256, 128, 4>;   // 4 warps, M <= 128 (20 KB static): four CTAs per SM hold all 512 rows of a
+                                                      // batch-32 round at once (no second wave)
 
 // In-place descending bitonic sort of n (power of two) u64 keys in smem; all kSelThreads threads call.
 __device__ __forceinline__ void block_bitonic_desc(unsigned long long *s, int n) {
     const int tid = threadIdx.x;
     for (int k = 2; k <= n; k <<= 1) {
         for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int i = tid; i < n; i += kSelThreads) {
+            for (int i = tid; i < n; i += (int)blockDim.x) {
                 int ixj = i ^ j;
                 if (ixj > i) {
                     unsigned long long a = s[i], b = s[ixj];
@@ -174,6 +178,13 @@ __device__ __forceinline__ void warp_bitonic_desc(unsigned long long *s, int n, 
     }
 }
 
+__device__ __forceinline__ void sel_span_mark(unsigned long long *span, int which) {
+    if (span && threadIdx.x == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        if (which == 0) atomicMin(span, t); else atomicMax(span + 1, t);
+    }
+}
 __device__ __forceinline__ int next_pow2(int x) { int p = 1; while (p < x) p <<= 1; return p; }
 
 // q-th largest (1-based, q <= 32) of the 32 lanes' keys: the largest T with #{key >= T} >= q, built bit by bit
@@ -193,7 +204,7 @@ __device__ __forceinline__ unsigned int warp_qth_largest(unsigned int key, int q
 // Rank `n` distinct keys by counting and hand the top M to `emit(rank, key)`; all threads call.
 template <typename F>
 __device__ __forceinline__ void block_rank_emit(const unsigned long long *keys, int n, int M, F emit) {
-    for (int i = threadIdx.x; i < n; i += kSelThreads) {
+    for (int i = threadIdx.x; i < n; i += (int)blockDim.x) {
         const unsigned long long mk = keys[i];
         int rank = 0;
         int j = 0;
@@ -241,7 +252,7 @@ __device__ __noinline__ SelWarpCtx sel_compact(SM &sm, SelWarpCtx c, int M) {
 // Filter the queued vectors, one vector per lane: append every element that can still be in the top M.
 // A batch adds at most SEG / 2 keys; the segment is compacted first when it could overflow.
 template <typename T, typename SM>
-__device__ __noinline__ SelWarpCtx sel_drain(SM &sm, SelWarpCtx c, int M, int V) {
+__device__ __noinline__ SelWarpCtx sel_drain(SM &sm, SelWarpCtx c, int M, int V, const T *rowp, bool aligned) {
     using Ops = SelOps<T>;
     constexpr int kVec = ElemTraits<T>::kVec;
     constexpr int kBatchKeys = SM::kSeg / 2;
@@ -250,24 +261,38 @@ __device__ __noinline__ SelWarpCtx sel_drain(SM &sm, SelWarpCtx c, int M, int V)
     unsigned long long *seg = sm.cand + warp * SM::kSeg;
     volatile unsigned int *vwcnt = sm.wcnt;
     __syncwarp();
-    for (int base = 0; base < c.qcnt; base += kLanes) {
-        if ((int)vwcnt[warp] > SM::kSeg - kBatchKeys) c = sel_compact(sm, c, M);
-        if (lane < kLanes && base + lane < c.qcnt) {
-            const uint4 v = sm.qv[warp][base + lane];
-            const int gv = sm.qi[warp][base + lane];
-            unsigned int mask = Ops::ge_mask(v, Ops::make_tau(c.tau_ord));      // usually one bit
-            while (mask) {
-                const int i = __ffs(mask) - 1;
-                mask &= mask - 1;
-                const unsigned int idx = (unsigned int)gv * kVec + i;
-                const unsigned long long key = ((unsigned long long)ord_key(Ops::elem(v, i)) << 32) | (unsigned long long)(0xFFFFFFFFu - idx);
-                if (key > c.wtau_key && idx < (unsigned int)V) {
-                    const unsigned int pos = atomicAdd(&sm.wcnt[warp], 1u);
-                    seg[pos] = key;
+    constexpr int kU = 4;                                           // vectors per lane in flight: one L2 round trip per 4 batches
+    for (int base0 = 0; base0 < c.qcnt; base0 += kLanes * kU) {
+        uint4 vv[kU];
+        int gvv[kU];
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            const int qi = base0 + u * kLanes + lane;
+            gvv[u] = (lane < kLanes && qi < c.qcnt) ? sm.qi[warp][qi] : -1;
+            vv[u] = make_uint4(0u, 0u, 0u, 0u);
+            if (gvv[u] >= 0) vv[u] = aligned ? ld_ro_v4(rowp + (size_t)gvv[u] * kVec) : Ops::load_scalar(rowp, (long long)gvv[u] * kVec, V);
+        }
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            if (base0 + u * kLanes >= c.qcnt) break;                 // warp-uniform
+            if ((int)vwcnt[warp] > SM::kSeg - kBatchKeys) c = sel_compact(sm, c, M);
+            if (gvv[u] >= 0) {
+                const uint4 v = vv[u];
+                const int gv = gvv[u];
+                unsigned int mask = Ops::ge_mask(v, Ops::make_tau(c.tau_ord));      // usually one bit
+                while (mask) {
+                    const int i = __ffs(mask) - 1;
+                    mask &= mask - 1;
+                    const unsigned int idx = (unsigned int)gv * kVec + i;
+                    const unsigned long long key = ((unsigned long long)ord_key(Ops::elem(v, i)) << 32) | (unsigned long long)(0xFFFFFFFFu - idx);
+                    if (key > c.wtau_key && idx < (unsigned int)V) {
+                        const unsigned int pos = atomicAdd(&sm.wcnt[warp], 1u);
+                        seg[pos] = key;
+                    }
                 }
             }
+            __syncwarp();
         }
-        __syncwarp();
     }
     c.qcnt = 0;
     return c;
@@ -291,8 +316,8 @@ __device__ __forceinline__ unsigned int sel_read_tau(SM &sm, const SelectParams 
     constexpr unsigned int kFull = 0xffffffffu;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     volatile unsigned int *vclaim = sm.claim, *vclaimM = sm.claimM;
-    unsigned int cw = (lane < kSelWarps) ? vclaim[lane] : 0xFFFFFFFFu;
-    unsigned int cm = (lane < kSelWarps) ? vclaimM[lane] : 0u;
+    unsigned int cw = (lane < SM::kWarps) ? vclaim[lane] : 0xFFFFFFFFu;
+    unsigned int cm = (lane < SM::kWarps) ? vclaimM[lane] : 0u;
 #pragma unroll
     for (int o = 4; o > 0; o >>= 1) {
         cw = min(cw, __shfl_xor_sync(kFull, cw, o));
@@ -308,24 +333,16 @@ __device__ __forceinline__ unsigned int sel_read_tau(SM &sm, const SelectParams 
 }
 // One vector slot of a warp: lanes whose vector holds an element >= tau queue it; a full queue is drained.
 template <typename T, typename SM>
-__device__ __forceinline__ SelWarpCtx sel_slot(SM &sm, SelWarpCtx c, const uint4 &x, bool hit, int gv, int M, int V) {
+__device__ __forceinline__ SelWarpCtx sel_slot(SM &sm, SelWarpCtx c, bool hit, int gv, int M, int V, const T *rowp, bool aligned) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-#ifdef DT_EXP_SELDRY
-    hit = false;
-#endif
     const unsigned int bal = __ballot_sync(0xffffffffu, hit);
     if (bal) {
         if (hit) {
             const int pos = c.qcnt + __popc(bal & ((1u << lane) - 1u));
-            sm.qv[warp][pos] = x;
             sm.qi[warp][pos] = gv;
         }
         c.qcnt += __popc(bal);
-#ifdef DT_EXP_NODRAIN
-        if (c.qcnt > SM::kQ - 32) c.qcnt = 0;
-#else
-        if (c.qcnt > SM::kQ - 32) c = sel_drain<T>(sm, c, M, V);
-#endif
+        if (c.qcnt > SM::kQ - 32) c = sel_drain<T>(sm, c, M, V, rowp, aligned);
     }
     return c;
 }
@@ -360,14 +377,14 @@ __device__ __forceinline__ void sel_epilogue(SM &sm, const SelectParams &p, int 
     if (c2 <= SM::kFin) {
         if (p.S == 1) { block_rank_emit(sm.fin, c2, M, out_single); return; }
         block_rank_emit(sm.fin, c2, M, out_part);
-        for (int i = c2 + tid; i < M; i += kSelThreads) part[i] = 0ull;      // chunk with fewer than M elements
+        for (int i = c2 + tid; i < M; i += (int)blockDim.x) part[i] = 0ull;      // chunk with fewer than M elements
     } else {
         // adversarial rows (more than kFin survivors): sort everything that was kept
         const int n = (int)sm.wcnt[warp];
         for (int i = n + lane; i < SM::kSeg; i += 32) seg[i] = 0ull;
         __syncthreads();
         block_bitonic_desc(sm.cand, SM::kCap);
-        for (int i = tid; i < M; i += kSelThreads) { if (p.S == 1) out_single(i, sm.cand[i]); else out_part(i, sm.cand[i]); }
+        for (int i = tid; i < M; i += (int)blockDim.x) { if (p.S == 1) out_single(i, sm.cand[i]); else out_part(i, sm.cand[i]); }
         if (p.S == 1) return;
     }
 
@@ -387,7 +404,7 @@ __device__ __forceinline__ void sel_epilogue(SM &sm, const SelectParams &p, int 
     __syncthreads();
     const int tot = p.S * M;                                   // <= SM::kCap (launcher)
     const unsigned long long *allp = p.part + (size_t)row * p.S * M;
-    for (int i = tid; i < tot; i += kSelThreads) {
+    for (int i = tid; i < tot; i += (int)blockDim.x) {
         const unsigned long long key = __ldcg(allp + i);
         sm.cand[i] = key;
         if ((unsigned int)(key >> 32) >= gtau && key != 0ull) {
@@ -401,10 +418,10 @@ __device__ __forceinline__ void sel_epilogue(SM &sm, const SelectParams &p, int 
         block_rank_emit(sm.fin, c3, M, out_single);
     } else {
         const int n2 = next_pow2(max(tot, 2));
-        for (int i = tot + tid; i < n2; i += kSelThreads) sm.cand[i] = 0ull;
+        for (int i = tot + tid; i < n2; i += (int)blockDim.x) sm.cand[i] = 0ull;
         __syncthreads();
         block_bitonic_desc(sm.cand, n2);
-        for (int i = tid; i < M; i += kSelThreads) out_single(i, sm.cand[i]);
+        for (int i = tid; i < M; i += (int)blockDim.x) out_single(i, sm.cand[i]);
     }
     if (tid == 0) { p.row_counter[row] = 0u; p.row_tau[row] = 0u; }
 }
@@ -473,15 +490,13 @@ __global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParam
         for (int u = 0; u < kSelU; ++u) {
             const Run m = Ops::vmax(X[u]);
             run = Ops::rmax(run, m);
-            c = sel_slot<T>(sm, c, X[u], Ops::pass(m, tau), gv0 + u * kSelThreads, M, V);
+            c = sel_slot<T>(sm, c, Ops::pass(m, tau), gv0 + u * kSelThreads, M, V, rowp, ALIGNED);
         }
-#ifndef DT_EXP_NOCLAIM
         if (t > 0 && (((t + 1) & t) == 0) && (t + 1 < n_tiles)) {
             sel_publish_claim<T>(sm, run, q);
             __syncwarp();
             c.tau_ord = max(c.tau_ord, sel_read_tau(sm, p, row));
         }
-#endif
     };
     for (int t = 0; t < n_tiles; t += 2) {      // ping-pong between the two register tiles
         if (t + 1 < n_tiles) load_tile(t + 1, Bn);
@@ -491,11 +506,12 @@ __global__ void __launch_bounds__(kSelThreads, 4) select_topm_kernel(SelectParam
             process(Bn, t + 1);
         }
     }
-    c = sel_drain<T>(sm, c, M, V);
-
+    // the queue is filtered against the chunk's final threshold
     sel_publish_claim<T>(sm, run, q);
     __syncthreads();
     c.tau_ord = max(c.tau_ord, sel_read_tau(sm, p, row));
+    c = sel_drain<T>(sm, c, M, V, rowp, ALIGNED);
+    __syncthreads();
     sel_epilogue(sm, p, row, s, c.tau_ord);
 }
 
@@ -524,33 +540,34 @@ __device__ __forceinline__ void sel_bulk_load(unsigned int dst, const void *src,
 
 constexpr int kSelTileVecs = kSelTileBytes / 16;
 constexpr int kBulkU = kSelTileVecs / 32;        // vectors per lane per tile
-constexpr size_t kSelBulkDynSmem = (size_t)kSelWarps * kSelStages * kSelTileBytes + (size_t)kSelWarps * kSelStages * 8;
+template <typename SM> constexpr size_t sel_bulk_dyn_smem() { return (size_t)SM::kWarps * kSelStages * kSelTileBytes + (size_t)SM::kWarps * kSelStages * 8; }
 
-template <typename T>
-__global__ void __launch_bounds__(kSelThreads, 2) select_topm_bulk_kernel(SelectParams p) {
+template <typename T, typename SM>
+__global__ void __launch_bounds__(SM::kWarps * 32, SM::kWarps == 4 ? 4 : 2) select_topm_bulk_kernel(SelectParams p) {
     using Ops = SelOps<T>;
     using Run = typename Ops::Run;
-    using SM = SelectSmemBig;
+    constexpr int kNW = SM::kWarps;
     constexpr int kVec = ElemTraits<T>::kVec;
     __shared__ __align__(16) SM sm;
     extern __shared__ __align__(128) unsigned char sel_dyn[];
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    sel_span_mark(p.span, 0);
     const int row = blockIdx.y, s = blockIdx.x;
     const int M = p.M, V = p.V;
-    const int q = (M + kSelWarps - 1) / kSelWarps;
+    const int q = (M + kNW - 1) / kNW;
     const T *rowp = reinterpret_cast<const T *>(p.logits) + (size_t)row * V;
     const int v0 = s * p.chunk_vecs;
     const int v1 = min(p.row_vecs, v0 + p.chunk_vecs);
     const int n_ctiles = (max(v1 - v0, 0) + kSelTileVecs - 1) / kSelTileVecs;       // 2 KB tiles of the chunk
-    const int n_w = (n_ctiles > warp) ? (n_ctiles - warp + kSelWarps - 1) / kSelWarps : 0;   // tiles of this warp
+    const int n_w = (n_ctiles > warp) ? (n_ctiles - warp + kNW - 1) / kNW : 0;   // tiles of this warp
 
     unsigned char *ring = sel_dyn + (size_t)warp * kSelStages * kSelTileBytes;
     const unsigned int ring_a = (unsigned int)__cvta_generic_to_shared(ring);
-    const unsigned int bar_a = (unsigned int)__cvta_generic_to_shared(sel_dyn + (size_t)kSelWarps * kSelStages * kSelTileBytes) +
+    const unsigned int bar_a = (unsigned int)__cvta_generic_to_shared(sel_dyn + (size_t)kNW * kSelStages * kSelTileBytes) +
                                (unsigned int)warp * kSelStages * 8;
 
-    if (tid < kSelWarps) { sm.wcnt[tid] = 0; sm.claim[tid] = 0; sm.claimM[tid] = 0; }
+    if (tid < kNW) { sm.wcnt[tid] = 0; sm.claim[tid] = 0; sm.claimM[tid] = 0; }
     if (tid == 0) { sm.cnt2 = 0; sm.is_last = 0; }
     if (lane == 0) {
         for (int i = 0; i < kSelStages; ++i) sel_mbar_init(bar_a + 8 * i, 1);
@@ -560,7 +577,7 @@ __global__ void __launch_bounds__(kSelThreads, 2) select_topm_bulk_kernel(Select
 
     // tile i of this warp = chunk tile warp + 8 i: vectors [tv0, tv0 + nv)
     auto issue = [&](int i) {
-        const int tv0 = v0 + (warp + kSelWarps * i) * kSelTileVecs;
+        const int tv0 = v0 + (warp + kNW * i) * kSelTileVecs;
         const int nv = min(kSelTileVecs, v1 - tv0);
         const int slot = i % kSelStages;
         sel_bulk_load(ring_a + slot * kSelTileBytes, rowp + (size_t)tv0 * kVec, (unsigned int)nv * 16u, bar_a + 8 * slot);
@@ -571,7 +588,7 @@ __global__ void __launch_bounds__(kSelThreads, 2) select_topm_bulk_kernel(Select
     c.tau_ord = 0; c.wtau_key = 0ull; c.qcnt = 0;
     Run run = Ops::lowest();
     auto load_slot = [&](int i, uint4 (&X)[kBulkU]) {            // lane's vectors u * 32 + lane of tile i
-        const int nv = min(kSelTileVecs, v1 - (v0 + (warp + kSelWarps * i) * kSelTileVecs));
+        const int nv = min(kSelTileVecs, v1 - (v0 + (warp + kNW * i) * kSelTileVecs));
         const uint4 *src = reinterpret_cast<const uint4 *>(ring + (size_t)(i % kSelStages) * kSelTileBytes);
 #pragma unroll
         for (int u = 0; u < kBulkU; ++u) X[u] = (u * 32 + lane < nv) ? src[u * 32 + lane] : Ops::lowest_vec();
@@ -597,12 +614,12 @@ __global__ void __launch_bounds__(kSelThreads, 2) select_topm_bulk_kernel(Select
             issue(i + kSelStages);
         }
         const Run tau = Ops::make_tau(c.tau_ord);
-        const int gv0 = v0 + (warp + kSelWarps * i) * kSelTileVecs + lane;
+        const int gv0 = v0 + (warp + kNW * i) * kSelTileVecs + lane;
 #pragma unroll
         for (int u = 0; u < kBulkU; ++u) {
             const Run m = Ops::vmax(X[u]);
             run = Ops::rmax(run, m);
-            c = sel_slot<T>(sm, c, X[u], Ops::pass(m, tau), gv0 + u * 32, M, V);
+            c = sel_slot<T>(sm, c, Ops::pass(m, tau), gv0 + u * 32, M, V, rowp, true);
         }
         if (i > 0 && (((i + 1) & i) == 0) && (i + 1 < n_w)) {
             sel_publish_claim<T>(sm, run, q);
@@ -610,12 +627,13 @@ __global__ void __launch_bounds__(kSelThreads, 2) select_topm_bulk_kernel(Select
             c.tau_ord = max(c.tau_ord, sel_read_tau(sm, p, row));
         }
     }
-    c = sel_drain<T>(sm, c, M, V);
-
     sel_publish_claim<T>(sm, run, q);
     __syncthreads();
     c.tau_ord = max(c.tau_ord, sel_read_tau(sm, p, row));
+    c = sel_drain<T>(sm, c, M, V, rowp, true);
+    __syncthreads();
     sel_epilogue(sm, p, row, s, c.tau_ord);
+    sel_span_mark(p.span, 1);
 }
 
 }  // namespace dt
