@@ -90,7 +90,7 @@ def compare_tree(gpu: dict, orc: "oracle.Tree", w: "oracle.Weights", hidden, roo
     assert np.all(gstar[1:] >= g_last - MARGIN), "GPU node scores below the oracle's B-th score by more than margin"
     for s in range(1, orc.n_nodes):
         if orc.scores[s] > g_last + MARGIN:
-            assert orc.path(s) in gpu_paths, f"oracle node {s} (score {orc.scores[s]:.6f}) missing from GPU tree"
+            assert tuple(orc.path(s)) in gpu_paths, f"oracle node {s} (score {orc.scores[s]:.6f}) missing from GPU tree"
     d = np.diff(gstar[1:])
     assert np.all(d <= MARGIN), "GPU pop order not non-increasing in oracle score (beyond margin)"
     err = np.abs(sc[1:nn].astype(np.float64) - gstar[1:])
