@@ -54,8 +54,19 @@ def load_peaks():
     if os.path.exists(p):
         with open(p) as f:
             d = json.load(f)
-        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "source": "measured"}
-    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)),
+                "bf16_tflops": float(d.get("bf16_tflops", 1590.0)), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "bf16_tflops": 1590.0, "source": "fallback"}
+
+
+def pctl(xs, q):
+    xs = sorted(xs)
+    if not xs:
+        return None
+    i = q * (len(xs) - 1)
+    lo = int(i)
+    hi = min(lo + 1, len(xs) - 1)
+    return xs[lo] + (xs[hi] - xs[lo]) * (i - lo)
 
 
 # ----------------------------------------------------------------------------------- clocks
@@ -291,6 +302,45 @@ def run_ours(args):
     phases_us = {n: 1e3 * v / Kp for n, v in phase_sum.items()}
     phase_round_us = 1e3 * tot_ph / Kp
 
+    # distribution over the replays: one event between consecutive replays (a separate pass: the timed region above is
+    # bracketed by exactly two events), and the split by input regime (even sets flat, odd sets peaked)
+    with torch.cuda.stream(st):
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
+        evs[0].record(st)
+        for i in range(K):
+            graphs[i % R].replay()
+            evs[i + 1].record(st)
+        st.synchronize()
+    per = [1e3 * evs[i].elapsed_time(evs[i + 1]) for i in range(K)]
+    by_regime = {"flat": [per[i] for i in range(K) if (i % R) % 2 == 0], "peaked": [per[i] for i in range(K) if (i % R) % 2 == 1]}
+    dist_us = {"p10": pctl(per, 0.1), "p50": pctl(per, 0.5), "p90": pctl(per, 0.9),
+               "by_regime_p50": {n: pctl(v, 0.5) for n, v in by_regime.items() if v}}
+    schedule = {}
+    with torch.cuda.stream(st):
+        for i in range(R):
+            graphs[i].replay()
+            st.synchronize()
+            if builder.get_option("expand_path_taken") == 6:
+                schedule["flat" if i % 2 == 0 else "peaked"] = "wavefront" if builder.get_option("schedule_chosen") else "lock-step"
+                if builder.get_option("schedule_chosen"):
+                    schedule["wavefront_steps_request0"] = builder.get_option("wave_steps")
+
+    # the select kernel's own duration inside the round: device-side span (first CTA start .. last CTA end, %globaltimer),
+    # free of the launch / event latency a CUDA-event pair around ONE kernel of a graph includes
+    span_us = None
+    try:
+        builder.set_option("select_span", 1)
+        with torch.cuda.stream(st):
+            sg = [capture(i) for i in range(R)]
+            tot_ns = 0
+            for i in range(4 * R):
+                sg[i % R].replay()
+                st.synchronize()
+                tot_ns += builder.get_option("select_span_ns")
+        span_us = tot_ns / (4 * R) / 1e3
+    finally:
+        builder.set_option("select_span", 0)
+
     # select alone, back to back on the rotating buffers (dt_select_topm)
     ids = torch.empty((batch * cfg.L, M), dtype=torch.int32, device="cuda")
     vals = torch.empty((batch * cfg.L, M), dtype=torch.float32, device="cuda")
@@ -303,11 +353,24 @@ def run_ours(args):
         ev3.record(st)
         st.synchronize()
     select_alone_us = 1e3 * ev2.elapsed_time(ev3) / 40
+    # L2-warm: the same 4 requests (64 rows, 19.4 MB) over and over
+    warm_rows = min(batch, 4) * cfg.L
+    with torch.cuda.stream(st):
+        wl_ = sets[0]["logits"][:min(batch, 4)]
+        for i in range(5):
+            builder.select_topm_into(wl_, M, ids[:warm_rows], vals[:warm_rows], stream=st)
+        ev2.record(st)
+        for i in range(40):
+            builder.select_topm_into(wl_, M, ids[:warm_rows], vals[:warm_rows], stream=st)
+        ev3.record(st)
+        st.synchronize()
+    select_warm_us = 1e3 * ev2.elapsed_time(ev3) / 40
 
     return dict(torch=torch, dtb=dtb, wl=wl, cfg=cfg, rank=rank, world=world, dev=dev, peaks=peaks, builder=builder,
                 w_cpu=w_cpu, sets_cpu=sets_cpu, sets=sets, outs=outs, graphs=graphs, st=st, R=R, W=W, K=K,
                 ms_per_step=ms_per_step, value=value, clocks=clk.summary(), phases_us=phases_us,
-                phase_round_us=phase_round_us, select_alone_us=select_alone_us,
+                phase_round_us=phase_round_us, select_alone_us=select_alone_us, select_warm_us=select_warm_us,
+                select_warm_rows=warm_rows, select_span_us=span_us, dist_us=dist_us, schedule=schedule,
                 launches_per_round=launches_per_round, create_s=create_s, barrier=barrier)
 
 
@@ -363,7 +426,9 @@ def measure_cpu_baseline(ctx):
         exact += bool(same)
         if same:
             max_dscore = max(max_dscore, float(np.max(np.abs(sc[b][:tr.n_nodes] - tr.scores[:tr.n_nodes]))))
-    base = {"value": n / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
+    _, sec1 = oracle_trees(ctx["w_cpu"], ctx["sets_cpu"][0], 0, 1, cfg, 1)
+    base = {"value": n / sec, "unit": UNIT, "cores": cores, "kind": "oracle", "single_thread_value": 1.0 / sec1,
+            "single_thread_s_per_tree": sec1,
             "sample": f"requests 0..{n - 1} of input set 0 of {cfg.name} (flat regime), one request per thread, "
                       f"{sec:.2f}s wall"}
     parity = {"requests": n, "tokens_parents_exact": exact, "max_abs_score_diff_on_exact": max_dscore,
@@ -555,24 +620,38 @@ def main():
     sel_bytes, exp_flops, pre_flops = algorithmic_counts(cfg, batch)
     ph = ctx["phases_us"]
     round_us = 1e3 * ctx["ms_per_step"]
-    sel_us = ph["select"]
+    # select: the kernel's duration inside the round = its device-side span; the CUDA-event phase (which also holds the launch
+    # and event latency of the graph's first node) and the back-to-back figure are reported beside it
+    sel_us = ctx["select_span_us"] or ph["select"]
     sel_gbs = sel_bytes / (sel_us * 1e-6) / 1e9
-    # `traffic`: dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures summarised in
-    # profiles/r1_select_ncu.md and profiles/r1_fused_ncu.md (C5 workload only; None for any other workload)
+    # `traffic`: dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures summarised under
+    # profiles/ (C5 workload only; None for any other workload): a constant of that capture, not measured by this run
     c5 = (cfg.name == "concurrent8b")
     roof_select = {"kernel": "select_topm_bulk_kernel", "bound": "hbm", "achieved": sel_gbs, "peak": peaks["hbm_gbs"],
                    "unit": "GB/s", "frac": sel_gbs / peaks["hbm_gbs"], "traffic": 159.66e6 if c5 else None,
+                   "traffic_source": "profiles/r2_select_ncu.md (ncu --set full, one launch)" if c5 else None,
                    "peak_source": peaks["source"], "algorithmic_bytes": sel_bytes, "us_per_launch": sel_us,
+                   "how": "device-side span of the kernel inside the round (L2 defeated by rotating inputs)",
+                   "us_event_phase": ph["select"], "gbs_event_phase": sel_bytes / (ph["select"] * 1e-6) / 1e9,
                    "share_of_step": sel_us / ctx["phase_round_us"],
-                   "alone_back_to_back_gbs": sel_bytes / (ctx["select_alone_us"] * 1e-6) / 1e9}
+                   "alone_back_to_back_gbs": sel_bytes / (ctx["select_alone_us"] * 1e-6) / 1e9,
+                   "alone_back_to_back_frac": sel_bytes / (ctx["select_alone_us"] * 1e-6) / 1e9 / peaks["hbm_gbs"],
+                   "l2_warm": {"rows": ctx["select_warm_rows"], "us": ctx["select_warm_us"],
+                               "gbs": ctx["select_warm_rows"] * cfg.V * 2 / (ctx["select_warm_us"] * 1e-6) / 1e9}}
     fma_peak_tflops = 148 * FP32_FMA_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
     exp_tflops = exp_flops / (ph["expand"] * 1e-6) / 1e12
-    roof_expand = {"kernel": "expansion phase (GRU step + correction/log-softmax/top-k + heap)", "bound": "alu",
-                   "achieved": exp_tflops, "peak": fma_peak_tflops, "unit": "TFLOP/s", "frac": exp_tflops / fma_peak_tflops,
-                   "traffic": 19.15e6 if c5 else None, "peak_source": "148 SMs x 128 fp32 FMA lanes x 2 x sm_max_mhz (DESIGN.md)",
-                   "algorithmic_flops": exp_flops, "us_per_round": ph["expand"],
-                   "share_of_step": ph["expand"] / ctx["phase_round_us"],
-                   "note": "a chain of B dependent steps: latency-bound, not throughput-bound"}
+    # the expansion is a chain of dependent steps: neither fraction is a target, the microseconds per step are
+    roof_expand = {"kernel": "expansion phase (wave_expand_kernel or fused_expand_kernel<0>, chosen per round on the device)",
+                   "bound": "latency", "achieved": exp_tflops, "unit": "TFLOP/s",
+                   "peak": fma_peak_tflops, "frac": exp_tflops / fma_peak_tflops,
+                   "peak_source": "148 SMs x 128 fp32 FMA lanes x 2 x sm_max_mhz (DESIGN.md)",
+                   "frac_of_bf16_tensor_peak": exp_tflops / peaks["bf16_tflops"],
+                   "bf16_tensor_peak": peaks["bf16_tflops"],
+                   "traffic": None, "algorithmic_flops": exp_flops, "us_per_round": ph["expand"],
+                   "share_of_step": ph["expand"] / ctx["phase_round_us"], "schedule": ctx["schedule"],
+                   "us_per_round_by_regime_p50": ctx["dist_us"]["by_regime_p50"],
+                   "note": "a chain of dependent GRU -> correction -> pop steps (32 lock-step steps, or ~9 wavefront steps of "
+                           "~4 nodes per request): latency-bound; 92 % of the flops run as bf16 hi/lo pairs on tcgen05"}
     dominant = roof_expand if ph["expand"] > sel_us else roof_select
 
     line = {
@@ -584,7 +663,7 @@ def main():
                    "launch": "one CUDA graph per round", "parallelism": f"dp{world} (independent requests, no collective)",
                    "l2": f"{ctx['R']} distinct input sets rotated ({ctx['R']} x {sel_bytes / 1e6:.1f} MB logits > 126 MB L2)",
                    "regimes": "flat / peaked alternating"},
-        "us_per_round": round_us,
+        "us_per_round": round_us, "us_per_round_dist": ctx["dist_us"],
         "phases_us": ph, "phase_pass_us_per_round": ctx["phase_round_us"],
         "select_hbm_gbs": sel_gbs,
         "roofline": dominant, "roofline_select": roof_select, "roofline_expand": roof_expand,
