@@ -128,6 +128,19 @@ int dt_build_trees_host(dt_handle *h, const void *marginal_logits_host, const vo
                         const dt_outputs *out_host, void *stream);
 
 /*
+ * dt_tree_links: first-child / next-sibling arrays of the trees of one round, for tree-verify kernels that walk the
+ * tree instead of reading the mask (Sec. 3.5 verifies all nodes in one pass under the ancestor-only mask;
+ * PAPER.md:187 runs the serving build on SGLang's EAGLE tree-verify kernel).  `tree` = the dt_outputs a dt_build_trees
+ * call filled (device pointers; parents and n_nodes are read), B the budget of that call (N = B + 1 slots).  Outputs
+ * (device, int32 [batch, N]): first_child[i] = the smallest slot j > i with parents[j] == i, next_sibling[i] = the
+ * smallest slot j > i with parents[j] == parents[i]; -1 where there is none, for the root's sibling and for dead-leaf
+ * padding slots.  Siblings are therefore chained in pop order (best first).  Asynchronous, capture-safe.
+ * Errors: INVALID_ARG for null pointers, batch or B out of range.
+ */
+int dt_tree_links(dt_handle *h, const dt_outputs *tree, int32_t batch, int32_t B, int32_t *first_child,
+                  int32_t *next_sibling, void *stream);
+
+/*
  * dt_commit_paths: longest-accepted-path commit over the trees of one round (Sec. 3.5: "we
  * commit the highest-scoring root-to-leaf path along which every edge is accepted").  `tree` holds the DEVICE
  * outputs of dt_build_trees for the same batch and B (tokens, parents, depths, scores, n_nodes are read; N = B+1).

@@ -17,7 +17,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libdominotree.so")
 
 DT_BF16, DT_F32 = 0, 1
-EXPORTS = ("dt_create", "dt_build_trees", "dt_select_topm", "dt_build_trees_host", "dt_commit_paths", "dt_adaptive_budget", "dt_set_option", "dt_get_option",
+EXPORTS = ("dt_create", "dt_build_trees", "dt_select_topm", "dt_build_trees_host", "dt_commit_paths", "dt_tree_links", "dt_adaptive_budget", "dt_set_option", "dt_get_option",
            "dt_kernel_launches", "dt_destroy", "dt_error_string", "dt_version", "dt_workspace_bytes",
            "dt_last_cuda_error", "dt_phase_timing", "dt_phase_slot", "dt_phase_elapsed_ms")
 PHASES = ("select", "precompute", "expand", "emit")
@@ -64,6 +64,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.dt_adaptive_budget.restype = ctypes.c_int
     lib.dt_commit_paths.argtypes = [vp, ctypes.POINTER(_Outputs), i32, i32, vp, vp, vp, vp, vp, vp]
     lib.dt_commit_paths.restype = ctypes.c_int
+    lib.dt_tree_links.argtypes = [vp, ctypes.POINTER(_Outputs), i32, i32, vp, vp, vp]
+    lib.dt_tree_links.restype = ctypes.c_int
     lib.dt_select_topm.argtypes = [vp, vp, i32, i32, vp, vp, vp]
     lib.dt_select_topm.restype = ctypes.c_int
     lib.dt_set_option.argtypes = [vp, ctypes.c_char_p, i64]
@@ -176,6 +178,8 @@ class DominoTreeBuilder:
             self._check_in(root_positions, (batch,), torch.int32, True)
         if out is None:
             out = alloc_outputs(batch, B, marginal_logits.device)
+        else:
+            self._check_out(out, batch, B, True)
         st = stream if stream is not None else torch.cuda.current_stream()
         os_ = out._struct()
         rc = self.lib.dt_build_trees(self._h, marginal_logits.data_ptr(), backbone_hidden.data_ptr(),
@@ -242,6 +246,19 @@ class DominoTreeBuilder:
         _check(self.lib, rc, "dt_commit_paths", self._h)
         return acc, path, bonus
 
+    def tree_links(self, tree: TreeBatch, B: int, stream=None):
+        """dt_tree_links: (first_child, next_sibling), int32 [batch, B+1] on the device."""
+        import torch
+        batch = tree.tokens.shape[0]
+        dev = tree.tokens.device
+        fc = torch.empty((batch, B + 1), dtype=torch.int32, device=dev)
+        ns = torch.empty((batch, B + 1), dtype=torch.int32, device=dev)
+        st = stream if stream is not None else torch.cuda.current_stream()
+        os_ = tree._struct()
+        rc = self.lib.dt_tree_links(self._h, ctypes.byref(os_), batch, B, fc.data_ptr(), ns.data_ptr(), st.cuda_stream)
+        _check(self.lib, rc, "dt_tree_links", self._h)
+        return fc, ns
+
     def build_trees_host(self, marginal_logits, backbone_hidden, root_tokens, root_positions, M: int, B: int,
                          temperature: float, out: Optional[TreeBatch] = None, stream=None) -> TreeBatch:
         """dt_build_trees_host: HOST tensors in, HOST tensors out; copies both ways and synchronises."""
@@ -254,6 +271,8 @@ class DominoTreeBuilder:
             self._check_in(root_positions, (batch,), torch.int32, False)
         if out is None:
             out = alloc_outputs(batch, B, "cpu", pin=True)
+        else:
+            self._check_out(out, batch, B, False)
         st = stream if stream is not None else torch.cuda.current_stream()
         os_ = out._struct()
         rc = self.lib.dt_build_trees_host(self._h, marginal_logits.data_ptr(), backbone_hidden.data_ptr(),
@@ -301,6 +320,16 @@ class DominoTreeBuilder:
         if tuple(t.shape) != tuple(shape) or t.dtype != dtype or not t.is_contiguous() or t.is_cuda != cuda:
             raise DominoTreeError(f"expected contiguous {'cuda' if cuda else 'cpu'} tensor {shape} {dtype}, "
                                   f"got {tuple(t.shape)} {t.dtype} cuda={t.is_cuda}")
+
+    def _check_out(self, out: TreeBatch, batch: int, B: int, cuda: bool):
+        """A caller-supplied TreeBatch must have exactly the shapes the kernels write: [batch, B+1] (mask [batch, B+1, B+1])."""
+        import torch
+        N = B + 1
+        for name in ("tokens", "parents", "depths", "positions"):
+            self._check_in(getattr(out, name), (batch, N), torch.int32, cuda)
+        self._check_in(out.scores, (batch, N), torch.float32, cuda)
+        self._check_in(out.mask, (batch, N, N), torch.uint8, cuda)
+        self._check_in(out.n_nodes, (batch,), torch.int32, cuda)
 
     def close(self):
         if self._h:

@@ -840,6 +840,19 @@ extern "C" int dt_commit_paths(dt_handle *h, const dt_outputs *tree, int32_t bat
     return DT_OK;
 }
 
+extern "C" int dt_tree_links(dt_handle *h, const dt_outputs *tree, int32_t batch, int32_t B, int32_t *first_child,
+                             int32_t *next_sibling, void *stream) {
+    if (!h || !tree) return DT_ERR_INVALID_ARG;
+    if (batch < 0 || batch > h->max_batch || B < 1 || B > h->max_B) return DT_ERR_INVALID_ARG;
+    h->launches = 0;
+    if (batch == 0) return DT_OK;
+    if (!tree->parents || !tree->n_nodes || !first_child || !next_sibling) return DT_ERR_INVALID_ARG;
+    tree_links_kernel<<<batch, 256, 0, (cudaStream_t)stream>>>(tree->parents, tree->n_nodes, B + 1, first_child, next_sibling);
+    h->launches++;
+    DT_CUDA(h, cudaGetLastError());
+    return DT_OK;
+}
+
 extern "C" int dt_build_trees_host(dt_handle *h, const void *logits_h, const void *hidden_h,
                                    const int32_t *roots_h, const int32_t *rpos_h, int32_t batch,
                                    int32_t M, int32_t B, float temperature, const dt_outputs *oh, void *stream) {

@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(256) commit_paths_kernel(CommitParams p) {
     __shared__ unsigned char sOk[256];
     __shared__ unsigned long long sBest[8];
     const int b = blockIdx.x, tid = threadIdx.x, N = p.N;
-    const int n = min(p.n_nodes[b], N);
+    const int n = max(1, min(p.n_nodes[b], N));              // the root always is a node
     const size_t base = (size_t)b * N;
     if (tid < N) {
         sPar[tid] = p.parents[base + tid];
@@ -71,6 +71,33 @@ __global__ void __launch_bounds__(256) commit_paths_kernel(CommitParams p) {
         for (int i = len; i >= 0; --i) { path[i] = u; u = (u == 0) ? 0 : sPar[u]; }
         if (p.bonus_token) p.bonus_token[b] = p.target_next ? sNext[end] : -1;
     }
+}
+
+// First-child / next-sibling link arrays for tree-verify kernels that walk the tree instead of reading the mask
+// (PAPER.md:169, 187): first_child[i] = smallest slot j > i with parents[j] == i, next_sibling[i] = smallest slot
+// j > i with parents[j] == parents[i]; -1 where there is none, for the root's sibling and for dead-leaf padding slots.
+// One CTA per request, one thread per slot, the parent links staged in shared memory.
+__global__ void __launch_bounds__(256) tree_links_kernel(const int32_t *parents, const int32_t *n_nodes, int N,
+                                                         int32_t *first_child, int32_t *next_sibling) {
+    __shared__ int sPar[256];
+    const int b = blockIdx.x, i = threadIdx.x;
+    const int n = max(1, min(n_nodes[b], N));
+    const size_t base = (size_t)b * N;
+    if (i < N) sPar[i] = parents[base + i];
+    __syncthreads();
+    if (i >= N) return;
+    int fc = -1, ns = -1;
+    if (i < n) {
+        const int par = sPar[i];
+        for (int j = i + 1; j < n; ++j) {
+            const int pj = sPar[j];
+            if (fc < 0 && pj == i) fc = j;
+            if (ns < 0 && i > 0 && pj == par) ns = j;
+            if (fc >= 0 && (ns >= 0 || i == 0)) break;
+        }
+    }
+    first_child[base + i] = fc;
+    next_sibling[base + i] = ns;
 }
 
 }  // namespace dt
