@@ -321,7 +321,7 @@ def run_ours(args):
             graphs[i].replay()
             st.synchronize()
             if builder.get_option("expand_path_taken") == 6:
-                schedule["flat" if i % 2 == 0 else "peaked"] = "wavefront" if builder.get_option("schedule_chosen") else "lock-step"
+                schedule["flat" if i % 2 == 0 else "peaked"] = "wavefront" if (builder.get_option("schedule_chosen") or B >= 48) else "lock-step"
                 if builder.get_option("schedule_chosen"):
                     schedule["wavefront_steps_request0"] = builder.get_option("wave_steps")
 
@@ -551,6 +551,7 @@ def run_trace(args):
     batch = args.trace_batch or cfg.batch
     w_gpu = {n: t.cuda() for n, t in wl.make_weights(cfg).items()}
     builder = dtb.DominoTreeBuilder(w_gpu, max_batch=batch, L=cfg.L, max_M=cfg.M, max_B=cfg.B, k=cfg.k, lib_path=lib_path)
+    builder.set_option("expand_path", 5)          # the timeline is the wavefront kernel's, whatever the adaptive schedule would pick
     if args.wave_width:
         builder.set_option("wave_width", args.wave_width)
     lib = builder.lib

@@ -620,7 +620,10 @@ static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st, int sel =
         f.partial = h->wv_partial + (size_t)b0 * kWvMaxW * f.P * p.r;
         f.desc = h->wv_desc + (size_t)b0 * kWvDescWords;
         f.flags = h->wv_flags; f.round_ctr = h->wv_round; f.err = h->wv_err; f.stats = (b0 == 0) ? h->wv_stats : nullptr;
-        if (sel >= 0) { f.sched_sel = h->sched_sel; f.sched_want = (unsigned int)sel; f.sched_thr = h->sched_thr; }
+        if (sel >= 0) {
+            f.sched_sel = h->sched_sel; f.sched_thr = h->sched_thr; f.run_peaked = (sel == 2);
+            f.W_peaked = W < 4 ? W : 4;
+        }
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof(cfg));
         cfg.gridDim = dim3(n_gru + (nb + kWvCS - 1) / kWvCS * kWvCS); cfg.blockDim = dim3(kWvThreads);
@@ -788,11 +791,16 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
             wave_regime_kernel<<<(rows + 7) / 8, 256, 0, st>>>(h->cand_val, rows, M, 1.0f / p.T_eff, h->sched_sel);
             h->launches++;
             DT_CUDA(h, cudaGetLastError());
-            rc = launch_wave(h, p, st, 1, false, true, false);
+            // chains longer than ~48 nodes: even a peaked round pays in the wavefront kernel (at a width of 4); shorter ones
+            // go to the lock-step kernel, whose step is shorter
+            const bool wave_only = B >= 48;
+            rc = launch_wave(h, p, st, wave_only ? 2 : 1, false, true, wave_only);
             if (rc) return rc < 0 ? rc : DT_ERR_CUDA;
-            const int64_t n = h->launches;
-            rc = launch_fused(h, p, st, false, 0, false, false, true);
-            h->launches = n + 1;
+            if (!wave_only) {
+                const int64_t n = h->launches;
+                rc = launch_fused(h, p, st, false, 0, false, false, true);
+                h->launches = n + 1;
+            }
             h->path_taken = 6;
             return rc < 0 ? rc : (rc ? DT_ERR_CUDA : DT_OK);
         }

@@ -71,7 +71,9 @@ struct WaveParams {
     unsigned int *round_ctr;       // rounds this handle has run (tags every hand-over word)
     unsigned int *err;             // set to 1 when a hand-over wait timed out (protocol slip: fail, do not hang)
     unsigned int *stats;           // [4] optional counters of request 0: steps, expansions (measurement aid)
-    const unsigned int *sched_sel; unsigned int sched_want, sched_thr;   // run only when (*sched_sel < sched_thr) == sched_want (null: always)
+    // adaptive schedule (null selector: always run, width W): the round is `flat` when *sched_sel < sched_thr; on a peaked round
+    // the kernel runs only if run_peaked, with the narrower width W_peaked (speculative nodes rarely pay on chains)
+    const unsigned int *sched_sel; unsigned int sched_thr; int run_peaked, W_peaked;
 };
 
 // ---- hand-over words ---------------------------------------------------------------------------------
@@ -162,15 +164,6 @@ __device__ __forceinline__ unsigned int wave_ld_acquire_u32(const unsigned int *
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-// two {value, tag} elements per access; each 64-bit element is read / written as one unit
-__device__ __forceinline__ void wave_st_pair2(uint2 *p, float a, float b, unsigned int tag) {
-    const unsigned long long x = ((unsigned long long)tag << 32) | __float_as_uint(a), y = ((unsigned long long)tag << 32) | __float_as_uint(b);
-    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(x), "l"(y) : "memory");
-}
-__device__ __forceinline__ void wave_ld_pair2(const uint2 *p, unsigned long long &x, unsigned long long &y) {
-    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(x), "=l"(y) : "l"(p) : "memory");
-}
-
 // TMEM -> registers without the wait: 8 / 16 consecutive fp32 columns of this thread's lane
 __device__ __forceinline__ void wave_tmem_ld8_nw(uint32_t taddr, uint32_t (&r)[8]) {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
@@ -929,16 +922,30 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                 mk[h] = is_old ? oK[i] : nKey[i - n_old];
                 mm[h] = is_old ? oM[i] : nMeta[i - n_old];
                 int rank = 0;
+                const unsigned long long mkh = mk[h];
                 if (is_old) rank = i;
                 else {                                               // old entries in front of it: the list is sorted
                     int lo = 0, hi = n_old;
-                    while (lo < hi) { const int mid = (lo + hi) >> 1; if (prec(oK[mid], oM[mid], mid, mk[h], mm[h], i)) lo = mid + 1; else hi = mid; }
+                    while (lo < hi) {
+                        const int mid = (lo + hi) >> 1;
+                        const unsigned long long km = oK[mid];
+                        if (km > mkh || (km == mkh && prec(km, oM[mid], mid, mkh, mm[h], i))) lo = mid + 1; else hi = mid;
+                    }
                     rank = lo;
                 }
+                // new entries in front of it: keys only, two per load; equal keys (the same score, depth and token under two
+                // parents: rare) go through the full comparator
+                int n_eq = 0, q = 0;
+                for (; q + 2 <= n_new; q += 2) {
+                    const ulonglong2 o = *reinterpret_cast<const ulonglong2 *>(nKey + q);
+                    rank += (o.x > mkh) + (o.y > mkh);
+                    n_eq += (o.x == mkh) + (o.y == mkh);
+                }
+                if (q < n_new) { rank += (nKey[q] > mkh); n_eq += (nKey[q] == mkh); }
+                if (n_eq > (is_old ? 0 : 1)) {
 #pragma unroll 1
-                for (int q = 0; q < n_new; ++q) {
-                    if (n_old + q == i) continue;
-                    rank += prec(nKey[q], nMeta[q], n_old + q, mk[h], mm[h], i) ? 1 : 0;
+                    for (int q2 = 0; q2 < n_new; ++q2)
+                        if (nKey[q2] == mkh && n_old + q2 != i) rank += prec(nKey[q2], nMeta[q2], n_old + q2, mkh, mm[h], i) ? 1 : 0;
                 }
                 rk[h] = rank;
             }
@@ -1091,7 +1098,10 @@ __global__ void __launch_bounds__(256) wave_regime_kernel(const float *cand_val,
 
 __global__ void __launch_bounds__(kWvThreads, 1) wave_expand_kernel(WaveParams p) {
     extern __shared__ __align__(1024) unsigned char wave_smem[];
-    if (p.sched_sel && (unsigned int)(*p.sched_sel < p.sched_thr) != p.sched_want) return;   // the other schedule was chosen (grid-uniform)
+    if (p.sched_sel && !(*p.sched_sel < p.sched_thr)) {            // a peaked round (grid-uniform)
+        if (!p.run_peaked) return;                                  // the lock-step kernel takes it
+        p.W = p.W_peaked;
+    }
     if ((int)blockIdx.x < p.n_gru) wave_gru_role(p, wave_smem);
     else if ((int)blockIdx.x - p.n_gru < p.e.batch) wave_req_role(p, wave_smem);   // CTAs padding the last cluster leave
 }
