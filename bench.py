@@ -519,6 +519,47 @@ def measure_sweep_and_arms(ctx):
         arms[name] = _time_graphs(torch, dtb, builder, st, lg, hd, rt, rp, 64, 16, 0.0)
     builder.set_option("scorer", 0)
     builder.close()
+    # the frontier schedule (dt_set_option "schedule" 1: the wavefront kernel at its maximal width) beside the adaptive heap
+    # schedule at the bench workload, and the select kernel over chunk counts and candidate widths
+    big = ctx["builder"]
+    s0 = ctx["sets"][0]
+    sched = {}
+    for name, val in (("adaptive", 0), ("frontier", 1)):
+        big.set_option("schedule", val)
+        o = dtb.alloc_outputs(cfg.batch, cfg.B)
+        with torch.cuda.stream(st):
+            big.build_trees(s0["logits"], s0["hidden"], s0["root_tokens"], s0["root_positions"], cfg.M, cfg.B, cfg.T, out=o, stream=st)
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=st):
+                big.build_trees(s0["logits"], s0["hidden"], s0["root_tokens"], s0["root_positions"], cfg.M, cfg.B, cfg.T, out=o, stream=st)
+            for _ in range(3):
+                g.replay()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st)
+            for _ in range(20):
+                g.replay()
+            e1.record(st)
+            st.synchronize()
+        sched[name] = 1e3 * e0.elapsed_time(e1) / 20
+    big.set_option("schedule", 0)
+    sel = {}
+    ids = torch.empty((cfg.batch * cfg.L, cfg.M), dtype=torch.int32, device="cuda")
+    vals = torch.empty((cfg.batch * cfg.L, cfg.M), dtype=torch.float32, device="cuda")
+    for S in (1, 2, 4):
+        big.set_option("select_chunks", S)
+        with torch.cuda.stream(st):
+            for i in range(ctx["R"]):
+                big.select_topm_into(ctx["sets"][i]["logits"], cfg.M, ids, vals, stream=st)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st)
+            for i in range(20):
+                big.select_topm_into(ctx["sets"][i % ctx["R"]]["logits"], cfg.M, ids, vals, stream=st)
+            e1.record(st)
+            st.synchronize()
+        sel[f"chunks_per_row_{S}"] = 1e3 * e0.elapsed_time(e1) / 20
+    big.set_option("select_chunks", 0)
+    sweep["schedules_at_bench_workload_flat_set"] = sched
+    sweep["select_us_by_chunks"] = sel
     return {"us_per_round": sweep, "note": "batch 1, flat / peaked inputs mixed, one CUDA graph per round"}, \
            {"us_per_round_batch1_B16_M64": arms}
 
@@ -629,7 +670,7 @@ def main():
     # profiles/ (C5 workload only; None for any other workload): a constant of that capture, not measured by this run
     c5 = (cfg.name == "concurrent8b")
     roof_select = {"kernel": "select_topm_bulk_kernel", "bound": "hbm", "achieved": sel_gbs, "peak": peaks["hbm_gbs"],
-                   "unit": "GB/s", "frac": sel_gbs / peaks["hbm_gbs"], "traffic": 159.66e6 if c5 else None,
+                   "unit": "GB/s", "frac": sel_gbs / peaks["hbm_gbs"], "traffic": 161.90e6 if c5 else None,
                    "traffic_source": "profiles/r2_select_ncu.md (ncu --set full, one launch)" if c5 else None,
                    "peak_source": peaks["source"], "algorithmic_bytes": sel_bytes, "us_per_launch": sel_us,
                    "how": "device-side span of the kernel inside the round (L2 defeated by rotating inputs)",

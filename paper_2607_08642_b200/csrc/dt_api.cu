@@ -761,8 +761,21 @@ extern "C" int dt_build_trees(dt_handle *h, const void *marginal_logits, const v
     p.tokens = out->tokens; p.parents = out->parents; p.depths = out->depths; p.positions = out->positions;
     p.n_nodes = out->n_nodes; p.scores = out->scores; p.mask = out->mask;
     p.root_tokens = root_tokens; p.root_positions = root_positions;
-    if (h->opt_schedule == 1 && h->opt_scorer == 0)  // frontier schedule of the DominoTree scorer
+    if (h->opt_schedule == 1 && h->opt_scorer == 0) {   // frontier schedule of the DominoTree scorer
+        // bf16: the frontier's per-depth GEMM over many nodes of many requests IS the wavefront kernel's GRU pass; at its
+        // maximal width a step expands every unexpanded member of the top-B frontier (up to 15 per request), on tcgen05.
+        // Shapes the wavefront kernel rejects (and fp32) take the depth-synchronous ledger kernels (warp FMA).
+        if (w.dtype == DT_BF16 && h->opt_expand_path == 0) {
+            const int64_t keep = h->opt_wave_width;
+            h->opt_wave_width = kWvMaxW;
+            h->opt_expand_path = 5;
+            rc = launch_wave(h, p, st);
+            h->opt_wave_width = keep;
+            h->opt_expand_path = 0;
+            if (rc <= 0) return rc;
+        }
         return (w.dtype == DT_BF16) ? launch_frontier<__nv_bfloat16>(h, p, st) : launch_frontier<float>(h, p, st);
+    }
     if (h->opt_scorer == 1) {                       // Marg: menus from the base logits alone, no GRU, no C
         ScorerParams sp;
         sp.e = p; sp.menu_tok = h->menu_tok; sp.menu_lp = h->menu_lp;

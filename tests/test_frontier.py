@@ -72,7 +72,8 @@ def test_frontier_qwen8b_shape_equals_heap():
     import gpu_util as gu
     case = gu.qwen8b_case()
     inp = wl.make_inputs(case.cfg, batch=2, seed=515, regime="flat")
-    out, _ = _frontier(case, inp, 64, 16, 0.0)
+    out, launches = _frontier(case, inp, 64, 16, 0.0)
+    assert launches <= 4            # select, precompute GEMM (2), ONE persistent kernel: the wavefront kernel at full width
     ne, nt = gu.check_batch(case, inp, 64, 16, 0.0, 2e-3, out=out)
     assert ne + nt == 2
     heap = case.run_gpu(inp, 64, 16, 0.0)
