@@ -502,6 +502,8 @@ extern "C" int dt_select_topm(dt_handle *h, const void *logits, int32_t rows, in
 static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool static_mode = false, int sel = -1, bool probe = false,
                         bool m_begin = true, bool m_end = true) {
     if (!h->fused_ok || h->opt_expand_path == 1) return 1;
+    // one-step rounds: GRU CTA 0 would bump the round counter before a late-starting CTA has read it
+    if (p.B < 2) return 1;
     int upc = 0;
     bool tcgen = false;
     // tcgen05 + TMEM GRU CTAs (16 units each) whenever the shape allows; the choice never depends on the batch
@@ -529,7 +531,7 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
     f.upc = upc; f.n_gru = p.g / upc; f.m_tiles = (3 * upc + 15) / 16;
     f.slot_stride = h->slot_stride;
     f.s_hi = h->s_hi; f.s_lo = h->s_lo; f.s32 = h->states; f.partial = h->partial; f.desc = h->desc; f.flags = h->flags; f.round_ctr = h->round_ctr;
-    f.static_mode = static_mode ? 1 : 0; f.menu_tok = h->menu_tok; f.menu_lp = h->menu_lp;
+    f.static_mode = static_mode ? 1 : 0; f.menu_tok = h->menu_tok; f.menu_lp = h->menu_lp; f.err = h->wv_err;
     f.w2_smem = 1;
     size_t rs = fused_req_smem(p.r, p.M, p.N, p.k, 1);
     if (rs > (size_t)h->max_smem_optin) { f.w2_smem = 0; rs = fused_req_smem(p.r, p.M, p.N, p.k, 0); }

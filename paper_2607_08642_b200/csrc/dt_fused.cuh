@@ -66,6 +66,7 @@ struct FusedParams {
     int static_mode;
     // adaptive schedule (dt_api.cu): the kernel runs only when (*sched_sel < sched_thr) == sched_want (null: always)
     const unsigned int *sched_sel; unsigned int sched_want, sched_thr;
+    unsigned int *err;             // device error word: a hand-over wait that times out raises it and gives up (no hang)
     int32_t *menu_tok;             // [batch, L, k]
     float *menu_lp;                // [batch, L, k]
 };
@@ -89,6 +90,23 @@ __device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long
     unsigned long long v;
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
+}
+// Bounded hand-over wait: spin on `ready`, look at the clock every 1024 polls, after 4 s (or when another CTA
+// has given up) raise the device error word and return false: a protocol slip fails the call instead of hanging the GPU.
+template <typename F>
+__device__ __forceinline__ bool fused_spin(F ready, unsigned int *err) {
+    unsigned long long t0 = 0ull;
+    unsigned int n = 0;
+    while (!ready()) {
+        if (((++n) & 1023u) == 0u && err) {
+            unsigned long long t;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+            if (n == 1024u) t0 = t;
+            if (*reinterpret_cast<volatile unsigned int *>(err) != 0u) return false;
+            if (t - t0 > 4000000000ull) { atomicExch(err, 1u); return false; }
+        }
+    }
+    return true;
 }
 __device__ __forceinline__ void st_relaxed_u32(unsigned int *p, unsigned int v) {
     asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
@@ -192,7 +210,7 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
                 int sidx = -1, tok = 0;
                 if (lane < nb) {
                     unsigned long long dsc;
-                    do { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride); } while (!fused_desc_is(dsc, t + 1, rnd));
+                    fused_spin([&] { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride); return fused_desc_is(dsc, t + 1, rnd); }, p.err);
                     sidx = fused_desc_sidx(dsc);
                     tok = (int)(dsc & 0xFFFFFFFFull);
                 }
@@ -467,7 +485,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                 int sidx = -1, tok = 0;
                 if (lane < nb) {
                     unsigned long long dsc;
-                    do { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride); } while (!fused_desc_is(dsc, t + 1, rnd));
+                    fused_spin([&] { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride); return fused_desc_is(dsc, t + 1, rnd); }, p.err);
                     sidx = fused_desc_sidx(dsc);
                     tok = (int)(dsc & 0xFFFFFFFFull);
                 }
@@ -717,7 +735,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         if (expand && tid < r) cpre = e.C[((size_t)b * L + depth) * r + tid];
         if (warp == 0) {
             for (int q = lane; q < p.n_gru; q += 32)
-                while ((int)(ld_relaxed_u32(p.flags + (size_t)q * kFusFlagStride) - (fbase + (unsigned int)(t + 1))) < 0) { }
+                fused_spin([&] { return (int)(ld_relaxed_u32(p.flags + (size_t)q * kFusFlagStride) - (fbase + (unsigned int)(t + 1))) >= 0; }, p.err);
         }
         __syncthreads();
         // the live frontier is entries 1 .. n_front of buffer `cur` (entry 0 was popped by the previous step)
