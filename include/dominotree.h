@@ -103,6 +103,7 @@ int dt_create(dt_handle **h, const dt_weights *w, int32_t max_batch, int32_t L,
  * the whole round into one CUDA graph.  One handle serves one stream at a time.
  * Input values are assumed non-NaN (-inf logits are allowed and sort last).
  */
+/* (`stream` is a cudaStream_t passed as void * so that this header needs no CUDA header.) */
 int dt_build_trees(dt_handle *h, const void *marginal_logits, const void *backbone_hidden,
                    const int32_t *root_tokens, const int32_t *root_positions, int32_t batch,
                    int32_t M, int32_t B, float temperature, const dt_outputs *out, void *stream);
@@ -177,17 +178,32 @@ int dt_adaptive_budget(dt_handle *h, const dt_outputs *tree, int32_t batch, int3
  *                   1 Marg (base logits alone, one menu per depth, no GRU),
  *                   2 Cond-static (correction once per depth along Domino's greedy chain, menu shared per depth;
  *                     bf16 shapes the fused kernel accepts, else dt_build_trees returns DT_ERR_UNSUPPORTED);
- *   "schedule"      0 best-first heap (Algorithm 1; default), 1 the depth-synchronous frontier builder of the paper's
- *                   serving path with W = B lanes: the same tree on tie-free inputs;
+ *   "schedule"      0 best-first heap (Algorithm 1; default), 1 the frontier builder of the paper's serving path
+ *                    with W = B: the same tree on tie-free inputs (bf16 shapes: the wavefront
+ *                   kernel at its maximal width; fp32 and odd shapes: depth-synchronous ledger kernels);
+ *   "adaptive_schedule"  1 (default): per round the device picks, from the mean top-1 probability of the base slices,
+ *                   the wavefront kernel (bushy trees) or the lock-step kernel (chains); both give the same tree, scores
+ *                   agree to fp32 rounding.  0: always the wavefront kernel when the shape allows (bitwise batch
+ *                   invariance of the scores then holds for any mix of requests);
  *   "wave_width"    nodes a request may expand per dependent step of the wavefront kernel (0 = auto, 1 = the plain heap
  *                   schedule, up to 15); any value gives the same tree;
- *   "expand_path", "select_chunks", "select_kernel", "precompute_gemm"   tuning / test switches of the kernels. */
+ *   "expand_path"   0 auto, 1 per-step kernels, 2 / 3 lock-step kernel on mma.sync, 4 lock-step kernel on tcgen05,
+ *                   5 wavefront kernel;
+ *   "select_chunks", "select_kernel", "select_span", "precompute_gemm", "precompute_serial"   tuning / measurement
+ *                   switches of the kernels.
+ * Batch sizes: any batch <= max_batch runs on the persistent kernels (bf16): a launch of the wavefront kernel holds up to
+ * 64 requests beside the g / 16 GRU CTAs, larger batches run as consecutive launches inside the same call; the lock-step
+ * kernel needs g / 16 + batch <= SM count and is simply not chosen otherwise. */
 int dt_set_option(dt_handle *h, const char *name, int64_t value);
 
 /* dt_get_option: read-back values; unknown name -> INVALID_ARG.  The device-side words synchronise the device first
  * (not capture-safe).
  *   "expand_path_taken"  expansion path the last dt_build_trees enqueued: 1 per-step kernels, 2 / 3 lock-step fused kernel
- *                        on mma.sync, 4 lock-step fused kernel on tcgen05, 5 wavefront kernel (dt_wave.cuh);
+ *                        on mma.sync, 4 lock-step fused kernel on tcgen05, 5 wavefront kernel (dt_wave.cuh), 6 adaptive
+ *                        (both persistent kernels enqueued, the device lets one run);
+ *   "schedule_chosen"    adaptive rounds: 1 if the last round's statistic said `flat` (wavefront kernel), else 0;
+ *   "select_span_ns"     with "select_span" 1: device-side span of the last bulk select kernel (first CTA start to last
+ *                        CTA end, %globaltimer);
  *   "state_slots"        GRU state slots per request in the workspace;
  *   "device_error"       1 after a hand-over wait inside a persistent kernel timed out (the round's outputs are invalid);
  *   "wave_steps", "wave_expansions"   dependent steps and CHILDREN evaluations request 0 needed in the last wavefront round. */
