@@ -593,6 +593,7 @@ def run_trace(args):
     w_gpu = {n: t.cuda() for n, t in wl.make_weights(cfg).items()}
     builder = dtb.DominoTreeBuilder(w_gpu, max_batch=batch, L=cfg.L, max_M=cfg.M, max_B=cfg.B, k=cfg.k, lib_path=lib_path)
     builder.set_option("expand_path", 5)          # the timeline is the wavefront kernel's, whatever the adaptive schedule would pick
+    builder.set_option("wave_groups", 1)          # one request group: GRU step i and request step i are the same step
     if args.wave_width:
         builder.set_option("wave_width", args.wave_width)
     lib = builder.lib

@@ -45,6 +45,7 @@ struct dt_handle {
     // wavefront expansion (dt_wave.cuh): per-item partials, multi-item descriptors, device error word, counters
     float *wv_partial; unsigned long long *wv_desc; unsigned int *wv_err, *wv_stats, *wv_flags, *wv_round; int wave_ok, slot_stride;
     int64_t opt_wave_width;         // items per request per step (0 = auto)
+    int64_t opt_wave_groups;        // request groups the GRU CTAs serve in turn: 0 auto (2), 1 .. 4
     int64_t opt_adaptive;           // 1 (default): the device picks wavefront or lock-step per round (wave_regime_kernel)
     unsigned int *sched_sel;        // device word: sum over the rows of p1 in 16-bit fixed point (wave_regime_kernel)
     unsigned int sched_thr;         // wavefront schedule when the sum is below this
@@ -143,6 +144,11 @@ extern "C" int dt_set_option(dt_handle *h, const char *name, int64_t value) {
     if (!strcmp(name, "wave_width")) {
         if (value < 0 || value > kWvMaxW) return DT_ERR_INVALID_ARG;
         h->opt_wave_width = value;
+        return DT_OK;
+    }
+    if (!strcmp(name, "wave_groups")) {
+        if (value < 0 || value > 4) return DT_ERR_INVALID_ARG;
+        h->opt_wave_groups = value;
         return DT_OK;
     }
     if (!strcmp(name, "adaptive_schedule")) {
@@ -615,6 +621,8 @@ static int launch_wave(dt_handle *h, ExpandParams &p, cudaStream_t st, int sel =
         f.e.positions = p.positions + (size_t)b0 * p.N; f.e.scores = p.scores + (size_t)b0 * p.N;
         f.e.mask = p.mask + (size_t)b0 * p.N * p.N; f.e.n_nodes = p.n_nodes + b0;
         f.e.root_tokens = p.root_tokens + b0; f.e.root_positions = p.root_positions ? p.root_positions + b0 : nullptr;
+        f.n_groups = h->opt_wave_groups ? (int)h->opt_wave_groups : 2;
+        if (f.n_groups > nb) f.n_groups = nb;
         f.n_gru = n_gru; f.slot_stride = h->slot_stride; f.W = W; f.n_slices = nsl; f.e_max = e_max;
         f.P = n_gru / kWvCS; f.rpc = 16 * ((p.r + 16 * kWvCS - 1) / (16 * kWvCS));
         const size_t so = (size_t)b0 * h->slot_stride * p.g;

@@ -59,6 +59,7 @@ struct WaveParams {
     int n_gru;                     // GRU CTAs = g / 16
     int slot_stride;               // state slots per request (slot 0 = zeros, expansion x lives in slot x + 1)
     int W;                         // items a request may publish per step (1 .. kWvMaxW)
+    int n_groups;                  // 1 .. 4: the requests of a launch form groups the GRU CTAs serve in turn (ping-pong)
     int n_slices;                  // W2 slices in a request CTA's shared memory
     int e_max;                     // expansions per request = slot_stride - 1
     int P;                         // partial vectors per item = n_gru / kWvCS (one per cluster of GRU CTAs)
@@ -280,11 +281,20 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
     // moment is a hot spot; the order depends on the CTA only, never on the batch, so results stay batch-invariant
     const int kshift = cta % n_kc;
     const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 10;
-    for (int s = 0;; ++s) {
+    // Ping-pong: the requests form up to four groups served in turn, so that while the request CTAs of one group score their
+    // nodes the GRU CTAs already run the other group's pass (a group's step still costs pass + hand-over + request role,
+    // but two groups share that time).  Each group has its own step counter and its own flag word.
+    const int G = p.n_groups, gsplit = (batch + G - 1) / G;
+    int sg[4] = {0, 0, 0, 0};
+    bool glive[4] = {true, G > 1, G > 2, G > 3};
+    for (int grp = 0; glive[0] || glive[1] || glive[2] || glive[3]; grp = (grp + 1 == G) ? 0 : grp + 1) {
+        if (!glive[grp]) continue;
+        const int s = sg[grp];
+        const int b_lo = grp * gsplit, b_hi = min(batch, b_lo + gsplit);
         // ---- item lines of step s: a half-warp per request, a lane per word of its 128-byte line
-        for (int b0 = 2 * warp; b0 < batch; b0 += 2 * (kWvThreads / 32)) {
+        for (int b0 = b_lo + 2 * warp; b0 < b_hi; b0 += 2 * (kWvThreads / 32)) {
             const int b = b0 + (lane >> 4), j = lane & 15;
-            const bool have = b < batch;
+            const bool have = b < b_hi;
             const unsigned long long *wp = p.desc + (size_t)(have ? b : 0) * kWvDescWords + j;
             unsigned long long w = 0ull, t0 = 0ull;
             bool v = false, ok = !have;
@@ -319,7 +329,7 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
             const bool ok = wave_spin([&] {
                 bool all = true;
                 for (int q = lane; q < p.n_gru; q += 32)
-                    all = all && ((int)(wave_ld_acquire_u32(p.flags + (size_t)q * kFusFlagStride) - want) >= 0);
+                    all = all && ((int)(wave_ld_acquire_u32(p.flags + (size_t)q * kFusFlagStride + grp) - want) >= 0);
                 return all; }, p.err);
             if (!ok) sCtl[2] = 1;
         }
@@ -327,7 +337,7 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
         // ---- compaction: every warp scans the counts (two requests per lane), warp w packs requests w, w + 8, ..
         int total;
         {
-            const int r0 = (lane < batch) ? sCnt[lane] : -1, r1 = (lane + 32 < batch) ? sCnt[lane + 32] : -1;
+            const int r0 = (lane >= b_lo && lane < b_hi) ? sCnt[lane] : -1, r1 = (lane + 32 >= b_lo && lane + 32 < b_hi) ? sCnt[lane + 32] : -1;
             const int c0 = max(r0, 0), c1 = max(r1, 0);
             int i0 = c0, i1 = c1;
 #pragma unroll
@@ -339,8 +349,9 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
             total = tot0 + __shfl_sync(0xffffffffu, i1, 31);
             const int ex0 = i0 - c0, ex1 = tot0 + i1 - c1;
             const bool live = __any_sync(0xffffffffu, r0 >= 0 || r1 >= 0);
-            if (sCtl[2] || !live) break;                             // abort, or every request is done (block-uniform)
-            for (int b = warp; b < batch; b += kWvThreads / 32) {
+            if (sCtl[2]) break;                                      // abort (block-uniform)
+            if (!live) { glive[grp] = false; __syncthreads(); continue; }   // every request of the group is done
+            for (int b = b_lo + warp; b < b_hi; b += kWvThreads / 32) {
                 const int off = __shfl_sync(0xffffffffu, (b < 32) ? ex0 : ex1, b & 31);
                 const int cb = __shfl_sync(0xffffffffu, (b < 32) ? c0 : c1, b & 31);
                 const int first = 1 + sCum[b];
@@ -611,9 +622,10 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
         if (sCtl[2]) break;
         if (tid == 0) {
             fence_release_gpu();                                     // states and partials of this step are visible before the flag
-            st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, fbase + (unsigned int)(s + 1));
+            st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride + grp, fbase + (unsigned int)(s + 1));
         }
         WV_TR(0, cta == 0, s, 7);
+        sg[grp] = s + 1;
     }
     __syncthreads();
     if (pend2) wave_cluster_wait();
@@ -667,6 +679,7 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
     const int r = e.r, M = e.M, k = e.k, N = e.N, L = e.L, B = e.B;
     const int W = p.W, nsl = p.n_slices, e_max = p.e_max, P = p.P;
     const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 10;
+    const int my_grp = b / ((e.batch + p.n_groups - 1) / p.n_groups);
     const size_t slice_bytes = wave_slice_bytes(r, M);
     const int Ka = (r + 63) / 64, nvec = r / 8;
 
@@ -756,7 +769,7 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
             const bool ok = wave_spin([&] {
                 bool all = true;
                 for (int q = lane; q < p.n_gru; q += 32)
-                    all = all && ((int)(wave_ld_acquire_u32(p.flags + (size_t)q * kFusFlagStride) - want) >= 0);
+                    all = all && ((int)(wave_ld_acquire_u32(p.flags + (size_t)q * kFusFlagStride + my_grp) - want) >= 0);
                 return all; }, p.err);
             if (!ok) ctl.abort_ = 1;
         }
