@@ -535,6 +535,8 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
     memset(&f, 0, sizeof(f));
     f.e = p;
     f.upc = upc; f.n_gru = p.g / upc; f.m_tiles = (3 * upc + 15) / 16;
+    // two groups when the batch allows (ping-pong between the GRU CTAs and the request CTAs), at most kFusChunk requests each
+    f.gsz = (p.batch <= 16) ? p.batch : ((p.batch + 1) / 2 < kFusChunk ? (p.batch + 1) / 2 : kFusChunk);
     f.slot_stride = h->slot_stride;
     f.s_hi = h->s_hi; f.s_lo = h->s_lo; f.s32 = h->states; f.partial = h->partial; f.desc = h->desc; f.flags = h->flags; f.round_ctr = h->round_ctr;
     f.static_mode = static_mode ? 1 : 0; f.menu_tok = h->menu_tok; f.menu_lp = h->menu_lp; f.err = h->wv_err;

@@ -53,6 +53,8 @@ constexpr int kFusFlagStride = 32; // u32 words between two GRU CTAs' flags     
 struct FusedParams {
     ExpandParams e;
     int n_gru, upc, m_tiles;       // GRU CTAs, units per CTA, ceil(3*upc/16)
+    int gsz;                       // requests per GRU pass (<= kFusChunk): the batch is served in groups of gsz, each with its own
+                                   // flag word, so the request CTAs of one group work while the GRU CTAs run the next group's pass
     int slot_stride;               // state slots per request = max_B + 2 (slot 0 = zeros, node t at t+1)
     int w2_smem;                   // request CTAs stage the M W2 rows in shared memory
     __nv_bfloat16 *s_hi, *s_lo;    // [batch, slot_stride, g]
@@ -202,8 +204,8 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
 
     const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 8;   // this round's tag / flag base
     for (int t = 0; t < e.B; ++t) {
-        for (int c0 = 0; c0 < batch; c0 += kFusChunk) {
-            const int nb = min(kFusChunk, batch - c0);
+        for (int c0 = 0; c0 < batch; c0 += p.gsz) {
+            const int nb = min(p.gsz, batch - c0);
             const int ntiles = (nb + 7) >> 3;
             // wait for the descriptors of step t (lane = request), then broadcast through shared memory
             if (warp == 0) {
@@ -375,8 +377,8 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
                 }
             }
             __syncthreads();
+            if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride + c0 / p.gsz, fbase + (unsigned int)(t + 1)); }
         }
-        if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, fbase + (unsigned int)(t + 1)); }
     }
     if (cta == 0 && tid == 0) st_relaxed_u32(p.round_ctr, rnd + 1u);      // every CTA read it long ago
 }
@@ -471,8 +473,8 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
 
     const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 8;   // this round's tag / flag base
     for (int t = 0; t < e.B; ++t) {
-        for (int c0 = 0; c0 < batch; c0 += kFusChunk) {
-            const int nb = min(kFusChunk, batch - c0);
+        for (int c0 = 0; c0 < batch; c0 += p.gsz) {
+            const int nb = min(p.gsz, batch - c0);
             // Columns of the hidden-half GEMM: requests' hi halves in rows [0, lo_off), lo halves in [lo_off, 2 lo_off);
             // N shrinks with the batch (8 columns serve up to 4 requests), and so do the ring traffic and the MMA time.
             const int ncol = (nb <= 4) ? 8 : (nb <= 8) ? 16 : (nb <= 16) ? 32 : 64;
@@ -643,8 +645,8 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             }
             tc::fence_before_sync();
             __syncthreads();
+            if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride + c0 / p.gsz, fbase + (unsigned int)(t + 1)); }
         }
-        if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride, fbase + (unsigned int)(t + 1)); }
     }
     __syncthreads();
     if (warp == 0) tc::tmem_free<kTcCols>(tmem);
@@ -735,7 +737,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         if (expand && tid < r) cpre = e.C[((size_t)b * L + depth) * r + tid];
         if (warp == 0) {
             for (int q = lane; q < p.n_gru; q += 32)
-                fused_spin([&] { return (int)(ld_relaxed_u32(p.flags + (size_t)q * kFusFlagStride) - (fbase + (unsigned int)(t + 1))) >= 0; }, p.err);
+                fused_spin([&] { return (int)(ld_relaxed_u32(p.flags + (size_t)q * kFusFlagStride + b / p.gsz) - (fbase + (unsigned int)(t + 1))) >= 0; }, p.err);
         }
         __syncthreads();
         // the live frontier is entries 1 .. n_front of buffer `cur` (entry 0 was popped by the previous step)
