@@ -672,6 +672,48 @@ __host__ __device__ inline size_t wave_req_smem2(int r, int M, int B, int k, int
     return s + 1024;
 }
 
+// Rank of frontier entry i (old entry i < n_old, or new candidate i - n_old) in the merged order; strict total order: key
+// desc, then parent position asc, then index asc (old entries before new ones).  Out of line on purpose: the request
+// role's step loop has to stay inside the instruction cache (it runs once per step, on one latency chain).
+__device__ __noinline__ int wave_merge_rank(const unsigned long long *oK, const unsigned int *oM, int n_old,
+                                            const unsigned long long *nKey, const unsigned int *nMeta, int n_new,
+                                            const int *ePos, int i, unsigned long long mkh, unsigned int mmh) {
+    auto prec = [&](unsigned long long ka, unsigned int ma, int ia, unsigned long long kb, unsigned int mb, int ib) {
+        if (ka != kb) return ka > kb;
+        const int pa = ePos[(ma >> 16) & 0x3FFu], pb = ePos[(mb >> 16) & 0x3FFu];
+        if (pa != pb) return pa < pb;
+        return ia < ib;
+    };
+    const bool is_old = i < n_old;
+    int rank = 0;
+    if (is_old) rank = i;
+    else {                                               // old entries in front of it: the list is sorted
+        int lo = 0, hi = n_old;
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            const unsigned long long km = oK[mid];
+            if (km > mkh || (km == mkh && prec(km, oM[mid], mid, mkh, mmh, i))) lo = mid + 1; else hi = mid;
+        }
+        rank = lo;
+    }
+    // new entries in front of it: keys only, two per load; equal keys (the same score, depth and token under two
+    // parents: rare) go through the full comparator
+    int n_eq = 0, q = 0;
+#pragma unroll 2
+    for (; q + 2 <= n_new; q += 2) {
+        const ulonglong2 o = *reinterpret_cast<const ulonglong2 *>(nKey + q);
+        rank += (o.x > mkh) + (o.y > mkh);
+        n_eq += (o.x == mkh) + (o.y == mkh);
+    }
+    if (q < n_new) { rank += (nKey[q] > mkh); n_eq += (nKey[q] == mkh); }
+    if (n_eq > (is_old ? 0 : 1)) {
+#pragma unroll 1
+        for (int q2 = 0; q2 < n_new; ++q2)
+            if (nKey[q2] == mkh && n_old + q2 != i) rank += prec(nKey[q2], nMeta[q2], n_old + q2, mkh, mmh, i) ? 1 : 0;
+    }
+    return rank;
+}
+
 __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char *smem_raw) {
     const ExpandParams &e = p.e;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -917,13 +959,6 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
             const unsigned int *oM = gMeta[cur];
             unsigned long long *dK = gKey[cur ^ 1];
             unsigned int *dM = gMeta[cur ^ 1];
-            // strict total order: key desc, then parent position asc, then index asc (old entries before new ones)
-            auto prec = [&](unsigned long long ka, unsigned int ma, int ia, unsigned long long kb, unsigned int mb, int ib) {
-                if (ka != kb) return ka > kb;
-                const int pa = ePos[(ma >> 16) & 0x3FFu], pb = ePos[(mb >> 16) & 0x3FFu];
-                if (pa != pb) return pa < pb;
-                return ia < ib;
-            };
             int rk[2] = {0, 0};
             unsigned long long mk[2] = {0ull, 0ull};
             unsigned int mm[2] = {0u, 0u};
@@ -934,32 +969,7 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                 const bool is_old = i < n_old;
                 mk[h] = is_old ? oK[i] : nKey[i - n_old];
                 mm[h] = is_old ? oM[i] : nMeta[i - n_old];
-                int rank = 0;
-                const unsigned long long mkh = mk[h];
-                if (is_old) rank = i;
-                else {                                               // old entries in front of it: the list is sorted
-                    int lo = 0, hi = n_old;
-                    while (lo < hi) {
-                        const int mid = (lo + hi) >> 1;
-                        const unsigned long long km = oK[mid];
-                        if (km > mkh || (km == mkh && prec(km, oM[mid], mid, mkh, mm[h], i))) lo = mid + 1; else hi = mid;
-                    }
-                    rank = lo;
-                }
-                // new entries in front of it: keys only, two per load; equal keys (the same score, depth and token under two
-                // parents: rare) go through the full comparator
-                int n_eq = 0, q = 0;
-                for (; q + 2 <= n_new; q += 2) {
-                    const ulonglong2 o = *reinterpret_cast<const ulonglong2 *>(nKey + q);
-                    rank += (o.x > mkh) + (o.y > mkh);
-                    n_eq += (o.x == mkh) + (o.y == mkh);
-                }
-                if (q < n_new) { rank += (nKey[q] > mkh); n_eq += (nKey[q] == mkh); }
-                if (n_eq > (is_old ? 0 : 1)) {
-#pragma unroll 1
-                    for (int q2 = 0; q2 < n_new; ++q2)
-                        if (nKey[q2] == mkh && n_old + q2 != i) rank += prec(nKey[q2], nMeta[q2], n_old + q2, mkh, mm[h], i) ? 1 : 0;
-                }
+                const int rank = wave_merge_rank(oK, oM, n_old, nKey, nMeta, n_new, ePos, i, mk[h], mm[h]);
                 rk[h] = rank;
             }
             __syncthreads();                                         // every rank is computed from the old positions

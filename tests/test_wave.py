@@ -171,3 +171,29 @@ def test_adaptive_schedule_picks_by_regime():
         assert case.builder.get_option("expand_path_taken") == 6
         chosen[regime] = case.builder.get_option("schedule_chosen")
     assert chosen == {"flat": 1, "peaked": 0}, chosen
+
+
+@pytest.mark.parametrize("path,schedule", [(5, 0), (4, 0), (0, 1)])
+def test_exact_fp32_ties_give_a_valid_tree(path, schedule):
+    """Saturated slices (a planted token 40 nats above the row): log p of the top child is exactly 0 in fp32, so a child's
+    score EQUALS its parent's and sibling subtrees tie bit for bit.  Every schedule must still return a valid best-first tree
+    (parents before children, the same node set up to the comparator's margin): reading A17 / ADVICE r1."""
+    gu = _gu()
+    case = _small(gu, 256, 40, 8)
+    inp = wl.make_inputs(case.cfg, batch=6, seed=2300, regime="peaked")
+    lg = inp["logits"].float()
+    rows = torch.arange(case.cfg.L)
+    for b in range(6):
+        lg[b, rows, inp["planted"][b]] = lg[b].max(dim=1).values + 40.0
+    inp["logits"] = lg.to(inp["logits"].dtype)
+    case.builder.set_option("schedule", schedule)
+    try:
+        with _with(case, expand_path=path):
+            out = case.run_gpu(inp, 24, 40, 1.0)
+            ne, nt = gu.check_batch(case, inp, 24, 40, 1.0, BF16_TOL, out=out)
+    finally:
+        case.builder.set_option("schedule", 0)
+    sc = out.scores[:, 1:6].cpu().numpy()
+    assert (sc[:, 0] == 0.0).all(), "the inputs were meant to saturate: top child log p == 0"
+    print(f"exact {ne} tolerant {nt}")
+    assert ne + nt == 6
