@@ -7,6 +7,8 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <mutex>
+#include <vector>
 
 #include "../../include/dominotree.h"
 #include "dt_budget.cuh"
@@ -73,6 +75,36 @@ struct dt_handle {
     int last_cuda;
     int num_sms;
 };
+
+// The input-half table P = E W_ih^T (1.87 GB at the 8B shape) depends on the weights alone: handles created on the same
+// borrowed weight tensors (same device, pointers, shapes, dtype -- e.g. one handle per stream of a serving process) share
+// one copy, reference-counted; the weights are immutable while a handle borrows them (dominotree.h).
+struct PEntry { const void *embed, *w_ih; int V, d, g, dtype, dev; float *P; int refs; };
+static std::mutex g_p_mutex;
+static std::vector<PEntry> g_p_cache;
+static float *p_cache_acquire(const dt_weights &w, int dev) {
+    std::lock_guard<std::mutex> lk(g_p_mutex);
+    for (auto &e : g_p_cache)
+        if (e.embed == w.embed && e.w_ih == w.gru_w_ih && e.V == w.V && e.d == w.d && e.g == w.g && e.dtype == (int)w.dtype && e.dev == dev) {
+            e.refs += 1;
+            return e.P;
+        }
+    return nullptr;
+}
+static void p_cache_insert(const dt_weights &w, int dev, float *P) {
+    std::lock_guard<std::mutex> lk(g_p_mutex);
+    g_p_cache.push_back(PEntry{w.embed, w.gru_w_ih, w.V, w.d, w.g, (int)w.dtype, dev, P, 1});
+}
+static void p_cache_release(float *P) {      // frees P when the last handle lets go (also for tables that never got into the cache)
+    if (!P) return;
+    std::lock_guard<std::mutex> lk(g_p_mutex);
+    for (size_t i = 0; i < g_p_cache.size(); ++i)
+        if (g_p_cache[i].P == P) {
+            if (--g_p_cache[i].refs == 0) { cudaFree(P); g_p_cache.erase(g_p_cache.begin() + i); }
+            return;
+        }
+    cudaFree(P);
+}
 
 #define DT_CUDA(h, call)                                                   \
     do {                                                                   \
@@ -339,7 +371,10 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     h->ws_bytes = off;
     h->p_bytes = (size_t)w->V * 3 * w->g * 4;
     if (cudaMalloc(&h->ws, h->ws_bytes) != cudaSuccess) { cudaGetLastError(); delete h; return DT_ERR_ALLOC; }
-    if (cudaMalloc(&h->P, h->p_bytes) != cudaSuccess) { cudaGetLastError(); cudaFree(h->ws); delete h; return DT_ERR_ALLOC; }
+    bool p_shared = false;
+    h->P = p_cache_acquire(*w, dev);
+    if (h->P) p_shared = true;
+    else if (cudaMalloc(&h->P, h->p_bytes) != cudaSuccess) { cudaGetLastError(); cudaFree(h->ws); delete h; return DT_ERR_ALLOC; }
     h->cand_id = (int32_t *)(h->ws + o_cid); h->cand_val = (float *)(h->ws + o_cval);
     h->sel_part = (unsigned long long *)(h->ws + o_part);
     h->sel_counter = (unsigned int *)(h->ws + o_cnt); h->sel_tau = (unsigned int *)(h->ws + o_tau);
@@ -358,7 +393,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     if (cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess) {
-        cudaGetLastError(); cudaFree(h->ws); cudaFree(h->P); delete h; return DT_ERR_CUDA;
+        cudaGetLastError(); cudaFree(h->ws); p_cache_release(h->P); delete h; return DT_ERR_CUDA;
     }
     if (h->fused_ok) {
         h->s_hi = (__nv_bfloat16 *)(h->ws + o_shi); h->s_lo = (__nv_bfloat16 *)(h->ws + o_slo);
@@ -401,14 +436,15 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
         }
     }
     // P = E W_ih^T  (weight-only table)
-    if (rc == DT_OK) {
+    if (rc == DT_OK && !p_shared) {
         if (w->dtype == DT_BF16)
             rc = launch_gemm_nt<__nv_bfloat16>(h, w->embed, w->d, w->gru_w_ih, w->d, h->P, 3LL * w->g, w->V, 3 * w->g, w->d, 0);
         else
             rc = launch_gemm_nt<float>(h, w->embed, w->d, w->gru_w_ih, w->d, h->P, 3LL * w->g, w->V, 3 * w->g, w->d, 0);
     }
     if (rc == DT_OK && cudaDeviceSynchronize() != cudaSuccess) { h->last_cuda = (int)cudaGetLastError(); rc = DT_ERR_CUDA; }
-    if (rc != DT_OK) { cudaFree(h->ws); cudaFree(h->P); delete h; return rc; }
+    if (rc != DT_OK) { cudaFree(h->ws); p_cache_release(h->P); delete h; return rc; }
+    if (!p_shared) p_cache_insert(*w, dev, h->P);
     h->launches = 0;
     *out = h;
     return DT_OK;
@@ -420,7 +456,7 @@ extern "C" int dt_destroy(dt_handle *h) {
     if (h->side) cudaStreamDestroy(h->side);
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->ev_join) cudaEventDestroy(h->ev_join);
-    cudaFree(h->ws); cudaFree(h->P);
+    cudaFree(h->ws); p_cache_release(h->P);
     if (h->stage) cudaFree(h->stage);
     delete h;
     return DT_OK;

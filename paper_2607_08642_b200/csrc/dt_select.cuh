@@ -261,7 +261,7 @@ __device__ __noinline__ SelWarpCtx sel_drain(SM &sm, SelWarpCtx c, int M, int V,
     unsigned long long *seg = sm.cand + warp * SM::kSeg;
     volatile unsigned int *vwcnt = sm.wcnt;
     __syncwarp();
-    constexpr int kU = 4;                                           // vectors per lane in flight: one L2 round trip per 4 batches
+    constexpr int kU = 4;                                           // vectors per lane in flight: one L2 round trip per 4 batches (8 spills)
     for (int base0 = 0; base0 < c.qcnt; base0 += kLanes * kU) {
         uint4 vv[kU];
         int gvv[kU];

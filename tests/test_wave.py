@@ -197,3 +197,21 @@ def test_exact_fp32_ties_give_a_valid_tree(path, schedule):
     assert (sc[:, 0] == 0.0).all(), "the inputs were meant to saturate: top child log p == 0"
     print(f"exact {ne} tolerant {nt}")
     assert ne + nt == 6
+
+
+def test_handles_on_the_same_weights_share_the_input_table():
+    """P = E W_ih^T is reference-counted across handles created on the same borrowed weight tensors: the second handle
+    gives the same trees, and closing either leaves the other working."""
+    import paper_2607_08642_b200 as dtb
+    gu = _gu()
+    case = _small(gu, 256, 40, 8)
+    inp = wl.make_inputs(case.cfg, batch=4, seed=2400)
+    ref = case.run_gpu(inp, 24, 20, 0.6)
+    b2 = dtb.DominoTreeBuilder(case.w_gpu, max_batch=4, L=case.cfg.L, max_M=32, max_B=48, k=8)
+    out2 = b2.build_trees(inp["logits"].cuda(), inp["hidden"].cuda(), inp["root_tokens"].cuda(), inp["root_positions"].cuda(), 24, 20, 0.6)
+    torch.cuda.synchronize()
+    for name in ("tokens", "parents", "scores", "mask"):
+        assert torch.equal(getattr(ref, name), getattr(out2, name)), name
+    b2.close()
+    again = case.run_gpu(inp, 24, 20, 0.6)
+    assert torch.equal(ref.tokens, again.tokens) and torch.equal(ref.scores, again.scores)
