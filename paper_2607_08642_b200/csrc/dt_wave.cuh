@@ -822,32 +822,54 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
         // ---- a_j = SiLU(C + W1[:, d:] S_j): the P cluster partials are summed in a fixed order (batch-invariant): two
         // neighbouring lanes per (node, four columns) take the even / the odd clusters, all loads of a lane in flight at once
         {
+            const int n_task = 2 * n_it * r4;
 #pragma unroll 1
-            for (int base = 0; base < 2 * n_it * r4; base += kWvThreads) {          // block-uniform trip count
-                const int idx = base + tid, pair = idx >> 1, h = idx & 1;
-                const bool act = base ? (pair < n_it * r4) : act0;
-                const int j = base ? (act ? pair / r4 : 0) : j0, jq = base ? (act ? pair - j * r4 : 0) : jq0;
-                float4 acc = make_float4(0.f, 0.f, 0.f, 0.f), cv = cv0;
-                if (act) {
-                    if (base && h == 0) cv = __ldg(reinterpret_cast<const float4 *>(e.C + ((size_t)b * L + eDep[itE[j]]) * r) + jq);
-                    const float4 *pp = reinterpret_cast<const float4 *>(p.partial + ((size_t)(b * kWvMaxW + j) * P) * r) + jq;
-#pragma unroll 1
-                    for (int q0 = h; q0 < P; q0 += 16) {
-                        float4 v[8];
+            for (int base = 0; base < n_task; base += 2 * kWvThreads) {             // block-uniform trip count; two tasks per thread,
+                bool act[2];                                                        // the loads of both in flight together
+                int jj[2], jq[2], hh[2];
+                float4 cv[2], v[2][8];
+                const float4 *pp[2];
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) v[i] = (q0 + 2 * i < P) ? __ldcg(pp + (size_t)(q0 + 2 * i) * r4) : make_float4(0.f, 0.f, 0.f, 0.f);
+                for (int t = 0; t < 2; ++t) {
+                    const int idx = base + t * kWvThreads + tid, pair = idx >> 1;
+                    hh[t] = idx & 1;
+                    const bool first = (base == 0 && t == 0);
+                    act[t] = first ? act0 : (pair < n_it * r4);
+                    jj[t] = first ? j0 : (act[t] ? pair / r4 : 0);
+                    jq[t] = first ? jq0 : (act[t] ? pair - jj[t] * r4 : 0);
+                    cv[t] = first ? cv0 : make_float4(0.f, 0.f, 0.f, 0.f);
+                    pp[t] = reinterpret_cast<const float4 *>(p.partial + ((size_t)(b * kWvMaxW + jj[t]) * P) * r) + jq[t];
+                    if (act[t]) {
+                        if (!first && hh[t] == 0) cv[t] = __ldg(reinterpret_cast<const float4 *>(e.C + ((size_t)b * L + eDep[itE[jj[t]]]) * r) + jq[t]);
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) { acc.x += v[i].x; acc.y += v[i].y; acc.z += v[i].z; acc.w += v[i].w; }
+                        for (int i = 0; i < 8; ++i)
+                            v[t][i] = (hh[t] + 2 * i < P) ? __ldcg(pp[t] + (size_t)(hh[t] + 2 * i) * r4) : make_float4(0.f, 0.f, 0.f, 0.f);
                     }
                 }
-                // even clusters + odd clusters, then C
-                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 1); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 1);
-                acc.z += __shfl_xor_sync(0xffffffffu, acc.z, 1); acc.w += __shfl_xor_sync(0xffffffffu, acc.w, 1);
-                if (act && h == 0) {
-                    float4 o;
-                    o.x = cv.x + acc.x; o.y = cv.y + acc.y; o.z = cv.z + acc.z; o.w = cv.w + acc.w;
-                    o.x *= sigmoidf_acc(o.x); o.y *= sigmoidf_acc(o.y); o.z *= sigmoidf_acc(o.z); o.w *= sigmoidf_acc(o.w);
-                    *reinterpret_cast<float4 *>(sA + (size_t)j * r + 4 * jq) = o;
+#pragma unroll
+                for (int t = 0; t < 2; ++t) {
+                    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (act[t]) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) { acc.x += v[t][i].x; acc.y += v[t][i].y; acc.z += v[t][i].z; acc.w += v[t][i].w; }
+#pragma unroll 1
+                        for (int q0 = hh[t] + 16; q0 < P; q0 += 16) {               // more than 16 clusters (g > 1024)
+                            float4 w8[8];
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) w8[i] = (q0 + 2 * i < P) ? __ldcg(pp[t] + (size_t)(q0 + 2 * i) * r4) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) { acc.x += w8[i].x; acc.y += w8[i].y; acc.z += w8[i].z; acc.w += w8[i].w; }
+                        }
+                    }
+                    // even clusters + odd clusters, then C
+                    acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 1); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 1);
+                    acc.z += __shfl_xor_sync(0xffffffffu, acc.z, 1); acc.w += __shfl_xor_sync(0xffffffffu, acc.w, 1);
+                    if (act[t] && hh[t] == 0) {
+                        float4 o;
+                        o.x = cv[t].x + acc.x; o.y = cv[t].y + acc.y; o.z = cv[t].z + acc.z; o.w = cv[t].w + acc.w;
+                        o.x *= sigmoidf_acc(o.x); o.y *= sigmoidf_acc(o.y); o.z *= sigmoidf_acc(o.z); o.w *= sigmoidf_acc(o.w);
+                        *reinterpret_cast<float4 *>(sA + (size_t)jj[t] * r + 4 * jq[t]) = o;
+                    }
                 }
             }
         }
@@ -857,6 +879,47 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
 
         // ---- z_m = ((base_m - base_0) + W2[cand_m, :] a) / T_eff   PAPER.md:143-144 (shift-invariant)
         // a warp takes 8 candidate rows (one swizzle row group), four lanes per row; two accumulation chains per lane
+        const int rb_n = (M + 31) >> 5;                              // 32-row blocks per node
+        if (n_it * rb_n >= kWvThreads / 32) {
+            // enough (node, row block) tasks for every warp: a lane owns one candidate row and walks all of it -- no cross-lane
+            // reduction, 8 accumulation chains -- with EXACTLY the association of the four-lanes-per-row form below (class
+            // c = piece index mod 4 is what lane group qq sums there; (q0 + q1) + (q2 + q3) is what its two shuffles add), so a
+            // node's scores do not depend on how many nodes share the step (batch invariance)
+#pragma unroll 1
+            for (int task = warp; task < n_it * rb_n; task += kWvThreads / 32) {
+                int j = 0, rb = task;
+                while (rb >= rb_n) { rb -= rb_n; ++j; }
+                const int si = ctl.d2s[eDep[itE[j]]];
+                const unsigned char *sl = sW2 + (size_t)si * slice_bytes;
+                const float *bs = slBase + si * M;
+                const float *aj = sA + (size_t)j * r;
+                const int m = 32 * rb + lane, mc = min(m, M - 1), rw = mc & 7;
+                const unsigned char *rowp = sl + (size_t)(mc >> 3) * Ka * 1024 + rw * 128;
+                float A0[4] = {0.f, 0.f, 0.f, 0.f}, A1[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll 2
+                for (int v0 = 0; v0 < nvec; v0 += 4) {
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        const int v = v0 + c;
+                        if (v < nvec) {
+                            const uint4 q = *reinterpret_cast<const uint4 *>(rowp + (size_t)(v >> 3) * 1024 + (((v & 7) ^ rw) << 4));
+                            const float4 a0 = *reinterpret_cast<const float4 *>(aj + (size_t)v * 8);
+                            const float4 a1 = *reinterpret_cast<const float4 *>(aj + (size_t)v * 8 + 4);
+                            float f[8];
+                            unpack8(q, f);
+                            A0[c] = fmaf(f[0], a0.x, A0[c]); A1[c] = fmaf(f[1], a0.y, A1[c]); A0[c] = fmaf(f[2], a0.z, A0[c]); A1[c] = fmaf(f[3], a0.w, A1[c]);
+                            A0[c] = fmaf(f[4], a1.x, A0[c]); A1[c] = fmaf(f[5], a1.y, A1[c]); A0[c] = fmaf(f[6], a1.z, A0[c]); A1[c] = fmaf(f[7], a1.w, A1[c]);
+                        }
+                    }
+                }
+                const float acc = ((A0[0] + A1[0]) + (A0[1] + A1[1])) + ((A0[2] + A1[2]) + (A0[3] + A1[3]));
+                if (m < M) {
+                    const float z = __fdiv_rn((bs[m] - bs[0]) + acc, e.T_eff);
+                    sZ[(size_t)j * M + m] = z;
+                    sKey[(size_t)j * M + m] = ((unsigned long long)ord_key(z) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned int)slTok[si * M + m]);
+                }
+            }
+        } else
 #pragma unroll 1
         for (int j = 0; j < n_it; ++j) {
             const int si = ctl.d2s[eDep[itE[j]]];
