@@ -572,7 +572,8 @@ GRU_STAMPS = ((0, "items polled + compacted"), (1, "pass begins"), (2, "P / prev
               (10, "TMEM loads, hi + lo shuffles, gates"), (11, "global + DSMEM state stores issued"), (12, "cluster barrier"),
               (4, "proxy fence + CTA barrier"), (13, "thread 0: D2 tcgen05.mma + commit issued"), (5, "D2 complete (mbarrier)"),
               (6, "partials stored + CTA barrier"), (7, "gpu fence + flag store"))
-REQ_STAMPS = ((0, "flags seen"), (1, "a = SiLU(C + partials)"), (2, "W2 slice dots"), (3, "slice log-softmax + top-k"),
+REQ_STAMPS = ((0, "flags seen"), (1, "a = SiLU(C + partials)"), (2, "W2 slice dots"), (10, "top-k: threshold from the lane maxima (warp 0)"),
+              (11, "top-k: ranks among the keys above it, log-softmax (warp 0)"), (3, "CTA barrier after the top-k"),
               (6, "merge into the sorted frontier"), (9, "nominate + publish (warp 0)"), (4, "CTA barrier"),
               (5, "slices staged (issue)"))
 

@@ -667,8 +667,8 @@ __host__ __device__ inline size_t wave_req_smem2(int r, int M, int B, int k, int
     s += 2 * al((size_t)B * 8) + 2 * al((size_t)B * 4);                     // frontier, two buffers
     s += al((size_t)W * k * 8) + al((size_t)W * k * 4);                     // new children
     s += 3 * al((size_t)e_max * 4);                                         // eDep, eSco, ePos
-    s += al((size_t)W * r * 4) + al((size_t)W * M * 4) + al((size_t)W * M * 8);
-    s += al((size_t)4 * kWvMaxW * 4) + al(256);
+    s += al((size_t)W * r * 4) + al((size_t)W * M * 8);
+    s += al((size_t)4 * kWvMaxW * 4) + al(256) + al((size_t)kWvThreads * 8) + al((size_t)kWvMaxW * 8);
     return s + 1024;
 }
 
@@ -742,9 +742,10 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
     float *eSco = reinterpret_cast<float *>(carve((size_t)e_max * 4));             // its score
     int *ePos = reinterpret_cast<int *>(carve((size_t)e_max * 4));                 // its position in the frontier (-1 root)
     float *sA = reinterpret_cast<float *>(carve((size_t)W * r * 4));
-    float *sZ = reinterpret_cast<float *>(carve((size_t)W * M * 4));
     unsigned long long *sKey = reinterpret_cast<unsigned long long *>(carve((size_t)W * M * 8));   // (z, ~token) of every candidate
     int *itE = reinterpret_cast<int *>(carve((size_t)4 * kWvMaxW * 4));
+    unsigned long long *sSvK = reinterpret_cast<unsigned long long *>(carve((size_t)kWvThreads * 8));   // per warp: keys at or above the top-k threshold
+    float2 *sStat = reinterpret_cast<float2 *>(carve((size_t)kWvMaxW * 8));        // per node: slice maximum, log-sum-exp
     int *itTok = itE + kWvMaxW, *itPs = itTok + kWvMaxW;
     WaveCtl &ctl = *reinterpret_cast<WaveCtl *>(carve(256));
 
@@ -915,7 +916,6 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                 const float acc = ((A0[0] + A1[0]) + (A0[1] + A1[1])) + ((A0[2] + A1[2]) + (A0[3] + A1[3]));
                 if (m < M) {
                     const float z = __fdiv_rn((bs[m] - bs[0]) + acc, e.T_eff);
-                    sZ[(size_t)j * M + m] = z;
                     sKey[(size_t)j * M + m] = ((unsigned long long)ord_key(z) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned int)slTok[si * M + m]);
                 }
             }
@@ -948,7 +948,6 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
                 const int m = 8 * rg + rw;
                 if (qq == 0 && m < M) {
                     const float z = __fdiv_rn((bs[m] - base0) + acc, e.T_eff);
-                    sZ[(size_t)j * M + m] = z;
                     sKey[(size_t)j * M + m] = ((unsigned long long)ord_key(z) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned int)slTok[si * M + m]);
                 }
             }
@@ -956,60 +955,114 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
         __syncthreads();
         WV_TR(1, b == 0, s, 2);
 
-        // ---- slice log-softmax (reading A1) and top-k by (z desc, token asc): rank by counting over the sortable keys, `tpc`
-        // neighbouring lanes per candidate, every warp working for ONE node (it computes that node's max and log-sum-exp
-        // itself); the k best become frontier candidates with score g_parent + logp
+        // ---- slice log-softmax (reading A1) and top-k by (z desc, token asc).  A warp per node finds the k best without
+        // anything that scales with M * M: (1) every lane takes the best of its own M / 32 keys and k rounds of a warp
+        // max reduction give L, the k-th best of the 32 lane maxima: at least k keys lie at or above L, so the true top k
+        // do; (2) the keys at or above L (k plus a few) are handed one to a lane and ranked among themselves by counting
+        // over the full 64-bit keys through shuffles.  The result is the exact top k in the exact order.  With at most
+        // four nodes a second warp per node computes the slice maximum and log-sum-exp meanwhile (named barrier 1 + j);
+        // otherwise the node's warp does both.  The k best become frontier candidates with score g_parent + logp
         {
-            int ltpc = 3;                                            // log2 of the lanes per candidate
-            while (ltpc > 0 && n_it * ((M << ltpc) + 31 >> 5) > kWvThreads / 32) --ltpc;
-            const int tpc = 1 << ltpc;
-            const int wpi = ((M << ltpc) + 31) >> 5;                 // warps per node
-            const int per = (M + tpc - 1) >> ltpc;
-            int jw = 0, wl = warp;                                   // node of this warp within a round, warp within the node
-            while (wl >= wpi) { wl -= wpi; ++jw; }
-            int ipr = 0;                                             // nodes per round
-            for (int w = wpi; w <= kWvThreads / 32; w += wpi) ++ipr;
-            if (ipr < 1) ipr = 1;
+            const int MI = (M + 31) >> 5;
+            const bool split = 2 * n_it <= kWvThreads / 32;
+            const bool stat_only = split && (warp & 1);
+            const int jstep = split ? kWvThreads / 64 : kWvThreads / 32;
+            unsigned long long *svK = sSvK + warp * 32;
 #pragma unroll 1
-            for (int j0s = 0; j0s < n_it; j0s += ipr) {
-                const int j = j0s + jw;
-                if (j >= n_it || jw >= ipr) continue;                // warp-uniform
+            for (int j = split ? (warp >> 1) : warp; j < n_it; j += jstep) {
                 const int x = itE[j];
-                const float *zj = sZ + (size_t)j * M;
                 const unsigned long long *kj = sKey + (size_t)j * M;
-                float zmax = -INFINITY;
-#pragma unroll 1
-                for (int m = lane; m < M; m += 32) zmax = fmaxf(zmax, zj[m]);
-                zmax = ord_key_inv(__reduce_max_sync(0xffffffffu, ord_key(zmax)));
-                float ssum = 0.f;
-#pragma unroll 1
-                for (int m = lane; m < M; m += 32) ssum += __expf(zj[m] - zmax);
-                ssum = warp_sum(ssum);
-                const float lse = __logf(ssum);
-                const int t = (wl * 32 + lane) >> ltpc, part = lane & (tpc - 1);   // candidate and the share of the keys it counts
-                const bool act = t < M;
-                const unsigned long long mk = act ? kj[t] : 0ull;
-                int rank = 0;
-                if (act) {
-                    const int m0 = part * per, m1 = min(M, m0 + per);
-                    int q = m0;
-                    if (!(m0 & 1))
-#pragma unroll 4
-                        for (; q + 2 <= m1; q += 2) {
-                            const ulonglong2 o = *reinterpret_cast<const ulonglong2 *>(kj + q);
-                            rank += (o.x > mk) + (o.y > mk);
+                float zmax = 0.f, lse = 0.f;
+                if (!split || stat_only) {
+                    float zr[8];
+                    zmax = -INFINITY;
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int m = lane + 32 * i;
+                        zr[i] = -INFINITY;
+                        if (i < MI && m < M) {
+                            zr[i] = ord_key_inv((unsigned int)(kj[m] >> 32));
+                            zmax = fmaxf(zmax, zr[i]);
                         }
+                    }
+                    zmax = ord_key_inv(__reduce_max_sync(0xffffffffu, ord_key(zmax)));
+                    float ssum = 0.f;
+#pragma unroll
+                    for (int i = 0; i < 8; ++i)
+                        if (i < MI && lane + 32 * i < M) ssum += __expf(zr[i] - zmax);
+                    ssum = warp_sum(ssum);
+                    lse = __logf(ssum);
+                    if (stat_only) {
+                        if (lane == 0) sStat[j] = make_float2(zmax, lse);
+                        __threadfence_block();
+                        asm volatile("bar.arrive %0, 64;" ::"r"(1 + j) : "memory");
+                        continue;
+                    }
+                }
+                unsigned long long kk[8];
+                unsigned int hmax = 0u;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const int m = lane + 32 * i;
+                    kk[i] = (i < MI && m < M) ? kj[m] : 0ull;
+                    hmax = max(hmax, (unsigned int)(kk[i] >> 32));
+                }
+                unsigned int cur = (hmax & ~31u) | (unsigned int)(31 - lane), L = 0u;   // lane in the low bits: all distinct
 #pragma unroll 1
-                    for (; q < m1; ++q) rank += (kj[q] > mk);
+                for (int rr = 0; rr < k; ++rr) {
+                    L = __reduce_max_sync(0xffffffffu, cur);
+                    if (cur == L) cur = 0u;
                 }
-                for (int o = 1; o < tpc; o <<= 1) rank += __shfl_xor_sync(0xffffffffu, rank, o);
-                if (act && part == 0 && rank < k) {
-                    const float lpm = (zj[t] - zmax) - lse;
-                    const int tok = (int)(0xFFFFFFFFu - (unsigned int)(mk & 0xFFFFFFFFull));
-                    const int cdep = eDep[x] + 1;
-                    nKey[j * k + rank] = wave_gkey(eSco[x] + lpm, cdep, tok);
-                    nMeta[j * k + rank] = (unsigned int)cdep | ((unsigned int)x << 16);
+                L &= ~31u;
+                WV_TR(1, b == 0, s, 10);
+                int ns = 0;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    if (i >= MI) break;
+                    const bool in = (unsigned int)(kk[i] >> 32) >= L && kk[i] != 0ull;
+                    const unsigned int bal = __ballot_sync(0xffffffffu, in);
+                    const int at = ns + __popc(bal & ((1u << lane) - 1u));
+                    if (in && at < 32) svK[at] = kk[i];
+                    ns += __popc(bal);
                 }
+                __syncwarp();
+                if (split) {
+                    asm volatile("bar.sync %0, 64;" ::"r"(1 + j) : "memory");
+                    const float2 st = sStat[j];
+                    zmax = st.x;
+                    lse = st.y;
+                }
+                const float gpar = eSco[x];
+                const int cdep = eDep[x] + 1;
+                if (ns <= 32) {
+                    const unsigned long long mk = lane < ns ? svK[lane] : 0ull;
+                    int rank = 0;
+#pragma unroll 4
+                    for (int q = 0; q < ns; ++q) rank += (__shfl_sync(0xffffffffu, mk, q) > mk);
+                    if (lane < ns && rank < k) {
+                        const float lpm = (ord_key_inv((unsigned int)(mk >> 32)) - zmax) - lse;
+                        const int tok = (int)(0xFFFFFFFFu - (unsigned int)(mk & 0xFFFFFFFFull));
+                        nKey[j * k + rank] = wave_gkey(gpar + lpm, cdep, tok);
+                        nMeta[j * k + rank] = (unsigned int)cdep | ((unsigned int)x << 16);
+                    }
+                } else {                                             // many equal keys at the threshold: count over the slice
+#pragma unroll 1
+                    for (int m = lane; m < M; m += 32) {
+                        const unsigned long long mk = kj[m];
+                        if ((unsigned int)(mk >> 32) < L) continue;
+                        int rank = 0;
+#pragma unroll 1
+                        for (int q = 0; q < M; ++q) rank += (kj[q] > mk);
+                        if (rank < k) {
+                            const float lpm = (ord_key_inv((unsigned int)(mk >> 32)) - zmax) - lse;
+                            const int tok = (int)(0xFFFFFFFFu - (unsigned int)(mk & 0xFFFFFFFFull));
+                            nKey[j * k + rank] = wave_gkey(gpar + lpm, cdep, tok);
+                            nMeta[j * k + rank] = (unsigned int)cdep | ((unsigned int)x << 16);
+                        }
+                    }
+                }
+                __syncwarp();
+                WV_TR(1, b == 0, s, 11);
             }
         }
         __syncthreads();
