@@ -567,7 +567,7 @@ def measure_sweep_and_arms(ctx):
 
 # ----------------------------------------------------------------------------------- in-kernel timeline
 # (stamp index, what has happened by then), in program order, for GRU CTA 0 / request CTA 0 (dt_wave.cuh WV_TR)
-GRU_STAMPS = ((0, "items polled + compacted"), (1, "pass begins"), (2, "P / previous-state loads issued"),
+GRU_STAMPS = ((0, "items polled + compacted"), (1, "pass begins"), (2, "P / previous-state loads issued"), (14, "producer thread 128: sources computed"), (15, "producer thread 128: first group issued"),
               (8, "issuer 0: first K chunk landed"), (9, "issuer 0: all tcgen05.mma + commit issued"), (3, "D1 complete (mbarrier)"),
               (10, "TMEM loads, hi + lo shuffles, gates"), (11, "global + DSMEM state stores issued"), (12, "cluster barrier"),
               (4, "proxy fence + CTA barrier"), (13, "thread 0: D2 tcgen05.mma + commit issued"), (5, "D2 complete (mbarrier)"),
@@ -576,6 +576,13 @@ REQ_STAMPS = ((0, "flags seen"), (1, "a = SiLU(C + partials)"), (2, "W2 slice do
               (11, "top-k: ranks among the keys above it, log-softmax (warp 0)"), (3, "CTA barrier after the top-k"),
               (6, "merge into the sorted frontier"), (9, "nominate + publish (warp 0)"), (4, "CTA barrier"),
               (5, "slices staged (issue)"))
+
+
+FUSED_GRU_STAMPS = ((0, "descriptors seen + CTA barrier"), (1, "state copies, P / previous-state loads issued"), (3, "D1 complete (copies landed, tcgen05.mma, mbarrier)"),
+                    (10, "TMEM -> shared + CTA barrier"), (11, "gates, state stores, W1 operand + CTA barrier"), (5, "D2 issued and complete"),
+                    (6, "partials stored + CTA barrier"), (7, "gpu fence + flag store"))
+FUSED_REQ_STAMPS = ((0, "flags seen"), (1, "a = SiLU(C + partials)"), (2, "W2 slice dots + online softmax statistics"), (3, "top-k + CTA barrier"),
+                    (9, "pop: next descriptor published (thread 0)"), (4, "merge + CTA barrier"))
 
 
 def run_trace(args):
@@ -593,8 +600,11 @@ def run_trace(args):
     batch = args.trace_batch or cfg.batch
     w_gpu = {n: t.cuda() for n, t in wl.make_weights(cfg).items()}
     builder = dtb.DominoTreeBuilder(w_gpu, max_batch=batch, L=cfg.L, max_M=cfg.M, max_B=cfg.B, k=cfg.k, lib_path=lib_path)
-    builder.set_option("expand_path", 5)          # the timeline is the wavefront kernel's, whatever the adaptive schedule would pick
-    builder.set_option("wave_groups", 1)          # one request group: GRU step i and request step i are the same step
+    fused = (args.trace_path == 4)
+    builder.set_option("expand_path", args.trace_path)   # the timeline of ONE kernel, whatever the adaptive schedule would pick
+    if not fused:
+        builder.set_option("wave_groups", 1)      # one request group: GRU step i and request step i are the same step
+    gru_stamps, req_stamps = (FUSED_GRU_STAMPS, FUSED_REQ_STAMPS) if fused else (GRU_STAMPS, REQ_STAMPS)
     if args.wave_width:
         builder.set_option("wave_width", args.wave_width)
     lib = builder.lib
@@ -602,7 +612,8 @@ def run_trace(args):
     lib.dt_trace_read.restype = ctypes.c_int
     S, K = 64, 16
     buf = np.zeros((2, S, K), dtype=np.uint64)
-    out = {"workload": cfg.name, "batch": batch, "wave_width": args.wave_width or "auto", "unit": "ns (median over steps)"}
+    out = {"workload": cfg.name, "batch": batch, "kernel": "fused_expand_kernel<0> (lock-step, two request groups)" if fused else "wave_expand_kernel (one request group)",
+           "wave_width": args.wave_width or "auto", "unit": "ns (median over steps)"}
     for regime in ("flat", "peaked"):
         inp = wl.make_inputs(cfg, batch=batch, regime=regime)
         dev = {k_: inp[k_].cuda() for k_ in ("logits", "hidden", "root_tokens", "root_positions")}
@@ -619,7 +630,7 @@ def run_trace(args):
         rows = {}
         g = t[0, 1:max(steps - 1, 2)]          # skip step 0 (weight load) and the last
         q = t[1, 1:max(steps - 1, 2)]
-        for role, arr, stamps in (("gru", g, GRU_STAMPS), ("req", q, REQ_STAMPS)):
+        for role, arr, stamps in (("gru", g, gru_stamps), ("req", q, req_stamps)):
             for (i0, _), (i1, name) in zip(stamps[:-1], stamps[1:]):
                 ok = (arr[:, i1] > 0) & (arr[:, i0] > 0)
                 rows[f"{role}: {name}"] = float(np.median((arr[:, i1] - arr[:, i0])[ok])) if ok.any() else None
@@ -631,7 +642,7 @@ def run_trace(args):
         period = np.diff(t[0, 1:steps, 0])
         rows["step period"] = float(np.median(period)) if len(period) else None
         rows["steps"] = steps
-        rows["expansions_request0"] = builder.get_option("wave_expansions")
+        rows["expansions_request0"] = cfg.B if fused else builder.get_option("wave_expansions")
         out[regime] = rows
     print(json.dumps({"trace": out}), flush=True)
     builder.close()
@@ -649,6 +660,7 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="also time the batch-1 B x M sweep and the three scorer arms")
     ap.add_argument("--trace", action="store_true", help="in-kernel timeline of the wavefront kernel (measurement build, not a bench value)")
     ap.add_argument("--trace-batch", type=int, default=0, help="batch of the --trace leg (default: the workload's)")
+    ap.add_argument("--trace-path", type=int, default=5, choices=(4, 5), help="kernel of the --trace leg: 5 = wavefront (default), 4 = lock-step fused")
     ap.add_argument("--wave-width", type=int, default=0, help="nodes a request may expand per step (0 = auto)")
     args = ap.parse_args()
     if args.impl == "reference":

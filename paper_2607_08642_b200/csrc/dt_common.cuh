@@ -79,4 +79,32 @@ template <typename T> __device__ __forceinline__ float ldf(const T *p, size_t i)
     return ElemTraits<T>::to_f32(p[i]);
 }
 
+__device__ __forceinline__ unsigned long long wave_timer() {
+    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
+}
+// In-kernel timeline of the persistent expansion kernels (measurement builds only: `python -m paper_2607_08642_b200.build --trace` compiles the separate
+// libdominotree_trace.so with -DDT_TRACE, read by `bench.py --trace`): thread 0 of GRU CTA 0 (role 0) and of request
+// CTA 0 (role 1) of dt_wave.cuh / dt_fused.cuh stamp %globaltimer at fixed points of the first kWvTraceSteps steps.
+constexpr int kWvTraceSteps = 64, kWvTraceStamps = 16;
+#ifdef DT_TRACE
+__device__ unsigned long long g_wv_trace[2][kWvTraceSteps][kWvTraceStamps];
+// one PREDICATED store by thread 0 (no branch: a thread-0-only branch would leave its warp diverged and slow every warp
+// collective after it; no store at all by the other threads: a release fence waits for every store in flight)
+#define WV_TR(role, cond, step, i) do { \
+        const bool wv_on__ = (threadIdx.x == 0) && (cond) && (step) < kWvTraceSteps; \
+        unsigned long long *wv_dst__ = &g_wv_trace[role][wv_on__ ? (step) : 0][i]; \
+        const unsigned long long wv_t__ = wave_timer(); \
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.global.u64 [%0], %1;\n\t}\n" \
+                     :: "l"(wv_dst__), "l"(wv_t__), "r"((unsigned int)wv_on__) : "memory"); } while (0)
+#define WV_TRT(tt, role, cond, step, i) do { \
+        const bool wv_on__ = (threadIdx.x == (tt)) && (cond) && (step) < kWvTraceSteps; \
+        unsigned long long *wv_dst__ = &g_wv_trace[role][wv_on__ ? (step) : 0][i]; \
+        const unsigned long long wv_t__ = wave_timer(); \
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.global.u64 [%0], %1;\n\t}\n" \
+                     :: "l"(wv_dst__), "l"(wv_t__), "r"((unsigned int)wv_on__) : "memory"); } while (0)
+#else
+#define WV_TR(role, cond, step, i) do { } while (0)
+#define WV_TRT(tt, role, cond, step, i) do { } while (0)
+#endif
+
 }  // namespace dt

@@ -494,6 +494,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                 sIdx[lane] = sidx; sTok[lane] = tok;
             }
             __syncthreads();
+            WV_TR(0, cta == 0 && c0 == 0, t, 0);
 
             // source rows of this thread's ring pieces (column n < 32: hi of request n, else lo of request n - 32)
             const int my_sidx = sIdx[my_rq];
@@ -509,8 +510,29 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                     cp_async16(dst + kb * 8192 + my_dst_lo, src_lo + k0 + kb * 64);
                 }
             };
+            // A group of at most 16 requests needs N <= 32 columns: with the k-blocks packed N rows apart (not 64) all of K fits
+            // the ring, so every chunk is in flight at once and the MMAs go out in ONE burst behind one wait and one barrier
+            // instead of a wait / barrier / issue / refill round per chunk (same accumulators, same order: same bits)
+            const int kb_bytes = (ncol >> 3) * 1024, slot_b = (kTcKC / 64) * kb_bytes;
+            const bool burst = (size_t)n_kc * slot_b <= (size_t)kTcSlots * kTcSlotBytes && ncol < 64;
+            if (burst) {
+                if (my_rq < lo_off) {
 #pragma unroll 1
-            for (int kc = 0; kc < kTcSlots; ++kc) { if (kc < n_kc) issue_chunk(kc); cp_async_commit(); }
+                    for (int kc = 0; kc < n_kc; ++kc) {
+                        unsigned char *dst = sRing + (size_t)kc * slot_b;
+                        const size_t k0 = (size_t)kc * kTcKC;
+#pragma unroll
+                        for (int kb = 0; kb < kTcKC / 64; ++kb) {
+                            cp_async16(dst + kb * kb_bytes + my_dst_hi, src_hi + k0 + kb * 64);
+                            cp_async16(dst + kb * kb_bytes + my_dst_lo, src_lo + k0 + kb * 64);
+                        }
+                    }
+                }
+                cp_async_commit();
+            } else {
+#pragma unroll 1
+                for (int kc = 0; kc < kTcSlots; ++kc) { if (kc < n_kc) issue_chunk(kc); cp_async_commit(); }
+            }
 
             // epilogue operands (input half from P, previous state): issued now, consumed after the MMAs
             float pr[PP], pz[PP], pn[PP], hp[PP];
@@ -526,7 +548,25 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                 }
             }
 
+            WV_TR(0, cta == 0 && c0 == 0, t, 1);
             // hidden half: D1[64 x 64] = W_hh slice [64 x g] . [S_hi | S_lo]^T, K streamed through the ring
+            if (burst) {
+                cp_async_wait<0>();
+                tc::fence_proxy_async();
+                __syncthreads();
+                if (warp < kTcIssuers && lane == 0) {
+                    tc::fence_after_sync();
+#pragma unroll 1
+                    for (int kc = 0; kc < n_kc; ++kc) {
+                        const uint64_t da = descA0 + (uint64_t)((kc * (kTcKC / 64) + warp) * 64);
+                        const uint64_t db = descB0 + (uint64_t)((kc * slot_b + warp * kb_bytes) >> 4);
+#pragma unroll
+                        for (int s4 = 0; s4 < 4; ++s4)
+                            tc::mma_bf16(tmem + 64 * warp, da + (uint64_t)(s4 * 2), db + (uint64_t)(s4 * 2), idesc1, (kc | s4) ? 1u : 0u);
+                    }
+                    tc::commit(mb0 + 16);
+                }
+            } else
 #pragma unroll 1
             for (int kc = 0; kc < n_kc; ++kc) {
                 cp_async_wait<kTcSlots - 1>();
@@ -554,6 +594,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             cp_async_wait<0>();
             tc::mbar_wait(mb0 + 16, ph_d1); ph_d1 ^= 1u;
             tc::fence_after_sync();
+            WV_TR(0, cta == 0 && c0 == 0, t, 3);
             // TMEM -> shared: row m = 16 w + i sits in lane 32 w + i (i < 16) for an M = 64 accumulator
             __syncwarp();
             if (warp < 3) {
@@ -593,6 +634,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             }
             tc::fence_before_sync();
             __syncthreads();
+            WV_TR(0, cta == 0 && c0 == 0, t, 10);
             // gates (reading A2): rows ul, 16 + ul, 32 + ul are the r, z, n pre-activations of unit ul
 #pragma unroll
             for (int i = 0; i < PP; ++i) {
@@ -619,6 +661,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             }
             tc::fence_proxy_async();
             __syncthreads();
+            WV_TR(0, cta == 0 && c0 == 0, t, 11);
             // this CTA's split-K share of W1[:, d:] S_t: D2[r x 64] = W1 slice [r x 16] . [S_hi | S_lo]^T
             if (tid == 0) {
                 tc::fence_after_sync();
@@ -630,6 +673,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             tc::mbar_wait(mb0 + 24, ph_d2); ph_d2 ^= 1u;
             tc::fence_after_sync();
             __syncwarp();
+            WV_TR(0, cta == 0 && c0 == 0, t, 5);
             for (int mt = warp >> 2; mt < m2_tiles; mt += 2) {
                 float vh[32], vl[32];
                 const uint32_t ta = tmem + ((uint32_t)(32 * (warp & 3)) << 16) + 256 + 64 * mt;
@@ -645,7 +689,9 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             }
             tc::fence_before_sync();
             __syncthreads();
+            WV_TR(0, cta == 0 && c0 == 0, t, 6);
             if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride + c0 / p.gsz, fbase + (unsigned int)(t + 1)); }
+            WV_TR(0, cta == 0 && c0 == 0, t, 7);
         }
     }
     __syncthreads();
@@ -740,6 +786,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                 fused_spin([&] { return (int)(ld_relaxed_u32(p.flags + (size_t)q * kFusFlagStride + b / p.gsz) - (fbase + (unsigned int)(t + 1))) >= 0; }, p.err);
         }
         __syncthreads();
+        WV_TR(1, b == 0, t, 0);
         // the live frontier is entries 1 .. n_front of buffer `cur` (entry 0 was popped by the previous step)
         const unsigned int *oHi = fHi + cur * kFusMaxFront + 1;
         const unsigned long long *oLo = fLo + cur * kFusMaxFront + 1;
@@ -787,6 +834,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             }
             cp_async_wait<0>();
             __syncthreads();
+            WV_TR(1, b == 0, t, 1);
             // z_m = ((base_m - base_0) + W2[cand_m, :] a) / T_eff     PAPER.md:143-144 (shift-invariant)
             // four lanes per candidate row, interleaved 16-byte pieces
             const float base0 = sBase[0];
@@ -837,47 +885,55 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                 if (lane == 0) { sWst[2 * warp] = wmx; sWst[2 * warp + 1] = wsm; }
             }
             __syncthreads();
-            // ... then every thread merges the 8 warps' (max, sum) pairs in warp order
-            float zmax = -INFINITY;
+            WV_TR(1, b == 0, t, 2);
+            // ... then warp 0 merges the 8 warps' (max, sum) pairs in warp order and picks the top-k by (logp desc, token asc)
+            // = (z desc, token asc) without anything that scales with M * M: every lane takes the best of its own M / 32
+            // sortable keys (ord(z), ~token) and k rounds of a warp max reduction give L, the k-th best of the 32 lane maxima
+            // (lane in the low bits, so the 32 values are distinct): at least k keys lie at or above L, so the true top k do;
+            // the keys at or above L (k plus a few) go one to a lane and are ranked among themselves by counting over the
+            // full keys through shuffles.  The exact top k in the exact order; the k winners become the new entries
+            if (warp == 0) {
+                float zmax = -INFINITY;
 #pragma unroll
-            for (int w = 0; w < kFusWarps; ++w) zmax = fmaxf(zmax, sWst[2 * w]);
-            float ssum = 0.f;
+                for (int w = 0; w < kFusWarps; ++w) zmax = fmaxf(zmax, sWst[2 * w]);
+                float ssum = 0.f;
 #pragma unroll
-            for (int w = 0; w < kFusWarps; ++w) { const float mw = sWst[2 * w]; if (mw > -INFINITY) ssum += sWst[2 * w + 1] * expf(mw - zmax); }
-            const float lse = logf(ssum);
-            const float gpar = nSco[t];
-            // top-k by (logp desc, token asc): rank by counting on z (logp is a monotone map of z), `tpc` lanes per
-            // candidate (a power of two <= 8, lanes of one candidate are neighbours in a warp); the k winners become
-            // the new entries
-            {
-                int tpc = 1;
-                while (tpc < 8 && M * tpc * 2 <= kFusThreads) tpc <<= 1;
-                const int m = tid / tpc, part = tid - m * tpc;
-                const bool act = (m < M);
-                const float mz = act ? sZ[m] : 0.f;
-                const int mtok = act ? sTok[m] : 0;
-                int rank = 0;
-                if (act) {
-                    const int per = (M + tpc - 1) / tpc;
-                    const int m0 = part * per, m1 = min(M, m0 + per);
-                    int q = m0;
-                    if (!(per & 3)) {
-                        for (; q + 4 <= m1; q += 4) {
-                            const float4 oz = *reinterpret_cast<const float4 *>(sZ + q);
-                            const int4 ot = *reinterpret_cast<const int4 *>(sTok + q);
-                            rank += (oz.x > mz) || (oz.x == mz && ot.x < mtok);
-                            rank += (oz.y > mz) || (oz.y == mz && ot.y < mtok);
-                            rank += (oz.z > mz) || (oz.z == mz && ot.z < mtok);
-                            rank += (oz.w > mz) || (oz.w == mz && ot.w < mtok);
-                        }
-                    }
-                    for (; q < m1; ++q) {
-                        const float oz = sZ[q];
-                        rank += (oz > mz) || (oz == mz && sTok[q] < mtok);
-                    }
+                for (int w = 0; w < kFusWarps; ++w) { const float mw = sWst[2 * w]; if (mw > -INFINITY) ssum += sWst[2 * w + 1] * expf(mw - zmax); }
+                const float lse = logf(ssum);
+                const float gpar = nSco[t];
+                unsigned long long *svK = reinterpret_cast<unsigned long long *>(sP);   // the group sums are dead
+                const int MI = (M + 31) >> 5;
+                unsigned long long kk[8];
+                unsigned int hmax = 0u;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const int m = lane + 32 * i;
+                    kk[i] = 0ull;
+                    if (i < MI && m < M)
+                        kk[i] = ((unsigned long long)ord_key(sZ[m]) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned int)sTok[m]);
+                    hmax = max(hmax, (unsigned int)(kk[i] >> 32));
                 }
-                for (int o = 1; o < tpc; o <<= 1) rank += __shfl_xor_sync(0xffffffffu, rank, o);
-                if (act && part == 0 && rank < k) {
+                unsigned int cur_l = (hmax & ~31u) | (unsigned int)(31 - lane), Lh = 0u;
+#pragma unroll 1
+                for (int rr = 0; rr < k; ++rr) {
+                    Lh = __reduce_max_sync(0xffffffffu, cur_l);
+                    if (cur_l == Lh) cur_l = 0u;
+                }
+                Lh &= ~31u;
+                int ns = 0;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    if (i >= MI) break;
+                    const bool in = (unsigned int)(kk[i] >> 32) >= Lh && kk[i] != 0ull;
+                    const unsigned int bal = __ballot_sync(0xffffffffu, in);
+                    const int at = ns + __popc(bal & ((1u << lane) - 1u));
+                    if (in && at < 32) svK[at] = kk[i];
+                    ns += __popc(bal);
+                }
+                __syncwarp();
+                auto emit = [&](unsigned long long mk, int rank) {
+                    const float mz = ord_key_inv((unsigned int)(mk >> 32));
+                    const int mtok = (int)(0xFFFFFFFFu - (unsigned int)(mk & 0xFFFFFFFFull));
                     const float lpm = (mz - zmax) - lse;
                     nHi[rank] = ord_key(gpar + lpm);
                     nLo[rank] = ((unsigned long long)(0xFFFFFFFFu - (unsigned int)mtok) << 32) |
@@ -886,32 +942,63 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                         p.menu_tok[((size_t)b * L + depth) * k + rank] = mtok;
                         p.menu_lp[((size_t)b * L + depth) * k + rank] = lpm;
                     }
+                };
+                if (ns <= 32) {
+                    const unsigned long long mk = lane < ns ? svK[lane] : 0ull;
+                    int rank = 0;
+#pragma unroll 4
+                    for (int q = 0; q < ns; ++q) rank += (__shfl_sync(0xffffffffu, mk, q) > mk);
+                    if (lane < ns && rank < k) emit(mk, rank);
+                } else {                                        // many equal keys at the threshold: count over the slice
+#pragma unroll 1
+                    for (int m = lane; m < M; m += 32) {
+                        const unsigned long long mk = ((unsigned long long)ord_key(sZ[m]) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned int)sTok[m]);
+                        if ((unsigned int)(mk >> 32) < Lh) continue;
+                        int rank = 0;
+#pragma unroll 1
+                        for (int q = 0; q < M; ++q)
+                            rank += ((((unsigned long long)ord_key(sZ[q]) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned int)sTok[q])) > mk);
+                        if (rank < k) emit(mk, rank);
+                    }
                 }
+                __syncwarp();
             }
             n_new = k;
-            __syncthreads();
+            WV_TR(1, b == 0, t, 3);
         }
-        // The node popped now is the better of the old frontier head and the best new entry: thread 0 publishes its
-        // descriptor BEFORE the merge, so the GRU CTAs start step t+1 while this CTA is still merging.
+        // The node popped now is the better of the old frontier head and the best new entry: warp 0 publishes its descriptor
+        // BEFORE the merge (and before the CTA barrier that hands the new entries to the other warps), so the GRU CTAs start
+        // step t+1 while this CTA is still merging.
         const int cap = B - t;                                  // pops still to do, this one included
         int tot = n_front + n_new;
-        if (tid == 0) {
+        if (warp == 0) {
             if (tot > 0) {
-                unsigned int h = 0; unsigned long long l = 0ull; bool have = false;
-                if (n_front > 0) { h = oHi[0]; l = oLo[0]; have = true; }
-                for (int j = 0; j < n_new; ++j)
-                    if (!have || front_gt(nHi[j], nLo[j], h, l)) { h = nHi[j]; l = nLo[j]; have = true; }
-                const int tok = (int)(0xFFFFFFFFu - (unsigned int)(l >> 32));
-                const int par = (int)(0xFFFFFFFFu - (unsigned int)(l & 0xFFFFFFFFull));
-                const int dep = nDep[par] + 1;
-                if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(t + 2, rnd, dep < L ? par + 1 : -1, tok));
-                nTok[t + 1] = tok; nPar[t + 1] = par; nDep[t + 1] = dep; nSco[t + 1] = ord_key_inv(h);
-                sm.n_valid = t + 2; sm.n_front = p.static_mode ? 0 : min(tot, cap) - 1; sm.cur = cur ^ 1;
-            } else {
+                // best new entry: max of (hi, lo) over the k new entries (lo's low word, ~parent, is the same for all)
+                unsigned int h = 0u; unsigned long long l = 0ull; bool have = false;
+                if (n_new > 0) {
+                    const unsigned int mh = (lane < n_new) ? nHi[lane] : 0u;
+                    const unsigned long long ml = (lane < n_new) ? nLo[lane] : 0ull;
+                    h = __reduce_max_sync(0xffffffffu, mh);
+                    const unsigned int l_hi = __reduce_max_sync(0xffffffffu, (lane < n_new && mh == h) ? (unsigned int)(ml >> 32) : 0u);
+                    l = ((unsigned long long)l_hi << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned int)t);
+                    have = true;
+                }
+                if (lane == 0) {
+                    if (n_front > 0 && (!have || !front_gt(h, l, oHi[0], oLo[0]))) { h = oHi[0]; l = oLo[0]; }
+                    const int tok = (int)(0xFFFFFFFFu - (unsigned int)(l >> 32));
+                    const int par = (int)(0xFFFFFFFFu - (unsigned int)(l & 0xFFFFFFFFull));
+                    const int dep = nDep[par] + 1;
+                    if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(t + 2, rnd, dep < L ? par + 1 : -1, tok));
+                    nTok[t + 1] = tok; nPar[t + 1] = par; nDep[t + 1] = dep; nSco[t + 1] = ord_key_inv(h);
+                    sm.n_valid = t + 2; sm.n_front = p.static_mode ? 0 : min(tot, cap) - 1; sm.cur = cur ^ 1;
+                }
+            } else if (lane == 0) {
                 sm.n_front = 0;
                 if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(t + 2, rnd, -1, 0));
             }
         }
+        WV_TR(1, b == 0, t, 9);
+        __syncthreads();                                        // the new entries (and the pop) are visible to every warp
         // merge the new entries into the sorted frontier (other buffer), truncated to the pops that remain
         if (tot > 0) {
             if (tid < n_front) {
@@ -937,6 +1024,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             if (tot > cap) tot = cap;
         }
         __syncthreads();
+        WV_TR(1, b == 0, t, 4);
         // the popped node is entry 0 of the other buffer; the live frontier becomes its entries 1..tot-1
         int next_dep = L;                                       // depth of the node popped now (L = none / leaf)
         if (tot > 0) next_dep = nDep[t + 1];

@@ -100,33 +100,13 @@ __device__ __forceinline__ unsigned long long wave_citem_pack(int tok, int ps, i
            ((unsigned long long)b << 40) | ((unsigned long long)j << 47);
 }
 
-__device__ __forceinline__ unsigned long long wave_timer() {
-    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
-}
-// In-kernel timeline (measurement builds only: `python -m paper_2607_08642_b200.build --trace` compiles the separate
-// libdominotree_trace.so with -DDT_TRACE, read by `bench.py --trace`): thread 0 of GRU CTA 0 (role 0) and of request
-// CTA 0 (role 1) stamp %globaltimer at fixed points of the first kWvTraceSteps steps.
-constexpr int kWvTraceSteps = 64, kWvTraceStamps = 16;
-#ifdef DT_TRACE
-__device__ unsigned long long g_wv_trace[2][kWvTraceSteps][kWvTraceStamps];
-// one PREDICATED store by thread 0 (no branch: a thread-0-only branch would leave its warp diverged and slow every warp
-// collective after it; no store at all by the other threads: a release fence waits for every store in flight)
-#define WV_TR(role, cond, step, i) do { \
-        const bool wv_on__ = (threadIdx.x == 0) && (cond) && (step) < kWvTraceSteps; \
-        unsigned long long *wv_dst__ = &g_wv_trace[role][wv_on__ ? (step) : 0][i]; \
-        const unsigned long long wv_t__ = wave_timer(); \
-        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.global.u64 [%0], %1;\n\t}\n" \
-                     :: "l"(wv_dst__), "l"(wv_t__), "r"((unsigned int)wv_on__) : "memory"); } while (0)
-#else
-#define WV_TR(role, cond, step, i) do { } while (0)
-#endif
 constexpr unsigned long long kWvTimeoutNs = 4000000000ull;     // 4 s: far beyond any round; a slip fails instead of hanging
 
 // shared-memory footprints (bytes)
 __host__ __device__ inline size_t wave_gru_smem(int g, int r) {
     const size_t rpc = (size_t)16 * ((r + 16 * kWvCS - 1) / (16 * kWvCS));
     return (size_t)48 * g * 2 + (size_t)kWvRingBytes + (size_t)kWvCS * 4096 + (size_t)kWvCS * rpc * 32 +
-           (size_t)kWvMaxItems * 8 + (size_t)(2 * kWvMaxBatch + 8) * 4 + 24 * 8 + 64 + 1024;
+           (size_t)kWvMaxItems * 12 + (size_t)(2 * kWvMaxBatch + 8) * 4 + 24 * 8 + 64 + 1024;
 }
 __host__ __device__ inline size_t wave_slice_bytes(int r, int M) {
     return (size_t)((M + 7) / 8) * (size_t)((r + 63) / 64) * 1024;
@@ -215,6 +195,7 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
     unsigned long long *mbar = reinterpret_cast<unsigned long long *>(sCum + kWvMaxBatch + 8);   // [0..7] slot full, [8..15] slot empty, [16] D1, [17] D2, [18] first group of chunks full
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(mbar + 24);
     int *sCtl = reinterpret_cast<int *>(tmem_slot + 2);               // [2] abort
+    uint32_t *sOff = reinterpret_cast<uint32_t *>(sCtl + 8);          // [kWvMaxItems] parent state row of an item, in 16-byte pieces
 
     {   // resident weights
         const __nv_bfloat16 *whh = reinterpret_cast<const __nv_bfloat16 *>(e.w_hh);
@@ -359,6 +340,7 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                     const unsigned long long w = sRaw[b * kWvDescWords + lane];
                     const int tok = min((int)(w >> 44), e.V - 1), ps = (int)((w >> 34) & 0x3FFull);
                     sItems[off + lane] = wave_citem_pack(tok, ps, first + lane, b, lane);
+                    sOff[off + lane] = (uint32_t)(b * stride + ps) * (uint32_t)(g >> 3);
                 }
                 __syncwarp();
                 if (lane == 0) sCum[b] = first - 1 + cb;
@@ -385,7 +367,10 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
             float4 pr = make_float4(0.f, 0.f, 0.f, 0.f), pz4 = pr, pn = pr, hp = pr;
             const bool mine = (my_node < n);
             int my_new = 0, my_it = 0;
-            if (mine) {
+            // (the producer warps issue theirs after the operand copies: the copies head the pass's critical path and the
+            // load / store unit serves both in order)
+            auto load_mine = [&]() {
+                if (!mine) return;
                 const unsigned long long it = sItems[p0 + my_node];
                 const int tok = (int)(it & 0xFFFFFull), ps = (int)((it >> 20) & 0x3FFull), bq = (int)((it >> 40) & 0x7Full);
                 my_new = bq * stride + (int)((it >> 30) & 0x3FFull);
@@ -395,7 +380,8 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                 pz4 = __ldg(reinterpret_cast<const float4 *>(prow + g));
                 pn = __ldg(reinterpret_cast<const float4 *>(prow + 2 * g));
                 if (ps) hp = __ldcg(reinterpret_cast<const float4 *>(p.s32 + ((size_t)bq * stride + ps) * g + u0 + my_u));
-            }
+            };
+            if (warp < 4) load_mine();
             WV_TR(0, cta == 0 && p0 == 0, s, 2);
 
             // ---- D1[64 x N] = W_hh slice . [S_hi | S_lo]^T, K streamed through the ring by a warp-specialised pipeline
@@ -407,25 +393,29 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                 const int r7 = ptid >> 4;                            // rho & 7, the same for all rows of a thread
                 const uint32_t doff = tc::smem_u32(sRing) + (uint32_t)(kb * kb_bytes + r7 * 128 + ((pc ^ r7) << 4));
                 const int nfirst = min(nslot, n_kc), ngrp = N >> 3;
-                // source of this thread's piece of row group i (null: the row is not in use)
-                auto src_of = [&](int i) -> const __nv_bfloat16 * {
+                // source of this thread's piece of row group i, in 16-byte pieces from s_hi (kNoRow: the row is not in use).
+                // Branch-free (clamped index), so that the shared-memory loads of all row groups are in flight together
+                constexpr uint32_t kNoRow = 0xFFFFFFFFu;
+                const uint32_t lo_delta = (uint32_t)((p.s_lo - p.s_hi) >> 3);
+                auto off_of = [&](int i) -> uint32_t {
                     const int rho = r7 + 8 * i;
                     const int hl = (rho >= nh), node = rho - (hl ? nh : 0);
-                    if (node >= n) return nullptr;
-                    const unsigned long long it = sItems[p0 + node];
-                    const size_t row = (size_t)((unsigned int)(it >> 40) & 0x7Fu) * stride + (size_t)((unsigned int)(it >> 20) & 0x3FFu);
-                    return (hl ? p.s_lo : p.s_hi) + row * g + (size_t)piece * 8;
+                    const uint32_t o = sOff[p0 + min(node, n - 1)] + (uint32_t)piece + (hl ? lo_delta : 0u);
+                    return (node < n) ? o : kNoRow;
                 };
                 // A copy instruction occupies the LSU for ~14 cycles even with every lane predicated off, divisions and address
                 // conversions cost hundreds of cycles with one warp per scheduler: real (uniform) branches around unused row
                 // groups, no division, shared-space addresses.  The chunks that fit the ring at once go row group by row group
                 // and share ONE arrive-on-completion (it sits in the copy queue: later copies would wait behind it).
                 if (nfirst == n_kc) {
+                    uint32_t o_next = off_of(0);
 #pragma unroll 2
                     for (int i = 0; i < ngrp; ++i) {
-                        const __nv_bfloat16 *sp = src_of(i);
-                        if (__ballot_sync(0xffffffffu, sp != nullptr) == 0u) continue;     // nobody in the warp has this row group
-                        if (sp) {
+                        const uint32_t o = o_next;
+                        if (i + 1 < ngrp) o_next = off_of(i + 1);
+                        if (__ballot_sync(0xffffffffu, o != kNoRow) == 0u) continue;     // nobody in the warp has this row group
+                        if (o != kNoRow) {
+                            const __nv_bfloat16 *sp = p.s_hi + ((size_t)o << 3);
                             int kcs = kshift;
 #pragma unroll 4
                             for (int kc = 0; kc < nfirst; ++kc) {
@@ -438,9 +428,10 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                 } else {
                     // a large pass streams through the ring: chunk by chunk, a slot refilled once the MMAs of its previous chunk
                     // have read it (at least 7 of the 16 row groups are in use, so the sources live in registers)
-                    const __nv_bfloat16 *src[16];
+                    uint32_t so[16];
 #pragma unroll
-                    for (int i = 0; i < 16; ++i) src[i] = (i < ngrp) ? src_of(i) : nullptr;
+                    for (int i = 0; i < 16; ++i) so[i] = (i < ngrp) ? off_of(i) : kNoRow;
+                    WV_TRT(128, 0, cta == 0 && p0 == 0, s, 14);
                     int sl = 0, kcs = kshift;
 #pragma unroll 1
                     for (int kc = 0; kc < n_kc; ++kc) {
@@ -449,16 +440,17 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                             ph_empty ^= 1u << sl;
                         }
                         const uint32_t dst = doff + (uint32_t)(sl * slot_bytes);
-                        const size_t k0 = (size_t)kcs * kWvKC;
+                        const __nv_bfloat16 *base = p.s_hi + (size_t)kcs * kWvKC;
 #pragma unroll
                         for (int i = 0; i < 16; ++i)
-                            if (src[i]) wave_cp_async16_s(dst + i * 1024, src[i] + k0);
-                        if (kc == nfirst - 1) wave_cp_async_arrive(mbGrp);
+                            if (so[i] != kNoRow) wave_cp_async16_s(dst + i * 1024, base + ((size_t)so[i] << 3));
+                        if (kc == nfirst - 1) { wave_cp_async_arrive(mbGrp); WV_TRT(128, 0, cta == 0 && p0 == 0, s, 15); }
                         else if (kc >= nfirst) wave_cp_async_arrive(mbFull + 8 * sl);
                         if (++sl == nslot) sl = 0;
                         if (++kcs == n_kc) kcs = 0;
                     }
                 }
+                load_mine();
             } else if (lane == 0) {
                 // consumer: warp w issues K = 16 steps 2 w, 2 w + 1 of every chunk into its own accumulator D1[w].  MMAs are issued
                 // in bursts: every wait -> proxy fence -> issue round costs a few hundred ns, the MMAs themselves tens, so the
