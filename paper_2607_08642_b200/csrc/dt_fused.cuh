@@ -781,9 +781,13 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         // C = H W1h^T of the node's depth does not depend on the GRU CTAs: fetch it while waiting for them
         float cpre = 0.f;
         if (expand && tid < r) cpre = e.C[((size_t)b * L + depth) * r + tid];
-        if (warp == 0) {
-            for (int q = lane; q < p.n_gru; q += 32)
-                fused_spin([&] { return (int)(ld_relaxed_u32(p.flags + (size_t)q * kFusFlagStride + b / p.gsz) - (fbase + (unsigned int)(t + 1))) >= 0; }, p.err);
+        if (warp == 0) {                                        // a lane's flags are polled together: one L2 round trip, not one each
+            const unsigned int want = fbase + (unsigned int)(t + 1);
+            const unsigned int *fl = p.flags + b / p.gsz;
+            fused_spin([&] {
+                bool ok = true;
+                for (int q = lane; q < p.n_gru; q += 32) ok = ok & ((int)(ld_relaxed_u32(fl + (size_t)q * kFusFlagStride) - want) >= 0);
+                return ok; }, p.err);
         }
         __syncthreads();
         WV_TR(1, b == 0, t, 0);
