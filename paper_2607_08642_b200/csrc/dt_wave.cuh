@@ -303,13 +303,13 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
                 if (!dn && j < cnt) sRaw[b * kWvDescWords + j] = w;
             }
         }
-        if (s > 0 && warp == 7) {
+        if (s > 0 && warp >= 6) {
             // the parents' states were written by other GRU CTAs in earlier steps: acquire their `states visible` words (they
             // were set long ago: a request only nominates after it has seen the partials of that step)
             const unsigned int want = fbase + (unsigned int)s;
             const bool ok = wave_spin([&] {
                 bool all = true;
-                for (int q = lane; q < p.n_gru; q += 32)
+                for (int q = tid - 192; q < p.n_gru; q += 64)        // one flag per lane (acquire loads complete in order)
                     all = all && ((int)(wave_ld_acquire_u32(p.flags + (size_t)q * kFusFlagStride + grp) - want) >= 0);
                 return all; }, p.err);
             if (!ok) sCtl[2] = 1;
@@ -798,12 +798,13 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
         const bool act0 = pair0 < n_it * r4;
         float4 cv0 = make_float4(0.f, 0.f, 0.f, 0.f);
         if (act0 && !(tid & 1)) cv0 = __ldg(reinterpret_cast<const float4 *>(e.C + ((size_t)b * L + eDep[itE[j0]]) * r) + jq0);
-        if (warp == 0) {
-            // all of a lane's flags are polled in one round trip per iteration
+        if (warp < 2) {
+            // two warps, so that with up to 64 GRU CTAs a lane has ONE flag: acquire loads of one thread complete in order,
+            // a second flag per lane would cost a second round trip to L2
             const unsigned int want = fbase + (unsigned int)(s + 1);
             const bool ok = wave_spin([&] {
                 bool all = true;
-                for (int q = lane; q < p.n_gru; q += 32)
+                for (int q = tid; q < p.n_gru; q += 64)
                     all = all && ((int)(wave_ld_acquire_u32(p.flags + (size_t)q * kFusFlagStride + my_grp) - want) >= 0);
                 return all; }, p.err);
             if (!ok) ctl.abort_ = 1;
