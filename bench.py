@@ -626,7 +626,7 @@ def run_trace(args):
         torch.cuda.synchronize()
         assert lib.dt_trace_read(buf.ctypes.data) == 0
         t = buf.astype(np.int64)
-        steps = int((t[0, :, 0] > 0).sum())
+        steps = int((t[0, :S - 1, 0] > 0).sum())
         rows = {}
         g = t[0, 1:max(steps - 1, 2)]          # skip step 0 (weight load) and the last
         q = t[1, 1:max(steps - 1, 2)]
@@ -639,6 +639,15 @@ def run_trace(args):
         gn = t[0, 2:max(steps, 3)]
         ok = (gn[:, 0] > 0) & (q[:len(gn), 9] > 0)
         rows["hop: request published -> GRU sees headers"] = float(np.median((gn[:, 0] - q[:len(gn), 9])[ok])) if ok.any() else None
+        kt = t[:, S - 1, :]                      # kernel-level stamps: entry, loop begins, loop ends, (request CTA) emitted
+        def span(r0, i0, r1, i1):
+            return float(kt[r1, i1] - kt[r0, i0]) if kt[r1, i1] > 0 and kt[r0, i0] > 0 else None
+        rows["kernel: GRU CTA 0 entry -> weights resident, step loop begins"] = span(0, 0, 0, 1)
+        rows["kernel: request CTA 0 entry -> root staged, step loop begins"] = span(1, 0, 1, 1)
+        rows["kernel: GRU CTA 0 step loop"] = span(0, 1, 0, 2)
+        rows["kernel: request CTA 0 step loop"] = span(1, 1, 1, 2)
+        rows["kernel: request CTA 0 emitter (tokens .. mask)"] = span(1, 2, 1, 3)
+        rows["kernel: GRU CTA 0 entry -> request CTA 0 done"] = span(0, 0, 1, 3)
         period = np.diff(t[0, 1:steps, 0])
         rows["step period"] = float(np.median(period)) if len(period) else None
         rows["steps"] = steps

@@ -435,18 +435,31 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
     {
         const __nv_bfloat16 *whh = reinterpret_cast<const __nv_bfloat16 *>(e.w_hh);
         const int vpr = g / 8;
+        // as asynchronous copies, all in flight at once: the weights come from HBM every round (the select has streamed
+        // 150 MB through L2 since the last one) and a load -> store loop pays that latency once per iteration
         for (int i = tid; i < 48 * vpr; i += kFusThreads) {
             const int m = i / vpr, c = i - m * vpr;                // local row m = gate * 16 + ul, k-chunk c
             const int gate = m >> 4, ul = m & 15;
-            const uint4 q = ld_ro_v4(whh + ((size_t)gate * g + u0 + ul) * g + (size_t)c * 8);
-            *reinterpret_cast<uint4 *>(sA + (size_t)(m >> 3) * sboA + (size_t)(c >> 3) * 1024 + (m & 7) * 128 + (((c & 7) ^ (m & 7)) << 4)) = q;
+            cp_async16(sA + (size_t)(m >> 3) * sboA + (size_t)(c >> 3) * 1024 + (m & 7) * 128 + (((c & 7) ^ (m & 7)) << 4),
+                       whh + ((size_t)gate * g + u0 + ul) * g + (size_t)c * 8);
         }
         const __nv_bfloat16 *w1 = reinterpret_cast<const __nv_bfloat16 *>(e.w1);
-        for (int i = tid; i < m2_tiles * 128 * 16; i += kFusThreads) {
-            const int j = i >> 4, ul = i & 15;
-            const __nv_bfloat16 v = (j < r) ? w1[(size_t)j * (e.d + g) + e.d + u0 + ul] : __float2bfloat16_rn(0.f);
-            *reinterpret_cast<__nv_bfloat16 *>(sA2 + (size_t)(j >> 3) * 256 + (ul >> 3) * 128 + (j & 7) * 16 + (ul & 7) * 2) = v;
+        if (((e.d | g) & 7) == 0 && (reinterpret_cast<uintptr_t>(w1) & 15) == 0) {                                // 8 units = one aligned 16-byte piece of a W1 row
+            for (int i = tid; i < m2_tiles * 128 * 2; i += kFusThreads) {
+                const int j = i >> 1, uh = i & 1;
+                unsigned char *dst = sA2 + (size_t)(j >> 3) * 256 + uh * 128 + (j & 7) * 16;
+                if (j < r) cp_async16(dst, w1 + (size_t)j * (e.d + g) + e.d + u0 + 8 * uh);
+                else *reinterpret_cast<uint4 *>(dst) = make_uint4(0u, 0u, 0u, 0u);
+            }
+        } else {
+            for (int i = tid; i < m2_tiles * 128 * 16; i += kFusThreads) {
+                const int j = i >> 4, ul = i & 15;
+                const __nv_bfloat16 v = (j < r) ? w1[(size_t)j * (e.d + g) + e.d + u0 + ul] : __float2bfloat16_rn(0.f);
+                *reinterpret_cast<__nv_bfloat16 *>(sA2 + (size_t)(j >> 3) * 256 + (ul >> 3) * 128 + (j & 7) * 16 + (ul & 7) * 2) = v;
+            }
         }
+        cp_async_commit();
+        cp_async_wait<0>();
         if (tid == 0) {
             tc::mbar_init(tc::smem_u32(mbar + 0), kTcIssuers);      // slot free
             tc::mbar_init(tc::smem_u32(mbar + 1), kTcIssuers);
@@ -472,6 +485,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
     const int my_c = tid & 7, my_rq = tid >> 3;
 
     const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 8;   // this round's tag / flag base
+    WV_TR(0, cta == 0, kWvTraceSteps - 1, 1);
     for (int t = 0; t < e.B; ++t) {
         for (int c0 = 0; c0 < batch; c0 += p.gsz) {
             const int nb = min(p.gsz, batch - c0);
@@ -695,6 +709,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
         }
     }
     __syncthreads();
+    WV_TR(0, cta == 0, kWvTraceSteps - 1, 2);
     if (warp == 0) tc::tmem_free<kTcCols>(tmem);
     if (cta == 0 && tid == 0) st_relaxed_u32(p.round_ctr, rnd + 1u);      // every CTA read it long ago
 }
@@ -770,6 +785,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     __syncthreads();
     stage_depth(0);
 
+    WV_TR(1, b == 0, kWvTraceSteps - 1, 1);
     for (int t = 0; t < B; ++t) {
         const int n_valid = sm.n_valid;
         const int n_front = sm.n_front, cur = sm.cur;
@@ -1037,6 +1053,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     __syncthreads();
 
     if (p.static_mode) return;                                  // menus are out; dt_scorers.cuh builds and emits the tree
+    WV_TR(1, b == 0, kWvTraceSteps - 1, 2);
     // emitter (a9): dead-leaf padding (reading A10), positions, ancestor-or-self mask
     const int n = sm.n_valid;
     const int rpos = e.root_positions ? e.root_positions[b] : 0;
@@ -1059,12 +1076,15 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         int a = i;
         while (a >= 0) { mk[(size_t)i * N + a] = 1; a = nPar[a]; }
     }
+    WV_TR(1, b == 0, kWvTraceSteps - 1, 3);
 }
 
 template <int UPC>
 __global__ void __launch_bounds__(kFusThreads, 1) fused_expand_kernel(FusedParams p) {
     extern __shared__ __align__(1024) unsigned char fused_smem[];
     if (p.sched_sel && (unsigned int)(*p.sched_sel < p.sched_thr) != p.sched_want) return;   // the other schedule was chosen (grid-uniform)
+    WV_TR(0, blockIdx.x == 0, kWvTraceSteps - 1, 0);
+    WV_TR(1, (int)blockIdx.x == p.n_gru, kWvTraceSteps - 1, 0);
     if ((int)blockIdx.x < p.n_gru) {
         if constexpr (UPC == 0) fused_gru_role_tc(p, fused_smem);
         else fused_gru_role<UPC>(p, fused_smem);

@@ -200,20 +200,34 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
     {   // resident weights
         const __nv_bfloat16 *whh = reinterpret_cast<const __nv_bfloat16 *>(e.w_hh);
         const int vpr = g / 8;
+        // as asynchronous copies, all in flight at once: the weights come from HBM every round (the select has streamed
+        // 150 MB through L2 since the last one) and a load -> store loop pays that latency once per iteration
         for (int i = tid; i < 48 * vpr; i += kWvThreads) {
             const int m = i / vpr, c = i - m * vpr;                // local row m = gate * 16 + unit, 16-byte piece c
             const int gate = m >> 4, ul = m & 15;
-            const uint4 q = ld_ro_v4(whh + ((size_t)gate * g + u0 + ul) * g + (size_t)c * 8);
-            *reinterpret_cast<uint4 *>(sW + (size_t)(m >> 3) * sboW + (size_t)(c >> 3) * 1024 + (m & 7) * 128 + (((c & 7) ^ (m & 7)) << 4)) = q;
+            cp_async16(sW + (size_t)(m >> 3) * sboW + (size_t)(c >> 3) * 1024 + (m & 7) * 128 + (((c & 7) ^ (m & 7)) << 4),
+                       whh + ((size_t)gate * g + u0 + ul) * g + (size_t)c * 8);
         }
         // W1 rows [crank * rpc, crank * rpc + rpc) x the 16 units of every CTA of the cluster (one K = 16 step each)
         const __nv_bfloat16 *w1 = reinterpret_cast<const __nv_bfloat16 *>(e.w1);
-        for (int i = tid; i < kWvCS * rpc * 16; i += kWvThreads) {
-            const int c = i / (rpc * 16), rem = i - c * rpc * 16;
-            const int jl = rem >> 4, ul = rem & 15, j = crank * rpc + jl;
-            const __nv_bfloat16 v = (j < r) ? w1[(size_t)j * (e.d + g) + e.d + (cbase + c) * 16 + ul] : __float2bfloat16_rn(0.f);
-            *reinterpret_cast<__nv_bfloat16 *>(sW1 + (size_t)c * rpc * 32 + (size_t)(jl >> 3) * 256 + (ul >> 3) * 128 + (jl & 7) * 16 + (ul & 7) * 2) = v;
+        if ((e.d & 7) == 0 && (reinterpret_cast<uintptr_t>(w1) & 15) == 0) {                                      // 8 units = one aligned 16-byte piece of a W1 row (g % 128 == 0)
+            for (int i = tid; i < kWvCS * rpc * 2; i += kWvThreads) {
+                const int c = i / (rpc * 2), rem = i - c * rpc * 2;
+                const int jl = rem >> 1, uh = rem & 1, j = crank * rpc + jl;
+                unsigned char *dst = sW1 + (size_t)c * rpc * 32 + (size_t)(jl >> 3) * 256 + uh * 128 + (jl & 7) * 16;
+                if (j < r) cp_async16(dst, w1 + (size_t)j * (e.d + g) + e.d + (cbase + c) * 16 + 8 * uh);
+                else *reinterpret_cast<uint4 *>(dst) = make_uint4(0u, 0u, 0u, 0u);
+            }
+        } else {
+            for (int i = tid; i < kWvCS * rpc * 16; i += kWvThreads) {
+                const int c = i / (rpc * 16), rem = i - c * rpc * 16;
+                const int jl = rem >> 4, ul = rem & 15, j = crank * rpc + jl;
+                const __nv_bfloat16 v = (j < r) ? w1[(size_t)j * (e.d + g) + e.d + (cbase + c) * 16 + ul] : __float2bfloat16_rn(0.f);
+                *reinterpret_cast<__nv_bfloat16 *>(sW1 + (size_t)c * rpc * 32 + (size_t)(jl >> 3) * 256 + (ul >> 3) * 128 + (jl & 7) * 16 + (ul & 7) * 2) = v;
+            }
         }
+        cp_async_commit();
+        cp_async_wait<0>();
         for (int i = tid; i < kWvCS * 1024; i += kWvThreads) reinterpret_cast<uint32_t *>(sS2)[i] = 0u;
         for (int i = tid; i < kWvMaxBatch; i += kWvThreads) sCum[i] = 0;
         if (tid == 0) {
@@ -266,6 +280,7 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
     // nodes the GRU CTAs already run the other group's pass (a group's step still costs pass + hand-over + request role,
     // but two groups share that time).  Each group has its own step counter and its own flag word.
     const int G = p.n_groups, gsplit = (batch + G - 1) / G;
+    WV_TR(0, cta == 0, kWvTraceSteps - 1, 1);
     int sg[4] = {0, 0, 0, 0};
     bool glive[4] = {true, G > 1, G > 2, G > 3};
     for (int grp = 0; glive[0] || glive[1] || glive[2] || glive[3]; grp = (grp + 1 == G) ? 0 : grp + 1) {
@@ -620,6 +635,7 @@ __device__ __forceinline__ void wave_gru_role(const WaveParams &p, unsigned char
         sg[grp] = s + 1;
     }
     __syncthreads();
+    WV_TR(0, cta == 0, kWvTraceSteps - 1, 2);
     if (pend2) wave_cluster_wait();
     if (warp == 0) tc::tmem_free<kWvTmemCols>(tmem);
     // every CTA of the grid has read the counter: a request is done only after all GRU CTAs finished step 0
@@ -789,6 +805,7 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
     stage_slices();
     if (tid == 0) ctl.n_stage = 0;                               // every thread read the list before the barrier inside
 
+    WV_TR(1, b == 0, kWvTraceSteps - 1, 1);
     for (int s = 0;; ++s) {
         const int n_it = ctl.n_items;
         // the first round of the partial sums: who am I, where are my partials, and C = H W1h^T of the node's depth (A12: row =
@@ -1179,6 +1196,7 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
     }
     __syncthreads();
 
+    WV_TR(1, b == 0, kWvTraceSteps - 1, 2);
     // emitter (a9): slots in frontier order, dead-leaf padding (reading A10), positions, ancestor-or-self mask
     const int n = ctl.abort_ ? 1 : ctl.nG + 1;
     const unsigned long long *fK = gKey[ctl.cur];
@@ -1209,6 +1227,7 @@ __device__ __forceinline__ void wave_req_role(const WaveParams &p, unsigned char
         int a = i;
         while (a >= 0) { mk[(size_t)i * N + a] = 1; a = nPar[a]; }
     }
+    WV_TR(1, b == 0, kWvTraceSteps - 1, 3);
 }
 
 // Which schedule pays is a property of the round's candidate tables: bushy trees (flat slices) finish in a few wide
@@ -1234,6 +1253,8 @@ __global__ void __launch_bounds__(kWvThreads, 1) wave_expand_kernel(WaveParams p
         if (!p.run_peaked) return;                                  // the lock-step kernel takes it
         p.W = p.W_peaked;
     }
+    WV_TR(0, blockIdx.x == 0, kWvTraceSteps - 1, 0);
+    WV_TR(1, (int)blockIdx.x == p.n_gru, kWvTraceSteps - 1, 0);
     if ((int)blockIdx.x < p.n_gru) wave_gru_role(p, wave_smem);
     else if ((int)blockIdx.x - p.n_gru < p.e.batch) wave_req_role(p, wave_smem);   // CTAs padding the last cluster leave
 }
