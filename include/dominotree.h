@@ -44,7 +44,8 @@ typedef enum {
     DT_ERR_INVALID_ARG = -1, /* null pointer, shape/parameter out of range                       */
     DT_ERR_UNSUPPORTED = -2, /* shape beyond the compiled limits (see DT_MAX_*)                  */
     DT_ERR_CUDA = -3,        /* a CUDA runtime call failed (dt_last_cuda_error gives the code)   */
-    DT_ERR_ALLOC = -4        /* device or host allocation failed                                 */
+    DT_ERR_ALLOC = -4,       /* device or host allocation failed                                 */
+    DT_ERR_STATIC_LIMIT = -5 /* dt_select_topm_static: shape beyond its static scratch limits    */
 } dt_status;
 
 /* compiled limits */
@@ -116,6 +117,32 @@ int dt_build_trees(dt_handle *h, const void *marginal_logits, const void *backbo
  */
 int dt_select_topm(dt_handle *h, const void *logits, int32_t rows, int32_t M,
                    int32_t *cand_id, float *cand_val, void *stream);
+
+/*
+ * dt_select_topm_static: the same operation as dt_select_topm for callers that cannot
+ * allocate: no handle, no cudaMalloc / cudaFree, no allocating library call, nothing to free.  The scratch
+ * memory the select kernels need (per-row arrival tickets and thresholds, per-chunk partial lists) is ONE
+ * file-scope device array of the library, 8 KiB + DT_STATIC_PART_BYTES (2 MiB) per GPU, held from the moment
+ * the library is loaded on that GPU until exit.
+ *   logits  [rows, V] device, element type `dtype` (DT_BF16 or DT_F32), row-major, contiguous
+ *   cand_id [rows, M] int32 device, cand_val [rows, M] float device: outputs, caller-owned; same
+ *           order as dt_select_topm: (value desc, token id asc), -0 == +0
+ *   stream  a cudaStream_t (as void *) of the CURRENT device; the call only enqueues a memset node and one
+ *           kernel on it (asynchronous)
+ * Limits: rows <= DT_STATIC_MAX_ROWS (1024) and M <= DT_MAX_M, else DT_ERR_STATIC_LIMIT (nothing is
+ * enqueued); rows < 0, V < 1, M < 1, M > V, a bad dtype or a null pointer with rows > 0: DT_ERR_INVALID_ARG;
+ * rows == 0 is a no-op.  Sharing: every call on a GPU uses the same array, which keeps the previous call's
+ * contents (what must start at zero is cleared on `stream` in front of the kernel): calls on one stream are
+ * safe back to back, calls that OVERLAP on the GPU (two streams, concurrent graph replays) race and give
+ * wrong candidates.  The first call on a device resolves the array's device address and sets kernel
+ * attributes (once per device, that device current; thread-safe); dt_static_init() does that set-up for the
+ * current device ahead of time, e.g. before a stream capture.
+ */
+#define DT_STATIC_MAX_ROWS 1024
+#define DT_STATIC_PART_BYTES (2u << 20)
+int dt_static_init(void);
+int dt_select_topm_static(const void *logits, int32_t dtype, int32_t rows, int32_t V, int32_t M,
+                          int32_t *cand_id, float *cand_val, void *stream);
 
 /*
  * dt_build_trees_host: the same round with HOST buffers (pinned or pageable): copies the inputs

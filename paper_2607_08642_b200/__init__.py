@@ -17,7 +17,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libdominotree.so")
 
 DT_BF16, DT_F32 = 0, 1
-EXPORTS = ("dt_create", "dt_build_trees", "dt_select_topm", "dt_build_trees_host", "dt_commit_paths", "dt_tree_links", "dt_adaptive_budget", "dt_set_option", "dt_get_option",
+EXPORTS = ("dt_create", "dt_build_trees", "dt_select_topm", "dt_select_topm_static", "dt_static_init", "dt_build_trees_host", "dt_commit_paths", "dt_tree_links", "dt_adaptive_budget", "dt_set_option", "dt_get_option",
            "dt_kernel_launches", "dt_destroy", "dt_error_string", "dt_version", "dt_workspace_bytes",
            "dt_last_cuda_error", "dt_phase_timing", "dt_phase_slot", "dt_phase_elapsed_ms")
 PHASES = ("select", "precompute", "expand", "emit")
@@ -67,6 +67,10 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.dt_tree_links.argtypes = [vp, ctypes.POINTER(_Outputs), i32, i32, vp, vp, vp]
     lib.dt_tree_links.restype = ctypes.c_int
     lib.dt_select_topm.argtypes = [vp, vp, i32, i32, vp, vp, vp]
+    lib.dt_select_topm_static.argtypes = [vp, i32, i32, i32, i32, vp, vp, vp]
+    lib.dt_select_topm_static.restype = ctypes.c_int
+    lib.dt_static_init.argtypes = []
+    lib.dt_static_init.restype = ctypes.c_int
     lib.dt_select_topm.restype = ctypes.c_int
     lib.dt_set_option.argtypes = [vp, ctypes.c_char_p, i64]
     lib.dt_set_option.restype = ctypes.c_int
@@ -100,6 +104,30 @@ def _check(lib, rc: int, what: str, handle=None):
         msg = lib.dt_error_string(rc).decode()
         extra = f" (cudaError {lib.dt_last_cuda_error(handle)})" if handle and rc == -3 else ""
         raise DominoTreeError(f"{what} failed: {msg}{extra}")
+
+
+STATIC_MAX_ROWS = 1024          # DT_STATIC_MAX_ROWS of include/dominotree.h
+
+
+def select_topm_static(logits, M: int, ids, vals, stream=None):
+    """dt_select_topm_static: top-M select of [rows, V] (or [batch, L, V]) bf16 / fp32 device logits into the caller's
+    `ids` (int32 [rows, M]) and `vals` (float32 [rows, M]) without a handle and without any device allocation (the
+    scratch is a static device array of the library: rows <= 1024, M <= 256; calls that overlap on the GPU race)."""
+    import torch
+    lib = load_library()
+    lg = logits.reshape(-1, logits.shape[-1])
+    if not (lg.is_cuda and lg.is_contiguous()) or lg.dtype not in (torch.bfloat16, torch.float32):
+        raise DominoTreeError("select_topm_static: logits must be a contiguous CUDA tensor of bfloat16 or float32")
+    rows, V = lg.shape
+    for t, dt_ in ((ids, torch.int32), (vals, torch.float32)):
+        if not (t.is_cuda and t.is_contiguous()) or t.dtype != dt_ or tuple(t.shape) != (rows, M) or t.device != lg.device:
+            raise DominoTreeError(f"select_topm_static: outputs must be contiguous [{rows}, {M}] int32 / float32 on {lg.device}")
+    st = stream if stream is not None else torch.cuda.current_stream(lg.device)
+    with torch.cuda.device(lg.device):
+        rc = lib.dt_select_topm_static(lg.data_ptr(), DT_BF16 if lg.dtype == torch.bfloat16 else DT_F32, rows, V, M,
+                                       ids.data_ptr(), vals.data_ptr(), st.cuda_stream)
+    _check(lib, rc, "dt_select_topm_static")
+    return ids, vals
 
 
 @dataclass

@@ -163,6 +163,7 @@ extern "C" const char *dt_error_string(int code) {
         case DT_ERR_UNSUPPORTED: return "unsupported shape (beyond compiled limits)";
         case DT_ERR_CUDA: return "CUDA runtime error";
         case DT_ERR_ALLOC: return "allocation failed";
+        case DT_ERR_STATIC_LIMIT: return "shape beyond the static scratch limits (DT_STATIC_MAX_ROWS rows, DT_MAX_M candidates)";
         default: return "unknown error";
     }
 }
@@ -972,6 +973,111 @@ extern "C" int dt_build_trees_host(dt_handle *h, const void *logits_h, const voi
     DT_CUDA(h, cudaMemcpyAsync(oh->mask, od.mask, (size_t)batch * Nb * Nb, cudaMemcpyDeviceToHost, st));
     DT_CUDA(h, cudaMemcpyAsync(oh->n_nodes, od.n_nodes, (size_t)batch * 4, cudaMemcpyDeviceToHost, st));
     DT_CUDA(h, cudaStreamSynchronize(st));
+    return DT_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// dt_select_topm_static: the top-M select (a1) for callers that cannot allocate -- no handle, no cudaMalloc / cudaFree, no
+// allocating library call.  The select kernels need scratch (per-row arrival tickets and shared thresholds, per-chunk
+// partial lists when a row is split into chunks); here it lives in ONE file-scope device array that every GPU which
+// loads the library holds until exit: 8 KiB of tickets / thresholds + 2 MiB of partials.  Every call shares it and it
+// keeps the last call's contents: the tickets and thresholds are cleared on `stream` in front of every launch, the
+// partials are written before they are read.  Two calls that overlap on the GPU (different streams, or graphs replayed
+// concurrently) race on it.
+constexpr int kStaticMaxRows = DT_STATIC_MAX_ROWS;
+constexpr size_t kStaticPartKeys = (size_t)DT_STATIC_PART_BYTES / 8;
+constexpr size_t kStaticCtlWords = 2 * (size_t)kStaticMaxRows * 4 / 8;      // u64 words of the ticket + threshold arrays
+static __device__ __align__(256) unsigned long long g_static_scratch[kStaticCtlWords + kStaticPartKeys];
+
+namespace {
+struct StaticDev { bool tried = false; int rc = DT_OK; unsigned long long *scratch = nullptr; int sms = 0; bool bulk_ok = false; };
+constexpr int kStaticMaxDev = 64;
+StaticDev g_static_dev[kStaticMaxDev];
+std::mutex g_static_mu;
+
+// Once per device, with that device current: in host code `g_static_scratch` is a host-side stand-in, not a device
+// address; the kernel gets what cudaGetSymbolAddress returns for the current device.
+int static_setup(int dev, StaticDev **out) {
+    if (dev < 0 || dev >= kStaticMaxDev) return DT_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    StaticDev &d = g_static_dev[dev];
+    if (!d.tried) {
+        d.tried = true;
+        void *ptr = nullptr;
+        if (cudaGetSymbolAddress(&ptr, g_static_scratch) != cudaSuccess || !ptr ||
+            cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || d.sms < 1) {
+            cudaGetLastError();
+            d.rc = DT_ERR_CUDA;
+        } else {
+            d.scratch = reinterpret_cast<unsigned long long *>(ptr);
+            d.bulk_ok =
+                cudaFuncSetAttribute(select_topm_bulk_kernel<__nv_bfloat16, SelectSmemBig>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_bulk_dyn_smem<SelectSmemBig>()) == cudaSuccess &&
+                cudaFuncSetAttribute(select_topm_bulk_kernel<float, SelectSmemBig>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_bulk_dyn_smem<SelectSmemBig>()) == cudaSuccess;
+            if (!d.bulk_ok) cudaGetLastError();
+        }
+    }
+    *out = &d;
+    return d.rc;
+}
+}  // namespace
+
+extern "C" int dt_static_init(void) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return DT_ERR_CUDA; }
+    StaticDev *d = nullptr;
+    return static_setup(dev, &d);
+}
+
+extern "C" int dt_select_topm_static(const void *logits, int32_t dtype, int32_t rows, int32_t V, int32_t M,
+                                     int32_t *cand_id, float *cand_val, void *stream) {
+    if (dtype != DT_BF16 && dtype != DT_F32) return DT_ERR_INVALID_ARG;
+    if (rows < 0 || V < 1 || M < 1 || M > V) return DT_ERR_INVALID_ARG;
+    if (rows > kStaticMaxRows || M > DT_MAX_M) return DT_ERR_STATIC_LIMIT;
+    if (rows == 0) return DT_OK;
+    if (!logits || !cand_id || !cand_val) return DT_ERR_INVALID_ARG;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return DT_ERR_CUDA; }
+    StaticDev *d = nullptr;
+    int rc = static_setup(dev, &d);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int kvec = (dtype == DT_BF16) ? 8 : 4;
+    const bool aligned = (V % kvec == 0) && ((reinterpret_cast<uintptr_t>(logits) & 15u) == 0);
+    const bool bulk = aligned && d->bulk_ok;
+    SelectParams p;
+    p.logits = logits; p.rows = rows; p.V = V; p.M = M;
+    p.row_vecs = (V + kvec - 1) / kvec;
+    // chunks per row: enough CTAs to fill the GPU, chunks long enough to keep a CTA's warps busy, the merging CTA's
+    // buffer holds S * M keys, and all partial lists fit the static array (S = 1 needs none)
+    int S = (3 * d->sms + rows - 1) / rows;
+    const int by_len = p.row_vecs / 4096 < 1 ? 1 : p.row_vecs / 4096;
+    if (S > by_len) S = by_len;
+    if (S > SelectSmemBig::kCap / M) S = SelectSmemBig::kCap / M;
+    if (S > kSelMaxChunks) S = kSelMaxChunks;
+    while (S > 1 && (size_t)rows * S * M > kStaticPartKeys) --S;
+    if (S < 1) S = 1;
+    p.S = S;
+    p.chunk_vecs = (p.row_vecs + S - 1) / S;
+    if (bulk) p.chunk_vecs = (p.chunk_vecs + kSelTileVecs - 1) / kSelTileVecs * kSelTileVecs;
+    p.cand_id = cand_id; p.cand_val = cand_val;
+    p.row_counter = reinterpret_cast<unsigned int *>(d->scratch);
+    p.row_tau = p.row_counter + kStaticMaxRows;
+    p.part = d->scratch + kStaticCtlWords;
+    p.span = nullptr;
+    // the array keeps the previous call's contents: tickets and thresholds must start at zero
+    if (cudaMemsetAsync(d->scratch, 0, kStaticCtlWords * 8, st) != cudaSuccess) { cudaGetLastError(); return DT_ERR_CUDA; }
+    const dim3 grid(S, rows);
+    if (bulk) {
+        if (dtype == DT_BF16) select_topm_bulk_kernel<__nv_bfloat16, SelectSmemBig><<<grid, 256, sel_bulk_dyn_smem<SelectSmemBig>(), st>>>(p);
+        else select_topm_bulk_kernel<float, SelectSmemBig><<<grid, 256, sel_bulk_dyn_smem<SelectSmemBig>(), st>>>(p);
+    } else if (dtype == DT_BF16) {
+        if (aligned) select_topm_kernel<__nv_bfloat16, true><<<grid, kSelThreads, 0, st>>>(p);
+        else select_topm_kernel<__nv_bfloat16, false><<<grid, kSelThreads, 0, st>>>(p);
+    } else {
+        if (aligned) select_topm_kernel<float, true><<<grid, kSelThreads, 0, st>>>(p);
+        else select_topm_kernel<float, false><<<grid, kSelThreads, 0, st>>>(p);
+    }
+    if (cudaGetLastError() != cudaSuccess) return DT_ERR_CUDA;
     return DT_OK;
 }
 
