@@ -217,6 +217,11 @@ int dt_adaptive_budget(dt_handle *h, const dt_outputs *tree, int32_t batch, int3
  *   "expand_path"   0 auto, 1 per-step kernels, 2 / 3 lock-step kernel on mma.sync, 4 lock-step kernel on tcgen05,
  *                   5 wavefront kernel;
  *   "select_chunks", "select_kernel", "select_span", "precompute_gemm", "precompute_serial"   tuning / measurement
+ *   "lockstep_speculation"  lock-step kernel: the GRU CTAs run the pass of the node a chain would pop next while the
+ *                     request CTA still scores its parent.  1 (default): on the rounds the adaptive schedule sends to the
+ *                     lock-step kernel (peaked ones), one request group; 2: always (tcgen05 shapes, V <= 2^24); 0: never.
+ *                     Changes when a node's state is computed, never the result (bit-identical outputs).
+ *   "lockstep_group"  lock-step kernel: requests per GRU pass (0 = automatic)
  *                   switches of the kernels.
  * Batch sizes: any batch <= max_batch runs on the persistent kernels (bf16): a launch of the wavefront kernel holds up to
  * 64 requests beside the g / 16 GRU CTAs, larger batches run as consecutive launches inside the same call; the lock-step
@@ -228,6 +233,7 @@ int dt_set_option(dt_handle *h, const char *name, int64_t value);
  *   "expand_path_taken"  expansion path the last dt_build_trees enqueued: 1 per-step kernels, 2 / 3 lock-step fused kernel
  *                        on mma.sync, 4 lock-step fused kernel on tcgen05, 5 wavefront kernel (dt_wave.cuh), 6 adaptive
  *                        (both persistent kernels enqueued, the device lets one run);
+ *   "lockstep_speculation_used"  1 if the last lock-step launch speculated
  *   "schedule_chosen"    adaptive rounds: 1 if the last round's statistic said `flat` (wavefront kernel), else 0;
  *   "select_span_ns"     with "select_span" 1: device-side span of the last bulk select kernel (first CTA start to last
  *                        CTA end, %globaltimer);

@@ -60,6 +60,9 @@ struct dt_handle {
     // options / bookkeeping
     int64_t opt_sel_span;           // 1: the bulk select kernel records its device-side span (first CTA start .. last CTA end)
     unsigned long long *sel_span;
+    int64_t opt_fused_spec;         // lock-step kernel: speculative GRU pass along the chain (dt_fused.cuh)
+    int64_t spec_used;              // the last lock-step launch speculated
+    int64_t opt_fused_gsz;          // lock-step kernel: requests per group (0 = automatic)
     int64_t opt_gemm_serial;        // 1: the precompute GEMM runs after the select on the caller's stream (no overlap)
     int64_t opt_select_chunks;
     int64_t opt_select_kernel;      // 0 auto, 1 register-tile kernel only
@@ -211,6 +214,8 @@ extern "C" int dt_set_option(dt_handle *h, const char *name, int64_t value) {
     }
     if (!strcmp(name, "select_span")) { h->opt_sel_span = value; return DT_OK; }
     if (!strcmp(name, "precompute_serial")) { h->opt_gemm_serial = value; return DT_OK; }
+    if (!strcmp(name, "lockstep_speculation")) { if (value < 0 || value > 2) return DT_ERR_INVALID_ARG; h->opt_fused_spec = value; return DT_OK; }
+    if (!strcmp(name, "lockstep_group")) { if (value < 0 || value > kFusChunk) return DT_ERR_INVALID_ARG; h->opt_fused_gsz = value; return DT_OK; }
     if (!strcmp(name, "select_kernel")) {
         if (value < 0 || value > 1) return DT_ERR_INVALID_ARG;
         h->opt_select_kernel = value;
@@ -229,6 +234,7 @@ extern "C" int dt_get_option(dt_handle *h, const char *name, int64_t *value) {
     if (!h || !name || !value) return DT_ERR_INVALID_ARG;
     if (!strcmp(name, "expand_path_taken")) { *value = h->path_taken; return DT_OK; }
     if (!strcmp(name, "state_slots")) { *value = h->slot_stride; return DT_OK; }
+    if (!strcmp(name, "lockstep_speculation_used")) { *value = h->spec_used; return DT_OK; }
     const bool dev_word = !strcmp(name, "device_error") || !strcmp(name, "wave_steps") || !strcmp(name, "wave_expansions") ||
                           !strcmp(name, "schedule_chosen") || !strcmp(name, "select_span_ns");
     if (!dev_word) return DT_ERR_INVALID_ARG;
@@ -313,6 +319,7 @@ extern "C" int dt_create(dt_handle **out, const dt_weights *w, int32_t max_batch
     h->max_batch = max_batch; h->L = L; h->max_M = max_M; h->max_B = max_B; h->k = k;
     h->heap_cap = max_B * k + k;
     h->opt_adaptive = 1;
+    h->opt_fused_spec = 1;
     h->esize = (w->dtype == DT_BF16) ? 2 : 4;
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess ||
@@ -574,6 +581,20 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
     f.upc = upc; f.n_gru = p.g / upc; f.m_tiles = (3 * upc + 15) / 16;
     // two groups when the batch allows (ping-pong between the GRU CTAs and the request CTAs), at most kFusChunk requests each
     f.gsz = (p.batch <= 16) ? p.batch : ((p.batch + 1) / 2 < kFusChunk ? (p.batch + 1) / 2 : kFusChunk);
+    // Speculation along the chain (dt_fused.cuh): by default on the rounds the adaptive schedule sends here, i.e. peaked
+    // ones, where most pops are the marginal top-1 child of the node just expanded (a hit overlaps the GRU pass with the
+    // request CTA's scoring, a miss costs a second pass); option 2 forces it, 0 disables it.  tcgen05 role only (its
+    // n_gru = g / 16 leaves room for a second partial buffer in the workspace, sized for g / 8 CTAs); token ids must leave
+    // the descriptor's top byte to the depth.  One group of up to 32 requests then: a hit's period is one pass.
+    const bool want_spec = h->opt_fused_spec == 2 || (h->opt_fused_spec == 1 && sel >= 0 && !static_mode);
+    f.spec = (tcgen && want_spec && p.V <= (1 << 24)) ? 1 : 0;
+    if (f.spec) f.gsz = p.batch < kFusChunk ? p.batch : kFusChunk;
+    if (h->opt_fused_gsz > 0) f.gsz = (int)h->opt_fused_gsz < p.batch ? (int)h->opt_fused_gsz : p.batch;
+    // (several groups share the GRU CTAs: their passes queue up behind one another and the speculation only adds passes;
+    // measured at batch 40: 491 vs 461 us per peaked round)
+    if (f.spec && h->opt_fused_spec != 2 && p.batch > f.gsz) { f.spec = 0; f.gsz = (p.batch + 1) / 2 < kFusChunk ? (p.batch + 1) / 2 : kFusChunk; }
+    if ((p.batch + f.gsz - 1) / f.gsz > kFusMaxGroups) f.spec = 0;
+    f.partial_buf = (size_t)(p.g / 16) * h->max_batch * p.r;
     f.slot_stride = h->slot_stride;
     f.s_hi = h->s_hi; f.s_lo = h->s_lo; f.s32 = h->states; f.partial = h->partial; f.desc = h->desc; f.flags = h->flags; f.round_ctr = h->round_ctr;
     f.static_mode = static_mode ? 1 : 0; f.menu_tok = h->menu_tok; f.menu_lp = h->menu_lp; f.err = h->wv_err;
@@ -584,6 +605,7 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
     const size_t gs = tcgen ? fused_tc_smem(p.g, p.r) : fused_gru_smem(p.g, p.r, upc, f.m_tiles);
     const size_t dsm = gs > rs ? gs : rs;
     if (probe) return DT_OK;
+    h->spec_used = f.spec;
     if (sel >= 0) { f.sched_sel = h->sched_sel; f.sched_want = (unsigned int)sel; f.sched_thr = h->sched_thr; }
     int rc = m_begin ? phase_mark(h, 2, st) : DT_OK;
     if (rc) return rc;

@@ -69,6 +69,11 @@ struct FusedParams {
     // adaptive schedule (dt_api.cu): the kernel runs only when (*sched_sel < sched_thr) == sched_want (null: always)
     const unsigned int *sched_sel; unsigned int sched_want, sched_thr;
     unsigned int *err;             // device error word: a hand-over wait that times out raises it and gives up (no hang)
+    // speculation (tcgen05 GRU role only): while the request CTAs score node t the GRU CTAs already run the pass of the
+    // node a chain would pop next (parent = node t, token = the marginal top-1 of the next depth) into the other of two
+    // partial buffers; a request whose pop is that node continues on the `speculative pass done` flag
+    int spec;
+    size_t partial_buf;            // floats between the two partial buffers
     int32_t *menu_tok;             // [batch, L, k]
     float *menu_lp;                // [batch, L, k]
 };
@@ -125,6 +130,7 @@ __device__ __forceinline__ bool fused_desc_is(unsigned long long d, int epoch, u
     return (unsigned int)(d >> 44) == (((unsigned int)epoch << 8) | (tag & 0xFFu));
 }
 __device__ __forceinline__ int fused_desc_sidx(unsigned long long d) { return (int)((d >> 32) & 0xFFFu) - 1; }
+constexpr int kFusMaxGroups = 8;   // request groups the speculation keeps predictions for
 
 // No initialisation kernel: the hand-over words carry the handle's round counter (flags: round * 256 + steps done,
 // compared as a signed difference; descriptors: an 8-bit round tag), each request CTA publishes its own root
@@ -202,7 +208,7 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
     const int nblk = g / kFusKB;
     const int blk0 = warp * nblk / kFusWarps, blk1 = (warp + 1) * nblk / kFusWarps;
 
-    const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 8;   // this round's tag / flag base
+    const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 10;  // this round's tag / flag base
     for (int t = 0; t < e.B; ++t) {
         for (int c0 = 0; c0 < batch; c0 += p.gsz) {
             const int nb = min(p.gsz, batch - c0);
@@ -212,7 +218,7 @@ __device__ __forceinline__ void fused_gru_role(const FusedParams &p, unsigned ch
                 int sidx = -1, tok = 0;
                 if (lane < nb) {
                     unsigned long long dsc;
-                    fused_spin([&] { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride); return fused_desc_is(dsc, t + 1, rnd); }, p.err);
+                    fused_spin([&] { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride + (t & 1)); return fused_desc_is(dsc, t + 1, rnd); }, p.err);
                     sidx = fused_desc_sidx(dsc);
                     tok = (int)(dsc & 0xFFFFFFFFull);
                 }
@@ -405,7 +411,7 @@ __host__ __device__ inline size_t fused_tc_smem(int g, int r) {
     const size_t a2 = (size_t)((r + 127) / 128) * 128 * 32;           // W1[:, d + u0 ..] slice [r_pad x 16] bf16
     const size_t b2 = 64 * 32;                                        // new states [64 cols x 16] bf16
     const size_t sh = 48 * 34 * 4;                                    // hidden-half pre-activations
-    return a + ring + a2 + b2 + sh + 3 * kFusChunk * 4 + 8 * 8 + 64 + 1024;
+    return a + ring + a2 + b2 + sh + 3 * kFusChunk * 4 + 8 * 8 + 64 + (size_t)(4 * kFusMaxGroups * kFusChunk + 32) * 4 + 1024;
 }
 
 __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned char *smem_raw) {
@@ -430,6 +436,16 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
     int *sTok = sIdx + kFusChunk;
     unsigned long long *mbar = reinterpret_cast<unsigned long long *>(sTok + 2 * kFusChunk);   // [0],[1] slot free, [2] D1, [3] D2
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(mbar + 8);
+    // per request (speculation, see the pass loop): predicted parent slot (-1 none, -2 nothing speculated) and token of node rE,
+    // the node whose descriptor is expected next, and the state (0 = A: a speculation for rE may exist, its descriptor
+    // decides; 1 = B: the real node rE ran in the previous pass; 2 = finished)
+    int *sPredIdx = reinterpret_cast<int *>(tmem_slot + 16);                  // [groups][32]
+    int *sPredTok = sPredIdx + kFusMaxGroups * kFusChunk;
+    int *rE = sPredTok + kFusMaxGroups * kFusChunk;
+    int *rSt = rE + kFusMaxGroups * kFusChunk;
+    int *sCtl = rSt + kFusMaxGroups * kFusChunk;                              // [0] this pass has columns, [1] the group is finished
+    int *sNode = sTok + kFusChunk;                                            // [32] node of this pass's column
+    for (int i = tid; i < kFusMaxGroups * kFusChunk; i += kFusThreads) { sPredIdx[i] = -2; sPredTok[i] = 0; rE[i] = 0; rSt[i] = 0; }
 
     // resident weights in core-matrix layout
     {
@@ -484,11 +500,25 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
     // (hi and lo, both 64-wide k-blocks of the slot); a warp instruction moves 4 whole 128-byte rows
     const int my_c = tid & 7, my_rq = tid >> 3;
 
-    const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 8;   // this round's tag / flag base
+    const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 10;  // this round's tag / flag base
     WV_TR(0, cta == 0, kWvTraceSteps - 1, 1);
-    for (int t = 0; t < e.B; ++t) {
+    // Passes, not steps.  Pass k serves every request of a group with ONE column: the node its descriptor asks for, or --
+    // speculation -- the node a chain would pop next (parent = the node just confirmed, token = the marginal top-1 of the
+    // next depth), computed while the request CTA still scores that parent.  Per request, identically in every GRU CTA
+    // (the decisions depend on descriptor CONTENTS only, never on their timing) and mirrored by the request CTA:
+    //   state A (a speculation for node e may exist): wait for descriptor e; if it is the speculated node (or a leaf, which
+    //            needs no state) e is final: speculate e + 1 in this pass and stay in A; else run the real node e -> B;
+    //   state B (the real node e ran in the previous pass): speculate e + 1 in this pass -> A.
+    // A hit costs a request one pass per node (and the pass overlaps its scoring), a miss two.  Without p.spec every
+    // pass runs the real node k of every request (the plain lock-step schedule).  Flag of pass k: round base + k + 1.
+    const int n_grp = (batch + p.gsz - 1) / p.gsz;
+    unsigned int done_mask = 0u;
+    __syncthreads();
+    for (int t = 0; done_mask != (1u << n_grp) - 1u; ++t) {     // t = pass index
         for (int c0 = 0; c0 < batch; c0 += p.gsz) {
             const int nb = min(p.gsz, batch - c0);
+            const int gi = c0 / p.gsz;
+            if ((done_mask >> gi) & 1u) continue;
             // Columns of the hidden-half GEMM: requests' hi halves in rows [0, lo_off), lo halves in [lo_off, 2 lo_off);
             // N shrinks with the batch (8 columns serve up to 4 requests), and so do the ring traffic and the MMA time.
             const int ncol = (nb <= 4) ? 8 : (nb <= 8) ? 16 : (nb <= 16) ? 32 : 64;
@@ -497,17 +527,64 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             const int n_lo = lo_off + my_rq;
             const uint32_t my_dst_hi = (uint32_t)((my_rq >> 3) * 1024 + (my_rq & 7) * 128 + ((my_c ^ (my_rq & 7)) << 4));
             const uint32_t my_dst_lo = (uint32_t)((n_lo >> 3) * 1024 + (n_lo & 7) * 128 + ((my_c ^ (n_lo & 7)) << 4));
+            unsigned int *my_flag = p.flags + (size_t)cta * kFusFlagStride + gi;
             if (warp == 0) {
-                int sidx = -1, tok = 0;
+                int c_sidx = -1, c_tok = 0, c_node = 0;          // this pass's column of request c0 + lane (none: -1)
+                int st = 2, en = 0;
                 if (lane < nb) {
-                    unsigned long long dsc;
-                    fused_spin([&] { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride); return fused_desc_is(dsc, t + 1, rnd); }, p.err);
-                    sidx = fused_desc_sidx(dsc);
-                    tok = (int)(dsc & 0xFFFFFFFFull);
+                    const int ri = gi * kFusChunk + lane;
+                    st = rSt[ri]; en = rE[ri];
+                    int pi = sPredIdx[ri], pt = sPredTok[ri];
+                    bool advance = false;                        // node en is final: go on to en + 1 with a speculation
+                    if (st == 0) {
+                        unsigned long long dsc;
+                        fused_spin([&] { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride + (en & 1)); return fused_desc_is(dsc, en + 1, rnd); }, p.err);
+                        const int sidx = fused_desc_sidx(dsc);
+                        int tok = (int)(dsc & 0xFFFFFFFFull), dep = 0;
+                        if (p.spec) { dep = (int)((unsigned int)tok >> 24); tok &= 0xFFFFFF; }
+                        const bool hit = p.spec ? (sidx < 0 || (sidx == pi && tok == pt)) : (sidx < 0);
+                        if (!hit) { c_sidx = sidx; c_tok = tok; c_node = en; st = 1; }
+                        advance = hit || !p.spec;                // (without speculation there is no state B: next node, next pass)
+                        // what a chain pops after node en: its marginal top-1 child
+                        pi = -1; pt = 0;
+                        if (p.spec && sidx >= 0 && dep + 1 < e.L) { pi = en + 1; pt = __ldg(e.cand_id + ((size_t)(c0 + lane) * e.L + dep) * e.M); }
+                    } else if (st == 1) advance = true;
+                    if (advance) {
+                        en += 1;
+                        if (!p.spec) st = (en >= e.B) ? 2 : 0;
+                        else if (en >= e.B) st = 2;
+                        else {
+                            st = 0;
+                            if (pi >= 0) { c_sidx = pi; c_tok = pt; c_node = en; }
+                            else pi = -2;                            // nothing speculated for en: only a leaf descriptor is a hit
+                        }
+                    }
+                    rSt[ri] = st; rE[ri] = en; sPredIdx[ri] = pi; sPredTok[ri] = pt;
                 }
-                sIdx[lane] = sidx; sTok[lane] = tok;
+                sIdx[lane] = c_sidx; sTok[lane] = c_tok; sNode[lane] = c_node;
+                const unsigned int anyc = __ballot_sync(0xffffffffu, c_sidx >= 0);
+                const unsigned int live = __ballot_sync(0xffffffffu, lane < nb && st != 2);
+                if (lane == 0) { sCtl[0] = anyc != 0u; sCtl[1] = live == 0u; }
+                if (p.spec && anyc != 0u && t > 0) {
+                    // the parents' states were written by the other GRU CTAs, at the latest in the previous pass (without
+                    // speculation a descriptor is only published once its request has seen every flag of that pass)
+                    const unsigned int want = fbase + (unsigned int)t;
+                    fused_spin([&] {
+                        bool ok = true;
+                        for (int q = lane; q < p.n_gru; q += 32) ok = ok & ((int)(ld_relaxed_u32(p.flags + (size_t)q * kFusFlagStride + gi) - want) >= 0);
+                        return ok; }, p.err);
+                }
             }
             __syncthreads();
+            {
+                const bool anyc = sCtl[0] != 0, fin = sCtl[1] != 0;
+                if (fin) done_mask |= 1u << gi;
+                if (!anyc) {                                     // nothing to compute: the pass still counts
+                    if (tid == 0) st_relaxed_u32(my_flag, fbase + (unsigned int)(t + 1));
+                    __syncthreads();                             // sCtl is rewritten by the next poll
+                    continue;
+                }
+            }
             WV_TR(0, cta == 0 && c0 == 0, t, 0);
 
             // source rows of this thread's ring pieces (column n < 32: hi of request n, else lo of request n - 32)
@@ -663,7 +740,7 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                 const __nv_bfloat16 hi = __float2bfloat16_rn(hnew);
                 const __nv_bfloat16 lo = __float2bfloat16_rn(hnew - __bfloat162float(hi));
                 if (sIdx[bl] >= 0) {                             // publish S_t (slot t+1): fp32 and the bf16 hi/lo split
-                    const size_t o = ((size_t)(c0 + bl) * stride + (t + 1)) * g + u0 + ul;
+                    const size_t o = ((size_t)(c0 + bl) * stride + (sNode[bl] + 1)) * g + u0 + ul;
                     __stcg(p.s32 + o, hnew);
                     p.s_hi[o] = hi;
                     p.s_lo[o] = lo;
@@ -688,6 +765,8 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
             tc::fence_after_sync();
             __syncwarp();
             WV_TR(0, cta == 0 && c0 == 0, t, 5);
+            const unsigned int live = __ballot_sync(0xffffffffu, lane < nb && sIdx[lane] >= 0);   // requests of this pass
+            const unsigned int odd = __ballot_sync(0xffffffffu, p.spec && (sNode[lane] & 1));       // their partial buffer (node parity)
             for (int mt = warp >> 2; mt < m2_tiles; mt += 2) {
                 float vh[32], vl[32];
                 const uint32_t ta = tmem + ((uint32_t)(32 * (warp & 3)) << 16) + 256 + 64 * mt;
@@ -698,13 +777,13 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                     float *o = p.partial + ((size_t)cta * batch + c0) * r + j;
 #pragma unroll
                     for (int c = 0; c < 32; ++c)
-                        if (c < nb) __stcg(o + (size_t)c * r, vh[c] + vl[c]);
+                        if ((live >> c) & 1u) __stcg(o + (size_t)c * r + (((odd >> c) & 1u) ? p.partial_buf : 0), vh[c] + vl[c]);
                 }
             }
             tc::fence_before_sync();
             __syncthreads();
             WV_TR(0, cta == 0 && c0 == 0, t, 6);
-            if (tid == 0) { fence_release_gpu(); st_relaxed_u32(p.flags + (size_t)cta * kFusFlagStride + c0 / p.gsz, fbase + (unsigned int)(t + 1)); }
+            if (tid == 0) { fence_release_gpu(); st_relaxed_u32(my_flag, fbase + (unsigned int)(t + 1)); }
             WV_TR(0, cta == 0 && c0 == 0, t, 7);
         }
     }
@@ -722,6 +801,8 @@ __device__ __forceinline__ bool front_gt(unsigned int ah, unsigned long long al,
 }
 
 struct FusedReqSmem {
+    int kwait;          // GRU pass that produces the current node's partials (its flag is waited for)
+    int kspec;          // GRU pass that speculates on the next node (see fused_gru_role_tc)
     int n_valid;        // tree slots filled so far (root included)
     int n_front;        // live frontier entries
     int cur;            // which of the two frontier buffers is live
@@ -734,7 +815,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     const int b = blockIdx.x - p.n_gru;
     const int r = e.r, M = e.M, k = e.k, N = e.N, L = e.L, batch = e.batch, B = e.B;
     const int ldw2 = r + kFusW2Pad;
-    const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 8;   // this round's tag / flag base
+    const unsigned int rnd = ld_relaxed_u32(p.round_ctr), fbase = rnd << 10;  // this round's tag / flag base
 
     // carve, every array 16-byte aligned: [W2 rows bf16] [frontier lo u64 x2] [new lo] [frontier hi u32 x2]
     // [new hi] [a] [z] [base] [cand tok] [tree tok / par / dep / score]
@@ -780,7 +861,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         nTok[0] = e.root_tokens[b]; nPar[0] = -1; nDep[0] = 0; nSco[0] = 0.f;
         // step-0 descriptor: the root, whose parent state is the zero slot (reading A4)
         st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(1, rnd, 0, min(max(e.root_tokens[b], 0), e.V - 1)));
-        sm.n_valid = 1; sm.n_front = 0; sm.cur = 0;
+        sm.n_valid = 1; sm.n_front = 0; sm.cur = 0; sm.kwait = 0; sm.kspec = 1;
     }
     __syncthreads();
     stage_depth(0);
@@ -798,7 +879,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         float cpre = 0.f;
         if (expand && tid < r) cpre = e.C[((size_t)b * L + depth) * r + tid];
         if (warp == 0) {                                        // a lane's flags are polled together: one L2 round trip, not one each
-            const unsigned int want = fbase + (unsigned int)(t + 1);
+            const unsigned int want = fbase + (unsigned int)((p.spec ? sm.kwait : t) + 1);
             const unsigned int *fl = p.flags + b / p.gsz;
             fused_spin([&] {
                 bool ok = true;
@@ -824,7 +905,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                 const int jq = tid % r4, qg = tid / r4;
                 if (qg < G) {
                     const size_t ps4 = ((size_t)batch * r) >> 2;
-                    const float4 *pp = reinterpret_cast<const float4 *>(p.partial + (size_t)b * r) + jq;
+                    const float4 *pp = reinterpret_cast<const float4 *>(p.partial + (size_t)(p.spec ? (t & 1) : 0) * p.partial_buf + (size_t)b * r) + jq;
                     const int q0 = qg * per, q1 = min(p.n_gru, q0 + per);
                     float4 s0 = make_float4(0.f, 0.f, 0.f, 0.f), s1 = s0;
                     int q = q0;
@@ -1008,13 +1089,20 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                     const int tok = (int)(0xFFFFFFFFu - (unsigned int)(l >> 32));
                     const int par = (int)(0xFFFFFFFFu - (unsigned int)(l & 0xFFFFFFFFull));
                     const int dep = nDep[par] + 1;
-                    if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(t + 2, rnd, dep < L ? par + 1 : -1, tok));
+                    // (the descriptor of step s lives in word s & 1 of the request's line: with speculation this CTA may publish
+                    // step t + 1 before every GRU CTA has read step t; the depth rides in the token's top byte)
+                    if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + ((t + 1) & 1),
+                                                  fused_desc_pack(t + 2, rnd, dep < L ? par + 1 : -1, p.spec ? (tok | (min(dep, 255) << 24)) : tok));
+                    // the GRU CTAs' prediction for step t + 1: the marginal top-1 child of the node expanded now
+                    // a hit (or a leaf, which needs no state) is served by the speculating pass, a miss by the pass after it
+                    const bool hit = dep >= L || (expand && par == t && tok == sTok[0]);
+                    sm.kwait = sm.kspec + (hit ? 0 : 1); sm.kspec = sm.kwait + 1;
                     nTok[t + 1] = tok; nPar[t + 1] = par; nDep[t + 1] = dep; nSco[t + 1] = ord_key_inv(h);
                     sm.n_valid = t + 2; sm.n_front = p.static_mode ? 0 : min(tot, cap) - 1; sm.cur = cur ^ 1;
                 }
             } else if (lane == 0) {
-                sm.n_front = 0;
-                if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(t + 2, rnd, -1, 0));
+                sm.n_front = 0; sm.kwait = sm.kspec; sm.kspec = sm.kwait + 1;
+                if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + ((t + 1) & 1), fused_desc_pack(t + 2, rnd, -1, 0));
             }
         }
         WV_TR(1, b == 0, t, 9);
