@@ -218,8 +218,9 @@ int dt_adaptive_budget(dt_handle *h, const dt_outputs *tree, int32_t batch, int3
  *                   5 wavefront kernel;
  *   "select_chunks", "select_kernel", "select_span", "precompute_gemm", "precompute_serial"   tuning / measurement
  *   "lockstep_speculation"  lock-step kernel: the GRU CTAs run the pass of the node a chain would pop next while the
- *                     request CTA still scores its parent.  1 (default): on the rounds the adaptive schedule sends to the
- *                     lock-step kernel (peaked ones), one request group; 2: always (tcgen05 shapes, V <= 2^24); 0: never.
+ *                     request CTA still scores its parent (or the frontier entry the request CTA hints at).  1 (default):
+ *                     whenever the batch fits one request group (<= 32) on tcgen05 shapes with V <= 2^24, DominoTree
+ *                     scorer; 2: also with several groups and for the Cond-static arm; 0: never.
  *                     Changes when a node's state is computed, never the result (bit-identical outputs).
  *   "lockstep_group"  lock-step kernel: requests per GRU pass (0 = automatic)
  *                   switches of the kernels.

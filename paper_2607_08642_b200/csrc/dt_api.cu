@@ -586,7 +586,7 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
     // request CTA's scoring, a miss costs a second pass); option 2 forces it, 0 disables it.  tcgen05 role only (its
     // n_gru = g / 16 leaves room for a second partial buffer in the workspace, sized for g / 8 CTAs); token ids must leave
     // the descriptor's top byte to the depth.  One group of up to 32 requests then: a hit's period is one pass.
-    const bool want_spec = h->opt_fused_spec == 2 || (h->opt_fused_spec == 1 && sel >= 0 && !static_mode);
+    const bool want_spec = h->opt_fused_spec == 2 || (h->opt_fused_spec == 1 && !static_mode);
     f.spec = (tcgen && want_spec && p.V <= (1 << 24)) ? 1 : 0;
     if (f.spec) f.gsz = p.batch < kFusChunk ? p.batch : kFusChunk;
     if (h->opt_fused_gsz > 0) f.gsz = (int)h->opt_fused_gsz < p.batch ? (int)h->opt_fused_gsz : p.batch;
@@ -606,6 +606,7 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
     const size_t dsm = gs > rs ? gs : rs;
     if (probe) return DT_OK;
     h->spec_used = f.spec;
+    f.stats = h->wv_stats;                           // read back as "wave_steps" / "wave_expansions"
     if (sel >= 0) { f.sched_sel = h->sched_sel; f.sched_want = (unsigned int)sel; f.sched_thr = h->sched_thr; }
     int rc = m_begin ? phase_mark(h, 2, st) : DT_OK;
     if (rc) return rc;

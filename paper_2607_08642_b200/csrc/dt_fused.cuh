@@ -74,6 +74,7 @@ struct FusedParams {
     // partial buffers; a request whose pop is that node continues on the `speculative pass done` flag
     int spec;
     size_t partial_buf;            // floats between the two partial buffers
+    unsigned int *stats;           // optional (measurement aid): [0] GRU passes request 0 needed, [1] the most any request needed
     int32_t *menu_tok;             // [batch, L, k]
     float *menu_lp;                // [batch, L, k]
 };
@@ -537,17 +538,23 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                     int pi = sPredIdx[ri], pt = sPredTok[ri];
                     bool advance = false;                        // node en is final: go on to en + 1 with a speculation
                     if (st == 0) {
-                        unsigned long long dsc;
-                        fused_spin([&] { dsc = ld_relaxed_u64(p.desc + (size_t)(c0 + lane) * kFusDescStride + (en & 1)); return fused_desc_is(dsc, en + 1, rnd); }, p.err);
+                        unsigned long long dsc, hnt = 0ull;     // descriptor and (speculation) the request's hint, both self-validating
+                        const unsigned long long *dw = p.desc + (size_t)(c0 + lane) * kFusDescStride + (en & 1);
+                        fused_spin([&] {
+                            dsc = ld_relaxed_u64(dw);
+                            if (!p.spec) return fused_desc_is(dsc, en + 1, rnd);
+                            hnt = ld_relaxed_u64(dw + 2);
+                            return fused_desc_is(dsc, en + 1, rnd) && fused_desc_is(hnt, en + 1, rnd); }, p.err);
                         const int sidx = fused_desc_sidx(dsc);
                         int tok = (int)(dsc & 0xFFFFFFFFull), dep = 0;
                         if (p.spec) { dep = (int)((unsigned int)tok >> 24); tok &= 0xFFFFFF; }
                         const bool hit = p.spec ? (sidx < 0 || (sidx == pi && tok == pt)) : (sidx < 0);
                         if (!hit) { c_sidx = sidx; c_tok = tok; c_node = en; st = 1; }
                         advance = hit || !p.spec;                // (without speculation there is no state B: next node, next pass)
-                        // what a chain pops after node en: its marginal top-1 child
+                        // the node to speculate on after en: the request's hint, else what a chain pops, en's marginal top-1 child
                         pi = -1; pt = 0;
-                        if (p.spec && sidx >= 0 && dep + 1 < e.L) { pi = en + 1; pt = __ldg(e.cand_id + ((size_t)(c0 + lane) * e.L + dep) * e.M); }
+                        if (p.spec && fused_desc_sidx(hnt) >= 0) { pi = fused_desc_sidx(hnt); pt = (int)(hnt & 0xFFFFFFull); }
+                        else if (p.spec && sidx >= 0 && dep + 1 < e.L) { pi = en + 1; pt = __ldg(e.cand_id + ((size_t)(c0 + lane) * e.L + dep) * e.M); }
                     } else if (st == 1) advance = true;
                     if (advance) {
                         en += 1;
@@ -803,6 +810,7 @@ __device__ __forceinline__ bool front_gt(unsigned int ah, unsigned long long al,
 struct FusedReqSmem {
     int kwait;          // GRU pass that produces the current node's partials (its flag is waited for)
     int kspec;          // GRU pass that speculates on the next node (see fused_gru_role_tc)
+    int pred_sidx, pred_tok;   // the frontier entry hinted for the next node (parent slot, token); -1: none, the chain child
     int n_valid;        // tree slots filled so far (root included)
     int n_front;        // live frontier entries
     int cur;            // which of the two frontier buffers is live
@@ -810,6 +818,7 @@ struct FusedReqSmem {
 
 __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned char *smem_raw) {
     __shared__ FusedReqSmem sm;
+    __shared__ float sLp1[DT_MAX_L];                            // marginal log-probability of every depth's top-1 candidate (hints)
     const ExpandParams &e = p.e;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int b = blockIdx.x - p.n_gru;
@@ -857,11 +866,23 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         cp_async_commit();
     };
 
+    if (p.spec) {                                               // slice log-softmax of the base logits at position 0 (sorted: v_0 is the max)
+        for (int row = warp; row < L; row += kFusWarps) {
+            const float *v = e.cand_val + ((size_t)b * L + row) * M;
+            const float v0 = v[0];
+            float ssum = 0.f;
+            for (int m = lane; m < M; m += 32) ssum += __expf((v[m] - v0) / e.T_eff);
+            ssum = warp_sum(ssum);
+            if (lane == 0) sLp1[row] = -__logf(ssum);
+        }
+    }
     if (tid == 0) {
         nTok[0] = e.root_tokens[b]; nPar[0] = -1; nDep[0] = 0; nSco[0] = 0.f;
         // step-0 descriptor: the root, whose parent state is the zero slot (reading A4)
+        if (p.spec) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + 2, fused_desc_pack(1, rnd, -1, 0));     // no hint
         st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(1, rnd, 0, min(max(e.root_tokens[b], 0), e.V - 1)));
-        sm.n_valid = 1; sm.n_front = 0; sm.cur = 0; sm.kwait = 0; sm.kspec = 1;
+        sm.n_valid = 1; sm.n_front = 0; sm.cur = 0; sm.kwait = 0; sm.kspec = 1; sm.pred_sidx = -1; sm.pred_tok = 0;
+        if (p.stats && b == 0) p.stats[1] = 0u;
     }
     __syncthreads();
     stage_depth(0);
@@ -1085,24 +1106,57 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                     have = true;
                 }
                 if (lane == 0) {
-                    if (n_front > 0 && (!have || !front_gt(h, l, oHi[0], oLo[0]))) { h = oHi[0]; l = oLo[0]; }
+                    const unsigned int hn = h; const unsigned long long ln = l;      // best new entry
+                    const bool pop_old = n_front > 0 && (!have || !front_gt(h, l, oHi[0], oLo[0]));
+                    if (pop_old) { h = oHi[0]; l = oLo[0]; }
                     const int tok = (int)(0xFFFFFFFFu - (unsigned int)(l >> 32));
                     const int par = (int)(0xFFFFFFFFu - (unsigned int)(l & 0xFFFFFFFFull));
                     const int dep = nDep[par] + 1;
+                    // Hint for the GRU CTAs' speculation on the node AFTER this one.  Default: this node's marginal top-1 child (a
+                    // chain).  But if the best entry left in the frontier beats the score that child can be expected to have
+                    // (this node's score + the marginal log-probability of the next depth's top-1), or this node is a leaf, the
+                    // frontier entry is the better guess.  Only a guess: a hit is decided by comparing with the real pop.
+                    int h_sidx = -1, h_tok = 0;
+                    if (p.spec && !p.static_mode && t + 2 < B) {
+                        unsigned int h2 = 0u; unsigned long long l2 = 0ull; bool have2 = false;
+                        if (pop_old) {
+                            if (n_front > 1) { h2 = oHi[1]; l2 = oLo[1]; have2 = true; }
+                            if (have && (!have2 || front_gt(hn, ln, h2, l2))) { h2 = hn; l2 = ln; have2 = true; }
+                        } else {
+                            if (n_front > 0) { h2 = oHi[0]; l2 = oLo[0]; have2 = true; }
+                            if (n_new > 1 && (!have2 || front_gt(nHi[1], nLo[1], h2, l2))) { h2 = nHi[1]; l2 = nLo[1]; have2 = true; }   // (ranked)
+                        }
+                        if (have2) {
+                            const int par2 = (int)(0xFFFFFFFFu - (unsigned int)(l2 & 0xFFFFFFFFull));
+                            const int dep2 = nDep[par2] + 1;
+                            if (dep2 < L && (dep >= L || ord_key_inv(h2) > ord_key_inv(h) + sLp1[dep])) {
+                                h_sidx = par2 + 1; h_tok = (int)(0xFFFFFFFFu - (unsigned int)(l2 >> 32));
+                            }
+                        }
+                    }
                     // (the descriptor of step s lives in word s & 1 of the request's line: with speculation this CTA may publish
                     // step t + 1 before every GRU CTA has read step t; the depth rides in the token's top byte)
-                    if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + ((t + 1) & 1),
-                                                  fused_desc_pack(t + 2, rnd, dep < L ? par + 1 : -1, p.spec ? (tok | (min(dep, 255) << 24)) : tok));
-                    // the GRU CTAs' prediction for step t + 1: the marginal top-1 child of the node expanded now
-                    // a hit (or a leaf, which needs no state) is served by the speculating pass, a miss by the pass after it
-                    const bool hit = dep >= L || (expand && par == t && tok == sTok[0]);
+                    if (t + 1 < B) {
+                        if (p.spec) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + 2 + ((t + 1) & 1), fused_desc_pack(t + 2, rnd, h_sidx, h_tok));
+                        st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + ((t + 1) & 1),
+                                       fused_desc_pack(t + 2, rnd, dep < L ? par + 1 : -1, p.spec ? (tok | (min(dep, 255) << 24)) : tok));
+                    }
+                    // What the GRU CTAs speculated for THIS node (told a step ago): the hinted frontier entry, else the marginal
+                    // top-1 child of the node expanded now.  A hit (or a leaf, which needs no state) is served by the
+                    // speculating pass, a miss by the pass after it
+                    const bool hit = dep >= L || (sm.pred_sidx >= 0 ? (par + 1 == sm.pred_sidx && tok == sm.pred_tok)
+                                                                    : (expand && par == t && tok == sTok[0]));
                     sm.kwait = sm.kspec + (hit ? 0 : 1); sm.kspec = sm.kwait + 1;
+                    sm.pred_sidx = h_sidx; sm.pred_tok = h_tok;
                     nTok[t + 1] = tok; nPar[t + 1] = par; nDep[t + 1] = dep; nSco[t + 1] = ord_key_inv(h);
                     sm.n_valid = t + 2; sm.n_front = p.static_mode ? 0 : min(tot, cap) - 1; sm.cur = cur ^ 1;
                 }
             } else if (lane == 0) {
-                sm.n_front = 0; sm.kwait = sm.kspec; sm.kspec = sm.kwait + 1;
-                if (t + 1 < B) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + ((t + 1) & 1), fused_desc_pack(t + 2, rnd, -1, 0));
+                sm.n_front = 0; sm.kwait = sm.kspec; sm.kspec = sm.kwait + 1; sm.pred_sidx = -1;
+                if (t + 1 < B) {
+                    if (p.spec) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + 2 + ((t + 1) & 1), fused_desc_pack(t + 2, rnd, -1, 0));
+                    st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + ((t + 1) & 1), fused_desc_pack(t + 2, rnd, -1, 0));
+                }
             }
         }
         WV_TR(1, b == 0, t, 9);
@@ -1140,6 +1194,11 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     }
     __syncthreads();
 
+    if (p.stats && tid == 0) {
+        const unsigned int np = (unsigned int)((p.spec ? sm.kwait : B - 1) + 1);
+        if (b == 0) p.stats[0] = np;
+        atomicMax(p.stats + 1, np);
+    }
     if (p.static_mode) return;                                  // menus are out; dt_scorers.cuh builds and emits the tree
     WV_TR(1, b == 0, kWvTraceSteps - 1, 2);
     // emitter (a9): dead-leaf padding (reading A10), positions, ancestor-or-self mask
