@@ -604,6 +604,10 @@ def run_trace(args):
     builder.set_option("expand_path", args.trace_path)   # the timeline of ONE kernel, whatever the adaptive schedule would pick
     if not fused:
         builder.set_option("wave_groups", 1)      # one request group: GRU step i and request step i are the same step
+    else:
+        # speculation (the default) makes GRU pass i and request step i different things: the plain chain (one pass per
+        # step, two request groups) unless --trace-spec; with it only the per-role segments and the periods are meaningful
+        builder.set_option("lockstep_speculation", 2 if args.trace_spec else 0)
     gru_stamps, req_stamps = (FUSED_GRU_STAMPS, FUSED_REQ_STAMPS) if fused else (GRU_STAMPS, REQ_STAMPS)
     if args.wave_width:
         builder.set_option("wave_width", args.wave_width)
@@ -612,7 +616,7 @@ def run_trace(args):
     lib.dt_trace_read.restype = ctypes.c_int
     S, K = 64, 16
     buf = np.zeros((2, S, K), dtype=np.uint64)
-    out = {"workload": cfg.name, "batch": batch, "kernel": "fused_expand_kernel<0> (lock-step, two request groups)" if fused else "wave_expand_kernel (one request group)",
+    out = {"workload": cfg.name, "batch": batch, "kernel": ("fused_expand_kernel<0> (lock-step, speculation, one request group)" if args.trace_spec else "fused_expand_kernel<0> (lock-step, no speculation, two request groups)") if fused else "wave_expand_kernel (one request group)",
            "wave_width": args.wave_width or "auto", "unit": "ns (median over steps)"}
     for regime in ("flat", "peaked"):
         inp = wl.make_inputs(cfg, batch=batch, regime=regime)
@@ -636,9 +640,23 @@ def run_trace(args):
                 rows[f"{role}: {name}"] = float(np.median((arr[:, i1] - arr[:, i0])[ok])) if ok.any() else None
         ok = (q[:, 0] > 0) & (g[:, 7] > 0)
         rows["hop: flag released -> request sees flags"] = float(np.median((q[:, 0] - g[:, 7])[ok])) if ok.any() else None
+        spec_on = fused and args.trace_spec
+        if spec_on:
+            rows["hop: flag released -> request sees flags"] = None
         gn = t[0, 2:max(steps, 3)]
         ok = (gn[:, 0] > 0) & (q[:len(gn), 9] > 0)
-        rows["hop: request published -> GRU sees headers"] = float(np.median((gn[:, 0] - q[:len(gn), 9])[ok])) if ok.any() else None
+        rows["hop: request published -> GRU sees headers"] = float(np.median((gn[:, 0] - q[:len(gn), 9])[ok])) if ok.any() and not spec_on else None
+        if spec_on:
+            rq = t[1, 1:min(cfg.B, S - 1), 0]
+            rq = rq[rq > 0]
+            rows["request step period"] = float(np.median(np.diff(rq))) if len(rq) > 1 else None
+            rows["gru_passes_request0"] = builder.get_option("wave_steps")
+            t00 = int(t[0, 0, 0])                                  # absolute timeline of the first passes / steps (ns)
+            rows["timeline_gru_pass_begins"] = [int(x - t00) for x in t[0, :14, 0] if x > 0]
+            rows["timeline_gru_flag_stored"] = [int(x - t00) for x in t[0, :14, 7] if x > 0]
+            rows["timeline_req_flags_seen"] = [int(x - t00) for x in t[1, :14, 0] if x > 0]
+            rows["timeline_req_published"] = [int(x - t00) for x in t[1, :14, 9] if x > 0]
+            rows["gru_passes_max"] = builder.get_option("wave_expansions")
         kt = t[:, S - 1, :]                      # kernel-level stamps: entry, loop begins, loop ends, (request CTA) emitted
         def span(r0, i0, r1, i1):
             return float(kt[r1, i1] - kt[r0, i0]) if kt[r1, i1] > 0 and kt[r0, i0] > 0 else None
@@ -669,6 +687,7 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="also time the batch-1 B x M sweep and the three scorer arms")
     ap.add_argument("--trace", action="store_true", help="in-kernel timeline of the wavefront kernel (measurement build, not a bench value)")
     ap.add_argument("--trace-batch", type=int, default=0, help="batch of the --trace leg (default: the workload's)")
+    ap.add_argument("--trace-spec", action="store_true", help="--trace --trace-path 4 with the speculation on (one request group)")
     ap.add_argument("--trace-path", type=int, default=5, choices=(4, 5), help="kernel of the --trace leg: 5 = wavefront (default), 4 = lock-step fused")
     ap.add_argument("--wave-width", type=int, default=0, help="nodes a request may expand per step (0 = auto)")
     args = ap.parse_args()
@@ -715,8 +734,9 @@ def main():
                    "traffic": None, "algorithmic_flops": exp_flops, "us_per_round": ph["expand"],
                    "share_of_step": ph["expand"] / ctx["phase_round_us"], "schedule": ctx["schedule"],
                    "us_per_round_by_regime_p50": ctx["dist_us"]["by_regime_p50"],
-                   "note": "a chain of dependent GRU -> correction -> pop steps (32 lock-step steps, or ~9 wavefront steps of "
-                           "~4 nodes per request): latency-bound; 92 % of the flops run as bf16 hi/lo pairs on tcgen05"}
+                   "note": "a chain of dependent GRU -> correction -> pop steps (lock-step: ~34 GRU passes for 32 nodes, the pass of "
+                           "the likely next node speculated while its parent is scored; wavefront: ~9 steps of ~4 nodes per "
+                           "request): latency-bound; 92 % of the flops run as bf16 hi/lo pairs on tcgen05"}
     dominant = roof_expand if ph["expand"] > sel_us else roof_select
 
     line = {

@@ -546,15 +546,15 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                             hnt = ld_relaxed_u64(dw + 2);
                             return fused_desc_is(dsc, en + 1, rnd) && fused_desc_is(hnt, en + 1, rnd); }, p.err);
                         const int sidx = fused_desc_sidx(dsc);
-                        int tok = (int)(dsc & 0xFFFFFFFFull), dep = 0;
-                        if (p.spec) { dep = (int)((unsigned int)tok >> 24); tok &= 0xFFFFFF; }
+                        int tok = (int)(dsc & 0xFFFFFFFFull);
+                        if (p.spec) tok &= 0xFFFFFF;
                         const bool hit = p.spec ? (sidx < 0 || (sidx == pi && tok == pt)) : (sidx < 0);
                         if (!hit) { c_sidx = sidx; c_tok = tok; c_node = en; st = 1; }
                         advance = hit || !p.spec;                // (without speculation there is no state B: next node, next pass)
-                        // the node to speculate on after en: the request's hint, else what a chain pops, en's marginal top-1 child
+                        // the node to speculate on after en: the request CTA's hint (en's marginal top-1 child -- a chain -- or the
+                        // best entry left in its frontier)
                         pi = -1; pt = 0;
                         if (p.spec && fused_desc_sidx(hnt) >= 0) { pi = fused_desc_sidx(hnt); pt = (int)(hnt & 0xFFFFFFull); }
-                        else if (p.spec && sidx >= 0 && dep + 1 < e.L) { pi = en + 1; pt = __ldg(e.cand_id + ((size_t)(c0 + lane) * e.L + dep) * e.M); }
                     } else if (st == 1) advance = true;
                     if (advance) {
                         en += 1;
@@ -572,15 +572,15 @@ __device__ __forceinline__ void fused_gru_role_tc(const FusedParams &p, unsigned
                 const unsigned int anyc = __ballot_sync(0xffffffffu, c_sidx >= 0);
                 const unsigned int live = __ballot_sync(0xffffffffu, lane < nb && st != 2);
                 if (lane == 0) { sCtl[0] = anyc != 0u; sCtl[1] = live == 0u; }
-                if (p.spec && anyc != 0u && t > 0) {
-                    // the parents' states were written by the other GRU CTAs, at the latest in the previous pass (without
-                    // speculation a descriptor is only published once its request has seen every flag of that pass)
-                    const unsigned int want = fbase + (unsigned int)t;
-                    fused_spin([&] {
-                        bool ok = true;
-                        for (int q = lane; q < p.n_gru; q += 32) ok = ok & ((int)(ld_relaxed_u32(p.flags + (size_t)q * kFusFlagStride + gi) - want) >= 0);
-                        return ok; }, p.err);
-                }
+            } else if (warp == 1 && p.spec && t > 0) {
+                // meanwhile: the parents' states were written by the other GRU CTAs, at the latest in the previous pass (every
+                // CTA flags every pass, so this never waits for long; without speculation a descriptor is only published once
+                // its request has seen every flag of that pass)
+                const unsigned int want = fbase + (unsigned int)t;
+                fused_spin([&] {
+                    bool ok = true;
+                    for (int q = lane; q < p.n_gru; q += 32) ok = ok & ((int)(ld_relaxed_u32(p.flags + (size_t)q * kFusFlagStride + gi) - want) >= 0);
+                    return ok; }, p.err);
             }
             __syncthreads();
             {
@@ -819,6 +819,7 @@ struct FusedReqSmem {
 __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned char *smem_raw) {
     __shared__ FusedReqSmem sm;
     __shared__ float sLp1[DT_MAX_L];                            // marginal log-probability of every depth's top-1 candidate (hints)
+    __shared__ int sTop1[DT_MAX_L];                             // and its token
     const ExpandParams &e = p.e;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int b = blockIdx.x - p.n_gru;
@@ -849,11 +850,38 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     const __nv_bfloat16 *w2 = reinterpret_cast<const __nv_bfloat16 *>(e.w2);
 
     // stage the candidate table of depth `dep` (row b*L + dep): ids, base logits, the M rows of W2
-    auto stage_depth = [&](int dep) {
+    // wait for the GRU CTAs' flags of pass `kpass` (warp 0; a lane's flags are polled together: one L2 round trip, not one each)
+    auto wait_flags = [&](int kpass) {
+        const unsigned int want = fbase + (unsigned int)(kpass + 1);
+        const unsigned int *fl = p.flags + b / p.gsz;
+        fused_spin([&] {
+            bool ok = true;
+            for (int q = lane; q < p.n_gru; q += 32) ok = ok & ((int)(ld_relaxed_u32(fl + (size_t)q * kFusFlagStride) - want) >= 0);
+            return ok; }, p.err);
+    };
+    // `kpass` >= 0: warp 0 also looks ONCE at the next step's flags here, under the latency of the candidate loads (with
+    // speculation they are usually set already, but even a successful poll is a round trip to L2); returns whether they
+    // were all there (warp 0; else the loop top waits for them, after the staging has been issued)
+    auto stage_depth = [&](int dep, int kpass) -> bool {
         const size_t row = (size_t)b * L + dep;
-        for (int m = tid; m < M; m += kFusThreads) {
-            sTok[m] = e.cand_id[row * M + m];
-            sBase[m] = e.cand_val[row * M + m];
+        int ctok[(DT_MAX_M + kFusThreads - 1) / kFusThreads];
+        float cval[(DT_MAX_M + kFusThreads - 1) / kFusThreads];
+#pragma unroll
+        for (int i = 0; i < (DT_MAX_M + kFusThreads - 1) / kFusThreads; ++i) {
+            const int m = tid + i * kFusThreads;
+            if (m < M) { ctok[i] = e.cand_id[row * M + m]; cval[i] = e.cand_val[row * M + m]; }
+        }
+        bool seen = false;
+        if (warp == 0 && kpass >= 0) {
+            const unsigned int want = fbase + (unsigned int)(kpass + 1);
+            bool ok = true;
+            for (int q = lane; q < p.n_gru; q += 32) ok = ok & ((int)(ld_relaxed_u32(p.flags + b / p.gsz + (size_t)q * kFusFlagStride) - want) >= 0);
+            seen = __all_sync(0xffffffffu, ok);
+        }
+#pragma unroll
+        for (int i = 0; i < (DT_MAX_M + kFusThreads - 1) / kFusThreads; ++i) {
+            const int m = tid + i * kFusThreads;
+            if (m < M) { sTok[m] = ctok[i]; sBase[m] = cval[i]; }
         }
         __syncthreads();
         if (p.w2_smem) {
@@ -864,6 +892,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             }
         }
         cp_async_commit();
+        return seen;
     };
 
     if (p.spec) {                                               // slice log-softmax of the base logits at position 0 (sorted: v_0 is the max)
@@ -873,19 +902,22 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             float ssum = 0.f;
             for (int m = lane; m < M; m += 32) ssum += __expf((v[m] - v0) / e.T_eff);
             ssum = warp_sum(ssum);
-            if (lane == 0) sLp1[row] = -__logf(ssum);
+            if (lane == 0) { sLp1[row] = -__logf(ssum); sTop1[row] = e.cand_id[((size_t)b * L + row) * M]; }
         }
+        __syncthreads();
     }
     if (tid == 0) {
         nTok[0] = e.root_tokens[b]; nPar[0] = -1; nDep[0] = 0; nSco[0] = 0.f;
         // step-0 descriptor: the root, whose parent state is the zero slot (reading A4)
-        if (p.spec) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + 2, fused_desc_pack(1, rnd, -1, 0));     // no hint
+        if (p.spec) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + 2,                   // hint for node 1: the root's top-1 child
+                                   fused_desc_pack(1, rnd, (1 < L && 1 < B) ? 1 : -1, sTop1[0]));
         st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(1, rnd, 0, min(max(e.root_tokens[b], 0), e.V - 1)));
-        sm.n_valid = 1; sm.n_front = 0; sm.cur = 0; sm.kwait = 0; sm.kspec = 1; sm.pred_sidx = -1; sm.pred_tok = 0;
+        sm.n_valid = 1; sm.n_front = 0; sm.cur = 0; sm.kwait = 0; sm.kspec = 1; sm.pred_sidx = (p.spec && 1 < L && 1 < B) ? 1 : -1; sm.pred_tok = sTop1[0];
         if (p.stats && b == 0) p.stats[1] = 0u;
     }
     __syncthreads();
-    stage_depth(0);
+    stage_depth(0, -1);
+    bool polled = false;                                        // the flags of the coming step were seen while staging
 
     WV_TR(1, b == 0, kWvTraceSteps - 1, 1);
     for (int t = 0; t < B; ++t) {
@@ -899,14 +931,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         // C = H W1h^T of the node's depth does not depend on the GRU CTAs: fetch it while waiting for them
         float cpre = 0.f;
         if (expand && tid < r) cpre = e.C[((size_t)b * L + depth) * r + tid];
-        if (warp == 0) {                                        // a lane's flags are polled together: one L2 round trip, not one each
-            const unsigned int want = fbase + (unsigned int)((p.spec ? sm.kwait : t) + 1);
-            const unsigned int *fl = p.flags + b / p.gsz;
-            fused_spin([&] {
-                bool ok = true;
-                for (int q = lane; q < p.n_gru; q += 32) ok = ok & ((int)(ld_relaxed_u32(fl + (size_t)q * kFusFlagStride) - want) >= 0);
-                return ok; }, p.err);
-        }
+        if (warp == 0 && !polled) wait_flags(p.spec ? sm.kwait : t);
         __syncthreads();
         WV_TR(1, b == 0, t, 0);
         // the live frontier is entries 1 .. n_front of buffer `cur` (entry 0 was popped by the previous step)
@@ -1117,6 +1142,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                     // (this node's score + the marginal log-probability of the next depth's top-1), or this node is a leaf, the
                     // frontier entry is the better guess.  Only a guess: a hit is decided by comparing with the real pop.
                     int h_sidx = -1, h_tok = 0;
+                    if (p.spec && t + 2 < B && dep + 1 < L) { h_sidx = t + 2; h_tok = sTop1[dep]; }     // the chain: slot of node t + 1
                     if (p.spec && !p.static_mode && t + 2 < B) {
                         unsigned int h2 = 0u; unsigned long long l2 = 0ull; bool have2 = false;
                         if (pop_old) {
@@ -1144,8 +1170,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                     // What the GRU CTAs speculated for THIS node (told a step ago): the hinted frontier entry, else the marginal
                     // top-1 child of the node expanded now.  A hit (or a leaf, which needs no state) is served by the
                     // speculating pass, a miss by the pass after it
-                    const bool hit = dep >= L || (sm.pred_sidx >= 0 ? (par + 1 == sm.pred_sidx && tok == sm.pred_tok)
-                                                                    : (expand && par == t && tok == sTok[0]));
+                    const bool hit = dep >= L || (sm.pred_sidx >= 0 && par + 1 == sm.pred_sidx && tok == sm.pred_tok);
                     sm.kwait = sm.kspec + (hit ? 0 : 1); sm.kspec = sm.kwait + 1;
                     sm.pred_sidx = h_sidx; sm.pred_tok = h_tok;
                     nTok[t + 1] = tok; nPar[t + 1] = par; nDep[t + 1] = dep; nSco[t + 1] = ord_key_inv(h);
@@ -1190,7 +1215,8 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         // the popped node is entry 0 of the other buffer; the live frontier becomes its entries 1..tot-1
         int next_dep = L;                                       // depth of the node popped now (L = none / leaf)
         if (tot > 0) next_dep = nDep[t + 1];
-        if (t + 1 < B && next_dep < L) stage_depth(next_dep);   // overlaps the GRU CTAs' step t+1
+        polled = false;
+        if (t + 1 < B && next_dep < L) polled = stage_depth(next_dep, p.spec ? sm.kwait : -1);   // overlaps the GRU CTAs' step t+1
     }
     __syncthreads();
 
