@@ -731,7 +731,9 @@ def main():
                    "peak_source": "148 SMs x 128 fp32 FMA lanes x 2 x sm_max_mhz (DESIGN.md)",
                    "frac_of_bf16_tensor_peak": exp_tflops / peaks["bf16_tflops"],
                    "bf16_tensor_peak": peaks["bf16_tflops"],
-                   "traffic": None, "algorithmic_flops": exp_flops, "us_per_round": ph["expand"],
+                   "traffic": 30.6e6, "traffic_source": "profiles/r2_fused_ncu.md (ncu --set full of the lock-step kernel on a peaked round: "
+                                                        "dram read 30.0 MB + write 0.6 MB; the wavefront kernel cannot be replayed by ncu)",
+                   "algorithmic_flops": exp_flops, "us_per_round": ph["expand"],
                    "share_of_step": ph["expand"] / ctx["phase_round_us"], "schedule": ctx["schedule"],
                    "us_per_round_by_regime_p50": ctx["dist_us"]["by_regime_p50"],
                    "note": "a chain of dependent GRU -> correction -> pop steps (lock-step: ~34 GRU passes for 32 nodes, the pass of "
