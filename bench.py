@@ -582,7 +582,7 @@ FUSED_GRU_STAMPS = ((0, "descriptors seen + CTA barrier"), (1, "state copies, P 
                     (10, "TMEM -> shared + CTA barrier"), (11, "gates, state stores, W1 operand + CTA barrier"), (5, "D2 issued and complete"),
                     (6, "partials stored + CTA barrier"), (7, "gpu fence + flag store"))
 FUSED_REQ_STAMPS = ((0, "flags seen"), (1, "a = SiLU(C + partials)"), (2, "W2 slice dots + online softmax statistics"), (3, "top-k + CTA barrier"),
-                    (9, "pop: next descriptor published (thread 0)"), (4, "merge + CTA barrier"))
+                    (9, "pop: next descriptor published (thread 0)"), (4, "CTA barrier, then warp 0: next flags seen (warps 1-7 merge + stage meanwhile)"))
 
 
 def run_trace(args):

@@ -1186,37 +1186,55 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         }
         WV_TR(1, b == 0, t, 9);
         __syncthreads();                                        // the new entries (and the pop) are visible to every warp
-        // merge the new entries into the sorted frontier (other buffer), truncated to the pops that remain
-        if (tot > 0) {
-            if (tid < n_front) {
-                const unsigned int h = oHi[tid]; const unsigned long long l = oLo[tid];
-                int c = 0;
-                for (int j = 0; j < n_new; ++j) c += front_gt(nHi[j], nLo[j], h, l);
-                const int pos = tid + c;
-                if (pos < cap) { wHi[pos] = h; wLo[pos] = l; }
-            }
-            if (tid >= kFusThreads - n_new) {                   // the last n_new threads place the new entries
-                const int j = tid - (kFusThreads - n_new);
-                const unsigned int h = nHi[j]; const unsigned long long l = nLo[j];
-                int c = 0;
-                for (int j2 = 0; j2 < n_new; ++j2) c += front_gt(nHi[j2], nLo[j2], h, l);
-                int lo = 0, hi = n_front;                        // first old entry that does not beat (h, l)
-                while (lo < hi) {
-                    const int mid = (lo + hi) >> 1;
-                    if (front_gt(oHi[mid], oLo[mid], h, l)) lo = mid + 1; else hi = mid;
-                }
-                const int pos = lo + c;
-                if (pos < cap) { wHi[pos] = h; wLo[pos] = l; }
-            }
-            if (tot > cap) tot = cap;
-        }
-        __syncthreads();
-        WV_TR(1, b == 0, t, 4);
-        // the popped node is entry 0 of the other buffer; the live frontier becomes its entries 1..tot-1
+        // Between two steps: warp 0 waits for the flags of the pass the NEXT node needs (with speculation they are usually there,
+        // but even a successful poll is a round trip to L2) while warps 1..7 merge the new entries into the sorted frontier
+        // (other buffer, truncated to the pops that remain) and stage the next depth's candidate rows; they meet at the
+        // barrier on top of the loop.
         int next_dep = L;                                       // depth of the node popped now (L = none / leaf)
         if (tot > 0) next_dep = nDep[t + 1];
         polled = false;
-        if (t + 1 < B && next_dep < L) polled = stage_depth(next_dep, p.spec ? sm.kwait : -1);   // overlaps the GRU CTAs' step t+1
+        if (warp == 0) {
+            if (t + 1 < B) { wait_flags(p.spec ? sm.kwait : t + 1); polled = true; }
+            WV_TR(1, b == 0, t, 4);
+        } else {
+            constexpr int nw = kFusThreads - 32;
+            const int wt = tid - 32;
+            if (tot > 0) {
+                for (int i = wt; i < n_front; i += nw) {
+                    const unsigned int h = oHi[i]; const unsigned long long l = oLo[i];
+                    int c = 0;
+                    for (int j = 0; j < n_new; ++j) c += front_gt(nHi[j], nLo[j], h, l);
+                    const int pos = i + c;
+                    if (pos < cap) { wHi[pos] = h; wLo[pos] = l; }
+                }
+                if (wt >= nw - n_new) {                         // the last n_new threads place the new entries
+                    const int j = wt - (nw - n_new);
+                    const unsigned int h = nHi[j]; const unsigned long long l = nLo[j];
+                    int c = 0;
+                    for (int j2 = 0; j2 < n_new; ++j2) c += front_gt(nHi[j2], nLo[j2], h, l);
+                    int lo = 0, hi = n_front;                    // first old entry that does not beat (h, l)
+                    while (lo < hi) {
+                        const int mid = (lo + hi) >> 1;
+                        if (front_gt(oHi[mid], oLo[mid], h, l)) lo = mid + 1; else hi = mid;
+                    }
+                    const int pos = lo + c;
+                    if (pos < cap) { wHi[pos] = h; wLo[pos] = l; }
+                }
+            }
+            if (t + 1 < B && next_dep < L) {                    // overlaps the GRU CTAs' next pass
+                const size_t row = (size_t)b * L + next_dep;
+                for (int m = wt; m < M; m += nw) { sTok[m] = e.cand_id[row * M + m]; sBase[m] = e.cand_val[row * M + m]; }
+                asm volatile("bar.sync 1, %0;" ::"n"(nw) : "memory");     // warps 1..7 only
+                if (p.w2_smem) {
+                    const int vpr = r / 8;
+                    for (int i = wt; i < M * vpr; i += nw) {
+                        const int m = i / vpr, v = i - m * vpr;
+                        cp_async16(sW2 + (size_t)m * ldw2 + v * 8, w2 + (size_t)sTok[m] * r + (size_t)v * 8);
+                    }
+                }
+                cp_async_commit();
+            }
+        }
     }
     __syncthreads();
 
