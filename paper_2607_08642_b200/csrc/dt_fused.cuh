@@ -149,8 +149,8 @@ __host__ __device__ inline size_t fused_gru_smem(int g, int r, int upc, int m_ti
 __host__ __device__ inline size_t fused_req_smem(int r, int M, int N, int k, int w2_smem) {
     auto al = [](size_t x) { return (x + 15) / 16 * 16; };
     size_t s = al((size_t)2 * kFusMaxFront * 8) + al((size_t)k * 8) + al((size_t)M * 8) + al((size_t)2 * kFusMaxFront * 4) +
-               al((size_t)k * 4) + 9 * al((size_t)r * 4) + 3 * al((size_t)M * 4) + 4 * al((size_t)N * 4);
-    if (w2_smem) s += al((size_t)M * (r + kFusW2Pad) * 2);
+               al((size_t)k * 4) + 9 * al((size_t)r * 4) + al((size_t)M * 4) + 2 * al((size_t)2 * M * 4) + 4 * al((size_t)N * 4);
+    if (w2_smem) s += al((size_t)2 * M * (r + kFusW2Pad) * 2);      // two staging buffers (current depth, prefetched depth)
     return s + 16 + 64;
 }
 
@@ -831,7 +831,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     // [new hi] [a] [z] [base] [cand tok] [tree tok / par / dep / score]
     size_t off = 0;
     auto carve = [&](size_t bytes) { unsigned char *q = smem_raw + off; off += (bytes + 15) / 16 * 16; return q; };
-    __nv_bfloat16 *sW2 = reinterpret_cast<__nv_bfloat16 *>(carve(p.w2_smem ? (size_t)M * ldw2 * 2 : 0));
+    __nv_bfloat16 *sW2_ = reinterpret_cast<__nv_bfloat16 *>(carve(p.w2_smem ? (size_t)2 * M * ldw2 * 2 : 0));   // [2 buffers][M rows]
     unsigned long long *fLo = reinterpret_cast<unsigned long long *>(carve((size_t)2 * kFusMaxFront * 8));
     unsigned long long *nLo = reinterpret_cast<unsigned long long *>(carve((size_t)k * 8));
     unsigned int *fHi = reinterpret_cast<unsigned int *>(carve((size_t)2 * kFusMaxFront * 4));
@@ -840,8 +840,8 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     float *sP = reinterpret_cast<float *>(carve((size_t)8 * r * 4));        // group sums of the split-K partials
     float *sWst = reinterpret_cast<float *>(carve((size_t)2 * kFusWarps * 4)); // per-warp softmax (max, sum)
     float *sZ = reinterpret_cast<float *>(carve((size_t)M * 4));
-    float *sBase = reinterpret_cast<float *>(carve((size_t)M * 4));
-    int *sTok = reinterpret_cast<int *>(carve((size_t)M * 4));
+    float *sBase_ = reinterpret_cast<float *>(carve((size_t)2 * M * 4));      // [2 buffers][M]
+    int *sTok_ = reinterpret_cast<int *>(carve((size_t)2 * M * 4));
     int *nTok = reinterpret_cast<int *>(carve((size_t)N * 4));
     int *nPar = reinterpret_cast<int *>(carve((size_t)N * 4));
     int *nDep = reinterpret_cast<int *>(carve((size_t)N * 4));
@@ -881,19 +881,41 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
 #pragma unroll
         for (int i = 0; i < (DT_MAX_M + kFusThreads - 1) / kFusThreads; ++i) {
             const int m = tid + i * kFusThreads;
-            if (m < M) { sTok[m] = ctok[i]; sBase[m] = cval[i]; }
+            if (m < M) { sTok_[m] = ctok[i]; sBase_[m] = cval[i]; }
         }
         __syncthreads();
         if (p.w2_smem) {
             const int vpr = r / 8;
             for (int i = tid; i < M * vpr; i += kFusThreads) {
                 const int m = i / vpr, v = i - m * vpr;
-                cp_async16(sW2 + (size_t)m * ldw2 + v * 8, w2 + (size_t)sTok[m] * r + (size_t)v * 8);
+                cp_async16(sW2_ + (size_t)m * ldw2 + v * 8, w2 + (size_t)sTok_[m] * r + (size_t)v * 8);
             }
         }
         cp_async_commit();
         return seen;
     };
+
+    // warps 1..7 (224 threads, named barrier 1) stage depth `dep` into staging buffer `buf` while warp 0 does something else
+    auto stage_side = [&](int dep, int buf) {
+        constexpr int nw = kFusThreads - 32;
+        const int wt = tid - 32;
+        const size_t row = (size_t)b * L + dep;
+        int *dTok = sTok_ + buf * M;
+        float *dBase = sBase_ + buf * M;
+        __nv_bfloat16 *dW2 = sW2_ + (size_t)buf * M * ldw2;
+        for (int m = wt; m < M; m += nw) { dTok[m] = e.cand_id[row * M + m]; dBase[m] = e.cand_val[row * M + m]; }
+        asm volatile("bar.sync 1, %0;" ::"n"(nw) : "memory");
+        if (p.w2_smem) {
+            const int vpr = r / 8;
+            for (int i = wt; i < M * vpr; i += nw) {
+                const int m = i / vpr, v = i - m * vpr;
+                cp_async16(dW2 + (size_t)m * ldw2 + v * 8, w2 + (size_t)dTok[m] * r + (size_t)v * 8);
+            }
+        }
+        cp_async_commit();
+    };
+    int cb = 0;                                                 // staging buffer of the current node's depth
+    int buf_dep0 = 0, buf_dep1 = -1;                            // depth whose rows each staging buffer holds (or is being filled with)
 
     if (p.spec) {                                               // slice log-softmax of the base logits at position 0 (sorted: v_0 is the max)
         for (int row = warp; row < L; row += kFusWarps) {
@@ -926,6 +948,9 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         const bool node_ok = (t < n_valid);
         const int depth = node_ok ? nDep[t] : L;
         const bool expand = node_ok && depth < L;               // block-uniform
+        __nv_bfloat16 *const sW2 = sW2_ + (size_t)cb * M * ldw2;
+        float *const sBase = sBase_ + cb * M;
+        int *const sTok = sTok_ + cb * M;
         // Every request CTA waits for the GRU CTAs' step t, expanded or not: nobody runs ahead, so the
         // descriptor word and the partial buffer are never overwritten while still in use.
         // C = H W1h^T of the node's depth does not depend on the GRU CTAs: fetch it while waiting for them
@@ -1033,6 +1058,13 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             }
             __syncthreads();
             WV_TR(1, b == 0, t, 2);
+            // While warp 0 picks the top-k and the pop, the other warps prefetch the candidate rows of the NEXT depth into the
+            // other staging buffer: a chain (and most pops of a bushy tree's subtree) goes one level down, and the fetch of
+            // M W2 rows takes longer than what is left between two steps.  A different depth is staged after the pop.
+            if (depth + 1 < L && t + 1 < B && (cb ? buf_dep0 : buf_dep1) != depth + 1) {
+                if (warp != 0) stage_side(depth + 1, cb ^ 1);       // (what that buffer held was waited for before the dots)
+                if (cb) buf_dep0 = depth + 1; else buf_dep1 = depth + 1;
+            }
             // ... then warp 0 merges the 8 warps' (max, sum) pairs in warp order and picks the top-k by (logp desc, token asc)
             // = (z desc, token asc) without anything that scales with M * M: every lane takes the best of its own M / 32
             // sortable keys (ord(z), ~token) and k rounds of a warp max reduction give L, the k-th best of the 32 lane maxima
@@ -1221,21 +1253,20 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                     if (pos < cap) { wHi[pos] = h; wLo[pos] = l; }
                 }
             }
-            if (t + 1 < B && next_dep < L) {                    // overlaps the GRU CTAs' next pass
-                const size_t row = (size_t)b * L + next_dep;
-                for (int m = wt; m < M; m += nw) { sTok[m] = e.cand_id[row * M + m]; sBase[m] = e.cand_val[row * M + m]; }
-                asm volatile("bar.sync 1, %0;" ::"n"(nw) : "memory");     // warps 1..7 only
-                if (p.w2_smem) {
-                    const int vpr = r / 8;
-                    for (int i = wt; i < M * vpr; i += nw) {
-                        const int m = i / vpr, v = i - m * vpr;
-                        cp_async16(sW2 + (size_t)m * ldw2 + v * 8, w2 + (size_t)sTok[m] * r + (size_t)v * 8);
-                    }
-                }
-                cp_async_commit();
+            // neither the prefetched depth nor the current one (a sibling): stage it now (overlaps the GRU CTAs' next pass), once
+            // whatever is still landing in that buffer has landed
+            if (t + 1 < B && next_dep < L && next_dep != buf_dep0 && next_dep != buf_dep1) {
+                cp_async_wait<0>();
+                asm volatile("bar.sync 1, %0;" ::"n"(nw) : "memory");
+                stage_side(next_dep, cb ^ 1);
             }
         }
+        if (t + 1 < B && next_dep < L) {                        // (block-uniform) which buffer holds the next node's rows
+            if (next_dep != buf_dep0 && next_dep != buf_dep1) { if (cb) buf_dep0 = next_dep; else buf_dep1 = next_dep; }
+            cb = (next_dep == buf_dep0) ? 0 : 1;
+        }
     }
+    cp_async_wait<0>();                                         // (a prefetch nobody used)
     __syncthreads();
 
     if (p.stats && tid == 0) {
