@@ -598,8 +598,9 @@ static int launch_fused(dt_handle *h, ExpandParams &p, cudaStream_t st, bool sta
     f.slot_stride = h->slot_stride;
     f.s_hi = h->s_hi; f.s_lo = h->s_lo; f.s32 = h->states; f.partial = h->partial; f.desc = h->desc; f.flags = h->flags; f.round_ctr = h->round_ctr;
     f.static_mode = static_mode ? 1 : 0; f.menu_tok = h->menu_tok; f.menu_lp = h->menu_lp; f.err = h->wv_err;
-    f.w2_smem = 1;
-    size_t rs = fused_req_smem(p.r, p.M, p.N, p.k, 1);
+    f.w2_smem = 1; f.w2_bufs = 2;
+    size_t rs = fused_req_smem(p.r, p.M, p.N, p.k, 1, 2);
+    if (rs > (size_t)h->max_smem_optin) { f.w2_bufs = 1; rs = fused_req_smem(p.r, p.M, p.N, p.k, 1, 1); }
     if (rs > (size_t)h->max_smem_optin) { f.w2_smem = 0; rs = fused_req_smem(p.r, p.M, p.N, p.k, 0); }
     if (rs > (size_t)h->max_smem_optin) return 1;
     const size_t gs = tcgen ? fused_tc_smem(p.g, p.r) : fused_gru_smem(p.g, p.r, upc, f.m_tiles);

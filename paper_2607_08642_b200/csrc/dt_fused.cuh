@@ -57,6 +57,7 @@ struct FusedParams {
                                    // flag word, so the request CTAs of one group work while the GRU CTAs run the next group's pass
     int slot_stride;               // state slots per request = max_B + 2 (slot 0 = zeros, node t at t+1)
     int w2_smem;                   // request CTAs stage the M W2 rows in shared memory
+    int w2_bufs;                   // ... in two buffers (the next depth is prefetched) or, if they do not fit, one
     __nv_bfloat16 *s_hi, *s_lo;    // [batch, slot_stride, g]
     float *s32;                    // [batch, slot_stride, g]
     float *partial;                // [n_gru, batch, r]
@@ -146,11 +147,11 @@ __host__ __device__ inline size_t fused_gru_smem(int g, int r, int upc, int m_ti
     (void)upc;
     return w + (ring > red ? ring : red) + w1 + snew + 3 * kFusChunk * 4 + 64;
 }
-__host__ __device__ inline size_t fused_req_smem(int r, int M, int N, int k, int w2_smem) {
+__host__ __device__ inline size_t fused_req_smem(int r, int M, int N, int k, int w2_smem, int w2_bufs = 2) {
     auto al = [](size_t x) { return (x + 15) / 16 * 16; };
     size_t s = al((size_t)2 * kFusMaxFront * 8) + al((size_t)k * 8) + al((size_t)M * 8) + al((size_t)2 * kFusMaxFront * 4) +
                al((size_t)k * 4) + 9 * al((size_t)r * 4) + al((size_t)M * 4) + 2 * al((size_t)2 * M * 4) + 4 * al((size_t)N * 4);
-    if (w2_smem) s += al((size_t)2 * M * (r + kFusW2Pad) * 2);      // two staging buffers (current depth, prefetched depth)
+    if (w2_smem) s += al((size_t)w2_bufs * M * (r + kFusW2Pad) * 2);   // staging buffers: current depth (+ prefetched depth)
     return s + 16 + 64;
 }
 
@@ -831,7 +832,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     // [new hi] [a] [z] [base] [cand tok] [tree tok / par / dep / score]
     size_t off = 0;
     auto carve = [&](size_t bytes) { unsigned char *q = smem_raw + off; off += (bytes + 15) / 16 * 16; return q; };
-    __nv_bfloat16 *sW2_ = reinterpret_cast<__nv_bfloat16 *>(carve(p.w2_smem ? (size_t)2 * M * ldw2 * 2 : 0));   // [2 buffers][M rows]
+    __nv_bfloat16 *sW2_ = reinterpret_cast<__nv_bfloat16 *>(carve(p.w2_smem ? (size_t)p.w2_bufs * M * ldw2 * 2 : 0));   // [buffers][M rows]
     unsigned long long *fLo = reinterpret_cast<unsigned long long *>(carve((size_t)2 * kFusMaxFront * 8));
     unsigned long long *nLo = reinterpret_cast<unsigned long long *>(carve((size_t)k * 8));
     unsigned int *fHi = reinterpret_cast<unsigned int *>(carve((size_t)2 * kFusMaxFront * 4));
@@ -915,6 +916,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
         cp_async_commit();
     };
     int cb = 0;                                                 // staging buffer of the current node's depth
+    const bool two_bufs = !p.w2_smem || p.w2_bufs == 2;         // (without staged rows only ids / base logits are buffered)
     int buf_dep0 = 0, buf_dep1 = -1;                            // depth whose rows each staging buffer holds (or is being filled with)
 
     if (p.spec) {                                               // slice log-softmax of the base logits at position 0 (sorted: v_0 is the max)
@@ -1061,7 +1063,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             // While warp 0 picks the top-k and the pop, the other warps prefetch the candidate rows of the NEXT depth into the
             // other staging buffer: a chain (and most pops of a bushy tree's subtree) goes one level down, and the fetch of
             // M W2 rows takes longer than what is left between two steps.  A different depth is staged after the pop.
-            if (depth + 1 < L && t + 1 < B && (cb ? buf_dep0 : buf_dep1) != depth + 1) {
+            if (two_bufs && depth + 1 < L && t + 1 < B && (cb ? buf_dep0 : buf_dep1) != depth + 1) {
                 if (warp != 0) stage_side(depth + 1, cb ^ 1);       // (what that buffer held was waited for before the dots)
                 if (cb) buf_dep0 = depth + 1; else buf_dep1 = depth + 1;
             }
@@ -1258,11 +1260,11 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             if (t + 1 < B && next_dep < L && next_dep != buf_dep0 && next_dep != buf_dep1) {
                 cp_async_wait<0>();
                 asm volatile("bar.sync 1, %0;" ::"n"(nw) : "memory");
-                stage_side(next_dep, cb ^ 1);
+                stage_side(next_dep, two_bufs ? cb ^ 1 : 0);
             }
         }
         if (t + 1 < B && next_dep < L) {                        // (block-uniform) which buffer holds the next node's rows
-            if (next_dep != buf_dep0 && next_dep != buf_dep1) { if (cb) buf_dep0 = next_dep; else buf_dep1 = next_dep; }
+            if (next_dep != buf_dep0 && next_dep != buf_dep1) { if (cb || !two_bufs) buf_dep0 = next_dep; else buf_dep1 = next_dep; }
             cb = (next_dep == buf_dep0) ? 0 : 1;
         }
     }

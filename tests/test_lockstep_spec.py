@@ -106,6 +106,20 @@ def test_speculation_full_size_bitwise_equal_to_plain_lockstep(batch, M, B, regi
     assert ne + nt == min(batch, 3)
 
 
+def test_widest_candidate_set_uses_one_staging_buffer():
+    """M = 256 (DT_MAX_M): two staging buffers of W2 rows do not fit a request CTA's shared memory, so the kernel keeps one
+    and does not prefetch; the tree still matches the oracle, with and without speculation."""
+    gu = _gu()
+    case = gu.get_case("qwen8b-m256", wl.CONFIGS["qwen8b"], max_batch=1, max_M=256, max_B=16, k=8)
+    inp = wl.make_inputs(case.cfg, batch=1, seed=5500, regime="peaked")
+    for spec in (2, 0):
+        with _Opts(case, expand_path=4, lockstep_speculation=spec):
+            ne, nt = gu.check_batch(case, inp, 256, 16, 0.6, BF16_TOL)
+            assert case.builder.get_option("expand_path_taken") == 4
+            assert case.builder.get_option("device_error") == 0
+        assert ne + nt == 1
+
+
 def test_speculation_cond_static_arm_unchanged():
     """The Cond-static arm walks the greedy chain with the same kernel (static mode): same trees with and without."""
     gu = _gu()
