@@ -933,10 +933,12 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
     if (tid == 0) {
         nTok[0] = e.root_tokens[b]; nPar[0] = -1; nDep[0] = 0; nSco[0] = 0.f;
         // step-0 descriptor: the root, whose parent state is the zero slot (reading A4)
-        if (p.spec) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + 2,                   // hint for node 1: the root's top-1 child
-                                   fused_desc_pack(1, rnd, (1 < L && 1 < B) ? 1 : -1, sTop1[0]));
+        // (the hint words are written in every round, speculating or not, like the descriptors: a word then never outlives
+        // the round that wrote it, and the 8-bit round tag cannot alias)
+        st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + 2,                               // hint for node 1: the root's top-1 child
+                       fused_desc_pack(1, rnd, (p.spec && 1 < L && 1 < B) ? 1 : -1, p.spec ? sTop1[0] : 0));
         st_relaxed_u64(p.desc + (size_t)b * kFusDescStride, fused_desc_pack(1, rnd, 0, min(max(e.root_tokens[b], 0), e.V - 1)));
-        sm.n_valid = 1; sm.n_front = 0; sm.cur = 0; sm.kwait = 0; sm.kspec = 1; sm.pred_sidx = (p.spec && 1 < L && 1 < B) ? 1 : -1; sm.pred_tok = sTop1[0];
+        sm.n_valid = 1; sm.n_front = 0; sm.cur = 0; sm.kwait = 0; sm.kspec = 1; sm.pred_sidx = (p.spec && 1 < L && 1 < B) ? 1 : -1; sm.pred_tok = p.spec ? sTop1[0] : 0;
         if (p.stats && b == 0) p.stats[1] = 0u;
     }
     __syncthreads();
@@ -1197,7 +1199,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
                     // (the descriptor of step s lives in word s & 1 of the request's line: with speculation this CTA may publish
                     // step t + 1 before every GRU CTA has read step t; the depth rides in the token's top byte)
                     if (t + 1 < B) {
-                        if (p.spec) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + 2 + ((t + 1) & 1), fused_desc_pack(t + 2, rnd, h_sidx, h_tok));
+                        st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + 2 + ((t + 1) & 1), fused_desc_pack(t + 2, rnd, h_sidx, h_tok));
                         st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + ((t + 1) & 1),
                                        fused_desc_pack(t + 2, rnd, dep < L ? par + 1 : -1, p.spec ? (tok | (min(dep, 255) << 24)) : tok));
                     }
@@ -1213,7 +1215,7 @@ __device__ __forceinline__ void fused_req_role(const FusedParams &p, unsigned ch
             } else if (lane == 0) {
                 sm.n_front = 0; sm.kwait = sm.kspec; sm.kspec = sm.kwait + 1; sm.pred_sidx = -1;
                 if (t + 1 < B) {
-                    if (p.spec) st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + 2 + ((t + 1) & 1), fused_desc_pack(t + 2, rnd, -1, 0));
+                    st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + 2 + ((t + 1) & 1), fused_desc_pack(t + 2, rnd, -1, 0));
                     st_relaxed_u64(p.desc + (size_t)b * kFusDescStride + ((t + 1) & 1), fused_desc_pack(t + 2, rnd, -1, 0));
                 }
             }

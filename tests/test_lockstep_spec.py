@@ -106,6 +106,33 @@ def test_speculation_full_size_bitwise_equal_to_plain_lockstep(batch, M, B, regi
     assert ne + nt == min(batch, 3)
 
 
+def test_many_rounds_alternating_modes_on_one_handle():
+    """The hand-over words carry an 8-bit round tag and are never cleared: 600 rounds on one handle (past two wraps of the
+    tag), alternating speculation on / off, batch sizes, budgets and regimes, must reproduce each configuration's first
+    output bit for bit and never raise the device error word."""
+    gu = _gu()
+    case = _small(gu, 8)
+    confs = [(2, 33, 24, 40, "peaked"), (0, 7, 32, 48, "flat"), (2, 1, 8, 8, "peaked"), (0, 33, 24, 12, "peaked"), (2, 12, 16, 3, "flat")]
+    inputs = [wl.make_inputs(case.cfg, batch=c[1], seed=4300 + i, regime=c[4]) for i, c in enumerate(confs)]
+    first = {}
+    try:
+        case.builder.set_option("expand_path", 4)
+        for rnd in range(600):
+            i = (rnd * 7 + rnd // 5) % len(confs)
+            spec, batch, M, B, _ = confs[i]
+            case.builder.set_option("lockstep_speculation", spec)
+            out = case.run_gpu(inputs[i], M, B, 0.6)
+            if i not in first:
+                first[i] = out
+                continue
+            for name in FIELDS:
+                assert torch.equal(getattr(first[i], name), getattr(out, name)), (rnd, i, name)
+        assert case.builder.get_option("device_error") == 0
+    finally:
+        case.builder.set_option("expand_path", 0)
+        case.builder.set_option("lockstep_speculation", 1)
+
+
 def test_widest_candidate_set_uses_one_staging_buffer():
     """M = 256 (DT_MAX_M): two staging buffers of W2 rows do not fit a request CTA's shared memory, so the kernel keeps one
     and does not prefetch; the tree still matches the oracle, with and without speculation."""
